@@ -1,0 +1,151 @@
+/*
+ * dsmc_oracle.h -- CPU oracle for the neural DSMC collision step (TEST INFRASTRUCTURE).
+ *
+ * This is the plain, slow, single-threaded fp64 restatement of what the hot path
+ * computes, written from /root/reference/PAPER.md ("P:L<line>") and the readings
+ * listed in DESIGN.md ("Q<n>").  It is NOT part of the product: only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * call it.  It shares no code, header, table or constant generator with the CUDA
+ * path under paper_2602_21244_b200/csrc/.
+ *
+ * All pointers are HOST pointers.  Velocities are fp64 (fp32 inputs are promoted
+ * exactly by the caller).  Every function is deterministic and re-entrant.
+ *
+ * Parity status: every function below is pinned by tests/test_oracle_*.py
+ * (-m "not gpu") except the behaviour of *trained* networks (isotropy, cos(chi)
+ * PDF, viscosity, flow fields: P:L217-235), which needs the paper's
+ * weights and data and is "parity unpinned".
+ */
+#ifndef DSMC_ORACLE_H
+#define DSMC_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- flags (same numeric values as the product header; restated, not shared) ---- */
+#define ORC_F_NOISE 1u              /* feed sigma_xi*xi to the network (eq. 2/9) */
+#define ORC_F_ENERGY_SHELL 2u       /* eq. 5 projection */
+#define ORC_F_MOMENT_MATCH 4u       /* cell-wise correction, eqs. 10-11 P:L126-131 + P:L46 */
+#define ORC_F_ACCEPT 8u             /* NTC acceptance test */
+#define ORC_F_MATCH_ENERGY_ONLY 32u /* literal eq. 11 (scale raw velocities) */
+
+#define ORC_ACT_TANH 0
+#define ORC_ACT_RELU 1
+#define ORC_ACT_SILU 2
+
+#define ORC_OK 0
+#define ORC_ERR_INVALID_ARG (-1)
+#define ORC_ERR_BAD_CELL_INDEX (-2)
+
+#define ORC_KB 1.380649e-23 /* CODATA k_B, J/K (Q18) */
+
+/* h^(l) = act(W^(l) h^(l-1) + b^(l)); W[l] row-major [out][in], fp32 values */
+typedef struct {
+  int32_t n_layers; /* number of linear layers, 2..6 */
+  int32_t dims[8];  /* dims[0] inputs ... dims[n_layers] outputs */
+  int32_t act;      /* hidden activation */
+  const float *W[7];
+  const float *b[7];
+} orc_mlp;
+
+typedef struct {
+  double mass, sigma_v, T_scale, noise_sigma, shell_eps;
+  double d_ref, omega, T_ref; /* VHS cross-section, used iff ORC_F_ACCEPT */
+  int32_t pairs_per_cell;     /* >0 request per cell, -1 = floor(N_k/2) */
+  uint32_t flags;
+} orc_vhs_params;
+
+typedef struct {
+  double mass, b_max;
+  double lnE_min, lnE_max; /* normalisation of the chi-MLP energy input (Q15) */
+  int32_t chi_mode;        /* 0 = table, 1 = MLP */
+  int32_t pairs_per_cell;
+  uint32_t flags;
+} orc_abinitio_params;
+
+typedef struct { /* chi[iE*nB + iB], node (lnE_min + iE*dE, iB/(nB-1)), Q13 */
+  const float *chi;
+  int32_t nE, nB;
+  double lnE_min, lnE_max;
+} orc_chi_table;
+
+/* potentials for the deflection integral (eq. 16) */
+#define ORC_POT_LJ 0          /* 4 eps ((s/r)^12-(s/r)^6); p0 = eps [J], p1 = sigma [m]  (Q17) */
+#define ORC_POT_HARD_SPHERE 1 /* +inf for r<d; p0 = d */
+#define ORC_POT_INV_R 2       /* kappa / r;   p0 = kappa */
+#define ORC_POT_INV_R2 3      /* kappa / r^2; p0 = kappa */
+typedef struct {
+  int32_t kind;
+  double p0, p1;
+  double r_hi; /* scan start for r_min, must exceed the largest root */
+} orc_potential;
+
+/* ---- random numbers (a4) ---- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double orc_u01(uint32_t x); /* ((x>>8)+0.5)*2^-24 in (0,1) */
+/* pairing key of slot p in cell k at step t (stream 0) */
+uint32_t orc_pair_key(uint64_t seed, uint32_t step, uint32_t cell, uint32_t slot);
+/* per-pair uniforms (stream 1): U_acc, U_b, U_eps */
+void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double u[3]);
+/* per-pair latent xi ~ N(0, I3) by Box-Muller (stream 2) */
+void orc_pair_normals(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double xi[3]);
+
+/* ---- a1: stable counting sort by cell id, P:L140 ---- */
+int orc_bin(int64_t n, int32_t n_cells, const int32_t *cell, int32_t *perm, int32_t *cell_start);
+
+/* ---- a2: cell moments, eq. 10: moments[k] = (Px,Py,Pz,E=sum|v|^2) ---- */
+void orc_cell_moments(int32_t n_cells, const int32_t *cell_start, const double *vx,
+                      const double *vy, const double *vz, double *moments);
+/* mean velocity, centred Theta = sum|v-u|^2, T = m Theta/(3 kB N) of one segment (Q6) */
+void orc_cell_state(int64_t N, const double *vx, const double *vy, const double *vz, double mass,
+                    double ubar[3], double *Theta, double *T);
+
+/* ---- a3: disjoint random matching (Q7). pi[N] = slots sorted by (key,slot). returns M ---- */
+int32_t orc_pairing(uint64_t seed, uint32_t step, uint32_t cell, int32_t N, int32_t M_req,
+                    int32_t *pi);
+
+/* ---- operators ---- */
+void orc_mlp_forward(const orc_mlp *net, const double *x, double *out);
+double orc_vhs_sigma_g(double g, const orc_vhs_params *p); /* sigma_T(g)*g, P:L68 + BJ cfg 1 */
+void orc_rotate(const double g[3], double chi, double eps, double gp[3]); /* Q16 */
+double orc_chi_bilinear(const orc_chi_table *t, double lnE, double btilde);
+double orc_chi_mlp(const orc_mlp *net, double lnE_min, double lnE_max, double lnE, double btilde);
+
+/* ---- a8: moment matching against target moments, eqs. 10-11 + P:L46 (Q5) ---- */
+void orc_moment_match(int32_t n_cells, const int32_t *cell_start, double *vx, double *vy,
+                      double *vz, const double *target_moments, uint32_t flags);
+
+/* ---- fused steps (a2-a9).  pair_i/pair_j/accepted (may be NULL) are indexed
+ *      cell_start[k]+s for pair slot s<M_k and hold slots relative to cell_start[k].
+ *      gprime_out (may be NULL): 3 doubles per dump index = post-collision relative velocity,
+ *      hnorm_out (may be NULL): |h_hat| per dump index (VHS-NN only; Q21 gating). ---- */
+int orc_collide_vhs_nn(int64_t n, int32_t n_cells, const int32_t *cell_start, double *vx,
+                       double *vy, double *vz, const float *sigma_cr_max, const orc_mlp *net,
+                       const orc_vhs_params *p, uint64_t seed, uint32_t step, int32_t *pair_i,
+                       int32_t *pair_j, uint8_t *accepted, double *gprime_out, double *hnorm_out);
+int orc_collide_abinitio(int64_t n, int32_t n_cells, const int32_t *cell_start, double *vx,
+                         double *vy, double *vz, const float *cr_max, const orc_mlp *net,
+                         const orc_chi_table *table, const orc_abinitio_params *p, uint64_t seed,
+                         uint32_t step, int32_t *pair_i, int32_t *pair_j, uint8_t *accepted,
+                         double *gprime_out, double *chi_out);
+
+/* ---- a10: chi for independent (E_r/k_B [K], b [m]) pairs ---- */
+void orc_chi_batch(int64_t n, const float *E_over_k, const float *b, double *chi, int32_t chi_mode,
+                   const orc_mlp *net, const orc_chi_table *table, double b_max, double lnE_min,
+                   double lnE_max);
+
+/* ---- "Exact" deflection angle, eqs. 16/20/21 P:L272, P:L327, P:L338-342 ---- */
+double orc_potential_eval(const orc_potential *pot, double r);
+double orc_rmin(const orc_potential *pot, double E, double b);
+/* signed chi by composite Gauss-Legendre (n_panels x 64 points) after u=r_min/r, u=1-s^2 */
+double orc_chi_exact(const orc_potential *pot, double E, double b, int32_t n_panels);
+/* fills chi[nE*nB] with |chi| rounded to fp32 (Q14) */
+void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, double lnE_min,
+                         double lnE_max, double b_max, int32_t n_panels, float *chi);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
