@@ -36,8 +36,8 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* 24-bit uniform strictly inside (0,1); exact in fp32 and fp64 */
-double orc_u01(uint32_t x) { return ((double)(x >> 8) + 0.5) * (1.0 / 16777216.0); }
+/* 23-bit uniform + half step: strictly inside (0,1) and (24 significant bits) exact in fp32 and fp64 */
+double orc_u01(uint32_t x) { return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0); }
 
 static void philox_at(uint64_t seed, uint32_t index, uint32_t cell, uint32_t step, uint32_t stream,
                       uint32_t out[4]) {

@@ -84,7 +84,7 @@ typedef struct {
 
 /* ---- random numbers (a4) ---- */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
-double orc_u01(uint32_t x); /* ((x>>8)+0.5)*2^-24 in (0,1) */
+double orc_u01(uint32_t x); /* ((x>>9)+0.5)*2^-23 in (0,1), exact in fp32 */
 /* pairing key of slot p in cell k at step t (stream 0) */
 uint32_t orc_pair_key(uint64_t seed, uint32_t step, uint32_t cell, uint32_t slot);
 /* per-pair uniforms (stream 1): U_acc, U_b, U_eps */
