@@ -1,0 +1,189 @@
+/*
+ * dsmc.h -- C ABI of the B200-native neural DSMC collision step.
+ *
+ * Method: Roohi, Shoja-sani, Stefanov, "Physics Constrained Neural Collision Operators for
+ * Variable Hard Sphere Surrogates and Ab Initio Angle Prediction in DSMC" (arxiv 2602.21244).
+ * Citations "P:L<n>" are line numbers of the paper text; "Q<n>" are the readings
+ * listed in DESIGN.md.  One call = one stage of the per-step collision path:
+ *
+ *   dsmc_bin               sort particles by cell index
+ *   dsmc_collide_vhs_nn    fused step with the VHS-surrogate MLP (eqs. 1-11)
+ *   dsmc_collide_abinitio  fused step with chi(E,b) by table or MLP + rotation
+ *   dsmc_cell_moments      per-cell momentum / energy sums (eq. 10)
+ *   dsmc_moment_match      cell-wise correction on its own (eqs. 10-11)
+ *   dsmc_chi_batch         chi for independent (E_r, b) pairs
+ *   dsmc_step_host         bin + fused step on HOST buffers (copies inside), for end-to-end timing
+ *
+ * Conventions
+ *   - Plain C, no C++/torch types.  Every function returns an int status (0 = DSMC_OK).
+ *   - Unless marked HOST, array arguments are DEVICE pointers owned by the caller; the library
+ *     never allocates, frees or retains them.  Arrays need only their natural alignment.
+ *   - Work is enqueued asynchronously on the context's stream (dsmc_set_stream; default stream
+ *     0).  Argument errors detectable on the host are returned immediately and nothing is
+ *     launched.  Data errors found on the device (cell index out of range, cell larger than
+ *     DSMC_MAX_CELL_PARTICLES) set a sticky status word returned (and cleared) by
+ *     dsmc_sync_status(), which synchronises the stream; outputs of such a call are unspecified.
+ *   - One context per device and stream; a context is not thread-safe.
+ *   - There is no CPU fallback: every stage runs in this library's sm_100a kernels.
+ *
+ * Random numbers: Philox4x32-10, key = seed, counter =
+ * (index, cell, step, stream); stream 0 = pairing keys (slot p uses word p&3 of block p>>2),
+ * stream 1 = (U_acc, U_b, U_eps) of pair slot s, stream 2 = Box-Muller normals of pair slot s;
+ * u = ((x>>9)+0.5) 2^-23.  Results therefore depend only on (seed, step, cell, slot).
+ */
+#ifndef DSMC_H
+#define DSMC_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DSMC_OK 0
+#define DSMC_ERR_INVALID_ARG (-1)
+#define DSMC_ERR_BAD_CELL_INDEX (-2)
+#define DSMC_ERR_CELL_TOO_LARGE (-3)
+#define DSMC_ERR_NOT_CONFIGURED (-4)
+#define DSMC_ERR_CUDA (-5)
+#define DSMC_ERR_UNSUPPORTED_SHAPE (-6)
+
+/* largest cell the SMEM-resident fused step accepts */
+#define DSMC_MAX_CELL_PARTICLES 2048
+
+typedef struct dsmc_ctx dsmc_ctx;
+
+/* Create a context on CUDA device `device` sized for at most max_particles / max_cells.
+ * Owns: scan scratch, staged weights, the chi table copy, the status word. */
+int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_cells);
+int dsmc_destroy(dsmc_ctx *ctx);
+/* Borrow a cudaStream_t (e.g. torch's current stream); NULL = default stream. */
+int dsmc_set_stream(dsmc_ctx *ctx, void *cuda_stream);
+/* Synchronise the stream; return and clear the sticky device status. */
+int dsmc_sync_status(dsmc_ctx *ctx);
+const char *dsmc_strerror(int status);
+/* Number of kernels this context has launched so far (bench bookkeeping). */
+int64_t dsmc_launch_count(const dsmc_ctx *ctx);
+
+/* ---- operators ------------------------------------------------------------------------- */
+typedef enum { DSMC_ACT_TANH = 0, DSMC_ACT_RELU = 1, DSMC_ACT_SILU = 2 } dsmc_act;
+
+/* h^(l) = act(W^(l) h^(l-1) + b^(l)), last layer linear.
+ * W, b: HOST pointers, fp32, W[l] row-major [dims[l+1]][dims[l]]; copied during the call. */
+typedef struct {
+  int32_t n_layers; /* linear layers, 2..6 */
+  int32_t dims[8];  /* dims[0] = inputs, dims[n_layers] = outputs; every dim <= 256 */
+  int32_t act;      /* dsmc_act of the hidden layers */
+  const float *const *W;
+  const float *const *b;
+} dsmc_mlp_desc;
+
+/* slot 0: VHS-surrogate f_theta (eqs. 3-4): dims[0] = 8 (g/sigma_v (3), |g|/sigma_v,
+ *         T_cell/T_scale, sigma_xi*xi (3); BASELINE.json form, Q2-Q3) or 6 (g/sigma_v (+) xi,
+ *         the paper's eq. 3 as read in Q1); dims[n_layers] = 3.
+ * slot 1: chi-MLP: dims[0] = 2 ((E~-E~min)/(E~max-E~min), b~), output 1,
+ *         chi = expm1(softplus(z)) (Q15).
+ * The BF16 tensor-core path (DSMC_F_BF16_TC) needs n_layers = 3 and equal hidden widths in
+ * {64, 128}; other shapes run only on the FP32 path (DSMC_ERR_UNSUPPORTED_SHAPE otherwise). */
+int dsmc_set_mlp(dsmc_ctx *ctx, int slot, const dsmc_mlp_desc *desc);
+
+/* chi table: chi_host HOST fp32 [nE][nB] row-major, node (iE,iB) at
+ * E~ = lnE_min + iE (lnE_max-lnE_min)/(nE-1) with E~ = ln(E_r/k_B [K]), b~ = iB/(nB-1).
+ * Lookups clamp both coordinates to the grid (Q13).  Copied during the call. */
+int dsmc_set_chi_table(dsmc_ctx *ctx, const float *chi_host, int32_t nE, int32_t nB, float lnE_min,
+                       float lnE_max);
+
+/* ---- a1: binning ---------------------------------------------------------------
+ * Stable counting sort of n particles by cell[p] in [0, n_cells).  Outputs: cell_start
+ * [n_cells+1] (CSR offsets), perm[n] (sorted slot -> original particle id; ties keep the
+ * original order, so the result is unique), and the velocities gathered into sorted order.
+ * n == 0: cell_start is zero-filled.  Bad index: sticky DSMC_ERR_BAD_CELL_INDEX. */
+int dsmc_bin(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell, const float *vx,
+             const float *vy, const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm,
+             int32_t *cell_start);
+
+/* ---- fused collision steps -------------------------------------------------------------- */
+enum {
+  DSMC_F_NOISE = 1,             /* feed sigma_xi * xi, xi ~ N(0,I3), to f_theta (eq. 2/9)      */
+  DSMC_F_ENERGY_SHELL = 2,      /* g' = |g| h/|h| (eq. 5, guard Q4); else g' = sigma_v h */
+  DSMC_F_MOMENT_MATCH = 4,      /* restore the cell's pre-collision momentum and energy (Q5)   */
+  DSMC_F_ACCEPT = 8,            /* NTC acceptance test; needs the *_max array          */
+  DSMC_F_BF16_TC = 16,          /* MLP layers as tcgen05 BF16 GEMMs over 128-pair tiles        */
+  DSMC_F_MATCH_ENERGY_ONLY = 32 /* literal eq. 11: scale raw velocities by sqrt(E_pre/E_post)  */
+};
+
+typedef struct {
+  float mass;        /* kg */
+  float sigma_v;     /* global velocity scale */
+  float T_scale;     /* K, normalises the T_cell feature */
+  float noise_sigma; /* sigma_xi (BASELINE.json cfg 1: 0.1) */
+  float shell_eps;   /* |h| below this skips the collision (Q4) */
+  float d_ref, omega, T_ref; /* VHS sigma_T(g), used iff DSMC_F_ACCEPT */
+  int32_t pairs_per_cell;    /* > 0: request per cell; -1: floor(N_k/2).  M_k = min(req, N_k/2) */
+  uint32_t flags;
+} dsmc_vhs_params;
+
+typedef struct {
+  float mass;
+  float b_max;            /* m; b = b_max sqrt(U_b) */
+  float lnE_min, lnE_max; /* normalisation of the chi-MLP energy input (Q15) */
+  int32_t chi_mode;       /* 0 = table, 1 = MLP (slot 1) */
+  int32_t pairs_per_cell;
+  uint32_t flags;         /* NOISE / ENERGY_SHELL are ignored here */
+} dsmc_abinitio_params;
+
+/* Optional debug output (any member may be NULL).  All arrays have n entries; pair slot s of
+ * cell k is written at index cell_start[k] + s (s < M_k): pair_i/pair_j = the two particle
+ * slots RELATIVE to cell_start[k]; accepted = 0/1; gprime = post-collision relative velocity
+ * (3 floats per index); aux = |h_hat| (VHS-NN) or chi (ab initio).  Other entries untouched. */
+typedef struct {
+  int32_t *pair_i;
+  int32_t *pair_j;
+  uint8_t *accepted;
+  float *gprime;
+  float *aux;
+} dsmc_pair_dump;
+
+/* Per cell k (contiguous segment [cell_start[k], cell_start[k+1]) of the sorted arrays):
+ * pre-collision moments -> disjoint random pairing (Q7) -> [acceptance] -> operator ->
+ * centre-of-mass update (eqs. 6-8) -> [moment matching over the whole cell] -> store.
+ * Velocities are updated in place.  Cells with N_k < 2 are untouched.
+ * sigma_cr_max / cr_max: [n_cells] fp32 caps for the acceptance test, or NULL (accept all). */
+int dsmc_collide_vhs_nn(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_start,
+                        float *vx_s, float *vy_s, float *vz_s, const float *sigma_cr_max,
+                        const dsmc_vhs_params *prm, uint64_t seed, uint32_t step,
+                        const dsmc_pair_dump *dump);
+int dsmc_collide_abinitio(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_start,
+                          float *vx_s, float *vy_s, float *vz_s, const float *cr_max,
+                          const dsmc_abinitio_params *prm, uint64_t seed, uint32_t step,
+                          const dsmc_pair_dump *dump);
+
+/* ---- cell sums and the stand-alone correction ------------------------------------------- */
+/* moments[k] = (Px, Py, Pz, E = sum |v|^2), fp64, eq. 10 */
+int dsmc_cell_moments(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_start,
+                      const float *vx_s, const float *vy_s, const float *vz_s, double *moments);
+/* v <- u_t + sqrt(Theta_t/Theta') (v - u') with (u_t, Theta_t) from target_moments[k] (Q5);
+ * flags & DSMC_F_MATCH_ENERGY_ONLY: v <- v sqrt(E_t/E') (eq. 11). */
+int dsmc_moment_match(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_start,
+                      float *vx_s, float *vy_s, float *vz_s, const double *target_moments,
+                      uint32_t flags);
+
+/* ---- a10: chi for n independent pairs (BASELINE.json cfg 4) ------------------------------
+ * E_over_k [K], b [m] -> chi [rad]; chi_mode 0 = table, 1 = MLP slot 1;
+ * flags & DSMC_F_BF16_TC selects the tensor-core MLP. */
+int dsmc_chi_batch(dsmc_ctx *ctx, int64_t n, const float *E_over_k, const float *b, float *chi,
+                   int32_t chi_mode, float b_max, float lnE_min, float lnE_max, uint32_t flags);
+
+/* ---- end-to-end helper on HOST buffers ----------------------------------------------------
+ * Copies cell/vx/vy/vz (HOST, ideally pinned) to context-owned device buffers, runs dsmc_bin and
+ * one fused ab initio (vhs == NULL) or VHS-NN (abi == NULL) step, copies the sorted post-collision
+ * velocities, perm and cell_start back to the HOST outputs, and synchronises. */
+int dsmc_step_host(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_h,
+                   const float *vx_h, const float *vy_h, const float *vz_h, float *vx_out_h,
+                   float *vy_out_h, float *vz_out_h, int32_t *perm_h, int32_t *cell_start_h,
+                   const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi, uint64_t seed,
+                   uint32_t step);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,334 @@
+// C-ABI entry points of libdsmc_b200.so (see include/dsmc.h): context management, operator
+// staging, argument checks, and dispatch to the kernel launchers.  No compute happens here.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "dsmc_internal.h"
+
+using namespace dsmc;
+
+#define CK(x)                                  \
+  do {                                         \
+    if ((x) != cudaSuccess) return DSMC_ERR_CUDA; \
+  } while (0)
+
+extern "C" {
+
+int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_cells) {
+  if (!out || max_particles < 0 || max_cells < 0 || max_particles >= (int64_t(1) << 31)) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(device));
+  dsmc_ctx *c = new (std::nothrow) dsmc_ctx();
+  if (!c) return DSMC_ERR_CUDA;
+  memset(c, 0, sizeof(*c));
+  c->device = device;
+  c->stream = 0;
+  c->max_particles = max_particles;
+  c->max_cells = max_cells;
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, device));
+  c->num_sms = prop.multiProcessorCount;
+  CK(cudaMalloc(&c->d_status, sizeof(int32_t)));
+  CK(cudaMemset(c->d_status, 0, sizeof(int32_t)));
+  CK(cudaMalloc(&c->d_cursor, sizeof(int32_t) * (size_t)(max_cells + 2)));
+  *out = c;
+  return DSMC_OK;
+}
+
+int dsmc_destroy(dsmc_ctx *c) {
+  if (!c) return DSMC_OK;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  cudaFree(c->d_status);
+  cudaFree(c->d_cursor);
+  for (int s = 0; s < 2; ++s) {
+    cudaFree(c->d_weights[s]);
+    cudaFree(c->d_tc_blob[s]);
+  }
+  cudaFree(c->d_table);
+  cudaFree(c->h_cell);
+  for (int a = 0; a < 3; ++a) { cudaFree(c->h_v[a]); cudaFree(c->h_vs[a]); }
+  cudaFree(c->h_perm);
+  cudaFree(c->h_cell_start);
+  delete c;
+  return DSMC_OK;
+}
+
+int dsmc_set_stream(dsmc_ctx *c, void *cuda_stream) {
+  if (!c) return DSMC_ERR_INVALID_ARG;
+  c->stream = (cudaStream_t)cuda_stream;
+  return DSMC_OK;
+}
+
+int dsmc_sync_status(dsmc_ctx *c) {
+  if (!c) return DSMC_ERR_INVALID_ARG;
+  int32_t st = 0;
+  CK(cudaMemcpyAsync(&st, c->d_status, sizeof(st), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (st != 0) CK(cudaMemsetAsync(c->d_status, 0, sizeof(int32_t), c->stream));
+  return st;
+}
+
+const char *dsmc_strerror(int s) {
+  switch (s) {
+    case DSMC_OK: return "ok";
+    case DSMC_ERR_INVALID_ARG: return "invalid argument";
+    case DSMC_ERR_BAD_CELL_INDEX: return "cell index out of range";
+    case DSMC_ERR_CELL_TOO_LARGE: return "cell has more particles than DSMC_MAX_CELL_PARTICLES";
+    case DSMC_ERR_NOT_CONFIGURED: return "operator (MLP or chi table) not set";
+    case DSMC_ERR_CUDA: return "CUDA runtime error";
+    case DSMC_ERR_UNSUPPORTED_SHAPE: return "MLP shape not supported by the requested path";
+    default: return "unknown status";
+  }
+}
+
+int64_t dsmc_launch_count(const dsmc_ctx *c) { return c ? c->launches : 0; }
+
+int dsmc_set_mlp(dsmc_ctx *c, int slot, const dsmc_mlp_desc *d) {
+  if (!c || !d || slot < 0 || slot > 1 || !d->W || !d->b) return DSMC_ERR_INVALID_ARG;
+  if (d->n_layers < 2 || d->n_layers > 6) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  if (d->act < 0 || d->act > 2) return DSMC_ERR_INVALID_ARG;
+  int dmax = 0;
+  size_t total = 0;
+  for (int l = 0; l <= d->n_layers; ++l) {
+    if (d->dims[l] < 1 || d->dims[l] > 256) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    dmax = d->dims[l] > dmax ? d->dims[l] : dmax;
+    if (l < d->n_layers) total += (size_t)d->dims[l] * d->dims[l + 1] + d->dims[l + 1];
+  }
+  if (slot == 0 && (!(d->dims[0] == 8 || d->dims[0] == 6) || d->dims[d->n_layers] != 3)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  if (slot == 1 && (d->dims[0] != 2 || d->dims[d->n_layers] != 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  // stage transposed fp32 weights: Wt[l][in][out]
+  std::vector<float> host((total + 3) & ~size_t(3));
+  MlpDev m{};
+  m.n_layers = d->n_layers;
+  m.act = d->act;
+  m.dmax = (dmax + 3) & ~3;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  cudaFree(c->d_weights[slot]);
+  c->d_weights[slot] = nullptr;
+  CK(cudaMalloc(&c->d_weights[slot], sizeof(float) * host.size()));
+  size_t off = 0;
+  for (int l = 0; l < d->n_layers; ++l) {
+    const int din = d->dims[l], dout = d->dims[l + 1];
+    m.dims[l] = din;
+    m.dims[l + 1] = dout;
+    if (!d->W[l] || !d->b[l]) return DSMC_ERR_INVALID_ARG;
+    m.Wt[l] = c->d_weights[slot] + off;
+    for (int i = 0; i < din; ++i)
+      for (int o = 0; o < dout; ++o) host[off + (size_t)i * dout + o] = d->W[l][(size_t)o * din + i];
+    off += (size_t)din * dout;
+    m.b[l] = c->d_weights[slot] + off;
+    for (int o = 0; o < dout; ++o) host[off + o] = d->b[l][o];
+    off += dout;
+  }
+  CK(cudaMemcpy(c->d_weights[slot], host.data(), sizeof(float) * host.size(), cudaMemcpyHostToDevice));
+  c->mlp[slot] = m;
+  c->has_mlp[slot] = true;
+  // tensor-core image when the shape allows it
+  cudaFree(c->d_tc_blob[slot]);
+  c->d_tc_blob[slot] = nullptr;
+  memset(&c->mlp_tc[slot], 0, sizeof(MlpTcDev));
+  int rc = build_tc_blob(d, &c->d_tc_blob[slot], &c->mlp_tc[slot], c->stream);
+  if (rc != DSMC_OK && rc != DSMC_ERR_UNSUPPORTED_SHAPE) return rc;
+  return DSMC_OK;
+}
+
+int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t nB, float lnE_min, float lnE_max) {
+  if (!c || !chi_host || nE < 2 || nB < 2 || !(lnE_max > lnE_min)) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  cudaFree(c->d_table);
+  c->d_table = nullptr;
+  CK(cudaMalloc(&c->d_table, sizeof(float) * (size_t)nE * nB));
+  CK(cudaMemcpy(c->d_table, chi_host, sizeof(float) * (size_t)nE * nB, cudaMemcpyHostToDevice));
+  c->table.chi = c->d_table;
+  c->table.nE = nE;
+  c->table.nB = nB;
+  c->table.lnE_min = lnE_min;
+  c->table.inv_dlnE = (float)((double)(nE - 1) / ((double)lnE_max - (double)lnE_min));
+  c->has_table = true;
+  return DSMC_OK;
+}
+
+static int check_sorted_args(dsmc_ctx *c, int64_t n, int32_t K, const void *cs, const void *x, const void *y,
+                             const void *z) {
+  if (!c || n < 0 || K < 0 || n >= (int64_t(1) << 31)) return DSMC_ERR_INVALID_ARG;
+  if (n == 0 || K == 0) return 1;  // nothing to do
+  if (!cs || !x || !y || !z) return DSMC_ERR_INVALID_ARG;
+  return DSMC_OK;
+}
+
+int dsmc_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const float *vx, const float *vy,
+             const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm, int32_t *cell_start) {
+  if (!c || n < 0 || K < 0 || n >= (int64_t(1) << 31) || K > c->max_cells) return DSMC_ERR_INVALID_ARG;
+  if (!cell_start) return DSMC_ERR_INVALID_ARG;
+  if (n > 0 && (!cell || !vx || !vy || !vz || !vx_s || !vy_s || !vz_s || !perm)) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_bin(c, n, K, cell, vx, vy, vz, vx_s, vy_s, vz_s, perm, cell_start);
+}
+
+int dsmc_cell_moments(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, const float *vx, const float *vy,
+                      const float *vz, double *moments) {
+  if (!c || n < 0 || K < 0) return DSMC_ERR_INVALID_ARG;
+  if (K == 0) return DSMC_OK;
+  if (!cs || !moments || (n > 0 && (!vx || !vy || !vz))) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_cell_moments(c, n, K, cs, vx, vy, vz, moments);
+}
+
+int dsmc_moment_match(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, float *vx, float *vy, float *vz,
+                      const double *target, uint32_t flags) {
+  int rc = check_sorted_args(c, n, K, cs, vx, vy, vz);
+  if (rc != DSMC_OK) return rc == 1 ? DSMC_OK : rc;
+  if (!target) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_moment_match(c, n, K, cs, vx, vy, vz, target, flags);
+}
+
+static void fill_common(StepParams &p, dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, float *vx, float *vy,
+                        float *vz, const float *cap, uint64_t seed, uint32_t step, const dsmc_pair_dump *dump) {
+  memset(&p, 0, sizeof(p));
+  p.n = n; p.n_cells = K; p.cell_start = cs;
+  p.vx = vx; p.vy = vy; p.vz = vz;
+  p.cap = cap;
+  p.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu);
+  p.seed_hi = (uint32_t)(seed >> 32);
+  p.step = step;
+  if (dump) p.dump = *dump;
+  p.status = c->d_status;
+}
+
+int dsmc_collide_vhs_nn(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, float *vx, float *vy, float *vz,
+                        const float *sigma_cr_max, const dsmc_vhs_params *prm, uint64_t seed, uint32_t step,
+                        const dsmc_pair_dump *dump) {
+  if (!prm) return DSMC_ERR_INVALID_ARG;
+  int rc = check_sorted_args(c, n, K, cs, vx, vy, vz);
+  if (rc != DSMC_OK) return rc == 1 ? DSMC_OK : rc;
+  if (!c->has_mlp[0]) return DSMC_ERR_NOT_CONFIGURED;
+  if (!(prm->sigma_v > 0.f) || !(prm->T_scale > 0.f) || !(prm->mass > 0.f)) return DSMC_ERR_INVALID_ARG;
+  StepParams p;
+  fill_common(p, c, n, K, cs, vx, vy, vz, sigma_cr_max, seed, step, dump);
+  p.flags = prm->flags;
+  p.pairs_per_cell = prm->pairs_per_cell;
+  p.op = 0;
+  p.mass = prm->mass;
+  p.sigma_v = prm->sigma_v;
+  p.inv_sigma_v = 1.0f / prm->sigma_v;
+  p.inv_T_scale = 1.0f / prm->T_scale;
+  p.noise_sigma = prm->noise_sigma;
+  p.shell_eps = prm->shell_eps;
+  if ((prm->flags & DSMC_F_ACCEPT) && sigma_cr_max) {
+    // sigma_T(g) g = pi d^2 (2 kB T_ref / (m_r g^2))^(omega-1/2) / Gamma(5/2-omega) * g, m_r = m/2
+    const double mr = 0.5 * (double)prm->mass, kB = 1.380649e-23;
+    p.vhs_c = (float)(M_PI * (double)prm->d_ref * prm->d_ref * pow(2.0 * kB * prm->T_ref / mr, prm->omega - 0.5) /
+                      tgamma(2.5 - prm->omega));
+    p.vhs_e = (float)(2.0 - 2.0 * (double)prm->omega);
+  }
+  CK(cudaSetDevice(c->device));
+  if (prm->flags & DSMC_F_BF16_TC) {
+    if (c->mlp_tc[0].H == 0) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    return launch_collide_tc(c, p, &c->mlp_tc[0]);
+  }
+  return launch_collide(c, p, &c->mlp[0]);
+}
+
+int dsmc_collide_abinitio(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, float *vx, float *vy, float *vz,
+                          const float *cr_max, const dsmc_abinitio_params *prm, uint64_t seed, uint32_t step,
+                          const dsmc_pair_dump *dump) {
+  if (!prm) return DSMC_ERR_INVALID_ARG;
+  int rc = check_sorted_args(c, n, K, cs, vx, vy, vz);
+  if (rc != DSMC_OK) return rc == 1 ? DSMC_OK : rc;
+  if (prm->chi_mode != 0 && prm->chi_mode != 1) return DSMC_ERR_INVALID_ARG;
+  if (prm->chi_mode == 0 && !c->has_table) return DSMC_ERR_NOT_CONFIGURED;
+  if (prm->chi_mode == 1 && !c->has_mlp[1]) return DSMC_ERR_NOT_CONFIGURED;
+  if (!(prm->mass > 0.f)) return DSMC_ERR_INVALID_ARG;
+  if (prm->chi_mode == 1 && !(prm->lnE_max > prm->lnE_min)) return DSMC_ERR_INVALID_ARG;
+  StepParams p;
+  fill_common(p, c, n, K, cs, vx, vy, vz, cr_max, seed, step, dump);
+  p.flags = prm->flags & ~(uint32_t)(DSMC_F_NOISE | DSMC_F_ENERGY_SHELL);
+  p.pairs_per_cell = prm->pairs_per_cell;
+  p.op = prm->chi_mode == 0 ? 1 : 2;
+  p.mass = prm->mass;
+  p.e_coef = (float)((double)prm->mass / (4.0 * 1.380649e-23));
+  p.lnE_min = prm->lnE_min;
+  p.inv_lnE_range = prm->chi_mode == 1 ? 1.0f / (prm->lnE_max - prm->lnE_min) : 0.f;
+  p.table = c->table;
+  CK(cudaSetDevice(c->device));
+  if (prm->chi_mode == 1 && (prm->flags & DSMC_F_BF16_TC)) {
+    if (c->mlp_tc[1].H == 0) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    return launch_collide_tc(c, p, &c->mlp_tc[1]);
+  }
+  return launch_collide(c, p, prm->chi_mode == 1 ? &c->mlp[1] : nullptr);
+}
+
+int dsmc_chi_batch(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, int32_t chi_mode,
+                   float b_max, float lnE_min, float lnE_max, uint32_t flags) {
+  if (!c || n < 0 || (chi_mode != 0 && chi_mode != 1) || !(b_max > 0.f)) return DSMC_ERR_INVALID_ARG;
+  if (n == 0) return DSMC_OK;
+  if (!E_over_k || !b || !chi) return DSMC_ERR_INVALID_ARG;
+  if (chi_mode == 0 && !c->has_table) return DSMC_ERR_NOT_CONFIGURED;
+  if (chi_mode == 1 && !c->has_mlp[1]) return DSMC_ERR_NOT_CONFIGURED;
+  if (chi_mode == 1 && !(lnE_max > lnE_min)) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  if (chi_mode == 1 && (flags & DSMC_F_BF16_TC)) {
+    if (c->mlp_tc[1].H == 0) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    return launch_chi_batch_tc(c, n, E_over_k, b, chi, b_max, lnE_min, lnE_max, &c->mlp_tc[1]);
+  }
+  return launch_chi_batch(c, n, E_over_k, b, chi, chi_mode, b_max, lnE_min, lnE_max, &c->mlp[1]);
+}
+
+static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
+  if (n <= c->host_cap_n && K <= c->host_cap_cells) return DSMC_OK;
+  cudaFree(c->h_cell);
+  for (int a = 0; a < 3; ++a) { cudaFree(c->h_v[a]); cudaFree(c->h_vs[a]); }
+  cudaFree(c->h_perm);
+  cudaFree(c->h_cell_start);
+  c->host_cap_n = 0;
+  CK(cudaMalloc(&c->h_cell, sizeof(int32_t) * (size_t)n));
+  for (int a = 0; a < 3; ++a) {
+    CK(cudaMalloc(&c->h_v[a], sizeof(float) * (size_t)n));
+    CK(cudaMalloc(&c->h_vs[a], sizeof(float) * (size_t)n));
+  }
+  CK(cudaMalloc(&c->h_perm, sizeof(int32_t) * (size_t)n));
+  CK(cudaMalloc(&c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1)));
+  c->host_cap_n = n;
+  c->host_cap_cells = K;
+  return DSMC_OK;
+}
+
+int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, const float *vx_h, const float *vy_h,
+                   const float *vz_h, float *vx_out_h, float *vy_out_h, float *vz_out_h, int32_t *perm_h,
+                   int32_t *cell_start_h, const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi,
+                   uint64_t seed, uint32_t step) {
+  if (!c || n <= 0 || K <= 0 || K > c->max_cells || (!vhs && !abi) || (vhs && abi)) return DSMC_ERR_INVALID_ARG;
+  if (!cell_h || !vx_h || !vy_h || !vz_h || !vx_out_h || !vy_out_h || !vz_out_h) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  int rc = ensure_host_staging(c, n, K);
+  if (rc != DSMC_OK) return rc;
+  cudaStream_t s = c->stream;
+  const float *src[3] = {vx_h, vy_h, vz_h};
+  float *dst[3] = {vx_out_h, vy_out_h, vz_out_h};
+  CK(cudaMemcpyAsync(c->h_cell, cell_h, sizeof(int32_t) * (size_t)n, cudaMemcpyHostToDevice, s));
+  for (int a = 0; a < 3; ++a) CK(cudaMemcpyAsync(c->h_v[a], src[a], sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, s));
+  rc = dsmc_bin(c, n, K, c->h_cell, c->h_v[0], c->h_v[1], c->h_v[2], c->h_vs[0], c->h_vs[1], c->h_vs[2], c->h_perm,
+                c->h_cell_start);
+  if (rc != DSMC_OK) return rc;
+  if (vhs)
+    rc = dsmc_collide_vhs_nn(c, n, K, c->h_cell_start, c->h_vs[0], c->h_vs[1], c->h_vs[2], nullptr, vhs, seed, step,
+                             nullptr);
+  else
+    rc = dsmc_collide_abinitio(c, n, K, c->h_cell_start, c->h_vs[0], c->h_vs[1], c->h_vs[2], nullptr, abi, seed,
+                               step, nullptr);
+  if (rc != DSMC_OK) return rc;
+  for (int a = 0; a < 3; ++a) CK(cudaMemcpyAsync(dst[a], c->h_vs[a], sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, s));
+  if (perm_h) CK(cudaMemcpyAsync(perm_h, c->h_perm, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost, s));
+  if (cell_start_h)
+    CK(cudaMemcpyAsync(cell_start_h, c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1), cudaMemcpyDeviceToHost, s));
+  return dsmc_sync_status(c);
+}
+
+}  // extern "C"

@@ -1,0 +1,110 @@
+// Internal declarations shared by the translation units of libdsmc_b200.so (product code only;
+// nothing here is seen by, or shared with, oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dsmc.h"
+
+namespace dsmc {
+
+constexpr int kChunk = 1024;                          // chunk granularity (particles)
+constexpr int kMaxCell = DSMC_MAX_CELL_PARTICLES;     // largest resident cell
+constexpr int kNlocMax = kChunk + kMaxCell;           // most particles one CTA can own
+constexpr int kActMax = kChunk / 2 + 2;               // most cells with N>=2 in one chunk
+constexpr int kThreads = 256;
+constexpr float kBoltzmann = 1.380649e-23f;
+
+// MLP staged on the device: Wt[l] is W[l] transposed, [in][out] row-major (fp32).
+struct MlpDev {
+  int n_layers;
+  int dims[8];
+  int act;
+  int dmax;
+  const float *Wt[7];
+  const float *b[7];
+};
+
+// BF16 tensor-core image of a 3-layer MLP (in<=16 -> H -> H -> out<=16), see dsmc_collide_tc.cu
+struct MlpTcDev {
+  int H;                      // 64 or 128, 0 = not available
+  int d_in, d_out, act;
+  const void *w_blob;         // bf16 weights already in UMMA K-major core-matrix layout
+  const float *b1, *b2, *b3;  // fp32 biases (b3 padded to 16)
+  uint32_t blob_bytes;
+};
+
+struct ChiTableDev {
+  const float *chi;
+  int nE, nB;
+  float lnE_min, inv_dlnE;  // inv_dlnE = (nE-1)/(lnE_max-lnE_min)
+};
+
+struct StepParams {
+  // common
+  int64_t n;
+  int32_t n_cells;
+  const int32_t *cell_start;
+  float *vx, *vy, *vz;
+  const float *cap;  // sigma_cr_max / cr_max or nullptr
+  uint32_t seed_lo, seed_hi, step;
+  uint32_t flags;
+  int32_t pairs_per_cell;
+  int32_t op;  // 0 = VHS-NN, 1 = ab initio table, 2 = ab initio MLP
+  float mass;
+  // VHS-NN
+  float inv_sigma_v, sigma_v, inv_T_scale, noise_sigma, shell_eps;
+  float vhs_c, vhs_e;  // sigma_T(g) g = vhs_c * g^vhs_e
+  // ab initio
+  float lnE_min, inv_lnE_range;
+  float e_coef;  // m / (4 kB)
+  ChiTableDev table;
+  dsmc_pair_dump dump;
+  int32_t *status;
+};
+
+}  // namespace dsmc
+
+struct dsmc_ctx {
+  int device;
+  cudaStream_t stream;
+  int64_t max_particles;
+  int32_t max_cells;
+  int32_t *d_status;
+  int32_t *d_cursor;  // [max_cells + 1] scatter cursors / counts
+  int64_t launches;
+  int num_sms;
+  // operators
+  bool has_mlp[2];
+  dsmc::MlpDev mlp[2];
+  dsmc::MlpTcDev mlp_tc[2];
+  float *d_weights[2];
+  void *d_tc_blob[2];
+  bool has_table;
+  dsmc::ChiTableDev table;
+  float *d_table;
+  // dsmc_step_host staging
+  int32_t *h_cell;
+  float *h_v[3], *h_vs[3];
+  int32_t *h_perm, *h_cell_start;
+  int64_t host_cap_n;
+  int32_t host_cap_cells;
+};
+
+namespace dsmc {
+// launchers (each returns a DSMC_* status and bumps ctx->launches)
+int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const float *vx, const float *vy,
+               const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm, int32_t *cell_start);
+int launch_cell_moments(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, const float *vx, const float *vy,
+                        const float *vz, double *moments);
+int launch_moment_match(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, float *vx, float *vy, float *vz,
+                        const double *target, uint32_t flags);
+int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
+int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
+int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
+                     float lnE_min, float lnE_max, const MlpDev *net);
+int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
+                        float lnE_min, float lnE_max, const MlpTcDev *net);
+// host-side packing of the tensor-core weight image (dsmc_collide_tc.cu)
+int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStream_t s);
+}  // namespace dsmc

@@ -1,0 +1,279 @@
+"""Thin Python binding of libdsmc_b200.so (include/dsmc.h): argument marshalling only.
+
+Same names as the C ABI.  PyTorch is used for device memory and streams; every step of the
+path runs in the library's sm_100a kernels.  There is no CPU fallback: importing this module
+raises if the shared library is missing, and every call raises ``DsmcError`` on a non-zero status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_DIR, "libdsmc_b200.so")
+
+OK = 0
+ERR_INVALID_ARG, ERR_BAD_CELL_INDEX, ERR_CELL_TOO_LARGE = -1, -2, -3
+ERR_NOT_CONFIGURED, ERR_CUDA, ERR_UNSUPPORTED_SHAPE = -4, -5, -6
+MAX_CELL_PARTICLES = 2048
+
+F_NOISE, F_ENERGY_SHELL, F_MOMENT_MATCH, F_ACCEPT, F_BF16_TC, F_MATCH_ENERGY_ONLY = 1, 2, 4, 8, 16, 32
+ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
+
+EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",
+           "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
+           "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
+           "dsmc_step_host"]
+
+
+class DsmcError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__("%s failed: %d (%s)" % (where, status, strerror(status)))
+
+
+class _MlpDesc(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("dims", C.c_int32 * 8), ("act", C.c_int32),
+                ("W", C.POINTER(C.POINTER(C.c_float))), ("b", C.POINTER(C.POINTER(C.c_float)))]
+
+
+class _VhsParams(C.Structure):
+    _fields_ = [("mass", C.c_float), ("sigma_v", C.c_float), ("T_scale", C.c_float),
+                ("noise_sigma", C.c_float), ("shell_eps", C.c_float), ("d_ref", C.c_float),
+                ("omega", C.c_float), ("T_ref", C.c_float), ("pairs_per_cell", C.c_int32),
+                ("flags", C.c_uint32)]
+
+
+class _AbiParams(C.Structure):
+    _fields_ = [("mass", C.c_float), ("b_max", C.c_float), ("lnE_min", C.c_float), ("lnE_max", C.c_float),
+                ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32), ("flags", C.c_uint32)]
+
+
+class _PairDump(C.Structure):
+    _fields_ = [("pair_i", C.c_void_p), ("pair_j", C.c_void_p), ("accepted", C.c_void_p),
+                ("gprime", C.c_void_p), ("aux", C.c_void_p)]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "libdsmc_b200.so is missing (%s). Build it with `python -m paper_2602_21244_b200.build`; "
+            "there is no CPU fallback." % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    lib.dsmc_strerror.restype = C.c_char_p
+    lib.dsmc_launch_count.restype = C.c_int64
+    lib.dsmc_launch_count.argtypes = [C.c_void_p]
+    return lib
+
+
+_lib = _load()
+
+
+def strerror(status: int) -> str:
+    return _lib.dsmc_strerror(C.c_int(status)).decode()
+
+
+def _chk(rc, where):
+    if rc != 0:
+        raise DsmcError(rc, where)
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_cuda and t.is_contiguous(), "device, contiguous tensors only"
+    if dtype is not None:
+        assert t.dtype == dtype, (t.dtype, dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+@dataclass
+class VhsParams:
+    mass: float = 6.63e-26
+    sigma_v: float = 337.2
+    T_scale: float = 273.0
+    noise_sigma: float = 0.1
+    shell_eps: float = 1e-20
+    d_ref: float = 4.17e-10
+    omega: float = 0.81
+    T_ref: float = 273.0
+    pairs_per_cell: int = -1
+    flags: int = F_NOISE | F_ENERGY_SHELL | F_MOMENT_MATCH
+
+    def c(self):
+        return _VhsParams(self.mass, self.sigma_v, self.T_scale, self.noise_sigma, self.shell_eps, self.d_ref,
+                          self.omega, self.T_ref, self.pairs_per_cell, self.flags)
+
+
+@dataclass
+class AbinitioParams:
+    mass: float = 6.63e-26
+    b_max: float = 1e-9
+    lnE_min: float = float(np.log(5.0))
+    lnE_max: float = float(np.log(6.0e4))
+    chi_mode: int = 0
+    pairs_per_cell: int = -1
+    flags: int = F_MOMENT_MATCH
+
+    def c(self):
+        return _AbiParams(self.mass, self.b_max, self.lnE_min, self.lnE_max, self.chi_mode, self.pairs_per_cell,
+                          self.flags)
+
+
+class PairDump:
+    """Optional debug outputs of a fused step (device tensors with n entries)."""
+
+    def __init__(self, n, device, gprime=True):
+        self.pair_i = torch.full((n,), -1, dtype=torch.int32, device=device)
+        self.pair_j = torch.full((n,), -1, dtype=torch.int32, device=device)
+        self.accepted = torch.zeros(n, dtype=torch.uint8, device=device)
+        self.gprime = torch.zeros((n, 3), dtype=torch.float32, device=device) if gprime else None
+        self.aux = torch.zeros(n, dtype=torch.float32, device=device)
+
+    def c(self):
+        return _PairDump(_ptr(self.pair_i), _ptr(self.pair_j), _ptr(self.accepted), _ptr(self.gprime),
+                         _ptr(self.aux))
+
+
+class Context:
+    """dsmc_ctx wrapper.  Work is enqueued on torch's current stream at call time."""
+
+    def __init__(self, max_particles: int, max_cells: int, device: int = 0):
+        self._h = C.c_void_p()
+        self.device = torch.device("cuda", device)
+        _chk(_lib.dsmc_create(C.byref(self._h), C.c_int(device), C.c_int64(max_particles), C.c_int32(max_cells)),
+             "dsmc_create")
+
+    def close(self):
+        if self._h:
+            _lib.dsmc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _stream(self):
+        _chk(_lib.dsmc_set_stream(self._h, C.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)),
+             "dsmc_set_stream")
+
+    def sync_status(self) -> int:
+        return _lib.dsmc_sync_status(self._h)
+
+    def check(self):
+        _chk(self.sync_status(), "dsmc_sync_status")
+
+    def launch_count(self) -> int:
+        return int(_lib.dsmc_launch_count(self._h))
+
+    # ---- operators
+    def set_mlp(self, slot: int, weights, biases, act: int):
+        L = len(weights)
+        Ws = [np.ascontiguousarray(w, np.float32) for w in weights]
+        bs = [np.ascontiguousarray(b, np.float32) for b in biases]
+        d = _MlpDesc()
+        d.n_layers = L
+        d.act = act
+        d.dims[0] = Ws[0].shape[1]
+        for l in range(L):
+            d.dims[l + 1] = Ws[l].shape[0]
+        Wp = (C.POINTER(C.c_float) * L)(*[w.ctypes.data_as(C.POINTER(C.c_float)) for w in Ws])
+        bp = (C.POINTER(C.c_float) * L)(*[b.ctypes.data_as(C.POINTER(C.c_float)) for b in bs])
+        d.W, d.b = Wp, bp
+        self._stream()
+        _chk(_lib.dsmc_set_mlp(self._h, C.c_int(slot), C.byref(d)), "dsmc_set_mlp")
+
+    def set_chi_table(self, chi: np.ndarray, lnE_min: float, lnE_max: float):
+        chi = np.ascontiguousarray(chi, np.float32)
+        self._stream()
+        _chk(_lib.dsmc_set_chi_table(self._h, chi.ctypes.data_as(C.POINTER(C.c_float)), C.c_int32(chi.shape[0]),
+                                     C.c_int32(chi.shape[1]), C.c_float(lnE_min), C.c_float(lnE_max)),
+             "dsmc_set_chi_table")
+
+    # ---- a1
+    def bin(self, cell, vx, vy, vz, n_cells: int, out=None):
+        n = cell.shape[0]
+        dev = cell.device
+        if out is None:
+            out = (torch.empty(n, dtype=torch.float32, device=dev), torch.empty(n, dtype=torch.float32, device=dev),
+                   torch.empty(n, dtype=torch.float32, device=dev), torch.empty(n, dtype=torch.int32, device=dev),
+                   torch.empty(n_cells + 1, dtype=torch.int32, device=dev))
+        vx_s, vy_s, vz_s, perm, cell_start = out
+        self._stream()
+        _chk(_lib.dsmc_bin(self._h, C.c_int64(n), C.c_int32(n_cells), _ptr(cell, torch.int32),
+                           _ptr(vx, torch.float32), _ptr(vy, torch.float32), _ptr(vz, torch.float32),
+                           _ptr(vx_s), _ptr(vy_s), _ptr(vz_s), _ptr(perm), _ptr(cell_start)), "dsmc_bin")
+        return vx_s, vy_s, vz_s, perm, cell_start
+
+    # ---- fused steps (in place on vx_s, vy_s, vz_s)
+    def collide_vhs_nn(self, cell_start, vx_s, vy_s, vz_s, prm: VhsParams, seed: int, step: int,
+                       sigma_cr_max=None, dump: PairDump = None):
+        p = prm.c()
+        d = dump.c() if dump is not None else None
+        self._stream()
+        _chk(_lib.dsmc_collide_vhs_nn(
+            self._h, C.c_int64(vx_s.shape[0]), C.c_int32(cell_start.shape[0] - 1), _ptr(cell_start, torch.int32),
+            _ptr(vx_s, torch.float32), _ptr(vy_s, torch.float32), _ptr(vz_s, torch.float32),
+            _ptr(sigma_cr_max, torch.float32) if sigma_cr_max is not None else C.c_void_p(0), C.byref(p),
+            C.c_uint64(seed), C.c_uint32(step), C.byref(d) if d is not None else None), "dsmc_collide_vhs_nn")
+
+    def collide_abinitio(self, cell_start, vx_s, vy_s, vz_s, prm: AbinitioParams, seed: int, step: int,
+                         cr_max=None, dump: PairDump = None):
+        p = prm.c()
+        d = dump.c() if dump is not None else None
+        self._stream()
+        _chk(_lib.dsmc_collide_abinitio(
+            self._h, C.c_int64(vx_s.shape[0]), C.c_int32(cell_start.shape[0] - 1), _ptr(cell_start, torch.int32),
+            _ptr(vx_s, torch.float32), _ptr(vy_s, torch.float32), _ptr(vz_s, torch.float32),
+            _ptr(cr_max, torch.float32) if cr_max is not None else C.c_void_p(0), C.byref(p),
+            C.c_uint64(seed), C.c_uint32(step), C.byref(d) if d is not None else None), "dsmc_collide_abinitio")
+
+    # ---- moments
+    def cell_moments(self, cell_start, vx_s, vy_s, vz_s, out=None):
+        K = cell_start.shape[0] - 1
+        if out is None:
+            out = torch.empty((K, 4), dtype=torch.float64, device=cell_start.device)
+        self._stream()
+        _chk(_lib.dsmc_cell_moments(self._h, C.c_int64(vx_s.shape[0]), C.c_int32(K), _ptr(cell_start, torch.int32),
+                                    _ptr(vx_s, torch.float32), _ptr(vy_s, torch.float32), _ptr(vz_s, torch.float32),
+                                    _ptr(out, torch.float64)), "dsmc_cell_moments")
+        return out
+
+    def moment_match(self, cell_start, vx_s, vy_s, vz_s, target, flags: int = F_MOMENT_MATCH):
+        self._stream()
+        _chk(_lib.dsmc_moment_match(self._h, C.c_int64(vx_s.shape[0]), C.c_int32(cell_start.shape[0] - 1),
+                                    _ptr(cell_start, torch.int32), _ptr(vx_s, torch.float32),
+                                    _ptr(vy_s, torch.float32), _ptr(vz_s, torch.float32),
+                                    _ptr(target, torch.float64), C.c_uint32(flags)), "dsmc_moment_match")
+
+    # ---- a10
+    def chi_batch(self, E_over_k, b, chi_mode: int, b_max: float, lnE_min=float(np.log(5.0)),
+                  lnE_max=float(np.log(6.0e4)), flags: int = 0, out=None):
+        if out is None:
+            out = torch.empty_like(E_over_k)
+        self._stream()
+        _chk(_lib.dsmc_chi_batch(self._h, C.c_int64(E_over_k.shape[0]), _ptr(E_over_k, torch.float32),
+                                 _ptr(b, torch.float32), _ptr(out, torch.float32), C.c_int32(chi_mode),
+                                 C.c_float(b_max), C.c_float(lnE_min), C.c_float(lnE_max), C.c_uint32(flags)),
+             "dsmc_chi_batch")
+        return out
+
+    # ---- end to end on host buffers (pinned CPU tensors)
+    def step_host(self, cell_h, vx_h, vy_h, vz_h, n_cells, out_h, vhs: VhsParams = None,
+                  abi: AbinitioParams = None, seed=0, step=0):
+        """out_h = (vx_out, vy_out, vz_out, perm, cell_start) CPU tensors.  Synchronous."""
+        pv = vhs.c() if vhs is not None else None
+        pa = abi.c() if abi is not None else None
+        hp = lambda t: C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+        self._stream()
+        _chk(_lib.dsmc_step_host(
+            self._h, C.c_int64(cell_h.shape[0]), C.c_int32(n_cells), hp(cell_h), hp(vx_h), hp(vy_h), hp(vz_h),
+            hp(out_h[0]), hp(out_h[1]), hp(out_h[2]), hp(out_h[3]), hp(out_h[4]),
+            C.byref(pv) if pv is not None else None, C.byref(pa) if pa is not None else None,
+            C.c_uint64(seed), C.c_uint32(step)), "dsmc_step_host")
