@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- collision pairs/s of the neural DSMC collision step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--chi table|mlp|mlp_tc] [--impl reference]
+
+A "step" is one pass of the whole hot path: dsmc_bin (a1) on the
+unsorted resident particle arrays, then the fused ab initio collision step (a2-a9) on the
+cell-sorted arrays, on the Mach-10 cylinder-shaped population of BASELINE.json (cfg 5:
+400x200 cells, 2e7 particles, pairs = floor(N_k/2) per cell).  Inputs are synthetic and seeded
+(paper_2602_21244_b200/workloads.py).  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "collision_pairs_per_s"
+UNIT = "pairs/s"
+NX, NY, N_TOTAL = 400, 200, 20_000_000
+TABLE_N = 1024
+B_MAX = 1e-9
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--chi", default="table", choices=["table", "mlp", "mlp_tc"])
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the population (debug only; marks the line)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-variants", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d["hbm_gbs"], d["bf16_tflops"], d.get("bf16_tflops_sustained", d["bf16_tflops"]), "measured"
+    return 6650.0, 1590.0, 1400.0, "fallback"
+
+
+def population(args, rank=0):
+    from paper_2602_21244_b200 import workloads as wl
+    s = args.scale
+    nx, ny = max(8, int(round(NX * s ** 0.5))), max(4, int(round(NY * s ** 0.5)))
+    return wl.mach10_cylinder(seed=4 + 1000 * rank, nx=nx, ny=ny, n_total=int(N_TOTAL * s))
+
+
+def config_dict(args, pop, pairs):
+    return {"workload": "cfg5 Mach-10 cylinder population %dx%d cells, %d particles, %d pairs/step, ab initio chi "
+                        "by %s + rotation + moment matching; step = dsmc_bin + fused collide" % (
+                            NX if args.scale == 1.0 else -1, NY if args.scale == 1.0 else -1, pop.n, pairs, args.chi),
+            "chi_mode": args.chi, "n_particles": pop.n, "n_cells": pop.n_cells, "pairs_per_step": pairs,
+            "table": "%dx%d fp32 LJ 12-6 (oracle quadrature)" % (TABLE_N, TABLE_N),
+            "l2_policy": "inputs larger than L2 (%.0f MB touched per step)" % (pop.n * 48 / 1e6),
+            "scale": args.scale}
+
+
+# ----------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on a bounded sample of the same workload
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(pop, chi, target_pairs=150_000):
+    """Contiguous cell range holding about target_pairs pairs, starting at the first shock-band cell
+    row so the sample mixes freestream, shock and wake cells like the whole population."""
+    counts = pop.counts
+    half = counts // 2
+    cum = np.cumsum(half)
+    k0 = int(pop.n_cells * 0.30)
+    base = cum[k0 - 1] if k0 > 0 else 0
+    k1 = int(np.searchsorted(cum, base + target_pairs))
+    k1 = min(max(k1, k0 + 1), pop.n_cells)
+    keep = (pop.cell >= k0) & (pop.cell < k1)
+    return k0, k1, keep
+
+
+def time_oracle(pop, chi, table, mlp_w, steps, warmup, target_pairs=150_000):
+    import oracle
+    k0, k1, keep = oracle_sample(pop, chi, target_pairs)
+    cell = (pop.cell[keep] - k0).astype(np.int32)
+    vx, vy, vz = pop.vx[keep], pop.vy[keep], pop.vz[keep]
+    K = k1 - k0
+    pairs = int((pop.counts[k0:k1] // 2).sum())
+    otab = oracle.ChiTable(table.chi, table.lnE_min, table.lnE_max)
+    net = oracle.Mlp(mlp_w[0], mlp_w[1], oracle.ACT_SILU)
+    prm = oracle.AbinitioParams(chi_mode=0 if chi == "table" else 1)
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        rc, perm, cs = oracle.bin_particles(cell, K)
+        v = [a[perm].astype(np.float64) for a in (vx, vy, vz)]
+        oracle.collide_abinitio(cs, *v, prm, 4, it, net=net, table=otab)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    return pairs / t, t, pairs, "cells [%d,%d) of the cfg5 population: %d particles, %d pairs, bin + fused ab initio " \
+                               "(%s) step, fp64 single thread" % (k0, k1, int(keep.sum()), pairs, chi)
+
+
+def build_operators(chi_needed=True):
+    """chi table by the oracle's quadrature (allowed: it is an INPUT, built once, outside timing)
+    and the random-init chi-MLP 2->128->128->1 (seed 3)."""
+    import oracle
+    from paper_2602_21244_b200 import workloads as wl
+    t0 = time.perf_counter()
+    table = oracle.build_chi_table(oracle.lj_argon(), TABLE_N, TABLE_N, b_max=B_MAX, n_panels=1)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    return table, (Ws, bs), time.perf_counter() - t0
+
+
+class ClockSampler(threading.Thread):
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    pop = population(args)
+    table, mlp_w, _ = build_operators()
+    chi = "table" if args.chi == "table" else "mlp"
+    v, t, pairs, sample = time_oracle(pop, chi, table, mlp_w, args.steps, args.warmup,
+                                      target_pairs=2_000_000 if chi == "table" else 150_000)
+    total_pairs = pop.pairs_per_step(-1)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(args, pop, total_pairs),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2602_21244_b200 import dsmc
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_peak, tc_burst, tc_sust, peak_src = peaks()
+
+    pop = population(args, rank)       # weak scaling: every rank owns one full cfg-5 population
+    table, mlp_w, t_table = build_operators()
+    pairs = pop.pairs_per_step(-1)
+    ctx = dsmc.Context(pop.n, pop.n_cells, device=local)
+    ctx.set_chi_table(table.chi, table.lnE_min, table.lnE_max)
+    ctx.set_mlp(1, mlp_w[0], mlp_w[1], dsmc.ACT_SILU)
+    dev = torch.device("cuda", local)
+    cell = torch.from_numpy(pop.cell).to(dev)
+    vin = [torch.from_numpy(a).to(dev) for a in (pop.vx, pop.vy, pop.vz)]
+    out = (torch.empty(pop.n, dtype=torch.float32, device=dev), torch.empty(pop.n, dtype=torch.float32, device=dev),
+           torch.empty(pop.n, dtype=torch.float32, device=dev), torch.empty(pop.n, dtype=torch.int32, device=dev),
+           torch.empty(pop.n_cells + 1, dtype=torch.int32, device=dev))
+
+    def params(chi):
+        flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi == "mlp_tc" else 0)
+        return dsmc.AbinitioParams(chi_mode=0 if chi == "table" else 1, flags=flags, b_max=B_MAX)
+
+    def one_step(chi, t, ev=None):
+        ctx.bin(cell, *vin, pop.n_cells, out=out)
+        if ev is not None:
+            ev[0].record()
+        ctx.collide_abinitio(out[4], out[0], out[1], out[2], params(chi), seed=4, step=t)
+        if ev is not None:
+            ev[1].record()
+
+    def timed(chi, steps, warmup, sampler=None):
+        for t in range(warmup):
+            one_step(chi, t)
+        ctx.check()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        l0 = ctx.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for t in range(steps):
+            one_step(chi, warmup + t, evs[t])
+        e1.record()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        ms = e0.elapsed_time(e1)
+        coll_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        if world > 1:
+            tt = torch.tensor([ms], device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ms = tt.item()
+        return ms / steps, coll_ms, ctx.launch_count() - l0
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_step, coll_ms, launches = timed(args.chi, args.steps, args.warmup)
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    st = ctx.sync_status()
+    if st != 0:
+        raise SystemExit("device status %d (%s)" % (st, dsmc.strerror(st)))
+
+    # end to end through the C-ABI host entry point: pinned host buffers, H2D + D2H inside the timing
+    hcell = torch.from_numpy(pop.cell).pin_memory()
+    hv = [torch.from_numpy(a).pin_memory() for a in (pop.vx, pop.vy, pop.vz)]
+    hout = [torch.empty(pop.n, dtype=torch.float32).pin_memory() for _ in range(3)] + \
+           [torch.empty(pop.n, dtype=torch.int32).pin_memory(), torch.empty(pop.n_cells + 1, dtype=torch.int32).pin_memory()]
+    e2e_steps = max(3, min(args.steps, 10))
+    for t in range(2):
+        ctx.step_host(hcell, *hv, pop.n_cells, hout, abi=params(args.chi), seed=4, step=t)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for t in range(e2e_steps):
+        ctx.step_host(hcell, *hv, pop.n_cells, hout, abi=params(args.chi), seed=4, step=10 + t)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        tt = torch.tensor([e2e_s], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = tt.item()
+    h2d = pop.n * 16
+    d2h = pop.n * 16 + (pop.n_cells + 1) * 4
+
+    variants = {}
+    if not args.no_variants and rank == 0 or (not args.no_variants and world > 1):
+        for chi in ("table", "mlp", "mlp_tc"):
+            if chi == args.chi:
+                variants[chi] = {"pairs_per_s": pairs / (ms_step * 1e-3), "collide_ms": coll_ms, "step_ms": ms_step}
+                continue
+            try:
+                m, c, _ = timed(chi, max(3, args.steps // 4), 2)
+                variants[chi] = {"pairs_per_s": pairs / (m * 1e-3), "collide_ms": c, "step_ms": m}
+            except dsmc.DsmcError as e:
+                variants[chi] = {"unavailable": str(e)}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (the fused collide kernel), north_star definition:
+    # the slower of the MLP FLOPs at tensor peak and the gathered + written bytes at HBM bandwidth
+    bytes_alg = pop.n * 24 + (pop.n_cells + 1) * 4
+    flops_alg = pairs * 2 * (2 * 128 + 128 * 128 + 128) if args.chi != "table" else 0
+    t_hbm = bytes_alg / (hbm_peak * 1e9)
+    t_tc = flops_alg / (tc_sust * 1e12)
+    if t_tc > t_hbm:
+        roof = {"bound": "tensor", "achieved": flops_alg / (coll_ms * 1e-3) / 1e12, "peak": tc_sust, "unit": "TFLOP/s"}
+    else:
+        roof = {"bound": "hbm", "achieved": bytes_alg / (coll_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["kernel"] = "fused collide (k_collide_*)"
+    roof["kernel_ms"] = coll_ms
+    roof["peak_source"] = peak_src
+    roof["algorithmic"] = {"bytes_per_launch": bytes_alg, "flops_per_launch": flops_alg}
+    bin_ms = ms_step - coll_ms
+    roof["bin"] = {"ms": bin_ms, "achieved_gbs": pop.n * 36 / (bin_ms * 1e-3) / 1e9, "frac": pop.n * 36 / (bin_ms * 1e-3) / 1e9 / hbm_peak}
+
+    line = {"metric": METRIC, "value": world * pairs / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if args.chi != "mlp_tc" else "bf16", "data": "synthetic",
+            "config": config_dict(args, pop, pairs), "clocks": sampler.summary(),
+            "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_s * 1e3, "api": "dsmc_step_host (pinned host buffers)"},
+            "gpu_launches": int(launches), "roofline": roof, "variants": variants,
+            "table_build_s": t_table}
+    if not args.no_cpu_baseline and world >= 1:
+        chi = "table" if args.chi == "table" else "mlp"
+        v, t, sp, sample = time_oracle(pop, chi, table, mlp_w, steps=3, warmup=1,
+                                       target_pairs=4_000_000 if chi == "table" else 300_000)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -76,7 +76,7 @@ def test_bin_reports_bad_cell_index_and_large_cells(dsmc):
     cell[3] = -1
     ctx.bin(dev(cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), 4)
     assert ctx.sync_status() == dsmc.ERR_BAD_CELL_INDEX
-    big = wl._populate("big", np.array([3000, 5]), np.full(2, 300.0), np.zeros(2), np.zeros(2), 1)
+    big = wl._populate("big", np.array([5000, 5]), np.full(2, 300.0), np.zeros(2), np.zeros(2), 1)
     ctx2 = dsmc.Context(big.n, 2)
     ctx2.bin(dev(big.cell), dev(big.vx), dev(big.vy), dev(big.vz), 2)
     assert ctx2.sync_status() == dsmc.ERR_CELL_TOO_LARGE
