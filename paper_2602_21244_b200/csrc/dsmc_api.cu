@@ -34,6 +34,9 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
   CK(cudaMalloc(&c->d_status, sizeof(int32_t)));
   CK(cudaMemset(c->d_status, 0, sizeof(int32_t)));
   CK(cudaMalloc(&c->d_cursor, sizeof(int32_t) * (size_t)(max_cells + 2)));
+  const size_t n_chunks = (size_t)(max_particles / kChunk + 2);
+  CK(cudaMalloc(&c->d_chunk_first, sizeof(int32_t) * n_chunks));
+  CK(cudaMalloc(&c->d_big, sizeof(int32_t) * (n_chunks + 1)));
   *out = c;
   return DSMC_OK;
 }
@@ -44,6 +47,8 @@ int dsmc_destroy(dsmc_ctx *c) {
   cudaStreamSynchronize(c->stream);
   cudaFree(c->d_status);
   cudaFree(c->d_cursor);
+  cudaFree(c->d_chunk_first);
+  cudaFree(c->d_big);
   for (int s = 0; s < 2; ++s) {
     cudaFree(c->d_weights[s]);
     cudaFree(c->d_tc_blob[s]);
@@ -143,20 +148,34 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
   CK(cudaStreamSynchronize(c->stream));
   cudaFree(c->d_table);
   c->d_table = nullptr;
-  CK(cudaMalloc(&c->d_table, sizeof(float) * (size_t)nE * nB));
-  CK(cudaMemcpy(c->d_table, chi_host, sizeof(float) * (size_t)nE * nB, cudaMemcpyHostToDevice));
-  c->table.chi = c->d_table;
+  // device layout: the 2x2 nodes of every grid cell side by side, so a lookup is one 16-byte load
+  const size_t nq = (size_t)(nE - 1) * (nB - 1);
+  std::vector<float> quad(4 * nq);
+  for (int iE = 0; iE + 1 < nE; ++iE)
+    for (int iB = 0; iB + 1 < nB; ++iB) {
+      float *q = &quad[4 * ((size_t)iE * (nB - 1) + iB)];
+      q[0] = chi_host[(size_t)iE * nB + iB];
+      q[1] = chi_host[(size_t)iE * nB + iB + 1];
+      q[2] = chi_host[(size_t)(iE + 1) * nB + iB];
+      q[3] = chi_host[(size_t)(iE + 1) * nB + iB + 1];
+    }
+  CK(cudaMalloc(&c->d_table, sizeof(float) * quad.size()));
+  CK(cudaMemcpy(c->d_table, quad.data(), sizeof(float) * quad.size(), cudaMemcpyHostToDevice));
+  c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
   c->table.nE = nE;
   c->table.nB = nB;
   c->table.lnE_min = lnE_min;
-  c->table.inv_dlnE = (float)((double)(nE - 1) / ((double)lnE_max - (double)lnE_min));
+  const double inv = (double)(nE - 1) / ((double)lnE_max - (double)lnE_min);
+  c->table.inv_dlnE = (float)inv;
+  c->table.c1 = (float)(0.6931471805599453 * inv);
+  c->table.c0 = (float)(-(double)lnE_min * inv);
   c->has_table = true;
   return DSMC_OK;
 }
 
 static int check_sorted_args(dsmc_ctx *c, int64_t n, int32_t K, const void *cs, const void *x, const void *y,
                              const void *z) {
-  if (!c || n < 0 || K < 0 || n >= (int64_t(1) << 31)) return DSMC_ERR_INVALID_ARG;
+  if (!c || n < 0 || K < 0 || n >= (int64_t(1) << 31) || n > c->max_particles) return DSMC_ERR_INVALID_ARG;
   if (n == 0 || K == 0) return 1;  // nothing to do
   if (!cs || !x || !y || !z) return DSMC_ERR_INVALID_ARG;
   return DSMC_OK;
@@ -199,6 +218,7 @@ static void fill_common(StepParams &p, dsmc_ctx *c, int64_t n, int32_t K, const 
   p.seed_hi = (uint32_t)(seed >> 32);
   p.step = step;
   if (dump) p.dump = *dump;
+  p.dump_any = (dump && (dump->pair_i || dump->pair_j || dump->accepted || dump->gprime || dump->aux)) ? 1 : 0;
   p.status = c->d_status;
 }
 
@@ -219,6 +239,7 @@ int dsmc_collide_vhs_nn(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
   p.sigma_v = prm->sigma_v;
   p.inv_sigma_v = 1.0f / prm->sigma_v;
   p.inv_T_scale = 1.0f / prm->T_scale;
+  p.T_coef = (float)((double)prm->mass / (3.0 * 1.380649e-23));
   p.noise_sigma = prm->noise_sigma;
   p.shell_eps = prm->shell_eps;
   if ((prm->flags & DSMC_F_ACCEPT) && sigma_cr_max) {

@@ -1,0 +1,443 @@
+// Chunk machinery shared by every variant of the fused collision kernel (product code only).
+//
+// A "chunk" is the run of whole cells whose first slot lies in [b*kChunk, (b+1)*kChunk) of the
+// cell-sorted arrays: one contiguous particle range, owned by one CTA, read from HBM once
+// (12 B / particle), processed entirely in shared memory and written once (12 B / particle).
+//
+//   begin     chunk -> cell range (precomputed map), cell discovery, one coalesced load
+//   pre       per 256-particle segment (one warp each): pivoted FP32 sums for eq. 10,
+//             Philox pairing keys (one block per 4 slots), bucket counts
+//   sort      exclusive scan of the bucket counts, placement, in-bucket ranking -> pi, the unique
+//             ascending order of (key << 32 | slot); pairs are (pi[2s], pi[2s+1])   (Q7)
+//   [pairs]   operator specific: table / FP32 MLP / tcgen05 MLP           (caller)
+//   finish    post-collision segment sums, moment matching folded into the store as one FMA per
+//             component: v <- alpha v + B, B = u_pre - alpha u_post (eqs. 10-11, Q5)
+//
+// Cell sums are accumulated in FP32 about a pivot near the cell mean (first particle before the
+// collisions, u_pre after them), 8 values per lane, and combined across lanes in FP32 and across
+// segments in FP64 in a fixed order, so results do not depend on scheduling.
+#pragma once
+#include "dsmc_device.cuh"
+#include "dsmc_internal.h"
+
+namespace dsmc {
+
+constexpr int kSeg = 256;  // particles per segment (multiple of 4: Philox blocks never straddle)
+constexpr int kWarps = kThreads / 32;
+
+struct __align__(16) CellInfo {
+  float ux, uy, uz, theta;  // pre-collision mean, sum |v-u|^2; finish_post overwrites: Bx,By,Bz,alpha
+  int32_t cell;             // global cell id
+  int32_t pair_off;         // first entry of this cell in pairs[]
+  uint16_t start, N, M, seg0;
+  int32_t collided;
+  int32_t pad[3];
+};
+static_assert(sizeof(CellInfo) == 48, "CellInfo layout");
+
+enum { MI_NACT = 0, MI_NSEG = 1, MI_NPAIRS = 2, MI_SCAN = 8 /* .. +40 */ };
+
+template <int LMAX_, int AMAX_>
+struct Chunk {
+  static constexpr int LMAX = LMAX_, AMAX = AMAX_;
+  static constexpr int SMAX = LMAX / kSeg + AMAX + 2;
+  float4 *v;        // [LMAX] velocities (x, y, z, unused)
+  float4 *part;     // [SMAX] segment partial sums
+  CellInfo *cells;  // [AMAX]
+  uint32_t *key;    // [LMAX]
+  int *cnt;         // [LMAX + 4]
+  uint32_t *pairs;  // [LMAX / 2] position of the pair's first member | active cell << 16
+  uint32_t *segs;   // [SMAX] active cell | piece << 16
+  int *misc;        // [64]
+  uint16_t *ord, *pi, *lc;  // [LMAX]
+
+  static constexpr size_t bytes() {
+    return sizeof(float4) * LMAX + sizeof(float4) * SMAX + sizeof(CellInfo) * AMAX + 4 * LMAX + 4 * (LMAX + 4) +
+           4 * (LMAX / 2) + 4 * SMAX + 4 * 64 + 2 * 3 * LMAX + 16;
+  }
+  __device__ __forceinline__ unsigned char *carve(unsigned char *base) {
+    v = reinterpret_cast<float4 *>(base);
+    part = v + LMAX;
+    cells = reinterpret_cast<CellInfo *>(part + SMAX);
+    key = reinterpret_cast<uint32_t *>(cells + AMAX);
+    cnt = reinterpret_cast<int *>(key + LMAX);
+    pairs = reinterpret_cast<uint32_t *>(cnt + LMAX + 4);
+    segs = pairs + LMAX / 2;
+    misc = reinterpret_cast<int *>(segs + SMAX);
+    ord = reinterpret_cast<uint16_t *>(misc + 64);
+    pi = ord + LMAX;
+    lc = pi + LMAX;
+    return reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(lc + LMAX) + 15) & ~(uintptr_t)15);
+  }
+};
+
+// Exclusive scan of a[0..L) in shared memory by the whole CTA; coalesced (conflict-free) sweeps.
+// `scratch` holds >= 2*kWarps ints.  Ends with __syncthreads().
+__device__ __forceinline__ void block_excl_scan_coalesced(int *a, int L, int *scratch) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int span = ((L + kWarps * 32 - 1) / (kWarps * 32)) * 32;  // per warp, multiple of 32
+  const int lo = min(warp * span, L), hi = min(lo + span, L);
+  int carry = 0;
+  for (int base = lo; base < hi; base += 32) {
+    const int i = base + lane;
+    const int x = i < hi ? a[i] : 0;
+    int inc = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (i < hi) a[i] = carry + inc - x;
+    carry += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  if (lane == 0) scratch[warp] = carry;
+  __syncthreads();
+  int off = 0;
+#pragma unroll
+  for (int w = 0; w < kWarps; ++w) off += (w < warp) ? scratch[w] : 0;
+  if (off != 0)
+    for (int i = lo + lane; i < hi; i += 32) a[i] += off;
+  __syncthreads();
+}
+
+__device__ __forceinline__ float warp_sum_f(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// begin: returns n_loc > 0 when there is work, 0 when the chunk has nothing to collide (nothing
+// to store either), -1 when the chunk does not fit this variant (caller defers it).
+// ---------------------------------------------------------------------------------------------
+template <class CK>
+__device__ int chunk_begin(const StepParams &P, CK &S, int chunk, int &q0_out) {
+  const int tid = threadIdx.x;
+  const int c_lo = __ldg(P.chunk_first + chunk);
+  const int c_hi = (chunk + 1 < P.n_chunks) ? __ldg(P.chunk_first + chunk + 1) : P.n_cells;
+  if (c_lo >= c_hi) return 0;
+  const int q0 = __ldg(P.cell_start + c_lo), q1 = __ldg(P.cell_start + c_hi);
+  const int n_loc = q1 - q0;
+  q0_out = q0;
+  if (n_loc <= 0) return 0;
+  if (n_loc > CK::LMAX) return -1;
+  for (int q = tid; q < n_loc; q += kThreads) S.cnt[q] = 0;
+  if (tid < 8) S.misc[tid] = 0;
+  __syncthreads();
+  // cell discovery (order of the active list is irrelevant to the results)
+  for (int c = c_lo + tid; c < c_hi; c += kThreads) {
+    const int gs = __ldg(P.cell_start + c), N = __ldg(P.cell_start + c + 1) - gs;
+    if (N == 1) S.cnt[gs - q0] = 1;  // lone particle: keeps bucket positions aligned with slots
+    if (N < 2) continue;
+    const int a = atomicAdd(&S.misc[MI_NACT], 1);
+    if (a >= CK::AMAX) continue;
+    int M = N >> 1;
+    if (P.pairs_per_cell >= 0 && P.pairs_per_cell < M) M = P.pairs_per_cell;
+    const int nseg = (N + kSeg - 1) / kSeg;
+    const int seg0 = atomicAdd(&S.misc[MI_NSEG], nseg);
+    CellInfo ci;
+    ci.ux = ci.uy = ci.uz = ci.theta = 0.f;
+    ci.cell = c;
+    ci.pair_off = atomicAdd(&S.misc[MI_NPAIRS], M);
+    ci.start = (uint16_t)(gs - q0);
+    ci.N = (uint16_t)N;
+    ci.M = (uint16_t)M;
+    ci.seg0 = (uint16_t)seg0;
+    ci.collided = (M > 0 && !(P.flags & DSMC_F_ACCEPT)) ? 1 : 0;
+    ci.pad[0] = ci.pad[1] = ci.pad[2] = 0;
+    S.cells[a] = ci;
+    for (int i = 0; i < nseg; ++i) S.segs[seg0 + i] = (uint32_t)a | ((uint32_t)i << 16);
+  }
+  // one coalesced read of the chunk
+  for (int q = tid; q < n_loc; q += kThreads) {
+    S.v[q] = make_float4(P.vx[q0 + q], P.vy[q0 + q], P.vz[q0 + q], 0.f);
+    S.lc[q] = 0xFFFFu;
+  }
+  __syncthreads();
+  if (S.misc[MI_NACT] > CK::AMAX) return -1;
+  if (S.misc[MI_NACT] == 0) return 0;
+  return n_loc;
+}
+
+// pre-collision segment sums + pairing keys + bucket counts; then cell finalisation + sort
+template <class CK>
+__device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
+  for (int sg = warp; sg < n_seg; sg += kWarps) {
+    const uint32_t e = S.segs[sg];
+    const int a = e & 0xFFFFu, piece = e >> 16;
+    const CellInfo &ci = S.cells[a];
+    const int start = ci.start, N = ci.N, M = ci.M, pair_off = ci.pair_off;
+    const uint32_t cell = (uint32_t)ci.cell;
+    const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
+    const float4 pv = S.v[start];
+    float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
+    for (int q = lo + lane; q < hi; q += 32) {
+      const float4 v = S.v[q];
+      const float dx = v.x - pv.x, dy = v.y - pv.y, dz = v.z - pv.z;
+      sx += dx; sy += dy; sz += dz;
+      s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
+      S.lc[q] = (uint16_t)a;
+    }
+    sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
+    if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
+    // pairing keys: Philox block blk serves slots 4 blk .. 4 blk + 3 of the cell (stream 0)
+    const int b_hi = min((piece + 1) * (kSeg / 4), (N + 3) >> 2);
+    for (int blk = piece * (kSeg / 4) + lane; blk < b_hi; blk += 32) {
+      const uint4 r = philox4x32_10((uint32_t)blk, cell, P.step, 0u, P.seed_lo, P.seed_hi);
+      const uint32_t k[4] = {r.x, r.y, r.z, r.w};
+      const int p = 4 * blk;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        if (p + w < N) {
+          S.key[start + p + w] = k[w];
+          atomicAdd(&S.cnt[start + (int)__umulhi(k[w], (uint32_t)N)], 1);
+        }
+      }
+      const int s = p >> 1;
+      if (s < M) S.pairs[pair_off + s] = (uint32_t)(start + p) | ((uint32_t)a << 16);
+      if (s + 1 < M) S.pairs[pair_off + s + 1] = (uint32_t)(start + p + 2) | ((uint32_t)a << 16);
+    }
+  }
+  __syncthreads();
+  // cell finalisation: u = pivot + mean(d), Theta = sum d^2 - N |mean(d)|^2   (eq. 10)
+  for (int a = tid; a < n_act; a += kThreads) {
+    CellInfo &ci = S.cells[a];
+    const int N = ci.N, nseg = (N + kSeg - 1) / kSeg;
+    double sx = 0, sy = 0, sz = 0, s2 = 0;
+    for (int i = 0; i < nseg; ++i) {
+      const float4 p = S.part[ci.seg0 + i];
+      sx += p.x; sy += p.y; sz += p.z; s2 += p.w;
+    }
+    const double inv = 1.0 / N;
+    const double dx = sx * inv, dy = sy * inv, dz = sz * inv;
+    const float4 pv = S.v[ci.start];
+    ci.ux = (float)((double)pv.x + dx);
+    ci.uy = (float)((double)pv.y + dy);
+    ci.uz = (float)((double)pv.z + dz);
+    ci.theta = (float)(s2 - N * (dx * dx + dy * dy + dz * dz));
+  }
+  block_excl_scan_coalesced(S.cnt, n_loc, S.misc + MI_SCAN);
+  // placement: cnt[bucket] ends as the bucket's end position
+  for (int q = tid; q < n_loc; q += kThreads) {
+    const int a = S.lc[q];
+    if (a == 0xFFFF) {
+      S.cnt[q] += 1;
+      continue;
+    }
+    const CellInfo &ci = S.cells[a];
+    const int bkt = ci.start + (int)__umulhi(S.key[q], (uint32_t)ci.N);
+    S.ord[atomicAdd(&S.cnt[bkt], 1)] = (uint16_t)q;
+  }
+  __syncthreads();
+  // in-bucket ranking by (key, slot): buckets hold ~1 particle on average
+  for (int q = tid; q < n_loc; q += kThreads) {
+    const int a = S.lc[q];
+    if (a == 0xFFFF) continue;
+    const CellInfo &ci = S.cells[a];
+    const uint32_t k = S.key[q];
+    const int bkt = ci.start + (int)__umulhi(k, (uint32_t)ci.N);
+    const int b0 = bkt > 0 ? S.cnt[bkt - 1] : 0, b1 = S.cnt[bkt];
+    int rank = 0;
+    for (int t = b0; t < b1; ++t) {
+      const int o = S.ord[t];
+      const uint32_t ko = S.key[o];
+      rank += (ko < k || (ko == k && o < q)) ? 1 : 0;
+    }
+    S.pi[b0 + rank] = (uint16_t)q;
+  }
+  __syncthreads();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-pair helpers
+// ---------------------------------------------------------------------------------------------
+struct PairCtx {
+  int a, s, i, j, start;  // active cell, pair slot, local particle indices, cell's first slot
+  uint32_t cell;
+  float4 vi, vj;
+  float gx, gy, gz, g2;
+  bool acc;
+  float U_b, U_eps;
+};
+
+template <class CK>
+__device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, int t, bool need_randoms) {
+  PairCtx c;
+  const uint32_t e = S.pairs[t];
+  const int pos = e & 0xFFFFu;
+  c.a = e >> 16;
+  const CellInfo &ci = S.cells[c.a];
+  c.start = ci.start;
+  c.cell = (uint32_t)ci.cell;
+  c.s = (pos - c.start) >> 1;
+  c.i = S.pi[pos];
+  c.j = S.pi[pos + 1];
+  c.vi = S.v[c.i];
+  c.vj = S.v[c.j];
+  c.gx = c.vi.x - c.vj.x;  // eq. 1
+  c.gy = c.vi.y - c.vj.y;
+  c.gz = c.vi.z - c.vj.z;
+  c.g2 = fmaf(c.gx, c.gx, fmaf(c.gy, c.gy, c.gz * c.gz));
+  c.acc = true;
+  c.U_b = 0.f;
+  c.U_eps = 0.f;
+  const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
+  if (need_randoms || accept) {
+    const uint4 r = philox4x32_10((uint32_t)c.s, c.cell, P.step, 1u, P.seed_lo, P.seed_hi);
+    c.U_b = u01(r.y);
+    c.U_eps = u01(r.z);
+    if (accept) {
+      const float cap = __ldg(P.cap + c.cell);
+      const float g = sqrtf(c.g2);
+      const float w = (P.op == 0) ? P.vhs_c * powf(g, P.vhs_e) : g;  // sigma_T(g) g  |  g
+      c.acc = u01(r.x) * cap < w;
+    }
+  }
+  return c;
+}
+
+template <class CK>
+__device__ __forceinline__ void pair_commit(const StepParams &P, CK &S, const PairCtx &c, float px, float py,
+                                            float pz, float aux, int q0) {
+  if (c.acc) {  // eqs. 6-8
+    const float cx = 0.5f * (c.vi.x + c.vj.x), cy = 0.5f * (c.vi.y + c.vj.y), cz = 0.5f * (c.vi.z + c.vj.z);
+    S.v[c.i] = make_float4(fmaf(0.5f, px, cx), fmaf(0.5f, py, cy), fmaf(0.5f, pz, cz), 0.f);
+    S.v[c.j] = make_float4(fmaf(-0.5f, px, cx), fmaf(-0.5f, py, cy), fmaf(-0.5f, pz, cz), 0.f);
+    if (P.flags & DSMC_F_ACCEPT) S.cells[c.a].collided = 1;
+  }
+  if (P.dump_any) {
+    const int64_t d = (int64_t)q0 + c.start + c.s;
+    if (P.dump.pair_i) P.dump.pair_i[d] = c.i - c.start;
+    if (P.dump.pair_j) P.dump.pair_j[d] = c.j - c.start;
+    if (P.dump.accepted) P.dump.accepted[d] = c.acc ? 1 : 0;
+    if (P.dump.gprime) { P.dump.gprime[3 * d] = px; P.dump.gprime[3 * d + 1] = py; P.dump.gprime[3 * d + 2] = pz; }
+    if (P.dump.aux) P.dump.aux[d] = aux;
+  }
+}
+
+// Rotation of g by deflection chi and azimuth eps = 2 pi U_eps (Q16).  MUFU sin/cos on
+// arguments inside [-pi, pi] (abs. error 2^-21.4): eps is taken as 2 pi (U - 1/2) with both signs flipped.
+__device__ __forceinline__ void rotate_fast(const PairCtx &c, float chi, float U_eps, float &px, float &py,
+                                            float &pz) {
+  float sc, cc, se, ce;
+  __sincosf(chi, &sc, &cc);
+  __sincosf(6.283185307179586f * (U_eps - 0.5f), &se, &ce);
+  se = -se;
+  ce = -ce;
+  const float gp2 = fmaf(c.gy, c.gy, c.gz * c.gz);
+  const float g = c.g2 * rsqrtf(c.g2);
+  if (gp2 <= 1e-30f * c.g2 * 1e-30f) {  // g_perp <= 1e-30 g
+    px = c.gx * cc;
+    py = fabsf(c.gx) * sc * ce;
+    pz = fabsf(c.gx) * sc * se;
+    return;
+  }
+  const float inv = rsqrtf(gp2), gperp = gp2 * inv;
+  const float sci = sc * inv;
+  px = fmaf(c.gx, cc, gperp * sc * se);
+  py = fmaf(c.gy, cc, sci * (g * c.gz * ce - c.gx * c.gy * se));
+  pz = fmaf(c.gz, cc, -sci * (g * c.gy * ce + c.gx * c.gz * se));
+}
+
+// table coordinate t_E = (ln x - lnE_min) (nE-1)/(lnE_max-lnE_min) from x = E_r/k_B, with the exponent
+// and mantissa of x handled separately (MUFU.LG2 only sees [1,2), abs. error 2^-22)
+__device__ __forceinline__ float table_tE(const ChiTableDev &T, float x) {
+  const int xi = __float_as_int(x);
+  const float e = (float)((xi >> 23) - 127);
+  const float m = __int_as_float((xi & 0x007FFFFF) | 0x3F800000);
+  return fmaf(__log2f(m), T.c1, fmaf(e, T.c1, T.c0));
+}
+
+// bilinear chi(E~, b~) from the L2-resident quad table, coordinates clamped (Q13).
+// quad[iE (nB-1) + iB] = (chi[iE][iB], chi[iE][iB+1], chi[iE+1][iB], chi[iE+1][iB+1]): one 16 B load.
+__device__ __forceinline__ float chi_table_t(const ChiTableDev &T, float tE, float tB) {
+  tE = fminf(fmaxf(tE, 0.f), (float)(T.nE - 1));
+  tB = fminf(fmaxf(tB, 0.f), (float)(T.nB - 1));
+  const int iE = min((int)tE, T.nE - 2), iB = min((int)tB, T.nB - 2);
+  const float fE = tE - (float)iE, fB = tB - (float)iB;
+  const float4 q = __ldg(T.quad + (size_t)iE * (T.nB - 1) + iB);
+  const float lo = fmaf(fB, q.y - q.x, q.x), hi = fmaf(fB, q.w - q.z, q.z);
+  return fmaf(fE, hi - lo, lo);
+}
+
+// ---------------------------------------------------------------------------------------------
+// finish: post-collision sums, matching coefficients, single coalesced store
+// ---------------------------------------------------------------------------------------------
+template <class CK>
+__device__ void chunk_finish(const StepParams &P, CK &S, int n_loc, int q0) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
+  if (P.flags & DSMC_F_MOMENT_MATCH) {
+    for (int sg = warp; sg < n_seg; sg += kWarps) {
+      const uint32_t e = S.segs[sg];
+      const int a = e & 0xFFFFu, piece = e >> 16;
+      const CellInfo &ci = S.cells[a];
+      if (!ci.collided) continue;
+      const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
+      const float ux = ci.ux, uy = ci.uy, uz = ci.uz;
+      float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
+      for (int q = lo + lane; q < hi; q += 32) {
+        const float4 v = S.v[q];
+        const float dx = v.x - ux, dy = v.y - uy, dz = v.z - uz;
+        sx += dx; sy += dy; sz += dz;
+        s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
+      }
+      sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
+      if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
+    }
+    __syncthreads();
+    for (int a = tid; a < n_act; a += kThreads) {
+      CellInfo &ci = S.cells[a];
+      double alpha = 1.0, bx = 0.0, by = 0.0, bz = 0.0;
+      if (ci.collided) {
+        const int N = ci.N, nseg = (N + kSeg - 1) / kSeg;
+        double sx = 0, sy = 0, sz = 0, s2 = 0;
+        for (int i = 0; i < nseg; ++i) {
+          const float4 p = S.part[ci.seg0 + i];
+          sx += p.x; sy += p.y; sz += p.z; s2 += p.w;
+        }
+        const double inv = 1.0 / N;
+        const double dx = sx * inv, dy = sy * inv, dz = sz * inv;  // u_post - u_pre
+        const double th_post = s2 - N * (dx * dx + dy * dy + dz * dz);
+        const double ux = ci.ux, uy = ci.uy, uz = ci.uz;
+        if (P.flags & DSMC_F_MATCH_ENERGY_ONLY) {  // literal eq. 11: v <- v sqrt(E_pre / E_post)
+          const double px = ux + dx, py = uy + dy, pz = uz + dz;
+          const double e_pre = (double)ci.theta + N * (ux * ux + uy * uy + uz * uz);
+          const double e_post = th_post + N * (px * px + py * py + pz * pz);
+          if (e_post > 0.0) alpha = sqrt(e_pre / e_post);
+        } else {  // v <- u_pre + alpha (v - u_post)
+          if (th_post > 0.0) alpha = sqrt((double)ci.theta / th_post);
+          bx = ux - alpha * (ux + dx);
+          by = uy - alpha * (uy + dy);
+          bz = uz - alpha * (uz + dz);
+        }
+      }
+      ci.ux = (float)bx; ci.uy = (float)by; ci.uz = (float)bz; ci.theta = (float)alpha;
+    }
+    __syncthreads();
+    for (int q = tid; q < n_loc; q += kThreads) {
+      const int a = S.lc[q];
+      float4 v = S.v[q];
+      if (a != 0xFFFF) {
+        const float4 co = *reinterpret_cast<const float4 *>(&S.cells[a]);
+        v.x = fmaf(co.w, v.x, co.x);
+        v.y = fmaf(co.w, v.y, co.y);
+        v.z = fmaf(co.w, v.z, co.z);
+      }
+      P.vx[q0 + q] = v.x;
+      P.vy[q0 + q] = v.y;
+      P.vz[q0 + q] = v.z;
+    }
+  } else {
+    for (int q = tid; q < n_loc; q += kThreads) {
+      const float4 v = S.v[q];
+      P.vx[q0 + q] = v.x;
+      P.vy[q0 + q] = v.y;
+      P.vz[q0 + q] = v.z;
+    }
+  }
+}
+
+}  // namespace dsmc

@@ -8,10 +8,11 @@
 
 namespace dsmc {
 
-constexpr int kChunk = 1024;                          // chunk granularity (particles)
+constexpr int kChunk = 512;                           // chunk granularity (particles)
 constexpr int kMaxCell = DSMC_MAX_CELL_PARTICLES;     // largest resident cell
-constexpr int kNlocMax = kChunk + kMaxCell;           // most particles one CTA can own
-constexpr int kActMax = kChunk / 2 + 2;               // most cells with N>=2 in one chunk
+constexpr int kNlocMax = kChunk + kMaxCell;           // most particles one CTA can own (deferred variant)
+constexpr int kLmaxSmall = 1536, kAmaxSmall = 64;     // small-footprint variant: 4 CTAs / SM
+constexpr int kLmaxBig = kNlocMax, kAmaxBig = kChunk / 2;  // deferred variant: any legal chunk
 constexpr int kThreads = 256;
 constexpr float kBoltzmann = 1.380649e-23f;
 
@@ -35,9 +36,10 @@ struct MlpTcDev {
 };
 
 struct ChiTableDev {
-  const float *chi;
+  const float4 *quad;  // [(nE-1)(nB-1)] the four nodes around each grid cell (one 16 B load per lookup)
   int nE, nB;
   float lnE_min, inv_dlnE;  // inv_dlnE = (nE-1)/(lnE_max-lnE_min)
+  float c0, c1;             // t_E = c0 + c1 log2(E_r/k_B): c1 = ln2 inv_dlnE, c0 = -lnE_min inv_dlnE
 };
 
 struct StepParams {
@@ -54,13 +56,19 @@ struct StepParams {
   float mass;
   // VHS-NN
   float inv_sigma_v, sigma_v, inv_T_scale, noise_sigma, shell_eps;
+  float T_coef;        // m / (3 kB): T_cell = T_coef Theta / N
   float vhs_c, vhs_e;  // sigma_T(g) g = vhs_c * g^vhs_e
   // ab initio
   float lnE_min, inv_lnE_range;
   float e_coef;  // m / (4 kB)
   ChiTableDev table;
   dsmc_pair_dump dump;
+  int32_t dump_any;
   int32_t *status;
+  // chunk decomposition (filled by launch_chunk_map)
+  int32_t n_chunks;
+  const int32_t *chunk_first;  // [n_chunks + 1]
+  int32_t *big;                // [0] = count, [1..] deferred chunk ids
 };
 
 }  // namespace dsmc
@@ -72,6 +80,8 @@ struct dsmc_ctx {
   int32_t max_cells;
   int32_t *d_status;
   int32_t *d_cursor;  // [max_cells + 1] scatter cursors / counts
+  int32_t *d_chunk_first;  // [max_particles / kChunk + 2]
+  int32_t *d_big;          // [max_particles / kChunk + 2]
   int64_t launches;
   int num_sms;
   // operators
@@ -99,6 +109,7 @@ int launch_cell_moments(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, co
                         const float *vz, double *moments);
 int launch_moment_match(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, float *vx, float *vy, float *vz,
                         const double *target, uint32_t flags);
+int launch_chunk_map(dsmc_ctx *c, StepParams &p);
 int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
