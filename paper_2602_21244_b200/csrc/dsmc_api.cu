@@ -33,7 +33,18 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
   c->num_sms = prop.multiProcessorCount;
   CK(cudaMalloc(&c->d_status, sizeof(int32_t)));
   CK(cudaMemset(c->d_status, 0, sizeof(int32_t)));
-  CK(cudaMalloc(&c->d_cursor, sizeof(int32_t) * (size_t)(max_cells + 2)));
+  {
+    const size_t np = (size_t)(max_particles > 0 ? max_particles : 1);
+    const size_t tiles = (np + kBinTile - 1) / kBinTile;
+    const int passes = bin_num_passes(max_cells > 0 ? max_cells : 1);
+    if (passes > 3) return DSMC_ERR_INVALID_ARG;
+    CK(cudaMalloc(&c->d_bin_hist, sizeof(int32_t) * tiles * kBinMaxRadix));
+    CK(cudaMalloc(&c->d_bin_group, sizeof(int32_t) * (size_t)c->num_sms * kBinMaxRadix));
+    for (int i = 0; i < 2; ++i) {
+      CK(cudaMalloc(&c->d_bin_cell[i], sizeof(int32_t) * np));
+      if (i < passes - 1) CK(cudaMalloc(&c->d_bin_rec[i], sizeof(float4) * np));
+    }
+  }
   const size_t n_chunks = (size_t)(max_particles / kChunk + 2);
   CK(cudaMalloc(&c->d_chunk_first, sizeof(int32_t) * n_chunks));
   CK(cudaMalloc(&c->d_big, sizeof(int32_t) * (n_chunks + 1)));
@@ -46,7 +57,9 @@ int dsmc_destroy(dsmc_ctx *c) {
   cudaSetDevice(c->device);
   cudaStreamSynchronize(c->stream);
   cudaFree(c->d_status);
-  cudaFree(c->d_cursor);
+  cudaFree(c->d_bin_hist);
+  cudaFree(c->d_bin_group);
+  for (int i = 0; i < 2; ++i) { cudaFree(c->d_bin_rec[i]); cudaFree(c->d_bin_cell[i]); }
   cudaFree(c->d_chunk_first);
   cudaFree(c->d_big);
   for (int s = 0; s < 2; ++s) {
@@ -183,7 +196,8 @@ static int check_sorted_args(dsmc_ctx *c, int64_t n, int32_t K, const void *cs, 
 
 int dsmc_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const float *vx, const float *vy,
              const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm, int32_t *cell_start) {
-  if (!c || n < 0 || K < 0 || n >= (int64_t(1) << 31) || K > c->max_cells) return DSMC_ERR_INVALID_ARG;
+  if (!c || n < 0 || K < 0 || n >= (int64_t(1) << 31) || K > c->max_cells || n > c->max_particles)
+    return DSMC_ERR_INVALID_ARG;
   if (!cell_start) return DSMC_ERR_INVALID_ARG;
   if (n > 0 && (!cell || !vx || !vy || !vz || !vx_s || !vy_s || !vz_s || !perm)) return DSMC_ERR_INVALID_ARG;
   CK(cudaSetDevice(c->device));

@@ -240,6 +240,7 @@ __device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
     const int bkt = ci.start + (int)__umulhi(k, (uint32_t)ci.N);
     const int b0 = bkt > 0 ? S.cnt[bkt - 1] : 0, b1 = S.cnt[bkt];
     int rank = 0;
+#pragma unroll 1
     for (int t = b0; t < b1; ++t) {
       const int o = S.ord[t];
       const uint32_t ko = S.key[o];

@@ -14,6 +14,8 @@ constexpr int kNlocMax = kChunk + kMaxCell;           // most particles one CTA 
 constexpr int kLmaxSmall = 1536, kAmaxSmall = 64;     // small-footprint variant: 4 CTAs / SM
 constexpr int kLmaxBig = kNlocMax, kAmaxBig = kChunk / 2;  // deferred variant: any legal chunk
 constexpr int kThreads = 256;
+constexpr int kBinTile = 4096;      // particles per radix-sort tile (dsmc_bin)
+constexpr int kBinMaxRadix = 512;   // digit values per pass
 constexpr float kBoltzmann = 1.380649e-23f;
 
 // MLP staged on the device: Wt[l] is W[l] transposed, [in][out] row-major (fp32).
@@ -79,7 +81,11 @@ struct dsmc_ctx {
   int64_t max_particles;
   int32_t max_cells;
   int32_t *d_status;
-  int32_t *d_cursor;  // [max_cells + 1] scatter cursors / counts
+  // dsmc_bin workspace: tile histograms, group sums, ping-pong record / cell-id buffers
+  int32_t *d_bin_hist;   // [tiles][kBinMaxRadix]
+  int32_t *d_bin_group;  // [num_sms][kBinMaxRadix]
+  float4 *d_bin_rec[2];  // (idx, vx, vy, vz) between passes
+  int32_t *d_bin_cell[2];
   int32_t *d_chunk_first;  // [max_particles / kChunk + 2]
   int32_t *d_big;          // [max_particles / kChunk + 2]
   int64_t launches;
@@ -103,6 +109,7 @@ struct dsmc_ctx {
 
 namespace dsmc {
 // launchers (each returns a DSMC_* status and bumps ctx->launches)
+int bin_num_passes(int32_t K);
 int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const float *vx, const float *vy,
                const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm, int32_t *cell_start);
 int launch_cell_moments(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, const float *vx, const float *vy,

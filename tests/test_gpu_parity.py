@@ -76,9 +76,16 @@ def test_bin_reports_bad_cell_index_and_large_cells(dsmc):
     cell[3] = -1
     ctx.bin(dev(cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), 4)
     assert ctx.sync_status() == dsmc.ERR_BAD_CELL_INDEX
+    # a cell above DSMC_MAX_CELL_PARTICLES sorts fine but is refused by the SMEM-resident fused step
     big = wl._populate("big", np.array([5000, 5]), np.full(2, 300.0), np.zeros(2), np.zeros(2), 1)
     ctx2 = dsmc.Context(big.n, 2)
-    ctx2.bin(dev(big.cell), dev(big.vx), dev(big.vy), dev(big.vz), 2)
+    vx_s, vy_s, vz_s, perm, cs = ctx2.bin(dev(big.cell), dev(big.vx), dev(big.vy), dev(big.vz), 2)
+    assert ctx2.sync_status() == 0
+    rc, perm_o, cs_o = oracle.bin_particles(big.cell, 2)
+    np.testing.assert_array_equal(perm.cpu().numpy(), perm_o)
+    tab = _lj_table(16, 16)
+    ctx2.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    ctx2.collide_abinitio(cs, vx_s, vy_s, vz_s, dsmc.AbinitioParams(), 0, 0)
     assert ctx2.sync_status() == dsmc.ERR_CELL_TOO_LARGE
 
 
