@@ -26,6 +26,7 @@ constexpr int kBinThreads = 512;
 constexpr int kBinWarps = kBinThreads / 32;
 constexpr int kBinItems = kBinTile / kBinThreads;  // 8 per thread, 256 consecutive per warp
 static_assert(kBinItems == 8, "tile / threads");
+constexpr int kHistTiles = 4;  // tiles per k_tile_hist CTA
 
 struct BinPass {
   int shift, mask, R;  // digit = (cell >> shift) & mask, R = number of digit values (<= 512)
@@ -35,36 +36,56 @@ __device__ __forceinline__ int bin_digit(int c, const BinPass &ps) { return (c >
 
 // ---------------------------------------------------------------------------------------------
 // k_tile_hist: hist[t][d] = number of items of tile t with digit d; group[g][d] += the same.
-// FIRST pass also range-checks the cell ids (bad ids are dropped here and in the down-sweep).
+// One CTA covers kHistTiles consecutive tiles (same group) so that 32 loads per thread are in
+// flight before the first shared-memory atomic.  FIRST pass also range-checks the cell ids (bad
+// ids are dropped here and in the down-sweep).
 // ---------------------------------------------------------------------------------------------
 template <bool FIRST>
-__global__ void __launch_bounds__(kBinThreads) k_tile_hist(int64_t n, int32_t K, const int32_t *__restrict__ cell,
-                                                          BinPass ps, int tiles_per_group,
-                                                          int32_t *__restrict__ hist, int32_t *__restrict__ group,
+__global__ void __launch_bounds__(kBinThreads) k_tile_hist(int64_t n, int32_t K, int n_tiles,
+                                                          const int32_t *__restrict__ cell, BinPass ps,
+                                                          int tiles_per_group, int32_t *__restrict__ hist,
+                                                          int32_t *__restrict__ group,
                                                           int32_t *__restrict__ status) {
-  __shared__ int h[kBinMaxRadix];
+  __shared__ int h[kHistTiles][kBinMaxRadix];
   const int tid = threadIdx.x;
-  const int t = blockIdx.x;
-  h[tid] = 0;
-  __syncthreads();
-  const int64_t base = (int64_t)t * kBinTile;
+  const int t0 = blockIdx.x * kHistTiles;
 #pragma unroll
-  for (int r = 0; r < kBinItems; ++r) {
-    const int64_t i = base + r * kBinThreads + tid;
-    if (i < n) {
-      const int c = __ldg(cell + i);
-      if (FIRST && (c < 0 || c >= K)) {
-        *status = DSMC_ERR_BAD_CELL_INDEX;
-      } else {
-        atomicAdd(&h[bin_digit(c, ps)], 1);
-      }
+  for (int k = 0; k < kHistTiles; ++k) h[k][tid] = 0;
+  int c[kHistTiles][kBinItems];
+#pragma unroll
+  for (int k = 0; k < kHistTiles; ++k) {
+    const int64_t base = (int64_t)(t0 + k) * kBinTile;
+#pragma unroll
+    for (int r = 0; r < kBinItems; ++r) {
+      const int64_t i = base + r * kBinThreads + tid;
+      c[k][r] = i < n ? __ldg(cell + i) : -1;
     }
   }
   __syncthreads();
+  bool bad = false;
+#pragma unroll
+  for (int k = 0; k < kHistTiles; ++k) {
+#pragma unroll
+    for (int r = 0; r < kBinItems; ++r) {
+      const int cc = c[k][r];
+      const int64_t i = (int64_t)(t0 + k) * kBinTile + r * kBinThreads + tid;
+      if (FIRST && i < n && (cc < 0 || cc >= K)) bad = true;
+      if (cc >= 0 && (!FIRST || cc < K)) atomicAdd(&h[k][bin_digit(cc, ps)], 1);
+    }
+  }
+  if (FIRST && bad) *status = DSMC_ERR_BAD_CELL_INDEX;
+  __syncthreads();
   if (tid < ps.R) {
-    const int x = h[tid];
-    hist[(size_t)t * kBinMaxRadix + tid] = x;
-    if (x) atomicAdd(&group[(size_t)(t / tiles_per_group) * kBinMaxRadix + tid], x);
+    int sum = 0;
+#pragma unroll
+    for (int k = 0; k < kHistTiles; ++k) {
+      if (t0 + k < n_tiles) {
+        const int x = h[k][tid];
+        hist[(size_t)(t0 + k) * kBinMaxRadix + tid] = x;
+        sum += x;
+      }
+    }
+    if (sum) atomicAdd(&group[(size_t)(t0 / tiles_per_group) * kBinMaxRadix + tid], sum);
   }
 }
 
@@ -120,10 +141,14 @@ __global__ void __launch_bounds__(kBinThreads) k_prefix(int n_tiles, int n_group
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_downsweep: one CTA per tile.  Warp w owns items [256 w, 256 w + 256) of the tile and walks
-// them in index order, 32 at a time: lanes with the same digit find one another with
-// match.any, the first of them bumps the warp's private counter of that digit, so
+// k_downsweep: one CTA per tile.  The tile's cell ids and payload are staged in shared memory by
+// bulk async copies (cp.async.bulk + mbarrier) issued by one thread at kernel start, so the HBM
+// reads overlap the ranking.  Warp w owns items [256 w, 256 w + 256) of the tile and walks them in
+// index order, 32 at a time: lanes with the same digit find one another with match.any, the first
+// of them bumps the warp's private counter of that digit, so
 // rank = (items of this digit in earlier warps) + (earlier rounds) + (earlier lanes): stable.
+// The copy-out walks the sorted positions and gathers through the inverse permutation, writing
+// runs of consecutive records.
 // ---------------------------------------------------------------------------------------------
 struct BinIo {
   // FIRST pass input
@@ -137,35 +162,107 @@ struct BinIo {
   // LAST pass output
   float *vx_s, *vy_s, *vz_s;
   int32_t *perm, *cell_sorted;
+  int32_t bulk_ok;  // FIRST-pass inputs are 16-byte aligned
 };
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// global -> shared bulk copy; bytes > 0 and a multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
 
 template <bool FIRST, bool LAST>
 __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t K, BinPass ps, BinIo io,
                                                               const int32_t *__restrict__ hist) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  float4 *srec = reinterpret_cast<float4 *>(smem_raw);                    // [tile]
-  int32_t *scell = reinterpret_cast<int32_t *>(srec + kBinTile);          // [tile]
-  int32_t *tile_off = scell + kBinTile;                                   // [R]
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  // staging (unsorted, tile order): cell ids, then (FIRST) vx | vy | vz, else records
+  int32_t *scell = reinterpret_cast<int32_t *>(smem_raw);                 // [tile]
+  float *sv = reinterpret_cast<float *>(scell + kBinTile);                // FIRST: [3][tile]
+  float4 *srec = reinterpret_cast<float4 *>(scell + kBinTile);            // else:  [tile]
+  unsigned char *after = smem_raw + (size_t)kBinTile * (FIRST ? 16 : 20);
+  int32_t *tile_off = reinterpret_cast<int32_t *>(after);                 // [R]
   int32_t *gdst = tile_off + kBinMaxRadix;                                // [R]
   uint16_t *wc = reinterpret_cast<uint16_t *>(gdst + kBinMaxRadix);       // [warps][R]
+  uint16_t *inv = wc + kBinWarps * kBinMaxRadix;                          // [tile] sorted pos -> tile index
   __shared__ int scratch[kBinWarps + 1];
+  __shared__ __align__(8) uint64_t bar[2];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int t = blockIdx.x;
-  const int64_t base = (int64_t)t * kBinTile + warp * (32 * kBinItems);
+  const int64_t tbase = (int64_t)t * kBinTile;
+  const int cnt_tile = (int)min((int64_t)kBinTile, n - tbase);
   const int32_t *cin = FIRST ? io.cell : io.cell_in;
+  const bool bulk = !FIRST || io.bulk_ok;
+  const int n_bulk = bulk ? (cnt_tile & ~3) : 0;  // 4-byte arrays: whole 16-byte units only
 
+  if (tid == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (n_bulk > 0) {
+      mbar_expect_tx(&bar[0], (uint32_t)n_bulk * 4u);
+      bulk_g2s(scell, cin + tbase, (uint32_t)n_bulk * 4u, &bar[0]);
+    } else {
+      mbar_expect_tx(&bar[0], 0u);
+    }
+    if (FIRST) {
+      if (n_bulk > 0) {
+        mbar_expect_tx(&bar[1], (uint32_t)n_bulk * 12u);
+        bulk_g2s(sv, io.vx + tbase, (uint32_t)n_bulk * 4u, &bar[1]);
+        bulk_g2s(sv + kBinTile, io.vy + tbase, (uint32_t)n_bulk * 4u, &bar[1]);
+        bulk_g2s(sv + 2 * kBinTile, io.vz + tbase, (uint32_t)n_bulk * 4u, &bar[1]);
+      } else {
+        mbar_expect_tx(&bar[1], 0u);
+      }
+    } else {
+      mbar_expect_tx(&bar[1], (uint32_t)cnt_tile * 16u);
+      bulk_g2s(srec, io.rec_in + tbase, (uint32_t)cnt_tile * 16u, &bar[1]);
+    }
+  }
   for (int i = tid; i < kBinWarps * kBinMaxRadix / 2; i += kBinThreads) reinterpret_cast<uint32_t *>(wc)[i] = 0u;
-  int c[kBinItems];
-#pragma unroll
-  for (int r = 0; r < kBinItems; ++r) {
-    const int64_t i = base + r * 32 + lane;
-    c[r] = i < n ? __ldg(cin + i) : -1;
-    if (FIRST && c[r] >= K) c[r] = -1;  // dropped (status already set by k_tile_hist)
+  // items the bulk copies do not cover (ragged tail, or unaligned caller arrays)
+  for (int j = n_bulk + tid; j < cnt_tile; j += kBinThreads) {
+    scell[j] = __ldg(cin + tbase + j);
+    if (FIRST) {
+      sv[j] = __ldg(io.vx + tbase + j);
+      sv[kBinTile + j] = __ldg(io.vy + tbase + j);
+      sv[2 * kBinTile + j] = __ldg(io.vz + tbase + j);
+    }
   }
   __syncthreads();
+  mbar_wait(&bar[0], 0);
+
   uint16_t *mywc = wc + warp * kBinMaxRadix;
-  int lr[kBinItems];
+  const int jbase = warp * (32 * kBinItems) + lane;
+  int c[kBinItems], lr[kBinItems];
+#pragma unroll
+  for (int r = 0; r < kBinItems; ++r) {
+    const int j = jbase + r * 32;
+    c[r] = j < cnt_tile ? scell[j] : -1;
+    if (FIRST && c[r] >= K) c[r] = -1;  // dropped (status already set by k_tile_hist)
+  }
 #pragma unroll
   for (int r = 0; r < kBinItems; ++r) {
     const int d = c[r] >= 0 ? bin_digit(c[r], ps) : 0xFFFF;
@@ -209,34 +306,26 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
     gdst[tid] = __ldg(hist + (size_t)t * kBinMaxRadix + tid) - off;
   }
   __syncthreads();
-  // payload -> sorted position in shared memory
-  float4 rec[kBinItems];
-#pragma unroll
-  for (int r = 0; r < kBinItems; ++r) {
-    const int64_t i = base + r * 32 + lane;
-    if (c[r] >= 0) {
-      if (FIRST) {
-        rec[r] = make_float4(__int_as_float((int)i), __ldg(io.vx + i), __ldg(io.vy + i), __ldg(io.vz + i));
-      } else {
-        rec[r] = __ldg(io.rec_in + i);
-      }
-    }
-  }
 #pragma unroll
   for (int r = 0; r < kBinItems; ++r) {
     if (c[r] >= 0) {
       const int d = bin_digit(c[r], ps);
-      const int pos = tile_off[d] + mywc[d] + lr[r];
-      srec[pos] = rec[r];
-      scell[pos] = c[r];
+      inv[tile_off[d] + mywc[d] + lr[r]] = (uint16_t)(jbase + r * 32);
     }
   }
   __syncthreads();
+  mbar_wait(&bar[1], 0);
   const int kept = scratch[kBinWarps];
   for (int pos = tid; pos < kept; pos += kBinThreads) {
-    const int cc = scell[pos];
+    const int j = inv[pos];
+    const int cc = scell[j];
     const int64_t dst = (int64_t)gdst[bin_digit(cc, ps)] + pos;
-    const float4 rr = srec[pos];
+    float4 rr;
+    if (FIRST) {
+      rr = make_float4(__int_as_float((int)(tbase + j)), sv[j], sv[kBinTile + j], sv[2 * kBinTile + j]);
+    } else {
+      rr = srec[j];
+    }
     if (LAST) {
       io.perm[dst] = __float_as_int(rr.x);
       io.vx_s[dst] = rr.y;
@@ -250,23 +339,36 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
   }
 }
 
-// cell_start[c] = first sorted slot whose cell id is >= c (CSR offsets; covers empty cells)
+// cell_start[c] = first sorted slot whose cell id is >= c (CSR offsets; covers empty cells).
+// Four consecutive slots per thread (one 16-byte load + the left neighbour).
 __global__ void __launch_bounds__(256) k_cell_start(int64_t n, int32_t K, const int32_t *__restrict__ cell_sorted,
                                                    int32_t *__restrict__ cell_start) {
-  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (s > n) return;
-  int prev = s > 0 ? __ldg(cell_sorted + s - 1) : -1;
-  int cur = s < n ? __ldg(cell_sorted + s) : K;
-  prev = max(-1, min(prev, K));
-  cur = max(-1, min(cur, K));
-  for (int cc = prev + 1; cc <= cur; ++cc) cell_start[cc] = (int32_t)s;
+  const int64_t s0 = 4 * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
+  if (s0 > n) return;
+  int v[5];
+  v[0] = s0 > 0 ? __ldg(cell_sorted + s0 - 1) : -1;
+  if (s0 + 4 <= n) {
+    const int4 q = __ldg(reinterpret_cast<const int4 *>(cell_sorted + s0));
+    v[1] = q.x; v[2] = q.y; v[3] = q.z; v[4] = q.w;
+  } else {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v[1 + u] = s0 + u < n ? __ldg(cell_sorted + s0 + u) : K;
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    const int64_t s = s0 + u;
+    if (s > n) break;
+    const int prev = max(-1, min(v[u], K)), cur = max(-1, min(s < n ? v[u + 1] : K, K));
+    for (int cc = prev + 1; cc <= cur; ++cc) cell_start[cc] = (int32_t)s;
+  }
 }
 
 template <bool FIRST, bool LAST>
 static void launch_downsweep(int n_tiles, cudaStream_t s, int64_t n, int32_t K, const BinPass &ps, const BinIo &io,
                              const int32_t *hist) {
   auto kern = k_downsweep<FIRST, LAST>;
-  const size_t smem = (size_t)kBinTile * 20 + 2 * 4 * kBinMaxRadix + 2 * kBinWarps * kBinMaxRadix;
+  const size_t smem = (size_t)kBinTile * (FIRST ? 16 : 20) + 2 * 4 * kBinMaxRadix + 2 * kBinWarps * kBinMaxRadix +
+                      2 * kBinTile + 128;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   kern<<<n_tiles, kBinThreads, smem, s>>>(n, K, ps, io, hist);
 }
@@ -290,8 +392,9 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
   const int dbits = (bits + passes - 1) / passes;
   const int n_tiles = (int)((n + kBinTile - 1) / kBinTile);
   const int n_groups = std::min(n_tiles, c->num_sms);
-  const int tpg = (n_tiles + n_groups - 1) / n_groups;
+  const int tpg = (((n_tiles + n_groups - 1) / n_groups) + kHistTiles - 1) / kHistTiles * kHistTiles;
   const int groups = (n_tiles + tpg - 1) / tpg;
+  const int hist_grid = (n_tiles + kHistTiles - 1) / kHistTiles;
   for (int p = 0; p < passes; ++p) {
     BinPass ps;
     ps.shift = p * dbits;
@@ -307,13 +410,16 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     io.cell_out = c->d_bin_cell[p & 1];
     io.vx_s = vx_s; io.vy_s = vy_s; io.vz_s = vz_s; io.perm = perm;
     io.cell_sorted = c->d_bin_cell[p & 1];
+    io.bulk_ok = ((reinterpret_cast<uintptr_t>(cell) | reinterpret_cast<uintptr_t>(vx) |
+                   reinterpret_cast<uintptr_t>(vy) | reinterpret_cast<uintptr_t>(vz)) & 15) == 0;
     if (cudaMemsetAsync(c->d_bin_group, 0, sizeof(int32_t) * (size_t)groups * kBinMaxRadix, s) != cudaSuccess)
       return DSMC_ERR_CUDA;
     if (first)
-      k_tile_hist<true><<<n_tiles, kBinThreads, 0, s>>>(n, K, cell, ps, tpg, c->d_bin_hist, c->d_bin_group, c->d_status);
+      k_tile_hist<true><<<hist_grid, kBinThreads, 0, s>>>(n, K, n_tiles, cell, ps, tpg, c->d_bin_hist,
+                                                          c->d_bin_group, c->d_status);
     else
-      k_tile_hist<false><<<n_tiles, kBinThreads, 0, s>>>(n, K, io.cell_in, ps, tpg, c->d_bin_hist, c->d_bin_group,
-                                                         c->d_status);
+      k_tile_hist<false><<<hist_grid, kBinThreads, 0, s>>>(n, K, n_tiles, io.cell_in, ps, tpg, c->d_bin_hist,
+                                                           c->d_bin_group, c->d_status);
     k_prefix<<<groups, kBinThreads, 0, s>>>(n_tiles, groups, tpg, ps, c->d_bin_hist, c->d_bin_group);
     if (first && last) launch_downsweep<true, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
     else if (first) launch_downsweep<true, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
@@ -321,7 +427,7 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     else launch_downsweep<false, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
     c->launches += 3;
     if (last) {
-      k_cell_start<<<(int)((n + 1 + 255) / 256), 256, 0, s>>>(n, K, io.cell_sorted, cell_start);
+      k_cell_start<<<(int)((n / 4 + 1 + 255) / 256), 256, 0, s>>>(n, K, io.cell_sorted, cell_start);
       c->launches += 1;
     }
   }
