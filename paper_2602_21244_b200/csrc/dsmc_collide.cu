@@ -13,9 +13,13 @@ namespace dsmc {
 
 // k_chunk_map: chunk_first[b] = first cell whose first slot is >= b * kChunk; resets the deferred list.
 __global__ void k_chunk_map(int32_t K, const int32_t *__restrict__ cs, int32_t *__restrict__ chunk_first,
-                            int32_t *__restrict__ big) {
+                            int32_t *__restrict__ big, int32_t *__restrict__ work) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k == 0) big[0] = 0;
+  if (k == 0) {
+    big[0] = 0;
+    work[0] = 0;
+    work[1] = 0;
+  }
   if (k > K) return;
   const int s = __ldg(cs + k);
   const int lo = (k == 0) ? 0 : (__ldg(cs + k - 1) / kChunk + 1);
@@ -229,7 +233,9 @@ int launch_chunk_map(dsmc_ctx *c, StepParams &p) {
   p.n_chunks = (int32_t)((p.n + kChunk - 1) / kChunk);
   p.chunk_first = c->d_chunk_first;
   p.big = c->d_big;
-  k_chunk_map<<<(p.n_cells + 1 + 255) / 256, 256, 0, c->stream>>>(p.n_cells, p.cell_start, c->d_chunk_first, c->d_big);
+  p.work = c->d_work;
+  k_chunk_map<<<(p.n_cells + 1 + 255) / 256, 256, 0, c->stream>>>(p.n_cells, p.cell_start, c->d_chunk_first, c->d_big,
+                                                                  c->d_work);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }

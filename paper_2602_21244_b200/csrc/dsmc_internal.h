@@ -71,6 +71,7 @@ struct StepParams {
   int32_t n_chunks;
   const int32_t *chunk_first;  // [n_chunks + 1]
   int32_t *big;                // [0] = count, [1..] deferred chunk ids
+  int32_t *work;               // [0], [1]: next chunk / next deferred entry (persistent kernels)
 };
 
 }  // namespace dsmc
@@ -88,6 +89,7 @@ struct dsmc_ctx {
   int32_t *d_bin_cell[2];
   int32_t *d_chunk_first;  // [max_particles / kChunk + 2]
   int32_t *d_big;          // [max_particles / kChunk + 2]
+  int32_t *d_work;         // [4] work counters of the persistent kernels ([0] main pass, [1] deferred pass)
   int64_t launches;
   int num_sms;
   // operators

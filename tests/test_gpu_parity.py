@@ -361,3 +361,101 @@ def test_empty_inputs_and_unconfigured_operators(dsmc):
     with pytest.raises(dsmc.DsmcError) as e:  # BF16 TC path supports H in {64,128} only
         ctx.collide_vhs_nn(cs, v, v.clone(), v.clone(), dsmc.VhsParams(flags=dsmc.F_BF16_TC), 0, 0)
     assert e.value.status == dsmc.ERR_UNSUPPORTED_SHAPE
+
+
+# --------------------------------------------------------------------------- BF16 tcgen05 paths
+def _quantiles(x):
+    return "median %.2e, 99%% %.2e, 99.9%% %.2e, max %.2e" % tuple(np.quantile(x, [0.5, 0.99, 0.999, 1.0]))
+
+
+@pytest.mark.parametrize("H,act", [(128, "silu"), (64, "silu"), (128, "tanh"), (64, "relu")])
+def test_chi_batch_bf16_tc(dsmc, H, act):
+    """a10 on the tensor cores; tolerance Q26: abs(dchi) <= 2e-2 (1 + abs(chi))."""
+    n = 300_017  # 2343 full tiles + a ragged tail of 113 pairs
+    E, b = wl.abinitio_pair_batch(seed=3, n=n)
+    E[:4] = [1.0, 1e6, 5.0, 6e4]
+    a_g = {"silu": dsmc.ACT_SILU, "tanh": dsmc.ACT_TANH, "relu": dsmc.ACT_RELU}[act]
+    a_o = {"silu": oracle.ACT_SILU, "tanh": oracle.ACT_TANH, "relu": oracle.ACT_RELU}[act]
+    ctx = dsmc.Context(n, 1)
+    Ws, bs = wl.random_mlp(3, [2, H, H, 1])
+    ctx.set_mlp(1, Ws, bs, a_g)
+    got = ctx.chi_batch(dev(E), dev(b), 1, 1e-9, flags=dsmc.F_BF16_TC).cpu().numpy().astype(np.float64)
+    ctx.check()
+    lo, hi = float(np.float32(np.log(5.0))), float(np.float32(np.log(6.0e4)))
+    want = oracle.chi_batch(E, b, 1, 1e-9, net=oracle.Mlp(Ws, bs, a_o), lnE_min=lo, lnE_max=hi)
+    rel = np.abs(got - want) / (1 + np.abs(want))
+    print("chi bf16 H=%d %s: %s" % (H, act, _quantiles(rel)))
+    assert rel.max() <= 2e-2
+    ctx.close()
+
+
+def test_collide_abinitio_bf16_tc(dsmc):
+    pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    net = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    prm = dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC)
+    oprm = oracle.AbinitioParams(chi_mode=1, lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
+    for step in range(2):
+        v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+        dump = dsmc.PairDump(pop.n, "cuda")
+        ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=4, step=step, dump=dump)
+        ctx.check()
+        ref = oracle.collide_abinitio(cs_h, *v_in, oprm, 4, step, net=net)
+        sel = ref.pair_i >= 0
+        chi_g = dump.aux.cpu().numpy().astype(np.float64)
+        rel = np.abs(chi_g[sel] - ref.aux[sel]) / (1 + np.abs(ref.aux[sel]))
+        print("abinitio bf16 chi: %s" % _quantiles(rel))
+        assert rel.max() <= 2e-2  # Q26
+        # a chi difference rotates g' by exactly that angle: allow it on top of the fp32 rotation error
+        err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 3e-5, 1e-6, slope=1.01 * np.abs(chi_g - ref.aux))
+        assert err.max() <= 2e-2 * (1 + np.abs(ref.aux[sel]).max())
+        N = np.diff(cs_h)
+        pre = oracle.cell_moments(cs_h, *v_in)
+        got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+        ok = N >= 2
+        assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+        assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    ctx.close()
+
+
+@pytest.mark.parametrize("case", ["cfg1_tiny", "cfg3_cavity_small", "ragged6"])
+def test_collide_vhs_nn_bf16_tc(dsmc, case):
+    """BF16 tensor-core VHS-NN: bit-exact pairing, 2e-2 per pair on the gated set (Q21), 1e-6 on moments."""
+    n_in = 8
+    if case == "cfg1_tiny":
+        pop, H, ppc, sw = wl.tiny_box(), 64, 50, 0
+    elif case == "cfg3_cavity_small":
+        pop, H, ppc, sw = wl.cavity(nx=20, ny=20), 128, 50, 2
+    else:
+        rng = np.random.default_rng(3)
+        counts = rng.integers(0, 30, 400)
+        counts[5], counts[6], counts[7], counts[8] = 0, 1, 2, 3
+        counts[100] = 2048
+        pop, H, ppc, sw, n_in = wl._populate("ragged", counts, np.full(400, 273.0), np.zeros(400), np.zeros(400), 3), 64, -1, 0, 6
+    ctx, net = _setup_vhs(dsmc, pop, H, sw, n_in=n_in)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    flags = dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC
+    prm = dsmc.VhsParams(sigma_v=wl.SIGMA_V, pairs_per_cell=ppc, flags=flags)
+    oprm = oracle.VhsParams(sigma_v=float(np.float32(wl.SIGMA_V)), pairs_per_cell=ppc)
+    for step in range(2):
+        v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+        dump = dsmc.PairDump(pop.n, "cuda")
+        ctx.collide_vhs_nn(cs, vx_s, vy_s, vz_s, prm, seed=sw, step=step, dump=dump)
+        ctx.check()
+        ref = oracle.collide_vhs_nn(cs_h, *v_in, net, oprm, sw, step)
+        hn = ref.aux
+        med = np.median(hn[ref.pair_i >= 0])
+        err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 2e-2, 1e-6, gate=hn >= 0.25 * med)
+        print("vhs bf16 %s: all pairs %s; excluded %.2f%%" % (case, _quantiles(err), 100 * (1 - (hn[ref.pair_i >= 0] >= 0.25 * med).mean())))
+        N = np.diff(cs_h)
+        pre = oracle.cell_moments(cs_h, *v_in)
+        got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+        ok = N >= 2
+        assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+        assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    ctx.close()
