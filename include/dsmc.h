@@ -120,6 +120,8 @@ typedef struct {
   float d_ref, omega, T_ref; /* VHS sigma_T(g), used iff DSMC_F_ACCEPT */
   int32_t pairs_per_cell;    /* > 0: request per cell; -1: floor(N_k/2).  M_k = min(req, N_k/2) */
   uint32_t flags;
+  int32_t cell_base;         /* RNG cell coordinate of local cell 0: a rank that owns the global cell range
+                                [c0, c1) passes c0 and draws exactly the randoms of the unsharded run */
 } dsmc_vhs_params;
 
 typedef struct {
@@ -129,6 +131,7 @@ typedef struct {
   int32_t chi_mode;       /* 0 = table, 1 = MLP (slot 1) */
   int32_t pairs_per_cell;
   uint32_t flags;         /* NOISE / ENERGY_SHELL are ignored here */
+  int32_t cell_base;      /* as in dsmc_vhs_params */
 } dsmc_abinitio_params;
 
 /* Optional debug output (any member may be NULL).  All arrays have n entries; pair slot s of

@@ -51,13 +51,13 @@ class _Vhs(C.Structure):
     _fields_ = [("mass", C.c_double), ("sigma_v", C.c_double), ("T_scale", C.c_double),
                 ("noise_sigma", C.c_double), ("shell_eps", C.c_double), ("d_ref", C.c_double),
                 ("omega", C.c_double), ("T_ref", C.c_double), ("pairs_per_cell", C.c_int32),
-                ("flags", C.c_uint32)]
+                ("flags", C.c_uint32), ("cell_base", C.c_int32)]
 
 
 class _Abi(C.Structure):
     _fields_ = [("mass", C.c_double), ("b_max", C.c_double), ("lnE_min", C.c_double),
                 ("lnE_max", C.c_double), ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32),
-                ("flags", C.c_uint32)]
+                ("flags", C.c_uint32), ("cell_base", C.c_int32)]
 
 
 class _Table(C.Structure):
@@ -136,10 +136,11 @@ class VhsParams:
     T_ref: float = 273.0
     pairs_per_cell: int = -1
     flags: int = F_NOISE | F_ENERGY_SHELL | F_MOMENT_MATCH
+    cell_base: int = 0
 
     def c(self):
         return _Vhs(self.mass, self.sigma_v, self.T_scale, self.noise_sigma, self.shell_eps,
-                    self.d_ref, self.omega, self.T_ref, self.pairs_per_cell, self.flags)
+                    self.d_ref, self.omega, self.T_ref, self.pairs_per_cell, self.flags, self.cell_base)
 
 
 @dataclass
@@ -151,10 +152,11 @@ class AbinitioParams:
     chi_mode: int = 0
     pairs_per_cell: int = -1
     flags: int = F_MOMENT_MATCH
+    cell_base: int = 0
 
     def c(self):
         return _Abi(self.mass, self.b_max, self.lnE_min, self.lnE_max, self.chi_mode,
-                    self.pairs_per_cell, self.flags)
+                    self.pairs_per_cell, self.flags, self.cell_base)
 
 
 @dataclass

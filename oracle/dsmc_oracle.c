@@ -328,15 +328,15 @@ int orc_collide_vhs_nn(int64_t n, int32_t n_cells, const int32_t *cell_start, do
     orc_cell_state(N, cx, cy, cz, prm->mass, ubar, &Theta, &Tk);
     for (int32_t p = 0; p < N; ++p) E_pre += cx[p] * cx[p] + cy[p] * cy[p] + cz[p] * cz[p];
     int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
-    int32_t M = orc_pairing(seed, step, (uint32_t)k, N, prm->pairs_per_cell, pi);
+    int32_t M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, prm->pairs_per_cell, pi);
     int32_t n_collided = 0;
     for (int32_t s = 0; s < M; ++s) {
       int32_t i = pi[2 * s], j = pi[2 * s + 1];
       double g[3] = {cx[i] - cx[j], cy[i] - cy[j], cz[i] - cz[j]}; /* eq. 1 */
       double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
       double U[3], xi[3];
-      orc_pair_uniforms(seed, step, (uint32_t)k, (uint32_t)s, U);
-      orc_pair_normals(seed, step, (uint32_t)k, (uint32_t)s, xi);
+      orc_pair_uniforms(seed, step, (uint32_t)(k + prm->cell_base), (uint32_t)s, U);
+      orc_pair_normals(seed, step, (uint32_t)(k + prm->cell_base), (uint32_t)s, xi);
       int acc = 1;
       if ((prm->flags & ORC_F_ACCEPT) && sigma_cr_max != NULL)
         acc = (U[0] * (double)sigma_cr_max[k] < orc_vhs_sigma_g(gn, prm)) ? 1 : 0;
@@ -400,7 +400,7 @@ int orc_collide_abinitio(int64_t n, int32_t n_cells, const int32_t *cell_start, 
     orc_cell_state(N, cx, cy, cz, prm->mass, ubar, &Theta, &Tk);
     for (int32_t p = 0; p < N; ++p) E_pre += cx[p] * cx[p] + cy[p] * cy[p] + cz[p] * cz[p];
     int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
-    int32_t M = orc_pairing(seed, step, (uint32_t)k, N, prm->pairs_per_cell, pi);
+    int32_t M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, prm->pairs_per_cell, pi);
     int32_t n_collided = 0;
     for (int32_t s = 0; s < M; ++s) {
       int32_t i = pi[2 * s], j = pi[2 * s + 1];
@@ -408,7 +408,7 @@ int orc_collide_abinitio(int64_t n, int32_t n_cells, const int32_t *cell_start, 
       double g2 = g[0] * g[0] + g[1] * g[1] + g[2] * g[2];
       double gn = sqrt(g2);
       double U[3];
-      orc_pair_uniforms(seed, step, (uint32_t)k, (uint32_t)s, U);
+      orc_pair_uniforms(seed, step, (uint32_t)(k + prm->cell_base), (uint32_t)s, U);
       int acc = 1; /* constant sigma = pi b_max^2 => accept iff U g_max < g (Q9) */
       if ((prm->flags & ORC_F_ACCEPT) && cr_max != NULL) acc = (U[0] * (double)cr_max[k] < gn) ? 1 : 0;
       if (pair_i) pair_i[a + s] = i;

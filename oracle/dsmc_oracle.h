@@ -55,6 +55,7 @@ typedef struct {
   double d_ref, omega, T_ref; /* VHS cross-section, used iff ORC_F_ACCEPT */
   int32_t pairs_per_cell;     /* >0 request per cell, -1 = floor(N_k/2) */
   uint32_t flags;
+  int32_t cell_base;          /* RNG cell coordinate of local cell 0 (cell-range shards) */
 } orc_vhs_params;
 
 typedef struct {
@@ -63,6 +64,7 @@ typedef struct {
   int32_t chi_mode;        /* 0 = table, 1 = MLP */
   int32_t pairs_per_cell;
   uint32_t flags;
+  int32_t cell_base; /* RNG cell coordinate of local cell 0 */
 } orc_abinitio_params;
 
 typedef struct { /* chi[iE*nB + iB], node (lnE_min + iE*dE, iB/(nB-1)), Q13 */

@@ -251,6 +251,7 @@ int dsmc_collide_vhs_nn(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
   p.flags = prm->flags;
   p.pairs_per_cell = prm->pairs_per_cell;
   p.op = 0;
+  p.cell_base = (uint32_t)prm->cell_base;
   p.mass = prm->mass;
   p.sigma_v = prm->sigma_v;
   p.inv_sigma_v = 1.0f / prm->sigma_v;
@@ -289,6 +290,7 @@ int dsmc_collide_abinitio(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, 
   p.flags = prm->flags & ~(uint32_t)(DSMC_F_NOISE | DSMC_F_ENERGY_SHELL);
   p.pairs_per_cell = prm->pairs_per_cell;
   p.op = prm->chi_mode == 0 ? 1 : 2;
+  p.cell_base = (uint32_t)prm->cell_base;
   p.mass = prm->mass;
   p.e_coef = (float)((double)prm->mass / (4.0 * 1.380649e-23));
   p.lnE_min = prm->lnE_min;

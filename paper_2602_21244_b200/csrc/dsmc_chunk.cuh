@@ -169,7 +169,7 @@ __device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
     const int a = e & 0xFFFFu, piece = e >> 16;
     const CellInfo &ci = S.cells[a];
     const int start = ci.start, N = ci.N, M = ci.M, pair_off = ci.pair_off;
-    const uint32_t cell = (uint32_t)ci.cell;
+    const uint32_t cell = (uint32_t)ci.cell + P.cell_base;
     const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
     const float4 pv = S.v[start];
     float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
@@ -286,7 +286,7 @@ __device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, 
   c.U_eps = 0.f;
   const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
   if (need_randoms || accept) {
-    const uint4 r = philox4x32_10((uint32_t)c.s, c.cell, P.step, 1u, P.seed_lo, P.seed_hi);
+    const uint4 r = philox4x32_10((uint32_t)c.s, c.cell + P.cell_base, P.step, 1u, P.seed_lo, P.seed_hi);
     c.U_b = u01(r.y);
     c.U_eps = u01(r.z);
     if (accept) {

@@ -120,7 +120,7 @@ __device__ __forceinline__ void pairs_mlp_fp32(const StepParams &P, const MlpDev
         if (P.op == 0) {  // VHS-NN features (eqs. 1-3, Q1-Q3)
           float n0 = 0.f, n1 = 0.f, n2 = 0.f;
           if (P.flags & DSMC_F_NOISE) {
-            const uint4 r = philox4x32_10((uint32_t)c.s, c.cell, P.step, 2u, P.seed_lo, P.seed_hi);
+            const uint4 r = philox4x32_10((uint32_t)c.s, c.cell + P.cell_base, P.step, 2u, P.seed_lo, P.seed_hi);
             box_muller3(r, n0, n1, n2);
             n0 *= P.noise_sigma; n1 *= P.noise_sigma; n2 *= P.noise_sigma;
           }

@@ -52,6 +52,7 @@ struct StepParams {
   float *vx, *vy, *vz;
   const float *cap;  // sigma_cr_max / cr_max or nullptr
   uint32_t seed_lo, seed_hi, step;
+  uint32_t cell_base;  // RNG cell coordinate of local cell 0
   uint32_t flags;
   int32_t pairs_per_cell;
   int32_t op;  // 0 = VHS-NN, 1 = ab initio table, 2 = ab initio MLP

@@ -45,12 +45,13 @@ class _VhsParams(C.Structure):
     _fields_ = [("mass", C.c_float), ("sigma_v", C.c_float), ("T_scale", C.c_float),
                 ("noise_sigma", C.c_float), ("shell_eps", C.c_float), ("d_ref", C.c_float),
                 ("omega", C.c_float), ("T_ref", C.c_float), ("pairs_per_cell", C.c_int32),
-                ("flags", C.c_uint32)]
+                ("flags", C.c_uint32), ("cell_base", C.c_int32)]
 
 
 class _AbiParams(C.Structure):
     _fields_ = [("mass", C.c_float), ("b_max", C.c_float), ("lnE_min", C.c_float), ("lnE_max", C.c_float),
-                ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32), ("flags", C.c_uint32)]
+                ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32), ("flags", C.c_uint32),
+                ("cell_base", C.c_int32)]
 
 
 class _PairDump(C.Structure):
@@ -103,10 +104,11 @@ class VhsParams:
     T_ref: float = 273.0
     pairs_per_cell: int = -1
     flags: int = F_NOISE | F_ENERGY_SHELL | F_MOMENT_MATCH
+    cell_base: int = 0
 
     def c(self):
         return _VhsParams(self.mass, self.sigma_v, self.T_scale, self.noise_sigma, self.shell_eps, self.d_ref,
-                          self.omega, self.T_ref, self.pairs_per_cell, self.flags)
+                          self.omega, self.T_ref, self.pairs_per_cell, self.flags, self.cell_base)
 
 
 @dataclass
@@ -118,10 +120,11 @@ class AbinitioParams:
     chi_mode: int = 0
     pairs_per_cell: int = -1
     flags: int = F_MOMENT_MATCH
+    cell_base: int = 0
 
     def c(self):
         return _AbiParams(self.mass, self.b_max, self.lnE_min, self.lnE_max, self.chi_mode, self.pairs_per_cell,
-                          self.flags)
+                          self.flags, self.cell_base)
 
 
 class PairDump:

@@ -459,3 +459,34 @@ def test_collide_vhs_nn_bf16_tc(dsmc, case):
         assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
         assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
     ctx.close()
+
+
+# --------------------------------------------------------------------------------------- (e) sharding
+@pytest.mark.parametrize("tc", [False, True])
+def test_sharded_step_matches_unsharded(dsmc, tc):
+    """Two cell-range shards run one after the other on this GPU (independent launches, no rank waits on
+    another) give bit-identical velocities to the unsharded step: RNG is keyed by the GLOBAL cell id."""
+    from paper_2602_21244_b200 import sharding
+    pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    tab = _lj_table(64, 64)
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if tc else 0)
+    full = [t.clone() for t in (vx_s, vy_s, vz_s)]
+    ctx.collide_abinitio(cs, *full, dsmc.AbinitioParams(chi_mode=1 if tc else 0, flags=flags), seed=9, step=2)
+    ctx.check()
+    bounds = sharding.partition_cells(np.diff(cs_h), 2)
+    host = [t.cpu().numpy() for t in (vx_s, vy_s, vz_s)]
+    for rank in range(2):
+        c0, lcs, lv = sharding.shard_sorted(cs_h, host, bounds, rank)
+        lt = [dev(a) for a in lv]
+        ctx.collide_abinitio(dev(lcs), *lt, dsmc.AbinitioParams(chi_mode=1 if tc else 0, flags=flags, cell_base=c0), seed=9, step=2)
+        ctx.check()
+        q0 = int(cs_h[bounds[rank]])
+        for a, b in zip(lt, full):
+            assert torch.equal(a, b[q0:q0 + a.shape[0]])
+    ctx.close()
