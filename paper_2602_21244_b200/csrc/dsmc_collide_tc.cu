@@ -11,6 +11,7 @@
 
 #include "dsmc_chunk.cuh"
 #include "dsmc_tc.cuh"
+#include "dsmc_tc_pipe.cuh"
 
 namespace dsmc {
 
@@ -292,61 +293,98 @@ __device__ __forceinline__ unsigned char *align128(unsigned char *p) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// a10: chi for independent pairs, chi = expm1(softplus(z)) = exp(z) (Q15), z = MLP(E~_n, b~)
+// a10: chi for independent pairs, chi = expm1(softplus(z)) = exp(z) (Q15), z = MLP(E~_n, b~).
+// Persistent, warp-specialised (dsmc_tc_pipe.cuh): the k-th tile of a CTA goes through slot k & 1.
 // ---------------------------------------------------------------------------------------------
 template <int H>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kPipeThreads, 1)
     k_chi_batch_tc(int64_t n, const float *__restrict__ E, const float *__restrict__ b, float *__restrict__ chi,
                    const MlpTcDev net, float inv_bmax, float lnE_min, float inv_range) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  TcEngine<H, false> eng;
-  eng.init(align128(smem_raw), net.w_blob);
-  const int tid = threadIdx.x;
+  TcPipe<H> pipe;
+  pipe.init(align128(smem_raw), net.w_blob, kPipeActWarps, kPipeIoWarps);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n_tiles = (n + 127) / 128;
-  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const int64_t p = tile * 128 + tid;
-    if (tid < 128) {
+  const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const int64_t n_rounds = (mine + 1) / 2;  // two slots per round; a missing second tile runs as zeros
+  if (warp < kPipeActWarps) {
+    for (int64_t r = 0; r < n_rounds; ++r) {
+#pragma unroll 1
+      for (int layer = 0; layer < 2; ++layer) {
+        pipe.act_tile(net.act, 0, warp);
+        pipe.act_tile(net.act, 1, warp);
+      }
+    }
+  } else if (warp < kPipeActWarps + kPipeIoWarps) {
+    const int io_warp = warp - kPipeActWarps, row = io_warp * 32 + lane;
+    auto features = [&](int s, int64_t k) {  // tile k of this CTA -> layer-1 operand buffer (s, (k >> 1) & 1)
+      const int64_t p = (blockIdx.x + k * gridDim.x) * 128 + row;
       float x[8];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) x[k] = 0.f;
-      if (p < n) {
-        const float e = (logf(__ldg(E + p)) - lnE_min) * inv_range;
+      for (int j = 0; j < 8; ++j) x[j] = 0.f;
+      if (k < mine && p < n) {
+        const float e = (__logf(__ldg(E + p)) - lnE_min) * inv_range;
         x[0] = !(e > 0.f) ? 0.f : fminf(e, 1.f);
         const float bt = __ldg(b + p) * inv_bmax;
         x[1] = !(bt > 0.f) ? 0.f : fminf(bt, 1.f);
       }
-      eng.write_a1_row(tid, x);
+      pipe.write_a1_row(s, (int)((k >> 1) & 1), row, x);
+      pipe.io_publish(s);
+    };
+    if (n_rounds > 0) {
+      features(0, 0);
+      features(1, 1);
     }
-    eng.run(net.act);
-    if (tid < 128) {
-      float y[4];
-      eng.read_out(y);
-      if (p < n) chi[p] = __expf(y[0]);
+    for (int64_t r = 0; r < n_rounds; ++r) {
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {
+        const int64_t k = 2 * r + s;
+        if (r + 1 < n_rounds) features(s, k + 2);  // a round ahead: off the critical path
+        float y[4];
+        pipe.io_read_out(s, io_warp, y);
+        const int64_t p = (blockIdx.x + k * gridDim.x) * 128 + row;
+        if (k < mine && p < n) chi[p] = __expf(y[0]);
+      }
     }
-    tc::fence_before();
+  } else {
+    // issue order keeps one layer of the other slot between a slot's consecutive layers, and the next
+    // tile's layer 1 ahead of the other slot's layer 3
+    if (n_rounds > 0) {
+      pipe.mma_layer1(0, 0, true);
+      pipe.mma_layer1(1, 0, false);
+    }
+    for (int64_t r = 0; r < n_rounds; ++r) {
+      const bool more = r + 1 < n_rounds;
+      const int par = (int)((r + 1) & 1);
+      pipe.mma_layer2(0);
+      pipe.mma_layer2(1);
+      pipe.mma_layer3(0, r == 0);
+      if (more) pipe.mma_layer1(0, par, false);
+      pipe.mma_layer3(1, r == 0);
+      if (more) pipe.mma_layer1(1, par, false);
+    }
   }
-  eng.teardown();
+  pipe.teardown();
+}
+
+template <int H>
+static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
+                                 float lnE_min, float lnE_max, const MlpTcDev *net) {
+  const float inv_range = 1.0f / (lnE_max - lnE_min);
+  const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms);
+  const int smem = PipeShape<H>::SMEM_BYTES + 128;
+  if (cudaFuncSetAttribute(k_chi_batch_tc<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+    return DSMC_ERR_CUDA;
+  k_chi_batch_tc<H><<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, 1.0f / b_max, lnE_min, inv_range);
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
 
 int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
                         float lnE_min, float lnE_max, const MlpTcDev *net) {
   if (net->d_in != 2 || net->d_out != 1) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  const float inv_range = 1.0f / (lnE_max - lnE_min);
-  const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms * 2);
-  cudaError_t e;
-  if (net->H == 128) {
-    const int smem = TcShape<128, false>::SMEM_BYTES + 128;
-    e = cudaFuncSetAttribute(k_chi_batch_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return DSMC_ERR_CUDA;
-    k_chi_batch_tc<128><<<grid, kThreads, smem, c->stream>>>(n, E, b, chi, *net, 1.0f / b_max, lnE_min, inv_range);
-  } else {
-    const int smem = TcShape<64, false>::SMEM_BYTES + 128;
-    e = cudaFuncSetAttribute(k_chi_batch_tc<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return DSMC_ERR_CUDA;
-    k_chi_batch_tc<64><<<grid, kThreads, smem, c->stream>>>(n, E, b, chi, *net, 1.0f / b_max, lnE_min, inv_range);
-  }
-  c->launches += 1;
-  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+  return net->H == 128 ? launch_chi_batch_tc_h<128>(c, n, E, b, chi, b_max, lnE_min, lnE_max, net)
+                       : launch_chi_batch_tc_h<64>(c, n, E, b, chi, b_max, lnE_min, lnE_max, net);
 }
 
 // ---------------------------------------------------------------------------------------------
