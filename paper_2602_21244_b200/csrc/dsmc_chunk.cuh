@@ -71,10 +71,20 @@ struct Chunk {
   }
 };
 
-// Exclusive scan of a[0..L) in shared memory by the whole CTA; coalesced (conflict-free) sweeps.
+// A team = the kThreads threads that own one chunk: the whole CTA (bar 0) in the one-chunk-per-CTA
+// kernels, or one of several 256-thread groups of a warp-specialised CTA (named barrier bar > 0).
+struct Team {
+  int tid;  // 0 .. kThreads-1 within the team
+  int bar;  // hardware barrier id
+  __device__ __forceinline__ void sync() const {
+    asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(kThreads) : "memory");
+  }
+};
+
+// Exclusive scan of a[0..L) in shared memory by the whole team; coalesced (conflict-free) sweeps.
 // `scratch` holds >= 2*kWarps ints.  Ends with __syncthreads().
-__device__ __forceinline__ void block_excl_scan_coalesced(int *a, int L, int *scratch) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__device__ __forceinline__ void block_excl_scan_coalesced(const Team &T, int *a, int L, int *scratch) {
+  const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   const int span = ((L + kWarps * 32 - 1) / (kWarps * 32)) * 32;  // per warp, multiple of 32
   const int lo = min(warp * span, L), hi = min(lo + span, L);
   int carry = 0;
@@ -91,13 +101,13 @@ __device__ __forceinline__ void block_excl_scan_coalesced(int *a, int L, int *sc
     carry += __shfl_sync(0xffffffffu, inc, 31);
   }
   if (lane == 0) scratch[warp] = carry;
-  __syncthreads();
+  T.sync();
   int off = 0;
 #pragma unroll
   for (int w = 0; w < kWarps; ++w) off += (w < warp) ? scratch[w] : 0;
   if (off != 0)
     for (int i = lo + lane; i < hi; i += 32) a[i] += off;
-  __syncthreads();
+  T.sync();
 }
 
 __device__ __forceinline__ float warp_sum_f(float v) {
@@ -111,8 +121,8 @@ __device__ __forceinline__ float warp_sum_f(float v) {
 // to store either), -1 when the chunk does not fit this variant (caller defers it).
 // ---------------------------------------------------------------------------------------------
 template <class CK>
-__device__ int chunk_begin(const StepParams &P, CK &S, int chunk, int &q0_out) {
-  const int tid = threadIdx.x;
+__device__ int chunk_begin(const Team &T, const StepParams &P, CK &S, int chunk, int &q0_out) {
+  const int tid = T.tid;
   const int c_lo = __ldg(P.chunk_first + chunk);
   const int c_hi = (chunk + 1 < P.n_chunks) ? __ldg(P.chunk_first + chunk + 1) : P.n_cells;
   if (c_lo >= c_hi) return 0;
@@ -123,7 +133,7 @@ __device__ int chunk_begin(const StepParams &P, CK &S, int chunk, int &q0_out) {
   if (n_loc > CK::LMAX) return -1;
   for (int q = tid; q < n_loc; q += kThreads) S.cnt[q] = 0;
   if (tid < 8) S.misc[tid] = 0;
-  __syncthreads();
+  T.sync();
   // cell discovery (order of the active list is irrelevant to the results)
   for (int c = c_lo + tid; c < c_hi; c += kThreads) {
     const int gs = __ldg(P.cell_start + c), N = __ldg(P.cell_start + c + 1) - gs;
@@ -153,7 +163,7 @@ __device__ int chunk_begin(const StepParams &P, CK &S, int chunk, int &q0_out) {
     S.v[q] = make_float4(P.vx[q0 + q], P.vy[q0 + q], P.vz[q0 + q], 0.f);
     S.lc[q] = 0xFFFFu;
   }
-  __syncthreads();
+  T.sync();
   if (S.misc[MI_NACT] > CK::AMAX) return -1;
   if (S.misc[MI_NACT] == 0) return 0;
   return n_loc;
@@ -161,8 +171,8 @@ __device__ int chunk_begin(const StepParams &P, CK &S, int chunk, int &q0_out) {
 
 // pre-collision segment sums + pairing keys + bucket counts; then cell finalisation + sort
 template <class CK>
-__device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, int n_loc) {
+  const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
   for (int sg = warp; sg < n_seg; sg += kWarps) {
     const uint32_t e = S.segs[sg];
@@ -200,7 +210,7 @@ __device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
       if (s + 1 < M) S.pairs[pair_off + s + 1] = (uint32_t)(start + p + 2) | ((uint32_t)a << 16);
     }
   }
-  __syncthreads();
+  T.sync();
   // cell finalisation: u = pivot + mean(d), Theta = sum d^2 - N |mean(d)|^2   (eq. 10)
   for (int a = tid; a < n_act; a += kThreads) {
     CellInfo &ci = S.cells[a];
@@ -218,7 +228,7 @@ __device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
     ci.uz = (float)((double)pv.z + dz);
     ci.theta = (float)(s2 - N * (dx * dx + dy * dy + dz * dz));
   }
-  block_excl_scan_coalesced(S.cnt, n_loc, S.misc + MI_SCAN);
+  block_excl_scan_coalesced(T, S.cnt, n_loc, S.misc + MI_SCAN);
   // placement: cnt[bucket] ends as the bucket's end position
   for (int q = tid; q < n_loc; q += kThreads) {
     const int a = S.lc[q];
@@ -230,7 +240,7 @@ __device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
     const int bkt = ci.start + (int)__umulhi(S.key[q], (uint32_t)ci.N);
     S.ord[atomicAdd(&S.cnt[bkt], 1)] = (uint16_t)q;
   }
-  __syncthreads();
+  T.sync();
   // in-bucket ranking by (key, slot): buckets hold ~1 particle on average
   for (int q = tid; q < n_loc; q += kThreads) {
     const int a = S.lc[q];
@@ -248,7 +258,7 @@ __device__ void chunk_pre_and_sort(const StepParams &P, CK &S, int n_loc) {
     }
     S.pi[b0 + rank] = (uint16_t)q;
   }
-  __syncthreads();
+  T.sync();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -367,8 +377,8 @@ __device__ __forceinline__ float chi_table_t(const ChiTableDev &T, float tE, flo
 // finish: post-collision sums, matching coefficients, single coalesced store
 // ---------------------------------------------------------------------------------------------
 template <class CK>
-__device__ void chunk_finish(const StepParams &P, CK &S, int n_loc, int q0) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__device__ void chunk_finish(const Team &T, const StepParams &P, CK &S, int n_loc, int q0) {
+  const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
   if (P.flags & DSMC_F_MOMENT_MATCH) {
     for (int sg = warp; sg < n_seg; sg += kWarps) {
@@ -388,7 +398,7 @@ __device__ void chunk_finish(const StepParams &P, CK &S, int n_loc, int q0) {
       sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
       if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
     }
-    __syncthreads();
+    T.sync();
     for (int a = tid; a < n_act; a += kThreads) {
       CellInfo &ci = S.cells[a];
       double alpha = 1.0, bx = 0.0, by = 0.0, bz = 0.0;
@@ -417,7 +427,7 @@ __device__ void chunk_finish(const StepParams &P, CK &S, int n_loc, int q0) {
       }
       ci.ux = (float)bx; ci.uy = (float)by; ci.uz = (float)bz; ci.theta = (float)alpha;
     }
-    __syncthreads();
+    T.sync();
     for (int q = tid; q < n_loc; q += kThreads) {
       const int a = S.lc[q];
       float4 v = S.v[q];

@@ -178,8 +178,9 @@ __device__ __forceinline__ void pairs_mlp_fp32(const StepParams &P, const MlpDev
 template <class CK, bool OP_TABLE, int TP>
 __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev &net, CK &S, float *mlp, int chunk,
                                               bool deferred) {
+  const Team T{(int)threadIdx.x, 0};
   int q0 = 0;
-  const int n_loc = chunk_begin(P, S, chunk, q0);
+  const int n_loc = chunk_begin(T, P, S, chunk, q0);
   if (n_loc == 0) return;
   if (n_loc < 0) {
     if (threadIdx.x == 0) {
@@ -192,14 +193,14 @@ __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev 
     }
     return;
   }
-  chunk_pre_and_sort(P, S, n_loc);
+  chunk_pre_and_sort(T, P, S, n_loc);
   if (OP_TABLE) {
     pairs_table(P, S, q0);
   } else {
     pairs_mlp_fp32<TP>(P, net, S, mlp, q0);
   }
   __syncthreads();
-  chunk_finish(P, S, n_loc, q0);
+  chunk_finish(T, P, S, n_loc, q0);
 }
 
 template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB>

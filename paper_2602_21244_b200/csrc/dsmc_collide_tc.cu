@@ -475,8 +475,9 @@ __global__ void __launch_bounds__(kThreads, MINB) k_collide_tc(const StepParams 
     __syncthreads();
     if (w >= n_work) break;
     const int chunk = DEFERRED ? P.big[1 + w] : w;
+    const Team T{(int)threadIdx.x, 0};
     int q0 = 0;
-    const int n_loc = chunk_begin(P, S, chunk, q0);
+    const int n_loc = chunk_begin(T, P, S, chunk, q0);
     if (n_loc == 0) continue;
     if (n_loc < 0) {
       if (threadIdx.x == 0) {
@@ -489,10 +490,10 @@ __global__ void __launch_bounds__(kThreads, MINB) k_collide_tc(const StepParams 
       }
       continue;
     }
-    chunk_pre_and_sort(P, S, n_loc);
+    chunk_pre_and_sort(T, P, S, n_loc);
     pairs_tc<H, SPLIT>(P, net, S, eng, q0);
     __syncthreads();
-    chunk_finish(P, S, n_loc, q0);
+    chunk_finish(T, P, S, n_loc, q0);
     __syncthreads();
   }
   eng.teardown();

@@ -187,19 +187,18 @@ struct TcPipe {
     mma_hidden<16>(s, SH::OFF_W3, SH::OFF_B3, full_o + s, SH::COL_OUT, !first);
   }
 
-  // ---- ACT warps: act_warp in [0, 16): lane quadrant act_warp & 3, column quarter act_warp >> 2 ---
-  template <int ACT>
-  __device__ __forceinline__ void act_tile(int s, int act_warp) {
-    tc::mbar_wait(full_e + s, ph_e[s]);
-    ph_e[s] ^= 1u;
+  // ---- ACT warps: lane quadrant act_warp & 3, column group act_warp >> 2 of NQ groups -----------
+  // act_body: one (slot, layer) share of this warp; the caller has observed full_e[s]
+  template <int ACT, int NQ>
+  __device__ __forceinline__ void act_body(int s, int act_warp) {
     tc::fence_after();
     const uint32_t base = tmem + (((uint32_t)((act_warp & 3) * 32)) << 16) + s * SH::SLOT_COLS;
-    const int quarter = act_warp >> 2;
+    const int grp = act_warp >> 2;
     // software pipeline over 16-column chunks: the TMEM read port (64 B / clk / SM) and the XU pipe
     // (16 MUFU / clk / SM) are both needed ~1024 cycles per tile layer, so chunk c + 1 is in flight
     // while chunk c goes through the activation
-    constexpr int NC = H / 64;  // 16-column chunks per thread
-    const uint32_t d0 = base + SH::COL_D + quarter * (H / 4), a0 = base + SH::COL_A + quarter * (H / 8);
+    constexpr int NC = H / (16 * NQ);  // 16-column chunks per thread
+    const uint32_t d0 = base + SH::COL_D + grp * (H / NQ), a0 = base + SH::COL_A + grp * (H / (2 * NQ));
     uint32_t v[2][16];
     tc::tmem_ld16(d0, v[0]);
 #pragma unroll
@@ -229,10 +228,17 @@ struct TcPipe {
     tc::fence_before();
     warp_arrive(a_ready + s);
   }
+  template <int NQ>
+  __device__ __forceinline__ void act_body(int act, int s, int act_warp) {
+    if (act == DSMC_ACT_TANH) act_body<DSMC_ACT_TANH, NQ>(s, act_warp);
+    else if (act == DSMC_ACT_RELU) act_body<DSMC_ACT_RELU, NQ>(s, act_warp);
+    else act_body<DSMC_ACT_SILU, NQ>(s, act_warp);
+  }
+  // blocking form used by the fixed-schedule kernel (k_chi_batch_tc)
   __device__ __forceinline__ void act_tile(int act, int s, int act_warp) {
-    if (act == DSMC_ACT_TANH) act_tile<DSMC_ACT_TANH>(s, act_warp);
-    else if (act == DSMC_ACT_RELU) act_tile<DSMC_ACT_RELU>(s, act_warp);
-    else act_tile<DSMC_ACT_SILU>(s, act_warp);
+    tc::mbar_wait(full_e + s, ph_e[s]);
+    ph_e[s] ^= 1u;
+    act_body<kPipeActWarps / 4>(act, s, act_warp);
   }
 };
 
