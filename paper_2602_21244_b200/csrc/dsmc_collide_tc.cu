@@ -302,7 +302,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
                    const MlpTcDev net, float inv_bmax, float lnE_min, float inv_range) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TcPipe<H> pipe;
-  pipe.init(align128(smem_raw), net.w_blob, kPipeActWarps, kPipeIoWarps);
+  pipe.init(smem_raw, net.w_blob, kPipeActWarps, kPipeIoWarps);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n_tiles = (n + 127) / 128;
   const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -522,6 +522,7 @@ static int launch_tc_pair(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
   if (p_in.op == 0 && !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3)) return DSMC_ERR_UNSUPPORTED_SHAPE;
   if (p_in.op == 2 && !(net->d_in == 2 && net->d_out == 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  if (p_in.op == 2) return launch_collide_pipe(c, p_in, net);  // plain BF16: warp-specialised kernel
   StepParams p = p_in;
   int rc = launch_chunk_map(c, p);
   if (rc != DSMC_OK) return rc;

@@ -187,6 +187,39 @@ struct TcPipe {
     mma_hidden<16>(s, SH::OFF_W3, SH::OFF_B3, full_o + s, SH::COL_OUT, !first);
   }
 
+  // ---- non-blocking issue (polling MMA warp of the fused kernel; whole warp calls, operand known ready) ----
+  __device__ __forceinline__ void issue_layer1(int s, bool first) {
+    if ((threadIdx.x & 31) == 0) {
+      if (first) tc::mbar_wait(bar_w, 0);
+      tc::fence_after();
+      constexpr uint32_t idH = tc::instr_desc(128, H);
+      const uint32_t a1a = tc::smem_u32(a1 + 2 * s * SH::A1_BYTES), wa = tc::smem_u32(w);
+#pragma unroll
+      for (int ks = 0; ks < SH::K1 / 16; ++ks)
+        tc::mma_ss(tmem + s * SH::SLOT_COLS + SH::COL_D, tc::smem_desc(a1a + ks * 2 * 128 * 16, 128 * 16, 128),
+                   tc::smem_desc(wa + ks * 2 * H * 16, H * 16, 128), idH, ks > 0 ? 1u : 0u);
+      tc::mma_commit(full_e + s);
+    }
+    __syncwarp();
+  }
+  template <int N>
+  __device__ __forceinline__ void issue_hidden(int s, uint32_t off_w, uint32_t off_b, uint64_t *done, uint32_t col_d) {
+    if ((threadIdx.x & 31) == 0) {
+      tc::fence_after();
+      constexpr uint32_t idesc = tc::instr_desc(128, N);
+      const uint32_t tD = tmem + s * SH::SLOT_COLS + col_d, tA = tmem + s * SH::SLOT_COLS + SH::COL_A;
+      const uint32_t wa = tc::smem_u32(w);
+#pragma unroll
+      for (int ks = 0; ks < H / 16; ++ks)
+        tc::mma_ts(tD, tA + ks * 8, tc::smem_desc(wa + off_w + ks * 2 * N * 16, N * 16, 128), idesc, ks > 0 ? 1u : 0u);
+      tc::mma_ts(tD, tmem + s * SH::SLOT_COLS + SH::COL_BIAS, tc::smem_desc(wa + off_b, N * 16, 128), idesc, 1u);
+      tc::mma_commit(done);
+    }
+    __syncwarp();
+  }
+  __device__ __forceinline__ void issue_layer2(int s) { issue_hidden<H>(s, SH::OFF_W2, SH::OFF_B2, full_e + s, SH::COL_D); }
+  __device__ __forceinline__ void issue_layer3(int s) { issue_hidden<16>(s, SH::OFF_W3, SH::OFF_B3, full_o + s, SH::COL_OUT); }
+
   // ---- ACT warps: lane quadrant act_warp & 3, column group act_warp >> 2 of NQ groups -----------
   // act_body: one (slot, layer) share of this warp; the caller has observed full_e[s]
   template <int ACT, int NQ>
