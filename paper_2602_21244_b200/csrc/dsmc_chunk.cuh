@@ -22,7 +22,7 @@
 
 namespace dsmc {
 
-constexpr int kSeg = 256;  // particles per segment (multiple of 4: Philox blocks never straddle)
+constexpr int kSeg = 128;  // particles per segment = one warp pass of 32 Philox blocks (measured: 256 leaves warps idle, 64 half-fills the key loop)
 constexpr int kWarps = kThreads / 32;
 
 struct __align__(16) CellInfo {
@@ -49,11 +49,11 @@ struct Chunk {
   uint32_t *pairs;  // [LMAX / 2] position of the pair's first member | active cell << 16
   uint32_t *segs;   // [SMAX] active cell | piece << 16
   int *misc;        // [64]
-  uint16_t *ord, *pi, *lc;  // [LMAX]
+  uint16_t *ord, *pi;  // [LMAX]
 
   static constexpr size_t bytes() {
     return sizeof(float4) * LMAX + sizeof(float4) * SMAX + sizeof(CellInfo) * AMAX + 4 * LMAX + 4 * (LMAX + 4) +
-           4 * (LMAX / 2) + 4 * SMAX + 4 * 64 + 2 * 3 * LMAX + 16;
+           4 * (LMAX / 2) + 4 * SMAX + 4 * 64 + 2 * 2 * LMAX + 16;
   }
   __device__ __forceinline__ unsigned char *carve(unsigned char *base) {
     v = reinterpret_cast<float4 *>(base);
@@ -66,8 +66,7 @@ struct Chunk {
     misc = reinterpret_cast<int *>(segs + SMAX);
     ord = reinterpret_cast<uint16_t *>(misc + 64);
     pi = ord + LMAX;
-    lc = pi + LMAX;
-    return reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(lc + LMAX) + 15) & ~(uintptr_t)15);
+    return reinterpret_cast<unsigned char *>(pi + LMAX);
   }
 };
 
@@ -81,33 +80,43 @@ struct Team {
   }
 };
 
-// Exclusive scan of a[0..L) in shared memory by the whole team; coalesced (conflict-free) sweeps.
-// `scratch` holds >= 2*kWarps ints.  Ends with __syncthreads().
+// Exclusive scan of a[0..L) in shared memory by the whole team.  a is 16-byte aligned and has room for
+// L rounded up to 4.  Each thread owns one int4 per 1024-element pass (conflict-free 16 B accesses),
+// scans it in registers, warp totals go through one shuffle scan.  `scratch` holds >= kWarps + 1 ints.
+// Ends with T.sync().
 __device__ __forceinline__ void block_excl_scan_coalesced(const Team &T, int *a, int L, int *scratch) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
-  const int span = ((L + kWarps * 32 - 1) / (kWarps * 32)) * 32;  // per warp, multiple of 32
-  const int lo = min(warp * span, L), hi = min(lo + span, L);
   int carry = 0;
-  for (int base = lo; base < hi; base += 32) {
-    const int i = base + lane;
-    const int x = i < hi ? a[i] : 0;
-    int inc = x;
+  for (int base = 0; base < L; base += 4 * kThreads) {
+    const int i = base + 4 * tid;
+    int4 x = make_int4(0, 0, 0, 0);
+    if (i < L) {
+      x = *reinterpret_cast<const int4 *>(a + i);
+      if (i + 1 >= L) x.y = 0;
+      if (i + 2 >= L) x.z = 0;
+      if (i + 3 >= L) x.w = 0;
+    }
+    const int s1 = x.x + x.y, s2 = s1 + x.z, tot = s2 + x.w;
+    int inc = tot;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const int t = __shfl_up_sync(0xffffffffu, inc, o);
       if (lane >= o) inc += t;
     }
-    if (i < hi) a[i] = carry + inc - x;
-    carry += __shfl_sync(0xffffffffu, inc, 31);
-  }
-  if (lane == 0) scratch[warp] = carry;
-  T.sync();
-  int off = 0;
+    if (lane == 31) scratch[warp] = inc;
+    T.sync();
+    int off = carry, all = 0;
 #pragma unroll
-  for (int w = 0; w < kWarps; ++w) off += (w < warp) ? scratch[w] : 0;
-  if (off != 0)
-    for (int i = lo + lane; i < hi; i += 32) a[i] += off;
-  T.sync();
+    for (int w = 0; w < kWarps; ++w) {
+      const int sw = scratch[w];
+      off += (w < warp) ? sw : 0;
+      all += sw;
+    }
+    const int e0 = off + inc - tot;  // exclusive prefix of x.x
+    if (i < L) *reinterpret_cast<int4 *>(a + i) = make_int4(e0, e0 + x.x, e0 + s1, e0 + s2);
+    carry += all;
+    T.sync();
+  }
 }
 
 __device__ __forceinline__ float warp_sum_f(float v) {
@@ -161,7 +170,6 @@ __device__ int chunk_begin(const Team &T, const StepParams &P, CK &S, int chunk,
   // one coalesced read of the chunk
   for (int q = tid; q < n_loc; q += kThreads) {
     S.v[q] = make_float4(P.vx[q0 + q], P.vy[q0 + q], P.vz[q0 + q], 0.f);
-    S.lc[q] = 0xFFFFu;
   }
   T.sync();
   if (S.misc[MI_NACT] > CK::AMAX) return -1;
@@ -188,7 +196,6 @@ __device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, in
       const float dx = v.x - pv.x, dy = v.y - pv.y, dz = v.z - pv.z;
       sx += dx; sy += dy; sz += dz;
       s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
-      S.lc[q] = (uint16_t)a;
     }
     sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
     if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
@@ -229,34 +236,40 @@ __device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, in
     ci.theta = (float)(s2 - N * (dx * dx + dy * dy + dz * dz));
   }
   block_excl_scan_coalesced(T, S.cnt, n_loc, S.misc + MI_SCAN);
-  // placement: cnt[bucket] ends as the bucket's end position
-  for (int q = tid; q < n_loc; q += kThreads) {
-    const int a = S.lc[q];
-    if (a == 0xFFFF) {
-      S.cnt[q] += 1;
-      continue;
+  // placement, one warp per segment (cell constants in registers): cnt[bucket] ends as the bucket's end
+  for (int sg = warp; sg < n_seg; sg += kWarps) {
+    const uint32_t e = S.segs[sg];
+    const CellInfo &ci = S.cells[e & 0xFFFFu];
+    const int start = ci.start, N = ci.N, piece = e >> 16;
+    const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
+    for (int q = lo + lane; q < hi; q += 32) {
+      const int bkt = start + (int)__umulhi(S.key[q], (uint32_t)N);
+      S.ord[atomicAdd(&S.cnt[bkt], 1)] = (uint16_t)q;
     }
-    const CellInfo &ci = S.cells[a];
-    const int bkt = ci.start + (int)__umulhi(S.key[q], (uint32_t)ci.N);
-    S.ord[atomicAdd(&S.cnt[bkt], 1)] = (uint16_t)q;
   }
   T.sync();
-  // in-bucket ranking by (key, slot): buckets hold ~1 particle on average
-  for (int q = tid; q < n_loc; q += kThreads) {
-    const int a = S.lc[q];
-    if (a == 0xFFFF) continue;
-    const CellInfo &ci = S.cells[a];
-    const uint32_t k = S.key[q];
-    const int bkt = ci.start + (int)__umulhi(k, (uint32_t)ci.N);
-    const int b0 = bkt > 0 ? S.cnt[bkt - 1] : 0, b1 = S.cnt[bkt];
-    int rank = 0;
+  // in-bucket ranking by (key, slot): buckets hold ~1 particle on average.  The first bucket of a cell
+  // begins at the cell's first slot, every other one where the previous bucket ends.
+  for (int sg = warp; sg < n_seg; sg += kWarps) {
+    const uint32_t e = S.segs[sg];
+    const CellInfo &ci = S.cells[e & 0xFFFFu];
+    const int start = ci.start, N = ci.N, piece = e >> 16;
+    const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
+    for (int q = lo + lane; q < hi; q += 32) {
+      const uint32_t k = S.key[q];
+      const int bkt = start + (int)__umulhi(k, (uint32_t)N);
+      const int b0 = bkt > start ? S.cnt[bkt - 1] : start, b1 = S.cnt[bkt];
+      int rank = 0;
+      if (b1 - b0 > 1) {
 #pragma unroll 1
-    for (int t = b0; t < b1; ++t) {
-      const int o = S.ord[t];
-      const uint32_t ko = S.key[o];
-      rank += (ko < k || (ko == k && o < q)) ? 1 : 0;
+        for (int t = b0; t < b1; ++t) {
+          const int o = S.ord[t];
+          const uint32_t ko = S.key[o];
+          rank += (ko < k || (ko == k && o < q)) ? 1 : 0;
+        }
+      }
+      S.pi[b0 + rank] = (uint16_t)q;
     }
-    S.pi[b0 + rank] = (uint16_t)q;
   }
   T.sync();
 }
@@ -428,25 +441,35 @@ __device__ void chunk_finish(const Team &T, const StepParams &P, CK &S, int n_lo
       ci.ux = (float)bx; ci.uy = (float)by; ci.uz = (float)bz; ci.theta = (float)alpha;
     }
     T.sync();
-    for (int q = tid; q < n_loc; q += kThreads) {
-      const int a = S.lc[q];
-      float4 v = S.v[q];
-      if (a != 0xFFFF) {
-        const float4 co = *reinterpret_cast<const float4 *>(&S.cells[a]);
-        v.x = fmaf(co.w, v.x, co.x);
-        v.y = fmaf(co.w, v.y, co.y);
-        v.z = fmaf(co.w, v.z, co.z);
+    // store, one warp per segment: v <- alpha v + B with the cell's coefficients in registers.  Cells in
+    // which nothing collided (and particles of cells with N < 2) are unchanged and not written.
+    for (int sg = warp; sg < n_seg; sg += kWarps) {
+      const uint32_t e = S.segs[sg];
+      const CellInfo &ci = S.cells[e & 0xFFFFu];
+      if (!ci.collided) continue;
+      const float4 co = *reinterpret_cast<const float4 *>(&ci);
+      const int piece = e >> 16;
+      const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
+      for (int q = lo + lane; q < hi; q += 32) {
+        const float4 v = S.v[q];
+        P.vx[q0 + q] = fmaf(co.w, v.x, co.x);
+        P.vy[q0 + q] = fmaf(co.w, v.y, co.y);
+        P.vz[q0 + q] = fmaf(co.w, v.z, co.z);
       }
-      P.vx[q0 + q] = v.x;
-      P.vy[q0 + q] = v.y;
-      P.vz[q0 + q] = v.z;
     }
   } else {
-    for (int q = tid; q < n_loc; q += kThreads) {
-      const float4 v = S.v[q];
-      P.vx[q0 + q] = v.x;
-      P.vy[q0 + q] = v.y;
-      P.vz[q0 + q] = v.z;
+    for (int sg = warp; sg < n_seg; sg += kWarps) {
+      const uint32_t e = S.segs[sg];
+      const CellInfo &ci = S.cells[e & 0xFFFFu];
+      if (!ci.collided) continue;
+      const int piece = e >> 16;
+      const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
+      for (int q = lo + lane; q < hi; q += 32) {
+        const float4 v = S.v[q];
+        P.vx[q0 + q] = v.x;
+        P.vy[q0 + q] = v.y;
+        P.vz[q0 + q] = v.z;
+      }
     }
   }
 }

@@ -248,7 +248,7 @@ int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {
   MlpDev nd{};
   const int big_grid = c->num_sms;
   if (p.op == 1) {
-    rc = launch_one<kLmaxSmall, kAmaxSmall, true, 64, false, 4>(c, p, nd, p.n_chunks, 0);
+    rc = launch_one<1024, kAmaxSmall, true, 64, false, 5>(c, p, nd, p.n_chunks, 0);
     if (rc != DSMC_OK) return rc;
     return launch_one<kLmaxBig, kAmaxBig, true, 64, true, 1>(c, p, nd, big_grid, 0);
   }
