@@ -40,7 +40,7 @@ enum { MI_NACT = 0, MI_NSEG = 1, MI_NPAIRS = 2, MI_SCAN = 8 /* .. +40 */ };
 template <int LMAX_, int AMAX_>
 struct Chunk {
   static constexpr int LMAX = LMAX_, AMAX = AMAX_;
-  static constexpr int SMAX = LMAX / kSeg + AMAX + 2;
+  static constexpr int SMAX = (LMAX / kSeg + AMAX + 2 + 3) & ~3;  // multiple of 4: keeps every array 16-byte aligned
   float4 *v;        // [LMAX] velocities (x, y, z, unused)
   float4 *part;     // [SMAX] segment partial sums
   CellInfo *cells;  // [AMAX]
@@ -66,6 +66,7 @@ struct Chunk {
     misc = reinterpret_cast<int *>(segs + SMAX);
     ord = reinterpret_cast<uint16_t *>(misc + 64);
     pi = ord + LMAX;
+    static_assert(LMAX % 8 == 0 && (sizeof(CellInfo) * AMAX) % 16 == 0, "chunk arrays must stay 16-byte aligned");
     return reinterpret_cast<unsigned char *>(pi + LMAX);
   }
 };
