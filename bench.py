@@ -52,6 +52,15 @@ def peaks():
     return 6650.0, 1590.0, 1400.0, "fallback"
 
 
+def measured_traffic(chi):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the fused collide kernel, per launch, from the committed
+    `ncu --set full` capture (profiles/r01_kernel_traffic.json); None if that file has no entry."""
+    p = os.path.join(ROOT, "profiles", "r01_kernel_traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(chi, {}).get("dram_bytes_per_launch")
+    return None
+
+
 def population(args, rank=0):
     from paper_2602_21244_b200 import workloads as wl
     s = args.scale
@@ -276,6 +285,31 @@ def run_b200(args):
             except dsmc.DsmcError as e:
                 variants[chi] = {"unavailable": str(e)}
 
+    # cfg 4 (a10): chi for 1e7 independent pairs, table and tensor-core MLP (context for the MLP engine alone)
+    cfg4 = {}
+    if not args.no_variants and rank == 0:
+        from paper_2602_21244_b200 import workloads as wl
+        n4 = int(10_000_000 * args.scale)
+        E4, b4 = wl.abinitio_pair_batch(seed=3, n=n4)
+        E4d, b4d = torch.from_numpy(E4).to(dev), torch.from_numpy(b4).to(dev)
+        o4 = torch.empty_like(E4d)
+        for name, mode, fl in (("table", 0, 0), ("mlp_tc", 1, dsmc.F_BF16_TC)):
+            for _ in range(3):
+                ctx.chi_batch(E4d, b4d, mode, B_MAX, flags=fl, out=o4)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a0.record()
+            for _ in range(10):
+                ctx.chi_batch(E4d, b4d, mode, B_MAX, flags=fl, out=o4)
+            a1.record()
+            torch.cuda.synchronize()
+            ms4 = a0.elapsed_time(a1) / 10
+            cfg4[name] = {"ms": ms4, "pairs_per_s": n4 / (ms4 * 1e-3)}
+        fl4 = n4 * 2 * (2 * 128 + 128 * 128 + 128)
+        cfg4["mlp_tc"]["tensor_frac"] = fl4 / (cfg4["mlp_tc"]["ms"] * 1e-3) / 1e12 / tc_sust
+        cfg4["table"]["hbm_frac"] = n4 * 12 / (cfg4["table"]["ms"] * 1e-3) / 1e9 / hbm_peak
+        del E4d, b4d, o4
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -292,7 +326,13 @@ def run_b200(args):
     else:
         roof = {"bound": "hbm", "achieved": bytes_alg / (coll_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
+    if args.chi != "table":
+        # extended bound: one MUFU per hidden activation, 16 / clk / SM (measured), at the
+        # SM clock sampled during the run
+        clk = (sampler.summary().get("sm_mhz") or 1965.0) * 1e6
+        t_xu = pairs * 256 / (16.0 * 148 * clk)
+        roof["xu_bound"] = {"ms": t_xu * 1e3, "frac": t_xu / (coll_ms * 1e-3)}
+    roof["traffic"] = measured_traffic("table" if args.chi == "table" else args.chi)
     roof["kernel"] = "fused collide (k_collide_*)"
     roof["kernel_ms"] = coll_ms
     roof["peak_source"] = peak_src
@@ -306,7 +346,7 @@ def run_b200(args):
             "config": config_dict(args, pop, pairs), "clocks": sampler.summary(),
             "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "api": "dsmc_step_host (pinned host buffers)"},
-            "gpu_launches": int(launches), "roofline": roof, "variants": variants,
+            "gpu_launches": int(launches), "roofline": roof, "variants": variants, "cfg4_chi_batch": cfg4,
             "table_build_s": t_table}
     if not args.no_cpu_baseline and world >= 1:
         chi = "table" if args.chi == "table" else "mlp"
