@@ -73,22 +73,26 @@ struct Chunk {
 
 // A team = the kThreads threads that own one chunk: the whole CTA (bar 0) in the one-chunk-per-CTA
 // kernels, or one of several 256-thread groups of a warp-specialised CTA (named barrier bar > 0).
-struct Team {
-  int tid;  // 0 .. kThreads-1 within the team
+template <int NT>
+struct TeamT {
+  static constexpr int kN = NT, kW = NT / 32;
+  int tid;  // 0 .. NT-1 within the team
   int bar;  // hardware barrier id
   __device__ __forceinline__ void sync() const {
-    asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(kThreads) : "memory");
+    asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(NT) : "memory");
   }
 };
+using Team = TeamT<kThreads>;
 
 // Exclusive scan of a[0..L) in shared memory by the whole team.  a is 16-byte aligned and has room for
 // L rounded up to 4.  Each thread owns one int4 per 1024-element pass (conflict-free 16 B accesses),
 // scans it in registers, warp totals go through one shuffle scan.  `scratch` holds >= kWarps + 1 ints.
 // Ends with T.sync().
-__device__ __forceinline__ void block_excl_scan_coalesced(const Team &T, int *a, int L, int *scratch) {
+template <class TM>
+__device__ __forceinline__ void block_excl_scan_coalesced(const TM &T, int *a, int L, int *scratch) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   int carry = 0;
-  for (int base = 0; base < L; base += 4 * kThreads) {
+  for (int base = 0; base < L; base += 4 * TM::kN) {
     const int i = base + 4 * tid;
     int4 x = make_int4(0, 0, 0, 0);
     if (i < L) {
@@ -108,7 +112,7 @@ __device__ __forceinline__ void block_excl_scan_coalesced(const Team &T, int *a,
     T.sync();
     int off = carry, all = 0;
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) {
+    for (int w = 0; w < TM::kW; ++w) {
       const int sw = scratch[w];
       off += (w < warp) ? sw : 0;
       all += sw;
@@ -130,8 +134,8 @@ __device__ __forceinline__ float warp_sum_f(float v) {
 // begin: returns n_loc > 0 when there is work, 0 when the chunk has nothing to collide (nothing
 // to store either), -1 when the chunk does not fit this variant (caller defers it).
 // ---------------------------------------------------------------------------------------------
-template <class CK>
-__device__ int chunk_begin(const Team &T, const StepParams &P, CK &S, int chunk, int &q0_out) {
+template <class TM, class CK>
+__device__ int chunk_begin(const TM &T, const StepParams &P, CK &S, int chunk, int &q0_out) {
   const int tid = T.tid;
   const int c_lo = __ldg(P.chunk_first + chunk);
   const int c_hi = (chunk + 1 < P.n_chunks) ? __ldg(P.chunk_first + chunk + 1) : P.n_cells;
@@ -141,11 +145,11 @@ __device__ int chunk_begin(const Team &T, const StepParams &P, CK &S, int chunk,
   q0_out = q0;
   if (n_loc <= 0) return 0;
   if (n_loc > CK::LMAX) return -1;
-  for (int q = tid; q < n_loc; q += kThreads) S.cnt[q] = 0;
+  for (int q = tid; q < n_loc; q += TM::kN) S.cnt[q] = 0;
   if (tid < 8) S.misc[tid] = 0;
   T.sync();
   // cell discovery (order of the active list is irrelevant to the results)
-  for (int c = c_lo + tid; c < c_hi; c += kThreads) {
+  for (int c = c_lo + tid; c < c_hi; c += TM::kN) {
     const int gs = __ldg(P.cell_start + c), N = __ldg(P.cell_start + c + 1) - gs;
     if (N == 1) S.cnt[gs - q0] = 1;  // lone particle: keeps bucket positions aligned with slots
     if (N < 2) continue;
@@ -169,7 +173,7 @@ __device__ int chunk_begin(const Team &T, const StepParams &P, CK &S, int chunk,
     for (int i = 0; i < nseg; ++i) S.segs[seg0 + i] = (uint32_t)a | ((uint32_t)i << 16);
   }
   // one coalesced read of the chunk
-  for (int q = tid; q < n_loc; q += kThreads) {
+  for (int q = tid; q < n_loc; q += TM::kN) {
     S.v[q] = make_float4(P.vx[q0 + q], P.vy[q0 + q], P.vz[q0 + q], 0.f);
   }
   T.sync();
@@ -179,11 +183,11 @@ __device__ int chunk_begin(const Team &T, const StepParams &P, CK &S, int chunk,
 }
 
 // pre-collision segment sums + pairing keys + bucket counts; then cell finalisation + sort
-template <class CK>
-__device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, int n_loc) {
+template <class TM, class CK>
+__device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int n_loc) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
-  for (int sg = warp; sg < n_seg; sg += kWarps) {
+  for (int sg = warp; sg < n_seg; sg += TM::kW) {
     const uint32_t e = S.segs[sg];
     const int a = e & 0xFFFFu, piece = e >> 16;
     const CellInfo &ci = S.cells[a];
@@ -220,7 +224,7 @@ __device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, in
   }
   T.sync();
   // cell finalisation: u = pivot + mean(d), Theta = sum d^2 - N |mean(d)|^2   (eq. 10)
-  for (int a = tid; a < n_act; a += kThreads) {
+  for (int a = tid; a < n_act; a += TM::kN) {
     CellInfo &ci = S.cells[a];
     const int N = ci.N, nseg = (N + kSeg - 1) / kSeg;
     double sx = 0, sy = 0, sz = 0, s2 = 0;
@@ -238,7 +242,7 @@ __device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, in
   }
   block_excl_scan_coalesced(T, S.cnt, n_loc, S.misc + MI_SCAN);
   // placement, one warp per segment (cell constants in registers): cnt[bucket] ends as the bucket's end
-  for (int sg = warp; sg < n_seg; sg += kWarps) {
+  for (int sg = warp; sg < n_seg; sg += TM::kW) {
     const uint32_t e = S.segs[sg];
     const CellInfo &ci = S.cells[e & 0xFFFFu];
     const int start = ci.start, N = ci.N, piece = e >> 16;
@@ -251,7 +255,7 @@ __device__ void chunk_pre_and_sort(const Team &T, const StepParams &P, CK &S, in
   T.sync();
   // in-bucket ranking by (key, slot): buckets hold ~1 particle on average.  The first bucket of a cell
   // begins at the cell's first slot, every other one where the previous bucket ends.
-  for (int sg = warp; sg < n_seg; sg += kWarps) {
+  for (int sg = warp; sg < n_seg; sg += TM::kW) {
     const uint32_t e = S.segs[sg];
     const CellInfo &ci = S.cells[e & 0xFFFFu];
     const int start = ci.start, N = ci.N, piece = e >> 16;
@@ -287,8 +291,9 @@ struct PairCtx {
   float U_b, U_eps;
 };
 
+// the two members of pair t, their velocities and relative velocity (eq. 1); no random numbers
 template <class CK>
-__device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, int t, bool need_randoms) {
+__device__ __forceinline__ PairCtx pair_load(const CK &S, int t) {
   PairCtx c;
   const uint32_t e = S.pairs[t];
   const int pos = e & 0xFFFFu;
@@ -308,6 +313,12 @@ __device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, 
   c.acc = true;
   c.U_b = 0.f;
   c.U_eps = 0.f;
+  return c;
+}
+
+template <class CK>
+__device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, int t, bool need_randoms) {
+  PairCtx c = pair_load(S, t);
   const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
   if (need_randoms || accept) {
     const uint4 r = philox4x32_10((uint32_t)c.s, c.cell + P.cell_base, P.step, 1u, P.seed_lo, P.seed_hi);
@@ -390,12 +401,12 @@ __device__ __forceinline__ float chi_table_t(const ChiTableDev &T, float tE, flo
 // ---------------------------------------------------------------------------------------------
 // finish: post-collision sums, matching coefficients, single coalesced store
 // ---------------------------------------------------------------------------------------------
-template <class CK>
-__device__ void chunk_finish(const Team &T, const StepParams &P, CK &S, int n_loc, int q0) {
+template <class TM, class CK>
+__device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc, int q0) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
   if (P.flags & DSMC_F_MOMENT_MATCH) {
-    for (int sg = warp; sg < n_seg; sg += kWarps) {
+    for (int sg = warp; sg < n_seg; sg += TM::kW) {
       const uint32_t e = S.segs[sg];
       const int a = e & 0xFFFFu, piece = e >> 16;
       const CellInfo &ci = S.cells[a];
@@ -413,7 +424,7 @@ __device__ void chunk_finish(const Team &T, const StepParams &P, CK &S, int n_lo
       if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
     }
     T.sync();
-    for (int a = tid; a < n_act; a += kThreads) {
+    for (int a = tid; a < n_act; a += TM::kN) {
       CellInfo &ci = S.cells[a];
       double alpha = 1.0, bx = 0.0, by = 0.0, bz = 0.0;
       if (ci.collided) {
@@ -444,7 +455,7 @@ __device__ void chunk_finish(const Team &T, const StepParams &P, CK &S, int n_lo
     T.sync();
     // store, one warp per segment: v <- alpha v + B with the cell's coefficients in registers.  Cells in
     // which nothing collided (and particles of cells with N < 2) are unchanged and not written.
-    for (int sg = warp; sg < n_seg; sg += kWarps) {
+    for (int sg = warp; sg < n_seg; sg += TM::kW) {
       const uint32_t e = S.segs[sg];
       const CellInfo &ci = S.cells[e & 0xFFFFu];
       if (!ci.collided) continue;
@@ -459,7 +470,7 @@ __device__ void chunk_finish(const Team &T, const StepParams &P, CK &S, int n_lo
       }
     }
   } else {
-    for (int sg = warp; sg < n_seg; sg += kWarps) {
+    for (int sg = warp; sg < n_seg; sg += TM::kW) {
       const uint32_t e = S.segs[sg];
       const CellInfo &ci = S.cells[e & 0xFFFFu];
       if (!ci.collided) continue;

@@ -86,11 +86,11 @@ __device__ float *mlp_tile_fp32(const MlpDev &net, float *buf) {
 // ---------------------------------------------------------------------------------------------
 // pair phases
 // ---------------------------------------------------------------------------------------------
-template <class CK>
-__device__ __forceinline__ void pairs_table(const StepParams &P, CK &S, int q0) {
+template <class TM, class CK>
+__device__ __forceinline__ void pairs_table(const TM &T, const StepParams &P, CK &S, int q0) {
   const int n_pairs = S.misc[MI_NPAIRS];
   const float nBm1 = (float)(P.table.nB - 1);
-  for (int t = threadIdx.x; t < n_pairs; t += kThreads) {
+  for (int t = T.tid; t < n_pairs; t += TM::kN) {
     PairCtx c = pair_setup(P, S, t, true);
     float px = c.gx, py = c.gy, pz = c.gz, chi = 0.f;
     if (c.acc) {
@@ -175,10 +175,10 @@ __device__ __forceinline__ void pairs_mlp_fp32(const StepParams &P, const MlpDev
 // kernels.  OP_TABLE: chi-table operator; otherwise FP32 MLP (P.op = 0 VHS-NN, 2 chi-MLP).
 // DEFERRED: persistent loop over the deferred chunk list instead of chunk = blockIdx.x.
 // ---------------------------------------------------------------------------------------------
-template <class CK, bool OP_TABLE, int TP>
+template <int NT, class CK, bool OP_TABLE, int TP>
 __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev &net, CK &S, float *mlp, int chunk,
                                               bool deferred) {
-  const Team T{(int)threadIdx.x, 0};
+  const TeamT<NT> T{(int)threadIdx.x, 0};
   int q0 = 0;
   const int n_loc = chunk_begin(T, P, S, chunk, q0);
   if (n_loc == 0) return;
@@ -195,37 +195,37 @@ __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev 
   }
   chunk_pre_and_sort(T, P, S, n_loc);
   if (OP_TABLE) {
-    pairs_table(P, S, q0);
+    pairs_table(T, P, S, q0);
   } else {
     pairs_mlp_fp32<TP>(P, net, S, mlp, q0);
   }
-  __syncthreads();
+  T.sync();
   chunk_finish(T, P, S, n_loc, q0);
 }
 
-template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB>
-__global__ void __launch_bounds__(kThreads, MINB) k_collide(const StepParams P, const MlpDev net) {
+template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB, int NT = kThreads>
+__global__ void __launch_bounds__(NT, MINB) k_collide(const StepParams P, const MlpDev net) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Chunk<LMAX, AMAX> S;
   float *mlp = reinterpret_cast<float *>(S.carve(smem_raw));
   if (!DEFERRED) {
-    process_chunk<Chunk<LMAX, AMAX>, OP_TABLE, TP>(P, net, S, mlp, blockIdx.x, false);
+    process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP>(P, net, S, mlp, blockIdx.x, false);
   } else {
     const int n_big = *reinterpret_cast<volatile const int32_t *>(P.big);
     for (int i = blockIdx.x; i < n_big; i += gridDim.x) {
-      process_chunk<Chunk<LMAX, AMAX>, OP_TABLE, TP>(P, net, S, mlp, P.big[1 + i], true);
+      process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP>(P, net, S, mlp, P.big[1 + i], true);
       __syncthreads();
     }
   }
 }
 
-template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB>
+template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB, int NT = kThreads>
 static int launch_one(dsmc_ctx *c, const StepParams &p, const MlpDev &nd, int grid, size_t mlp_bytes) {
-  auto kern = k_collide<LMAX, AMAX, OP_TABLE, TP, DEFERRED, MINB>;
+  auto kern = k_collide<LMAX, AMAX, OP_TABLE, TP, DEFERRED, MINB, NT>;
   const size_t smem = Chunk<LMAX, AMAX>::bytes() + mlp_bytes;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
-  kern<<<grid, kThreads, smem, c->stream>>>(p, nd);
+  kern<<<grid, NT, smem, c->stream>>>(p, nd);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
@@ -248,7 +248,7 @@ int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {
   MlpDev nd{};
   const int big_grid = c->num_sms;
   if (p.op == 1) {
-    rc = launch_one<1024, kAmaxSmall, true, 64, false, 5>(c, p, nd, p.n_chunks, 0);
+    rc = launch_one<1024, kAmaxSmall, true, 64, false, 6, 128>(c, p, nd, p.n_chunks, 0);
     if (rc != DSMC_OK) return rc;
     return launch_one<kLmaxBig, kAmaxBig, true, 64, true, 1>(c, p, nd, big_grid, 0);
   }

@@ -188,12 +188,12 @@ struct TcPipe {
   }
 
   // ---- non-blocking issue (polling MMA warp of the fused kernel; whole warp calls, operand known ready) ----
-  __device__ __forceinline__ void issue_layer1(int s, bool first) {
+  __device__ __forceinline__ void issue_layer1(int s, int par, bool first) {
     if ((threadIdx.x & 31) == 0) {
       if (first) tc::mbar_wait(bar_w, 0);
       tc::fence_after();
       constexpr uint32_t idH = tc::instr_desc(128, H);
-      const uint32_t a1a = tc::smem_u32(a1 + 2 * s * SH::A1_BYTES), wa = tc::smem_u32(w);
+      const uint32_t a1a = tc::smem_u32(a1 + (2 * s + par) * SH::A1_BYTES), wa = tc::smem_u32(w);
 #pragma unroll
       for (int ks = 0; ks < SH::K1 / 16; ++ks)
         tc::mma_ss(tmem + s * SH::SLOT_COLS + SH::COL_D, tc::smem_desc(a1a + ks * 2 * 128 * 16, 128 * 16, 128),
@@ -258,6 +258,13 @@ struct TcPipe {
       tc::tmem_st8(a0 + c * 8, o);
     }
     tc::wait_st();
+    tc::fence_before();
+    warp_arrive(a_ready + s);
+  }
+  // this warp's 32 rows hold no real pair: nothing to activate, only the hand-off (rows are independent, the
+  // stale operand rows produce outputs nobody reads)
+  __device__ __forceinline__ void act_skip(int s) {
+    tc::fence_after();
     tc::fence_before();
     warp_arrive(a_ready + s);
   }
