@@ -28,7 +28,9 @@
  *
  * Random numbers: Philox4x32-10, key = seed, counter =
  * (index, cell, step, stream); stream 0 = pairing keys (slot p uses word p&3 of block p>>2),
- * stream 1 = (U_acc, U_b, U_eps) of pair slot s, stream 2 = Box-Muller normals of pair slot s;
+ * stream 1 = (U_b, U_eps) of pair slot s (words 2(s&1), 2(s&1)+1 of block s>>1), stream 2 = Box-Muller
+ * normals of pair slot s, stream 3 = U_acc of pair slot s (word s&3 of block s>>2, drawn only with
+ * DSMC_F_ACCEPT); cell = local cell index + cell_base;
  * u = ((x>>9)+0.5) 2^-23.  Results therefore depend only on (seed, step, cell, slot).
  */
 #ifndef DSMC_H

@@ -53,13 +53,16 @@ uint32_t orc_pair_key(uint64_t seed, uint32_t step, uint32_t cell, uint32_t slot
   return r[slot & 3u];
 }
 
-/* stream 1: U_acc, U_b, U_eps for pair slot s */
+/* per-pair uniforms.  Stream 1: one Philox block serves two consecutive pair slots; pair s takes words
+ * 2(s&1), 2(s&1)+1 of block s>>1 as (U_b, U_eps).  Stream 3: U_acc of pair s is word s&3 of block s>>2
+ * (DESIGN.md "RNG addressing"). */
 void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double u[3]) {
-  uint32_t r[4];
-  philox_at(seed, s, cell, step, 1u, r);
-  u[0] = orc_u01(r[0]);
-  u[1] = orc_u01(r[1]);
-  u[2] = orc_u01(r[2]);
+  uint32_t r[4], a[4];
+  philox_at(seed, s >> 1, cell, step, 1u, r);
+  philox_at(seed, s >> 2, cell, step, 3u, a);
+  u[0] = orc_u01(a[s & 3u]);
+  u[1] = orc_u01(r[2u * (s & 1u)]);
+  u[2] = orc_u01(r[2u * (s & 1u) + 1u]);
 }
 
 /* stream 2: xi ~ N(0,I3), eq. 2, by Box-Muller on four uniforms */

@@ -89,7 +89,8 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 double orc_u01(uint32_t x); /* ((x>>9)+0.5)*2^-23 in (0,1), exact in fp32 */
 /* pairing key of slot p in cell k at step t (stream 0) */
 uint32_t orc_pair_key(uint64_t seed, uint32_t step, uint32_t cell, uint32_t slot);
-/* per-pair uniforms (stream 1): U_acc, U_b, U_eps */
+/* per-pair uniforms: U_acc (stream 3, word s&3 of block s>>2), U_b, U_eps (stream 1, words 2(s&1), 2(s&1)+1
+ * of block s>>1) */
 void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double u[3]);
 /* per-pair latent xi ~ N(0, I3) by Box-Muller (stream 2) */
 void orc_pair_normals(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double xi[3]);

@@ -321,14 +321,16 @@ __device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, 
   PairCtx c = pair_load(S, t);
   const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
   if (need_randoms || accept) {
-    const uint4 r = philox4x32_10((uint32_t)c.s, c.cell + P.cell_base, P.step, 1u, P.seed_lo, P.seed_hi);
-    c.U_b = u01(r.y);
-    c.U_eps = u01(r.z);
-    if (accept) {
+    // stream 1: one block per two pair slots, (U_b, U_eps) = words 2(s&1), 2(s&1)+1 of block s>>1
+    const uint4 r = philox4x32_10((uint32_t)c.s >> 1, c.cell + P.cell_base, P.step, 1u, P.seed_lo, P.seed_hi);
+    c.U_b = u01((c.s & 1) ? r.z : r.x);
+    c.U_eps = u01((c.s & 1) ? r.w : r.y);
+    if (accept) {  // stream 3: U_acc = word s&3 of block s>>2
+      const uint4 ra = philox4x32_10((uint32_t)c.s >> 2, c.cell + P.cell_base, P.step, 3u, P.seed_lo, P.seed_hi);
       const float cap = __ldg(P.cap + c.cell);
       const float g = sqrtf(c.g2);
       const float w = (P.op == 0) ? P.vhs_c * powf(g, P.vhs_e) : g;  // sigma_T(g) g  |  g
-      c.acc = u01(r.x) * cap < w;
+      c.acc = u01(word_of(ra, (uint32_t)c.s & 3u)) * cap < w;
     }
   }
   return c;

@@ -38,8 +38,12 @@ def test_rng_addressing_streams_are_distinct_and_keyed():
     seed = 0x1234567899
     r0 = oracle.philox4x32_10([5 >> 2, 7, 3, 0], [seed & 0xFFFFFFFF, seed >> 32])
     assert oracle.pair_key(seed, 3, 7, 5) == r0[5 & 3]
-    r1 = oracle.philox4x32_10([9, 7, 3, 1], [seed & 0xFFFFFFFF, seed >> 32])
-    np.testing.assert_array_equal(oracle.pair_uniforms(seed, 3, 7, 9), [oracle.u01(x) for x in r1[:3]])
+    # pair 9: (U_b, U_eps) = words 2, 3 of stream-1 block 9 >> 1; U_acc = word 9 & 3 of stream-3 block 9 >> 2
+    r1 = oracle.philox4x32_10([9 >> 1, 7, 3, 1], [seed & 0xFFFFFFFF, seed >> 32])
+    r3 = oracle.philox4x32_10([9 >> 2, 7, 3, 3], [seed & 0xFFFFFFFF, seed >> 32])
+    np.testing.assert_array_equal(oracle.pair_uniforms(seed, 3, 7, 9), [oracle.u01(x) for x in (r3[9 & 3], r1[2], r1[3])])
+    r1e = oracle.philox4x32_10([8 >> 1, 7, 3, 1], [seed & 0xFFFFFFFF, seed >> 32])
+    np.testing.assert_array_equal(oracle.pair_uniforms(seed, 3, 7, 8)[1:], [oracle.u01(x) for x in (r1e[0], r1e[1])])
     # normals: Box-Muller identity xi0^2 + xi1^2 = -2 ln u0
     r2 = oracle.philox4x32_10([9, 7, 3, 2], [seed & 0xFFFFFFFF, seed >> 32])
     xi = oracle.pair_normals(seed, 3, 7, 9)
