@@ -48,6 +48,8 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
   const size_t n_chunks = (size_t)(max_particles / kChunk + 2);
   CK(cudaMalloc(&c->d_chunk_first, sizeof(int32_t) * n_chunks));
   CK(cudaMalloc(&c->d_big, sizeof(int32_t) * (n_chunks + 1)));
+  CK(cudaMalloc(&c->d_chunk_meta, sizeof(int4) * n_chunks));
+  CK(cudaMalloc(&c->d_big2, sizeof(int32_t) * (n_chunks + 1)));
   CK(cudaMalloc(&c->d_work, sizeof(int32_t) * 4));
   *out = c;
   return DSMC_OK;
@@ -63,6 +65,8 @@ int dsmc_destroy(dsmc_ctx *c) {
   for (int i = 0; i < 2; ++i) { cudaFree(c->d_bin_rec[i]); cudaFree(c->d_bin_cell[i]); }
   cudaFree(c->d_chunk_first);
   cudaFree(c->d_big);
+  cudaFree(c->d_chunk_meta);
+  cudaFree(c->d_big2);
   cudaFree(c->d_work);
   for (int s = 0; s < 2; ++s) {
     cudaFree(c->d_weights[s]);

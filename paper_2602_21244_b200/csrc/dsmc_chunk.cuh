@@ -137,14 +137,24 @@ __device__ __forceinline__ float warp_sum_f(float v) {
 template <class TM, class CK>
 __device__ int chunk_begin(const TM &T, const StepParams &P, CK &S, int chunk, int &q0_out) {
   const int tid = T.tid;
-  const int c_lo = __ldg(P.chunk_first + chunk);
-  const int c_hi = (chunk + 1 < P.n_chunks) ? __ldg(P.chunk_first + chunk + 1) : P.n_cells;
+  const int4 meta = __ldg(P.chunk_meta + chunk);  // (first cell, end cell, first slot, end slot): one load
+  const int c_lo = meta.x, c_hi = meta.y, q0 = meta.z;
   if (c_lo >= c_hi) return 0;
-  const int q0 = __ldg(P.cell_start + c_lo), q1 = __ldg(P.cell_start + c_hi);
-  const int n_loc = q1 - q0;
+  const int n_loc = meta.w - q0;
   q0_out = q0;
   if (n_loc <= 0) return 0;
   if (n_loc > CK::LMAX) return -1;
+  // one coalesced read of the chunk, asynchronously (global -> shared without registers) so that its latency
+  // overlaps the cell discovery below
+  {
+    const uint32_t sv = (uint32_t)__cvta_generic_to_shared(S.v);
+    for (int q = tid; q < n_loc; q += TM::kN) {
+      const uint32_t d = sv + 16u * (uint32_t)q;
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(P.vx + q0 + q) : "memory");
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d + 4u), "l"(P.vy + q0 + q) : "memory");
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d + 8u), "l"(P.vz + q0 + q) : "memory");
+    }
+  }
   for (int q = tid; q < n_loc; q += TM::kN) S.cnt[q] = 0;
   if (tid < 8) S.misc[tid] = 0;
   T.sync();
@@ -172,10 +182,7 @@ __device__ int chunk_begin(const TM &T, const StepParams &P, CK &S, int chunk, i
     S.cells[a] = ci;
     for (int i = 0; i < nseg; ++i) S.segs[seg0 + i] = (uint32_t)a | ((uint32_t)i << 16);
   }
-  // one coalesced read of the chunk
-  for (int q = tid; q < n_loc; q += TM::kN) {
-    S.v[q] = make_float4(P.vx[q0 + q], P.vy[q0 + q], P.vz[q0 + q], 0.f);
-  }
+  asm volatile("cp.async.wait_all;" ::: "memory");
   T.sync();
   if (S.misc[MI_NACT] > CK::AMAX) return -1;
   if (S.misc[MI_NACT] == 0) return 0;

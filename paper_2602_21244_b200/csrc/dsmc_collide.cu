@@ -13,10 +13,11 @@ namespace dsmc {
 
 // k_chunk_map: chunk_first[b] = first cell whose first slot is >= b * kChunk; resets the deferred list.
 __global__ void k_chunk_map(int32_t K, const int32_t *__restrict__ cs, int32_t *__restrict__ chunk_first,
-                            int32_t *__restrict__ big, int32_t *__restrict__ work) {
+                            int32_t *__restrict__ big, int32_t *__restrict__ big2, int32_t *__restrict__ work) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k == 0) {
     big[0] = 0;
+    big2[0] = 0;
     work[0] = 0;
     work[1] = 0;
   }
@@ -25,6 +26,15 @@ __global__ void k_chunk_map(int32_t K, const int32_t *__restrict__ cs, int32_t *
   const int lo = (k == 0) ? 0 : (__ldg(cs + k - 1) / kChunk + 1);
   const int hi = s / kChunk;
   for (int b = lo; b <= hi; ++b) chunk_first[b] = k;
+}
+
+// k_chunk_meta: (first cell, end cell, first slot, end slot) of every chunk, so a CTA starts with one load
+__global__ void k_chunk_meta(int32_t n_chunks, int32_t K, const int32_t *__restrict__ cs,
+                             const int32_t *__restrict__ chunk_first, int4 *__restrict__ meta) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= n_chunks) return;
+  const int c_lo = chunk_first[b], c_hi = (b + 1 < n_chunks) ? chunk_first[b + 1] : K;
+  meta[b] = make_int4(c_lo, c_hi, __ldg(cs + min(c_lo, K)), __ldg(cs + min(c_hi, K)));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -175,20 +185,23 @@ __device__ __forceinline__ void pairs_mlp_fp32(const StepParams &P, const MlpDev
 // kernels.  OP_TABLE: chi-table operator; otherwise FP32 MLP (P.op = 0 VHS-NN, 2 chi-MLP).
 // DEFERRED: persistent loop over the deferred chunk list instead of chunk = blockIdx.x.
 // ---------------------------------------------------------------------------------------------
-template <int NT, class CK, bool OP_TABLE, int TP>
-__device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev &net, CK &S, float *mlp, int chunk,
-                                              bool deferred) {
+// SRC: where a CTA's chunks come from (0 = chunk blockIdx.x, 1 = deferred list P.big, 2 = second list P.big2,
+// walked grid-stride).  DST: where a chunk that does not fit this footprint goes (1 = P.big, 2 = P.big2,
+// 0 = nowhere: DSMC_ERR_CELL_TOO_LARGE).
+template <int NT, class CK, bool OP_TABLE, int TP, int DST>
+__device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev &net, CK &S, float *mlp, int chunk) {
   const TeamT<NT> T{(int)threadIdx.x, 0};
   int q0 = 0;
   const int n_loc = chunk_begin(T, P, S, chunk, q0);
   if (n_loc == 0) return;
   if (n_loc < 0) {
     if (threadIdx.x == 0) {
-      if (deferred) {
+      if (DST == 0) {
         *P.status = DSMC_ERR_CELL_TOO_LARGE;
       } else {
-        const int i = atomicAdd(P.big, 1);
-        P.big[1 + i] = chunk;
+        int32_t *list = DST == 1 ? P.big : P.big2;
+        const int i = atomicAdd(list, 1);
+        list[1 + i] = chunk;
       }
     }
     return;
@@ -203,25 +216,26 @@ __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev 
   chunk_finish(T, P, S, n_loc, q0);
 }
 
-template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB, int NT = kThreads>
+template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads>
 __global__ void __launch_bounds__(NT, MINB) k_collide(const StepParams P, const MlpDev net) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Chunk<LMAX, AMAX> S;
   float *mlp = reinterpret_cast<float *>(S.carve(smem_raw));
-  if (!DEFERRED) {
-    process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP>(P, net, S, mlp, blockIdx.x, false);
+  if (SRC == 0) {
+    process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP, DST>(P, net, S, mlp, blockIdx.x);
   } else {
-    const int n_big = *reinterpret_cast<volatile const int32_t *>(P.big);
-    for (int i = blockIdx.x; i < n_big; i += gridDim.x) {
-      process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP>(P, net, S, mlp, P.big[1 + i], true);
+    const int32_t *list = SRC == 1 ? P.big : P.big2;
+    const int n_list = *reinterpret_cast<volatile const int32_t *>(list);
+    for (int i = blockIdx.x; i < n_list; i += gridDim.x) {
+      process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP, DST>(P, net, S, mlp, list[1 + i]);
       __syncthreads();
     }
   }
 }
 
-template <int LMAX, int AMAX, bool OP_TABLE, int TP, bool DEFERRED, int MINB, int NT = kThreads>
+template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads>
 static int launch_one(dsmc_ctx *c, const StepParams &p, const MlpDev &nd, int grid, size_t mlp_bytes) {
-  auto kern = k_collide<LMAX, AMAX, OP_TABLE, TP, DEFERRED, MINB, NT>;
+  auto kern = k_collide<LMAX, AMAX, OP_TABLE, TP, SRC, DST, MINB, NT>;
   const size_t smem = Chunk<LMAX, AMAX>::bytes() + mlp_bytes;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
@@ -234,10 +248,14 @@ int launch_chunk_map(dsmc_ctx *c, StepParams &p) {
   p.n_chunks = (int32_t)((p.n + kChunk - 1) / kChunk);
   p.chunk_first = c->d_chunk_first;
   p.big = c->d_big;
+  p.big2 = c->d_big2;
   p.work = c->d_work;
   k_chunk_map<<<(p.n_cells + 1 + 255) / 256, 256, 0, c->stream>>>(p.n_cells, p.cell_start, c->d_chunk_first, c->d_big,
-                                                                  c->d_work);
-  c->launches += 1;
+                                                                  c->d_big2, c->d_work);
+  p.chunk_meta = c->d_chunk_meta;
+  k_chunk_meta<<<(p.n_chunks + 255) / 256, 256, 0, c->stream>>>(p.n_chunks, p.n_cells, p.cell_start, c->d_chunk_first,
+                                                             c->d_chunk_meta);
+  c->launches += 2;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
 
@@ -248,21 +266,25 @@ int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {
   MlpDev nd{};
   const int big_grid = c->num_sms;
   if (p.op == 1) {
-    rc = launch_one<1024, kAmaxSmall, true, 64, false, 6, 128>(c, p, nd, p.n_chunks, 0);
+    // three footprints: 704 slots at 8 CTAs/SM (chunks of cells up to ~230 particles), 1024 slots at 6 CTAs/SM
+    // (one ~1000-particle cell), then anything legal on one CTA per SM
+    rc = launch_one<704, kAmaxSmall, true, 64, 0, 1, 8, 128>(c, p, nd, p.n_chunks, 0);
     if (rc != DSMC_OK) return rc;
-    return launch_one<kLmaxBig, kAmaxBig, true, 64, true, 1>(c, p, nd, big_grid, 0);
+    rc = launch_one<1024, kAmaxSmall, true, 64, 1, 2, 6, 128>(c, p, nd, c->num_sms * 6, 0);
+    if (rc != DSMC_OK) return rc;
+    return launch_one<kLmaxBig, kAmaxBig, true, 64, 2, 0, 1>(c, p, nd, big_grid, 0);
   }
   nd = *net;
   if (nd.dmax <= 128) {
     const size_t mb = sizeof(float) * 2 * nd.dmax * 64;
-    rc = launch_one<kLmaxSmall, kAmaxSmall, false, 64, false, 1>(c, p, nd, p.n_chunks, mb);
+    rc = launch_one<kLmaxSmall, kAmaxSmall, false, 64, 0, 1, 1>(c, p, nd, p.n_chunks, mb);
     if (rc != DSMC_OK) return rc;
-    return launch_one<kLmaxBig, kAmaxBig, false, 64, true, 1>(c, p, nd, big_grid, mb);
+    return launch_one<kLmaxBig, kAmaxBig, false, 64, 1, 0, 1>(c, p, nd, big_grid, mb);
   }
   const size_t mb = sizeof(float) * 2 * nd.dmax * 32;
-  rc = launch_one<kLmaxSmall, kAmaxSmall, false, 32, false, 1>(c, p, nd, p.n_chunks, mb);
+  rc = launch_one<kLmaxSmall, kAmaxSmall, false, 32, 0, 1, 1>(c, p, nd, p.n_chunks, mb);
   if (rc != DSMC_OK) return rc;
-  return launch_one<kLmaxBig, kAmaxBig, false, 32, true, 1>(c, p, nd, big_grid, mb);
+  return launch_one<kLmaxBig, kAmaxBig, false, 32, 1, 0, 1>(c, p, nd, big_grid, mb);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -71,7 +71,9 @@ struct StepParams {
   // chunk decomposition (filled by launch_chunk_map)
   int32_t n_chunks;
   const int32_t *chunk_first;  // [n_chunks + 1]
+  const int4 *chunk_meta;      // [n_chunks] (first cell, end cell, first slot, end slot)
   int32_t *big;                // [0] = count, [1..] deferred chunk ids
+  int32_t *big2;               // second-level deferred list (chunks that did not fit the middle footprint)
   int32_t *work;               // [0], [1]: next chunk / next deferred entry (persistent kernels)
 };
 
@@ -89,7 +91,9 @@ struct dsmc_ctx {
   float4 *d_bin_rec[2];  // (idx, vx, vy, vz) between passes
   int32_t *d_bin_cell[2];
   int32_t *d_chunk_first;  // [max_particles / kChunk + 2]
+  int4 *d_chunk_meta;      // [max_particles / kChunk + 2]
   int32_t *d_big;          // [max_particles / kChunk + 2]
+  int32_t *d_big2;         // [max_particles / kChunk + 2]
   int32_t *d_work;         // [4] work counters of the persistent kernels ([0] main pass, [1] deferred pass)
   int64_t launches;
   int num_sms;
