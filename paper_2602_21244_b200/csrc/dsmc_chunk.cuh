@@ -85,23 +85,36 @@ struct TeamT {
 using Team = TeamT<kThreads>;
 
 // Exclusive scan of a[0..L) in shared memory by the whole team.  a is 16-byte aligned and has room for
-// L rounded up to 4.  Each thread owns one int4 per 1024-element pass (conflict-free 16 B accesses),
+// L rounded up to 4.  Each thread owns eight consecutive elements per pass (two 16 B accesses),
 // scans it in registers, warp totals go through one shuffle scan.  `scratch` holds >= kWarps + 1 ints.
 // Ends with T.sync().
 template <class TM>
 __device__ __forceinline__ void block_excl_scan_coalesced(const TM &T, int *a, int L, int *scratch) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   int carry = 0;
-  for (int base = 0; base < L; base += 4 * TM::kN) {
-    const int i = base + 4 * tid;
-    int4 x = make_int4(0, 0, 0, 0);
+  for (int base = 0; base < L; base += 8 * TM::kN) {  // eight consecutive elements per thread and pass
+    const int i = base + 8 * tid;
+    int x[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) x[u] = 0;
     if (i < L) {
-      x = *reinterpret_cast<const int4 *>(a + i);
-      if (i + 1 >= L) x.y = 0;
-      if (i + 2 >= L) x.z = 0;
-      if (i + 3 >= L) x.w = 0;
+      const int4 lo = *reinterpret_cast<const int4 *>(a + i);
+      x[0] = lo.x; x[1] = lo.y; x[2] = lo.z; x[3] = lo.w;
+      if (i + 4 < L) {
+        const int4 hi = *reinterpret_cast<const int4 *>(a + i + 4);
+        x[4] = hi.x; x[5] = hi.y; x[6] = hi.z; x[7] = hi.w;
+      }
+#pragma unroll
+      for (int u = 1; u < 8; ++u)
+        if (i + u >= L) x[u] = 0;
     }
-    const int s1 = x.x + x.y, s2 = s1 + x.z, tot = s2 + x.w;
+    int tot = 0;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {  // x[u] <- exclusive prefix inside the thread
+      const int t = x[u];
+      x[u] = tot;
+      tot += t;
+    }
     int inc = tot;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -117,8 +130,11 @@ __device__ __forceinline__ void block_excl_scan_coalesced(const TM &T, int *a, i
       off += (w < warp) ? sw : 0;
       all += sw;
     }
-    const int e0 = off + inc - tot;  // exclusive prefix of x.x
-    if (i < L) *reinterpret_cast<int4 *>(a + i) = make_int4(e0, e0 + x.x, e0 + s1, e0 + s2);
+    const int e0 = off + inc - tot;
+    if (i < L) {
+      *reinterpret_cast<int4 *>(a + i) = make_int4(e0 + x[0], e0 + x[1], e0 + x[2], e0 + x[3]);
+      if (i + 4 < L) *reinterpret_cast<int4 *>(a + i + 4) = make_int4(e0 + x[4], e0 + x[5], e0 + x[6], e0 + x[7]);
+    }
     carry += all;
     T.sync();
   }
