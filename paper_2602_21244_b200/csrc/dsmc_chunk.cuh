@@ -13,8 +13,8 @@
 //   finish    post-collision segment sums, moment matching folded into the store as one FMA per
 //             component: v <- alpha v + B, B = u_pre - alpha u_post (eqs. 10-11, Q5)
 //
-// Cell sums are accumulated in FP32 about a pivot near the cell mean (first particle before the
-// collisions, u_pre after them), 8 values per lane, and combined across lanes in FP32 and across
+// Cell sums are accumulated in FP32 about a pivot near the cell mean (mean of the first 32 particles
+// before the collisions, u_pre after them), 8 values per lane, and combined across lanes in FP32 and across
 // segments in FP64 in a fixed order, so results do not depend on scheduling.
 #pragma once
 #include "dsmc_device.cuh"
@@ -217,7 +217,23 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     const int start = ci.start, N = ci.N, M = ci.M, pair_off = ci.pair_off;
     const uint32_t cell = (uint32_t)ci.cell + P.cell_base;
     const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
-    const float4 pv = S.v[start];
+    // pivot = mean of the cell's first (up to) 32 particles: identical in every warp that works on this cell,
+    // and close enough to the cell mean that Theta = sum d^2 - N |mean d|^2 loses no digits to cancellation
+    float4 pv;
+    {
+      const int m = min(N, 32);
+      const float4 f = lane < m ? S.v[start + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float im = 1.0f / (float)m;
+      pv.x = warp_sum_f(f.x) * im;
+      pv.y = warp_sum_f(f.y) * im;
+      pv.z = warp_sum_f(f.z) * im;
+      pv.w = 0.f;
+      if (lane == 0 && piece == 0) {  // parked in the cell record until the finalisation below replaces it by u
+        S.cells[a].ux = pv.x;
+        S.cells[a].uy = pv.y;
+        S.cells[a].uz = pv.z;
+      }
+    }
     float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
     for (int q = lo + lane; q < hi; q += 32) {
       const float4 v = S.v[q];
@@ -257,10 +273,9 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     }
     const double inv = 1.0 / N;
     const double dx = sx * inv, dy = sy * inv, dz = sz * inv;
-    const float4 pv = S.v[ci.start];
-    ci.ux = (float)((double)pv.x + dx);
-    ci.uy = (float)((double)pv.y + dy);
-    ci.uz = (float)((double)pv.z + dz);
+    ci.ux = (float)((double)ci.ux + dx);  // pivot + mean(d)
+    ci.uy = (float)((double)ci.uy + dy);
+    ci.uz = (float)((double)ci.uz + dz);
     ci.theta = (float)(s2 - N * (dx * dx + dy * dy + dz * dz));
   }
   block_excl_scan_coalesced(T, S.cnt, n_loc, S.misc + MI_SCAN);

@@ -1,0 +1,138 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (-m gpu).
+
+The oracle cannot run 2e7 particles in seconds, so (prompt section 3):
+  * binning is checked exactly through properties that pin the unique stable sort (cell_start = cumulative
+    counts, perm a permutation, cells constant and ids ascending inside every segment);
+  * the fused step is checked (a) on SAMPLED cells that the oracle recomputes one by one -- cell_base makes
+    the oracle draw exactly the randoms of the full run -- with bit-exact pairing and the per-pair tolerances of
+    DESIGN.md, and (b) on ALL cells through the conserved moments (1e-6);
+  * the chi batch (cfg 4, 1e7 pairs) on a sample of outputs.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_21244_b200 import workloads as wl
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dsmc():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2602_21244_b200 import dsmc as mod
+    return mod
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _segment_moments(cs, vx, vy, vz):
+    """per-cell (Px, Py, Pz, E) in fp64 by prefix sums (numpy, independent of both implementations)."""
+    out = []
+    for a in (vx, vy, vz, vx * vx + vy * vy + vz * vz):
+        c = np.concatenate([[0.0], np.cumsum(a.astype(np.float64))])
+        out.append(c[cs[1:]] - c[cs[:-1]])
+    return np.stack(out, axis=1)
+
+
+def _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, seed, step, tol_pair, net=None, table=None,
+                         chi_tol_rel=None):
+    worst = 0.0
+    for k in cells:
+        q0, q1 = int(cs_h[k]), int(cs_h[k + 1])
+        if q1 - q0 < 2:
+            continue
+        loc = [a[q0:q1].astype(np.float64) for a in v_in]
+        lcs = np.array([0, q1 - q0], np.int32)
+        prm_o.cell_base = int(k)
+        ref = oracle.collide_abinitio(lcs, *loc, prm_o, seed, step, net=net, table=table)
+        # after moment matching every particle of the cell moved by the same affine map, so comparing final
+        # velocities tests pairing, operator, rotation and matching together
+        scale = np.sqrt((loc[0] ** 2 + loc[1] ** 2 + loc[2] ** 2).mean())
+        for a, want in zip(v_out, (ref.vx, ref.vy, ref.vz)):
+            d = np.abs(a[q0:q1].astype(np.float64) - want).max() / scale
+            worst = max(worst, d)
+    return worst
+
+
+@pytest.mark.parametrize("chi", ["table", "mlp_tc"])
+def test_cfg5_full_size(dsmc, chi):
+    pop = wl.mach10_cylinder()  # 400 x 200 cells, 2e7 particles
+    assert pop.n == 20_000_000 and pop.n_cells == 80_000
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    tab = oracle.build_chi_table(oracle.lj_argon(), 256, 256, n_panels=1)
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = ctx.bin(dev(pop.cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), pop.n_cells)
+    ctx.check()
+    cs_h, perm_h = cs.cpu().numpy(), perm.cpu().numpy()
+    # ---- a1: the unique stable sort
+    np.testing.assert_array_equal(cs_h, np.concatenate([[0], np.cumsum(pop.counts)]).astype(np.int32))
+    assert np.array_equal(np.sort(perm_h), np.arange(pop.n, dtype=np.int32))
+    sorted_cells = pop.cell[perm_h]
+    assert np.all(np.diff(sorted_cells) >= 0)
+    same = sorted_cells[1:] == sorted_cells[:-1]
+    assert np.all(np.diff(perm_h)[same] > 0)  # ties keep the original order
+    assert np.array_equal(vx_s.cpu().numpy(), pop.vx[perm_h])
+    # ---- a2-a9
+    v_in = [t.cpu().numpy() for t in (vx_s, vy_s, vz_s)]
+    pre = _segment_moments(cs_h, *v_in)
+    flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi == "mlp_tc" else 0)
+    cm = 0 if chi == "table" else 1
+    prm = dsmc.AbinitioParams(chi_mode=cm, flags=flags)
+    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=4, step=7)
+    ctx.check()
+    v_out = [t.cpu().numpy() for t in (vx_s, vy_s, vz_s)]
+    post = _segment_moments(cs_h, *v_out)
+    N = np.diff(cs_h)
+    ok = N >= 2
+    assert np.abs(post[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+    assert (np.linalg.norm(post[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    # untouched: cells with fewer than two particles
+    lone = np.flatnonzero(N == 1)[:100]
+    for k in lone:
+        assert v_out[0][cs_h[k]] == v_in[0][cs_h[k]]
+    # something did happen everywhere else
+    moved = np.abs(v_out[0] - v_in[0]) > 0
+    assert moved.mean() > 0.95
+    # sampled cells against the oracle (freestream, shock band, wake, boundary cells)
+    rng = np.random.default_rng(0)
+    sizes = np.unique(N[N >= 2])
+    cells = np.concatenate([rng.choice(np.flatnonzero(N == s), size=min(3, int((N == s).sum())), replace=False)
+                            for s in sizes[:: max(1, len(sizes) // 8)]] + [rng.choice(np.flatnonzero(ok), 24)])
+    lo, hi = float(np.float32(prm.lnE_min)), float(np.float32(prm.lnE_max))
+    prm_o = oracle.AbinitioParams(chi_mode=cm, lnE_min=lo, lnE_max=hi)
+    otab = oracle.ChiTable(tab.chi, float(np.float32(tab.lnE_min)), float(np.float32(tab.lnE_max)))
+    worst = _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, 4, 7, None,
+                                 net=oracle.Mlp(Ws, bs, oracle.ACT_SILU), table=otab)
+    print("cfg5 %s: worst sampled-cell velocity deviation / thermal scale = %.3e over %d cells" % (chi, worst, len(cells)))
+    # table: fp32 table coordinates move chi by up to ~2e-3 near the orbiting band (Q25); MLP: Q26 (2e-2 (1 + chi))
+    assert worst < (3e-3 if chi == "table" else 3e-2)
+    ctx.close()
+
+
+def test_cfg4_full_size_sampled(dsmc):
+    n = 10_000_000
+    E, b = wl.abinitio_pair_batch(seed=3, n=n)
+    ctx = dsmc.Context(n, 1)
+    tab = oracle.build_chi_table(oracle.lj_argon(), 256, 256, n_panels=1)
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    Ed, bd = dev(E), dev(b)
+    idx = np.concatenate([np.arange(0, 300), np.arange(n - 300, n), np.random.default_rng(1).choice(n, 20000, replace=False)])
+    lo, hi = float(np.float32(tab.lnE_min)), float(np.float32(tab.lnE_max))
+    got_t = ctx.chi_batch(Ed, bd, 0, 1e-9).cpu().numpy()[idx].astype(np.float64)
+    want_t = oracle.chi_batch(E[idx], b[idx], 0, 1e-9, table=oracle.ChiTable(tab.chi, lo, hi))
+    assert np.mean(np.abs(got_t - want_t) > 1e-5 * np.maximum(np.abs(want_t), 1)) < 0.01
+    assert np.abs(got_t - want_t).max() < 5e-3
+    got_m = ctx.chi_batch(Ed, bd, 1, 1e-9, flags=dsmc.F_BF16_TC).cpu().numpy()[idx].astype(np.float64)
+    want_m = oracle.chi_batch(E[idx], b[idx], 1, 1e-9, net=oracle.Mlp(Ws, bs, oracle.ACT_SILU), lnE_min=lo, lnE_max=hi)
+    assert (np.abs(got_m - want_m) / (1 + np.abs(want_m))).max() <= 2e-2
+    ctx.check()
+    ctx.close()
