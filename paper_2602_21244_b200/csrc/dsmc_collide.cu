@@ -20,6 +20,7 @@ __global__ void k_chunk_map(int32_t K, const int32_t *__restrict__ cs, int32_t *
     big2[0] = 0;
     work[0] = 0;
     work[1] = 0;
+    work[2] = 0;
   }
   if (k > K) return;
   const int s = __ldg(cs + k);

@@ -36,9 +36,9 @@ struct FuseCtl {
   int *done_ctr[2];      // the chunk's delivered-tile counter
   int n_valid[2];        // rows of the slot that are real pairs
   int done;              // chunk groups that ran out of work
-  int next[4];           // per group: chunk handed out by the work counter
-  int slot_of[8];        // per 128-row feeder: slot taken for the tile being submitted
-  int tiles_done[4][2];  // [group][buffer]
+  int next[5];           // per group: chunk handed out by the work counter
+  int slot_of[10];       // per 128-row feeder: slot taken for the tile being submitted
+  int tiles_done[5][2];  // [group][buffer]
 };
 
 __device__ __forceinline__ void half_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
@@ -113,7 +113,9 @@ constexpr size_t chunk_region_bytes() {
   return (Chunk<LMAX, AMAX>::bytes() + 127) & ~(size_t)127;
 }
 
-template <int H, int LMAX, int AMAX, int NG, int NT, int NBUF, bool DEFERRED>
+// SRC: 0 = every chunk (work counter 0), 1 = deferred list P.big (counter 1), 2 = second list P.big2 (counter 2).
+// DST: where a chunk that does not fit this footprint goes (1 = P.big, 2 = P.big2, 0 = DSMC_ERR_CELL_TOO_LARGE).
+template <int H, int LMAX, int AMAX, int NG, int NT, int NBUF, int SRC, int DST>
 __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const StepParams P, const MlpTcDev net) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   using CK = Chunk<LMAX, AMAX>;
@@ -135,7 +137,8 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
     // ---------------- chunk group ----------------
     const int g = warp / (NT / 32);
     const TeamT<NT> T{(int)threadIdx.x - g * NT, 1 + g};
-    const int n_work = DEFERRED ? ld_volatile(P.big) : P.n_chunks;
+    const int32_t *src_list = SRC == 1 ? P.big : P.big2;
+    const int n_work = SRC == 0 ? P.n_chunks : ld_volatile(src_list);
     bool more = true, have0 = false, have1 = false;
     int b = 0;
     for (;;) {
@@ -145,7 +148,7 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
       S.carve(base + (size_t)(g * NBUF + b) * REGION);
       if (more) {
         if (T.tid == 0) {
-          *reinterpret_cast<volatile int *>(&ctl->next[g]) = atomicAdd(P.work + (DEFERRED ? 1 : 0), 1);
+          *reinterpret_cast<volatile int *>(&ctl->next[g]) = atomicAdd(P.work + SRC, 1);
           *reinterpret_cast<volatile int *>(&ctl->tiles_done[g][b]) = 0;
         }
         T.sync();
@@ -154,15 +157,16 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
         if (w >= n_work) {
           more = false;
         } else {
-          const int chunk = DEFERRED ? P.big[1 + w] : w;
+          const int chunk = SRC == 0 ? w : src_list[1 + w];
           int q0 = 0;
           const int n_loc = chunk_begin(T, P, S, chunk, q0);
           if (n_loc < 0 && T.tid == 0) {
-            if (DEFERRED) {
+            if (DST == 0) {
               *P.status = DSMC_ERR_CELL_TOO_LARGE;
             } else {
-              const int i = atomicAdd(P.big, 1);
-              P.big[1 + i] = chunk;
+              int32_t *dst_list = DST == 1 ? P.big : P.big2;
+              const int i = atomicAdd(dst_list, 1);
+              dst_list[1 + i] = chunk;
             }
           }
           if (n_loc > 0) {
@@ -274,9 +278,9 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
   pipe.teardown();
 }
 
-template <int H, int LMAX, int AMAX, int NG, int NT, int NBUF, bool DEFERRED>
+template <int H, int LMAX, int AMAX, int NG, int NT, int NBUF, int SRC, int DST>
 static int launch_pipe_one(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net, int grid) {
-  auto kern = k_collide_pipe<H, LMAX, AMAX, NG, NT, NBUF, DEFERRED>;
+  auto kern = k_collide_pipe<H, LMAX, AMAX, NG, NT, NBUF, SRC, DST>;
   const size_t smem = NG * NBUF * chunk_region_bytes<LMAX, AMAX>() + PipeShape<H>::SMEM_BYTES + sizeof(FuseCtl) + 128;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
@@ -287,10 +291,14 @@ static int launch_pipe_one(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net
 
 template <int H>
 static int launch_pipe_h(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net) {
-  const int g_main = std::max(1, std::min((p.n_chunks + 3) / 4, c->num_sms));
-  int rc = launch_pipe_one<H, 1024, kAmaxSmall, 4, 128, 1, false>(c, p, net, g_main);
+  // three footprints, as in the table path: 704-slot chunks on five 128-thread groups per SM, 1024-slot chunks
+  // on four, then any legal chunk on one 256-thread group
+  const int g0 = std::max(1, std::min((p.n_chunks + 4) / 5, c->num_sms));
+  int rc = launch_pipe_one<H, 704, kAmaxSmall, 5, 128, 1, 0, 1>(c, p, net, g0);
   if (rc != DSMC_OK) return rc;
-  return launch_pipe_one<H, kLmaxBig, kAmaxBig, 1, 256, 1, true>(c, p, net, c->num_sms);
+  rc = launch_pipe_one<H, 1024, kAmaxSmall, 4, 128, 1, 1, 2>(c, p, net, c->num_sms);
+  if (rc != DSMC_OK) return rc;
+  return launch_pipe_one<H, kLmaxBig, kAmaxBig, 1, 256, 1, 2, 0>(c, p, net, c->num_sms);
 }
 
 // op 2 (ab initio chi-MLP), plain BF16: chunk map, main pass, deferred pass
