@@ -3,9 +3,10 @@
 // in shared memory by TMA").  See dsmc_tc.cuh for the tile algebra and operand layouts.
 //
 //   k_chi_batch_tc   a10: chi for independent (E_r, b) pairs                     (BASELINE.json cfg 4)
-//   k_collide_tc     a2-a9: persistent fused step; one CTA pulls chunks (dsmc_chunk.cuh) from a work
-//                    counter, keeps the packed weights resident, and feeds the chunk's pairs through
-//                    the tile engine 128 at a time
+//   k_collide_tc     a2-a9 with the VHS-NN operator (split-BF16 operands): persistent fused step; one CTA pulls
+//                    chunks (dsmc_chunk.cuh) from a work counter, keeps the packed weights resident, and feeds
+//                    the chunk's pairs through the tile engine 128 at a time
+//   (the ab initio chi-MLP fused step is the warp-specialised k_collide_pipe, dsmc_collide_pipe.cu)
 #include <algorithm>
 #include <vector>
 

@@ -1,4 +1,4 @@
-// Device-side helpers of the CUDA path: Philox4x32-10, uniforms, Box-Muller, warp/block scans.
+// Device-side helpers of the CUDA path: Philox4x32-10, uniforms, Box-Muller, warp sums, activations.
 // Written for sm_100a; shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
@@ -52,52 +52,6 @@ __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
-}
-
-// In-place exclusive scan of a[0..L) in shared memory by the whole CTA (blockDim.x threads,
-// multiple of 32, <= 1024).  `scratch` holds >= 33 ints.  Ends with __syncthreads().
-__device__ __forceinline__ void block_excl_scan(int *a, int L, int *scratch) {
-  const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int per = (L + nt - 1) / nt;
-  const int lo = min(tid * per, L), hi = min(lo + per, L);
-  int sum = 0;
-  for (int i = lo; i < hi; ++i) sum += a[i];
-  int inc = sum;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    int t = __shfl_up_sync(0xffffffffu, inc, o);
-    if (lane >= o) inc += t;
-  }
-  if (lane == 31) scratch[warp] = inc;
-  __syncthreads();
-  if (warp == 0) {
-    int w = (lane < (nt >> 5)) ? scratch[lane] : 0;
-    int winc = w;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      int t = __shfl_up_sync(0xffffffffu, winc, o);
-      if (lane >= o) winc += t;
-    }
-    scratch[lane] = winc - w;
-  }
-  __syncthreads();
-  int run = scratch[warp] + inc - sum;
-  for (int i = lo; i < hi; ++i) {
-    int t = a[i];
-    a[i] = run;
-    run += t;
-  }
-  __syncthreads();
-}
-
-// first index c in [0, K] with cs[c] >= value (cs non-decreasing, cs[K] = n)
-__device__ __forceinline__ int lower_bound_cells(const int32_t *__restrict__ cs, int K, int64_t value) {
-  int lo = 0, hi = K;
-  while (lo < hi) {
-    int mid = (lo + hi) >> 1;
-    if ((int64_t)__ldg(cs + mid) < value) lo = mid + 1; else hi = mid;
-  }
-  return lo;
 }
 
 __device__ __forceinline__ float act_apply(int act, float z) {

@@ -32,8 +32,7 @@ struct MlpDev {
 struct MlpTcDev {
   int H;                      // 64 or 128, 0 = not available
   int d_in, d_out, act;
-  const void *w_blob;         // bf16 weights already in UMMA K-major core-matrix layout
-  const float *b1, *b2, *b3;  // fp32 biases (b3 padded to 16)
+  const void *w_blob;         // bf16 weights and biases (hi + lo parts) in UMMA K-major core-matrix layout
   uint32_t blob_bytes;
 };
 

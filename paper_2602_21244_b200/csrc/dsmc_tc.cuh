@@ -3,13 +3,14 @@
 // One "tile" is 128 pairs = the 128 rows (TMEM lanes) of a UMMA with M = 128.  The three layers of
 // h1 = act(W1 x + b1), h2 = act(W2 h1 + b2), y = W3 h2 + b3 (eq. 4) run as
 //
-//   D[128 x H]  = A1[128 x 16]   . W1p^T     SS: A1 (features) and W1p in shared memory
+//   D[128 x H]  = A1[128 x 32]   . W1p^T     SS: A1 (features) and W1p in shared memory, K = 32
 //   D[128 x H]  = A2[128 x H+16] . W2p^T     TS: A2 = bf16(act(D)) written back to TMEM by tcgen05.st
 //   D[128 x 16] = A3[128 x H+16] . W3p^T     TS
 //
-// with BF16 operands and FP32 accumulation in tensor memory.  Biases ride in the GEMMs: every A
-// operand carries a constant 1 in column d_in (layer 1) or H (layers 2, 3) and the packed weights
-// carry the bias in that column, so the epilogue is activation + pack only.
+// with BF16 operands and FP32 accumulation in tensor memory.  Layer 1 runs in split precision inside one
+// operand: A1 = [x_hi | x_lo | x_hi | 1 1 0 ..] against W1p = [W_hi | W_hi | W_lo | b_hi b_lo 0 ..].  Biases
+// of layers 2, 3 ride in the GEMMs as one extra K = 16 step: a constant (1, 1, 0, ...) column block of the A
+// operand against (b_hi, b_lo, 0, ...), so the epilogue is activation + pack only.
 //
 // Shared-memory operand layout (no swizzle, K-major "panels"): element (row r, k) of an [R x K]
 // operand sits at byte (k / 8) * R * 16 + r * 16 + (k % 8) * 2, i.e. 8 x 16 B core matrices are
