@@ -4,8 +4,8 @@
 //
 //   chunk groups (NG teams of NT threads: 5 x 128 on 704-slot chunks, 4 x 128 on 1024-slot chunks, 1 x 256 on
 //       the rest)  each group pulls chunks (dsmc_chunk.cuh) from a work counter and owns NBUF shared-memory
-//       chunk buffers (NBUF = 1 as launched: shared memory goes to more groups rather than to double buffers).  Stage A of a chunk: load, cell moments, Philox pairing keys +
-//       sort, then its pairs are SUBMITTED 128 at a time to the MLP server (features -> A1 rows of a free
+//       chunk buffers (NBUF = 1 as launched: shared memory goes to more groups rather than to double buffers).
+//       Stage A of a chunk: load, cell moments, Philox pairing keys + sort, then its pairs are SUBMITTED 128 at a time to the MLP server (features -> A1 rows of a free
 //       slot; U_eps and the acceptance bit are parked in the chunk).  Stage B: when the server has delivered
 //       chi for all tiles of the chunk, rotate + commit, matching, store.  With NBUF = 2 a group runs stage A
 //       of its next chunk while the server works on the previous one, so the ALU-bound chunk work and the
