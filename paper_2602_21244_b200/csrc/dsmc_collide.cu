@@ -267,11 +267,11 @@ int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {
   MlpDev nd{};
   const int big_grid = c->num_sms;
   if (p.op == 1) {
-    // three footprints: 704 slots and 32 cells at 9 CTAs/SM (chunks of cells up to ~230 particles), 1024 slots at 6 CTAs/SM
+    // three footprints: 704 slots and 32 cells at 9 CTAs/SM (chunks of cells up to ~230 particles), 1024 slots / 8 cells at 7 CTAs/SM
     // (one ~1000-particle cell), then anything legal on one CTA per SM
     rc = launch_one<704, 32, true, 64, 0, 1, 9, 128>(c, p, nd, p.n_chunks, 0);
     if (rc != DSMC_OK) return rc;
-    rc = launch_one<1024, kAmaxSmall, true, 64, 1, 2, 6, 128>(c, p, nd, c->num_sms * 6, 0);
+    rc = launch_one<1024, 8, true, 64, 1, 2, 7, 128>(c, p, nd, c->num_sms * 7, 0);
     if (rc != DSMC_OK) return rc;
     return launch_one<kLmaxBig, kAmaxBig, true, 64, 2, 0, 1>(c, p, nd, big_grid, 0);
   }
