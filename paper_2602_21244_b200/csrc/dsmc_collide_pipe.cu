@@ -26,8 +26,7 @@
 
 namespace dsmc {
 
-constexpr int kFuseActWarps = 8;
-constexpr int fuse_threads(int ng, int nt) { return ng * nt + kFuseActWarps * 32 + 32; }
+constexpr int fuse_threads(int ng, int nt, int na) { return ng * nt + na * 32 + 32; }  // groups + ACT warps + MMA warp
 enum { MI_NLOC = 5, MI_Q0 = 6 };  // per-buffer chunk state parked in misc[] between stage A and stage B
 
 struct FuseCtl {
@@ -37,9 +36,9 @@ struct FuseCtl {
   int *done_ctr[2];      // the chunk's delivered-tile counter
   int n_valid[2];        // rows of the slot that are real pairs
   int done;              // chunk groups that ran out of work
-  int next[5];           // per group: chunk handed out by the work counter
-  int slot_of[10];       // per 128-row feeder: slot taken for the tile being submitted
-  int tiles_done[5][2];  // [group][buffer]
+  int next[6];           // per group: chunk handed out by the work counter
+  int slot_of[12];       // per 128-row feeder: slot taken for the tile being submitted
+  int tiles_done[6][2];  // [group][buffer]
 };
 
 __device__ __forceinline__ void half_sync(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
@@ -116,8 +115,8 @@ constexpr size_t chunk_region_bytes() {
 
 // SRC: 0 = every chunk (work counter 0), 1 = deferred list P.big (counter 1), 2 = second list P.big2 (counter 2).
 // DST: where a chunk that does not fit this footprint goes (1 = P.big, 2 = P.big2, 0 = DSMC_ERR_CELL_TOO_LARGE).
-template <int H, int LMAX, int AMAX, int NG, int NT, int NBUF, int SRC, int DST>
-__global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const StepParams P, const MlpTcDev net) {
+template <int H, int LMAX, int AMAX, int NG, int NT, int NA, int NBUF, int SRC, int DST>
+__global__ void __launch_bounds__(fuse_threads(NG, NT, NA), 1) k_collide_pipe(const StepParams P, const MlpTcDev net) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   using CK = Chunk<LMAX, AMAX>;
   constexpr size_t REGION = chunk_region_bytes<LMAX, AMAX>();
@@ -130,7 +129,7 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
     ctl->outcnt[0] = ctl->outcnt[1] = 0;
     ctl->done = 0;
   }
-  pipe.init(pipe_base, net.w_blob, kFuseActWarps, 4);  // ends with CTA-wide barriers
+  pipe.init(pipe_base, net.w_blob, NA, 4);  // ends with CTA-wide barriers
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   constexpr int GW = NG * NT / 32;  // warps of the chunk groups
@@ -202,7 +201,7 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
       __threadfence_block();
       atomicAdd(&ctl->done, 1);
     }
-  } else if (warp < GW + kFuseActWarps) {
+  } else if (warp < GW + NA) {
     // ---------------- MLP server: activation + delivery warps ----------------
     using SH = PipeShape<H>;
     const int aw = warp - GW;
@@ -232,12 +231,12 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
       bool any = false;
       if (tc::mbar_test(pipe.full_e + 0, ph0)) {
         ph0 ^= 1u;
-        pipe.template act_body<kFuseActWarps / 4>(net.act, 0, aw);
+        pipe.template act_body<NA / 4>(net.act, 0, aw);
         any = true;
       }
       if (tc::mbar_test(pipe.full_e + 1, ph1)) {
         ph1 ^= 1u;
-        pipe.template act_body<kFuseActWarps / 4>(net.act, 1, aw);
+        pipe.template act_body<NA / 4>(net.act, 1, aw);
         any = true;
       }
       if (aw < 4) {
@@ -279,13 +278,13 @@ __global__ void __launch_bounds__(fuse_threads(NG, NT), 1) k_collide_pipe(const 
   pipe.teardown();
 }
 
-template <int H, int LMAX, int AMAX, int NG, int NT, int NBUF, int SRC, int DST>
+template <int H, int LMAX, int AMAX, int NG, int NT, int NA, int NBUF, int SRC, int DST>
 static int launch_pipe_one(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net, int grid) {
-  auto kern = k_collide_pipe<H, LMAX, AMAX, NG, NT, NBUF, SRC, DST>;
+  auto kern = k_collide_pipe<H, LMAX, AMAX, NG, NT, NA, NBUF, SRC, DST>;
   const size_t smem = NG * NBUF * chunk_region_bytes<LMAX, AMAX>() + PipeShape<H>::SMEM_BYTES + sizeof(FuseCtl) + 128;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
-  kern<<<grid, fuse_threads(NG, NT), smem, c->stream>>>(p, net);
+  kern<<<grid, fuse_threads(NG, NT, NA), smem, c->stream>>>(p, net);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
@@ -295,11 +294,11 @@ static int launch_pipe_h(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net) 
   // three footprints, as in the table path: 704-slot chunks on five 128-thread groups per SM, 1024-slot chunks
   // on four, then any legal chunk on one 256-thread group
   const int g0 = std::max(1, std::min((p.n_chunks + 4) / 5, c->num_sms));
-  int rc = launch_pipe_one<H, 704, kAmaxSmall, 5, 128, 1, 0, 1>(c, p, net, g0);
+  int rc = launch_pipe_one<H, 704, kAmaxSmall, 5, 128, 8, 1, 0, 1>(c, p, net, g0);  // (6 groups + 4 ACT warps: slower)
   if (rc != DSMC_OK) return rc;
-  rc = launch_pipe_one<H, 1024, kAmaxSmall, 4, 128, 1, 1, 2>(c, p, net, c->num_sms);
+  rc = launch_pipe_one<H, 1024, kAmaxSmall, 4, 128, 8, 1, 1, 2>(c, p, net, c->num_sms);
   if (rc != DSMC_OK) return rc;
-  return launch_pipe_one<H, kLmaxBig, kAmaxBig, 1, 256, 1, 2, 0>(c, p, net, c->num_sms);
+  return launch_pipe_one<H, kLmaxBig, kAmaxBig, 1, 256, 8, 1, 2, 0>(c, p, net, c->num_sms);
 }
 
 // op 2 (ab initio chi-MLP), plain BF16: chunk map, main pass, deferred pass
