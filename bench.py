@@ -345,6 +345,20 @@ def run_b200(args):
             torch.cuda.synchronize()
             ms4 = a0.elapsed_time(a1) / 10
             cfg4[name] = {"ms": ms4, "pairs_per_s": n4 / (ms4 * 1e-3)}
+        # the computation the operators above replace: deflection-integral quadrature per pair
+        for _ in range(2):
+            ctx.chi_exact_batch(E4d, b4d, out=o4)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a0.record()
+        for _ in range(3):
+            ctx.chi_exact_batch(E4d, b4d, out=o4)
+        a1.record()
+        torch.cuda.synchronize()
+        msx = a0.elapsed_time(a1) / 3
+        cfg4["exact_quadrature_fp64"] = {"ms": msx, "pairs_per_s": n4 / (msx * 1e-3),
+                                         "table_speedup": msx / cfg4["table"]["ms"],
+                                         "mlp_tc_speedup": msx / cfg4["mlp_tc"]["ms"]}
         fl4 = n4 * 2 * (2 * 128 + 128 * 128 + 128)
         cfg4["mlp_tc"]["tensor_frac"] = fl4 / (cfg4["mlp_tc"]["ms"] * 1e-3) / 1e12 / tc_sust
         cfg4["table"]["hbm_frac"] = n4 * 12 / (cfg4["table"]["ms"] * 1e-3) / 1e9 / hbm_peak

@@ -12,6 +12,7 @@
  *   dsmc_cell_moments      per-cell momentum / energy sums (eq. 10)
  *   dsmc_moment_match      cell-wise correction on its own (eqs. 10-11)
  *   dsmc_chi_batch         chi for independent (E_r, b) pairs
+ *   dsmc_chi_exact_batch   chi by the deflection-integral quadrature itself (eq. 16), LJ 12-6
  *   dsmc_step_host         bin + fused step on HOST buffers (copies inside), for end-to-end timing
  *
  * Conventions
@@ -177,6 +178,16 @@ int dsmc_moment_match(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *
  * flags & DSMC_F_BF16_TC selects the tensor-core MLP. */
 int dsmc_chi_batch(dsmc_ctx *ctx, int64_t n, const float *E_over_k, const float *b, float *chi,
                    int32_t chi_mode, float b_max, float lnE_min, float lnE_max, uint32_t flags);
+
+/* ---- "exact" chi for n independent pairs (the computation the neural operators replace) ----
+ * Classical deflection integral of eq. 16 for a Lennard-Jones 12-6 potential with well depth
+ * eps_over_k [K] and diameter sigma [m], per pair, in FP64: largest root r_min of eq. 21, then
+ * Gauss-Legendre quadrature in the variable of P:L342 with the end-point singularity removed analytically.
+ * E_over_k [K], b [m] -> chi [rad], SIGNED (negative = attractive glancing collision, Q14) unless
+ * flags & DSMC_F_CHI_ABS.  b <= 0 gives pi.  Near the orbiting condition the integral is ill-conditioned (Q23). */
+#define DSMC_F_CHI_ABS 64u
+int dsmc_chi_exact_batch(dsmc_ctx *ctx, int64_t n, const float *E_over_k, const float *b, float *chi,
+                         float eps_over_k, float sigma, uint32_t flags);
 
 /* ---- end-to-end helper on HOST buffers ----------------------------------------------------
  * Copies cell/vx/vy/vz (HOST, ideally pinned) to context-owned device buffers, runs dsmc_bin and

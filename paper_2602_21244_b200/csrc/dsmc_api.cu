@@ -343,6 +343,15 @@ static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
   return DSMC_OK;
 }
 
+int dsmc_chi_exact_batch(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, float eps_over_k,
+                         float sigma, uint32_t flags) {
+  if (!c || n < 0 || !(eps_over_k > 0.f) || !(sigma > 0.f)) return DSMC_ERR_INVALID_ARG;
+  if (n == 0) return DSMC_OK;
+  if (!E_over_k || !b || !chi) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_chi_exact(c, n, E_over_k, b, chi, (double)eps_over_k, (double)sigma, (flags & DSMC_F_CHI_ABS) ? 1 : 0);
+}
+
 int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, const float *vx_h, const float *vy_h,
                    const float *vz_h, float *vx_out_h, float *vy_out_h, float *vz_out_h, int32_t *perm_h,
                    int32_t *cell_start_h, const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi,

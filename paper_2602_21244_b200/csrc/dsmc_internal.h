@@ -130,6 +130,8 @@ int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, flo
                      float lnE_min, float lnE_max, const MlpDev *net);
 int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
                         float lnE_min, float lnE_max, const MlpTcDev *net);
+int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, double eps_over_k,
+                     double sigma, int take_abs);
 // host-side packing of the tensor-core weight image (dsmc_collide_tc.cu)
 int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStream_t s);
 }  // namespace dsmc

@@ -21,13 +21,13 @@ ERR_INVALID_ARG, ERR_BAD_CELL_INDEX, ERR_CELL_TOO_LARGE = -1, -2, -3
 ERR_NOT_CONFIGURED, ERR_CUDA, ERR_UNSUPPORTED_SHAPE = -4, -5, -6
 MAX_CELL_PARTICLES = 2048
 
-F_NOISE, F_ENERGY_SHELL, F_MOMENT_MATCH, F_ACCEPT, F_BF16_TC, F_MATCH_ENERGY_ONLY = 1, 2, 4, 8, 16, 32
+F_NOISE, F_ENERGY_SHELL, F_MOMENT_MATCH, F_ACCEPT, F_BF16_TC, F_MATCH_ENERGY_ONLY, F_CHI_ABS = 1, 2, 4, 8, 16, 32, 64
 ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 
 EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
-           "dsmc_step_host"]
+           "dsmc_chi_exact_batch", "dsmc_step_host"]
 
 
 class DsmcError(RuntimeError):
@@ -265,6 +265,17 @@ class Context:
                                  _ptr(b, torch.float32), _ptr(out, torch.float32), C.c_int32(chi_mode),
                                  C.c_float(b_max), C.c_float(lnE_min), C.c_float(lnE_max), C.c_uint32(flags)),
              "dsmc_chi_batch")
+        return out
+
+    def chi_exact_batch(self, E_over_k, b, eps_over_k: float = 119.8, sigma: float = 3.405e-10, flags: int = 0,
+                        out=None):
+        """chi by the deflection-integral quadrature itself (LJ 12-6), signed unless flags & F_CHI_ABS."""
+        if out is None:
+            out = torch.empty_like(E_over_k)
+        self._stream()
+        _chk(_lib.dsmc_chi_exact_batch(self._h, C.c_int64(E_over_k.shape[0]), _ptr(E_over_k, torch.float32),
+                                       _ptr(b, torch.float32), _ptr(out, torch.float32), C.c_float(eps_over_k),
+                                       C.c_float(sigma), C.c_uint32(flags)), "dsmc_chi_exact_batch")
         return out
 
     # ---- end to end on host buffers (pinned CPU tensors)

@@ -490,3 +490,36 @@ def test_sharded_step_matches_unsharded(dsmc, tc):
         for a, b in zip(lt, full):
             assert torch.equal(a, b[q0:q0 + a.shape[0]])
     ctx.close()
+
+
+# --------------------------------------------------------------------------------------- (f3) exact chi
+def test_chi_exact_batch_golden_and_oracle(dsmc):
+    """dsmc_chi_exact_batch (deflection-integral quadrature on the GPU, FP64 inside, fp32 in / out) against
+    (a) the LJ worked values of tests/golden (SURVEY pin P8) and (b) the oracle's quadrature on a grid of
+    (E*, b*) away from the orbiting band (Q23).  fp32 inputs limit the agreement to ~1e-6."""
+    import os
+    eps_k, sig = 119.8, 3.405e-10
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "lj_chi_worked_values.txt"))
+            if l.strip() and not l.startswith("#")]
+    Es = np.array([float(r[0]) for r in rows]); bs = np.array([float(r[1]) for r in rows]); want = np.array([float(r[2]) for r in rows])
+    ctx = dsmc.Context(1 << 16, 1)
+    E32, b32 = (Es * eps_k).astype(np.float32), (bs * sig).astype(np.float32)
+    got = ctx.chi_exact_batch(dev(E32), dev(b32), eps_k, sig).cpu().numpy().astype(np.float64)
+    ctx.check()
+    assert np.abs(got - want).max() < 5e-6, np.abs(got - want).max()
+    # grid against the oracle, evaluated at the fp32-rounded inputs; E* >= 1 keeps clear of the orbiting band
+    rng = np.random.default_rng(5)
+    n = 4000
+    Er = np.exp(rng.uniform(np.log(1.0), np.log(500.0), n)); br = rng.uniform(0.0, 2.9, n)
+    E32, b32 = (Er * eps_k).astype(np.float32), (br * sig).astype(np.float32)
+    b32[:5] = 0.0
+    got = ctx.chi_exact_batch(dev(E32), dev(b32), eps_k, sig).cpu().numpy().astype(np.float64)
+    pot = oracle.lj_argon()
+    ref = np.array([oracle.chi_exact(pot, float(e) * KB, float(b)) for e, b in zip(E32, b32)])
+    d = np.abs(got - ref)
+    print("chi exact vs oracle: median %.2e, 99.9%% %.2e, max %.2e" % (np.median(d), np.quantile(d, 0.999), d.max()))
+    assert np.all(got[:5] == np.float32(np.pi))
+    assert np.quantile(d, 0.999) < 5e-6 and d.max() < 1e-3  # a handful of points sit next to the orbiting curve
+    absd = ctx.chi_exact_batch(dev(E32), dev(b32), eps_k, sig, flags=dsmc.F_CHI_ABS).cpu().numpy()
+    assert np.array_equal(absd, np.abs(got.astype(np.float32)))
+    ctx.close()
