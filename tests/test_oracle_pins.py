@@ -556,3 +556,25 @@ def test_workload_shapes_match_baseline_configs():
     assert ratio[-1] / ratio[0] > 15  # 16x density contrast between shock band and wake
     rc, perm, cs = oracle.bin_particles(p.cell, p.n_cells)
     np.testing.assert_array_equal(np.diff(cs), p.counts)
+
+
+def test_chapman_enskog_collision_integral_of_lj_matches_textbook():
+    """Pin P14 (physics level, independent of the oracle): the deflection angles of the oracle's quadrature,
+    pushed through Q^(2)(E) = 2 pi int (1 - cos^2 chi) b db (eq. 19) and the Maxwellian average of eq. 18
+    in its standard Chapman-Enskog form, must reproduce the tabulated reduced collision integral Omega^(2,2)* of
+    the Lennard-Jones gas (tests/golden/lj_omega22_textbook.txt).  A wrong sign, a wrong root or a dropped factor
+    in the quadrature moves these numbers by far more than the 0.5 % allowed here."""
+    pot = oracle.lj_argon()
+    eps, sig = 119.8 * KB, 3.405e-10
+    rows = [l.split() for l in open(os.path.join(GOLD, "lj_omega22_textbook.txt")) if l.strip() and not l.startswith("#")]
+    xs, ws = np.polynomial.laguerre.laggauss(20)
+    nb, bmax = 400, 4.0
+    bs = (np.arange(nb) + 0.5) * bmax / nb
+
+    def q2_star(Es):
+        chi = np.array([oracle.chi_exact(pot, Es * eps, b * sig) for b in bs])
+        return 3.0 * np.sum((1.0 - np.cos(chi) ** 2) * bs) * bmax / nb
+
+    for Ts, want in ((float(r[0]), float(r[1])) for r in rows):
+        got = sum(w * x ** 3 * q2_star(x * Ts) for x, w in zip(xs, ws)) / 6.0
+        assert abs(got / want - 1.0) < 5e-3, (Ts, got, want)
