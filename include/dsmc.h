@@ -13,6 +13,7 @@
  *   dsmc_moment_match      cell-wise correction on its own (eqs. 10-11)
  *   dsmc_chi_batch         chi for independent (E_r, b) pairs
  *   dsmc_chi_exact_batch   chi by the deflection-integral quadrature itself (eq. 16), LJ 12-6
+ *   dsmc_build_chi_table_lj  the chi table generated on the device by that quadrature
  *   dsmc_step_host         bin + fused step on HOST buffers (copies inside), for end-to-end timing
  *
  * Conventions
@@ -188,6 +189,13 @@ int dsmc_chi_batch(dsmc_ctx *ctx, int64_t n, const float *E_over_k, const float 
 #define DSMC_F_CHI_ABS 64u
 int dsmc_chi_exact_batch(dsmc_ctx *ctx, int64_t n, const float *E_over_k, const float *b, float *chi,
                          float eps_over_k, float sigma, uint32_t flags);
+
+/* Generates the chi table ON THE DEVICE by that quadrature (the paper's exact 512 x 512 table takes
+ * "several hours" on a CPU cluster) and installs it as the context's table exactly as dsmc_set_chi_table
+ * would: nodes as documented there, abs(chi) rounded to fp32 (Q14).  chi_out: optional DEVICE array [nE][nB] that
+ * receives the node values.  Synchronises the stream. */
+int dsmc_build_chi_table_lj(dsmc_ctx *ctx, int32_t nE, int32_t nB, float lnE_min, float lnE_max, float b_max,
+                            float eps_over_k, float sigma, float *chi_out);
 
 /* ---- end-to-end helper on HOST buffers ----------------------------------------------------
  * Copies cell/vx/vy/vz (HOST, ideally pinned) to context-owned device buffers, runs dsmc_bin and

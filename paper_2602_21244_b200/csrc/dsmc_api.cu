@@ -343,6 +343,39 @@ static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
   return DSMC_OK;
 }
 
+int dsmc_build_chi_table_lj(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, float lnE_max, float b_max,
+                            float eps_over_k, float sigma, float *chi_out) {
+  if (!c || nE < 2 || nB < 2 || !(lnE_max > lnE_min) || !(b_max > 0.f) || !(eps_over_k > 0.f) || !(sigma > 0.f))
+    return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  cudaFree(c->d_table);
+  c->d_table = nullptr;
+  c->has_table = false;
+  const size_t nq = (size_t)(nE - 1) * (nB - 1), nn = (size_t)nE * nB;
+  float *nodes = nullptr;
+  CK(cudaMalloc(&c->d_table, sizeof(float) * 4 * nq));
+  CK(cudaMalloc(&nodes, sizeof(float) * nn));
+  int rc = launch_chi_table_lj(c, nE, nB, (double)lnE_min, (double)lnE_max, (double)b_max, (double)eps_over_k,
+                               (double)sigma, nodes, reinterpret_cast<float4 *>(c->d_table));
+  if (rc == DSMC_OK && chi_out &&
+      cudaMemcpyAsync(chi_out, nodes, sizeof(float) * nn, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+    rc = DSMC_ERR_CUDA;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) rc = DSMC_ERR_CUDA;
+  cudaFree(nodes);
+  if (rc != DSMC_OK) return rc;
+  c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
+  c->table.nE = nE;
+  c->table.nB = nB;
+  c->table.lnE_min = lnE_min;
+  const double inv = (double)(nE - 1) / ((double)lnE_max - (double)lnE_min);
+  c->table.inv_dlnE = (float)inv;
+  c->table.c1 = (float)(0.6931471805599453 * inv);
+  c->table.c0 = (float)(-(double)lnE_min * inv);
+  c->has_table = true;
+  return DSMC_OK;
+}
+
 int dsmc_chi_exact_batch(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, float eps_over_k,
                          float sigma, uint32_t flags) {
   if (!c || n < 0 || !(eps_over_k > 0.f) || !(sigma > 0.f)) return DSMC_ERR_INVALID_ARG;

@@ -31,59 +31,87 @@ __device__ __forceinline__ double lj_over_E(double r, double inv_E) {  // V*(r) 
   return 4.0 * (i6 * i6 - i6) * inv_E;
 }
 
+// signed chi for reduced energy Es = E / eps and reduced impact parameter bs = b / sigma
+__device__ double chi_exact_lj(double Es, double bs) {
+  double out;
+  if (!(bs > 0.0) || !(Es > 0.0)) {
+    out = 3.141592653589793;
+  } else {
+    const double inv_E = 1.0 / Es, b2 = bs * bs;
+    // 1. largest root of F
+    double hi = fmax(50.0, 2.0 * bs), lo = hi;
+    {
+      const double q = 0.97;
+      for (int it = 0; it < 400; ++it) {
+        lo = hi * q;
+        const double F = 1.0 - b2 / (lo * lo) - lj_over_E(lo, inv_E);
+        if (F < 0.0) break;
+        hi = lo;
+      }
+    }
+    for (int it = 0; it < 64; ++it) {  // F(lo) < 0 <= F(hi)
+      const double mid = 0.5 * (lo + hi);
+      const double F = 1.0 - b2 / (mid * mid) - lj_over_E(mid, inv_E);
+      if (F < 0.0) lo = mid; else hi = mid;
+    }
+    const double rmin = hi, beta = bs / rmin, beta2 = beta * beta;
+    // 2. quadrature in s.  F~(1) = 0 at the root, so F~(u) = F~(u) - F~(1) = s^2 G(s) with
+    //    G = beta^2 (1 + u) + (4 / E) [a^12 P12(u) - a^6 P6(u)],  a = 1 / r_min,  Pn(u) = 1 + u + ... + u^(n-1)
+    //    (1 - u^n = (1 - u) Pn(u), 1 - u = s^2): the integrand s / sqrt(F~) = 1 / sqrt(G) is smooth and free of
+    //    cancellation.  Panel edges graded as (k / kPanels)^2 (G(0) is small near orbiting).
+    const double a2 = 1.0 / (rmin * rmin), a6 = a2 * a2 * a2, a12 = a6 * a6;
+    const double c12 = 4.0 * inv_E * a12, c6 = 4.0 * inv_E * a6;
+    double acc = 0.0;
+    for (int k = 0; k < kPanels; ++k) {
+      const double e0 = (double)(k * k) / (kPanels * kPanels), e1 = (double)((k + 1) * (k + 1)) / (kPanels * kPanels);
+      const double h = e1 - e0;
+      double part = 0.0;
+#pragma unroll 4
+      for (int j = 0; j < kGl; ++j) {
+        const double sx = e0 + h * c_gl_x[j];
+        const double u = 1.0 - sx * sx;
+        const double u2 = u * u, u3 = u2 * u;
+        const double p6 = (1.0 + u + u2) * (1.0 + u3);  // 1 + u + ... + u^5
+        const double p12 = p6 * (1.0 + u3 * u3);        // 1 + u + ... + u^11
+        const double G = beta2 * (1.0 + u) + c12 * p12 - c6 * p6;
+        part += c_gl_w[j] * rsqrt(fmax(G, 1e-300));
+      }
+      acc += h * part;
+    }
+    out = 3.141592653589793 - 4.0 * beta * acc;
+  }
+  return out;
+}
+
 __global__ void __launch_bounds__(128) k_chi_exact(int64_t n, const float *__restrict__ E_over_k,
                                                   const float *__restrict__ b, float *__restrict__ chi,
                                                   double inv_eps_k, double inv_sigma, int take_abs) {
   for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-    const double Es = (double)__ldg(E_over_k + p) * inv_eps_k, bs = (double)__ldg(b + p) * inv_sigma;
-    double out;
-    if (!(bs > 0.0) || !(Es > 0.0)) {
-      out = 3.141592653589793;
-    } else {
-      const double inv_E = 1.0 / Es, b2 = bs * bs;
-      // 1. largest root of F
-      double hi = fmax(50.0, 2.0 * bs), lo = hi;
-      {
-        const double q = 0.97;
-        for (int it = 0; it < 400; ++it) {
-          lo = hi * q;
-          const double F = 1.0 - b2 / (lo * lo) - lj_over_E(lo, inv_E);
-          if (F < 0.0) break;
-          hi = lo;
-        }
-      }
-      for (int it = 0; it < 64; ++it) {  // F(lo) < 0 <= F(hi)
-        const double mid = 0.5 * (lo + hi);
-        const double F = 1.0 - b2 / (mid * mid) - lj_over_E(mid, inv_E);
-        if (F < 0.0) lo = mid; else hi = mid;
-      }
-      const double rmin = hi, beta = bs / rmin, beta2 = beta * beta;
-      // 2. quadrature in s.  F~(1) = 0 at the root, so F~(u) = F~(u) - F~(1) = s^2 G(s) with
-      //    G = beta^2 (1 + u) + (4 / E) [a^12 P12(u) - a^6 P6(u)],  a = 1 / r_min,  Pn(u) = 1 + u + ... + u^(n-1)
-      //    (1 - u^n = (1 - u) Pn(u), 1 - u = s^2): the integrand s / sqrt(F~) = 1 / sqrt(G) is smooth and free of
-      //    cancellation.  Panel edges graded as (k / kPanels)^2 (G(0) is small near orbiting).
-      const double a2 = 1.0 / (rmin * rmin), a6 = a2 * a2 * a2, a12 = a6 * a6;
-      const double c12 = 4.0 * inv_E * a12, c6 = 4.0 * inv_E * a6;
-      double acc = 0.0;
-      for (int k = 0; k < kPanels; ++k) {
-        const double e0 = (double)(k * k) / (kPanels * kPanels), e1 = (double)((k + 1) * (k + 1)) / (kPanels * kPanels);
-        const double h = e1 - e0;
-        double part = 0.0;
-#pragma unroll 4
-        for (int j = 0; j < kGl; ++j) {
-          const double sx = e0 + h * c_gl_x[j];
-          const double u = 1.0 - sx * sx;
-          const double u2 = u * u, u3 = u2 * u;
-          const double p6 = (1.0 + u + u2) * (1.0 + u3);  // 1 + u + ... + u^5
-          const double p12 = p6 * (1.0 + u3 * u3);        // 1 + u + ... + u^11
-          const double G = beta2 * (1.0 + u) + c12 * p12 - c6 * p6;
-          part += c_gl_w[j] * rsqrt(fmax(G, 1e-300));
-        }
-        acc += h * part;
-      }
-      out = 3.141592653589793 - 4.0 * beta * acc;
-    }
+    const double out = chi_exact_lj((double)__ldg(E_over_k + p) * inv_eps_k, (double)__ldg(b + p) * inv_sigma);
     chi[p] = (float)(take_abs ? fabs(out) : out);
+  }
+}
+
+// chi table nodes (Q13): node (iE, iB) at E~ = lnE_min + iE dlnE (E~ = ln(E_r / k_B [K])), b~ = iB / (nB - 1);
+// stores abs(chi) (Q14) rounded to fp32, chi[iE * nB + iB]
+__global__ void __launch_bounds__(128) k_chi_table_lj(int nE, int nB, double lnE_min, double dlnE, double bmax_star,
+                                                     double inv_eps_k, float *__restrict__ table) {
+  const int64_t total = (int64_t)nE * nB;
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < total; p += (int64_t)gridDim.x * blockDim.x) {
+    const int iE = (int)(p / nB), iB = (int)(p % nB);
+    const double Es = exp(lnE_min + iE * dlnE) * inv_eps_k;
+    const double bs = bmax_star * ((double)iB / (double)(nB - 1));
+    table[p] = (float)fabs(chi_exact_lj(Es, bs));
+  }
+}
+
+// quad[iE (nB-1) + iB] = the four nodes around grid cell (iE, iB): one 16-byte load per lookup
+__global__ void k_quad_from_table(int nE, int nB, const float *__restrict__ table, float4 *__restrict__ quad) {
+  const int64_t total = (int64_t)(nE - 1) * (nB - 1);
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < total; p += (int64_t)gridDim.x * blockDim.x) {
+    const int iE = (int)(p / (nB - 1)), iB = (int)(p % (nB - 1));
+    const float *t = table + (size_t)iE * nB + iB;
+    quad[p] = make_float4(t[0], t[1], t[nB], t[nB + 1]);
   }
 }
 
@@ -109,8 +137,24 @@ static void gauss_legendre_01(int n, double *x, double *w) {
   }
 }
 
-int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, double eps_over_k,
-                     double sigma, int take_abs) {
+static int upload_gl_nodes(dsmc_ctx *c);
+
+// generates the table on the device and installs it as the context's chi table (device copy in `table_dev`,
+// nE * nB floats, owned by the caller / context)
+int launch_chi_table_lj(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_max, double b_max, double eps_over_k,
+                        double sigma, float *table_dev, float4 *quad_dev) {
+  int rc = upload_gl_nodes(c);
+  if (rc != DSMC_OK) return rc;
+  const int64_t total = (int64_t)nE * nB;
+  const int grid = (int)std::min<int64_t>((total + 127) / 128, (int64_t)c->num_sms * 16);
+  k_chi_table_lj<<<grid, 128, 0, c->stream>>>(nE, nB, lnE_min, (lnE_max - lnE_min) / (nE - 1), b_max / sigma,
+                                              1.0 / eps_over_k, table_dev);
+  k_quad_from_table<<<grid, 128, 0, c->stream>>>(nE, nB, table_dev, quad_dev);
+  c->launches += 2;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+static int upload_gl_nodes(dsmc_ctx *c) {
   static std::once_flag once[64];
   static cudaError_t upload_rc[64];
   const int dev = c->device < 64 ? c->device : 63;
@@ -120,7 +164,13 @@ int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float 
     upload_rc[dev] = cudaMemcpyToSymbol(c_gl_x, x, sizeof(x));
     if (upload_rc[dev] == cudaSuccess) upload_rc[dev] = cudaMemcpyToSymbol(c_gl_w, w, sizeof(w));
   });
-  if (upload_rc[dev] != cudaSuccess) return DSMC_ERR_CUDA;
+  return upload_rc[dev] == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, double eps_over_k,
+                     double sigma, int take_abs) {
+  const int rc = upload_gl_nodes(c);
+  if (rc != DSMC_OK) return rc;
   const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms * 16);
   k_chi_exact<<<grid, 128, 0, c->stream>>>(n, E_over_k, b, chi, 1.0 / eps_over_k, 1.0 / sigma, take_abs);
   c->launches += 1;

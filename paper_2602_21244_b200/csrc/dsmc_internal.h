@@ -132,6 +132,8 @@ int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, 
                         float lnE_min, float lnE_max, const MlpTcDev *net);
 int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, double eps_over_k,
                      double sigma, int take_abs);
+int launch_chi_table_lj(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_max, double b_max, double eps_over_k,
+                        double sigma, float *table_dev, float4 *quad_dev);
 // host-side packing of the tensor-core weight image (dsmc_collide_tc.cu)
 int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStream_t s);
 }  // namespace dsmc

@@ -27,7 +27,7 @@ ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
-           "dsmc_chi_exact_batch", "dsmc_step_host"]
+           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host"]
 
 
 class DsmcError(RuntimeError):
@@ -265,6 +265,18 @@ class Context:
                                  _ptr(b, torch.float32), _ptr(out, torch.float32), C.c_int32(chi_mode),
                                  C.c_float(b_max), C.c_float(lnE_min), C.c_float(lnE_max), C.c_uint32(flags)),
              "dsmc_chi_batch")
+        return out
+
+    def build_chi_table_lj(self, nE: int, nB: int, lnE_min=float(np.log(5.0)), lnE_max=float(np.log(6.0e4)),
+                           b_max: float = 1e-9, eps_over_k: float = 119.8, sigma: float = 3.405e-10,
+                           want_nodes: bool = False):
+        """Generate the LJ chi table on the device and install it; returns the [nE, nB] node tensor if asked."""
+        out = torch.empty((nE, nB), dtype=torch.float32, device=self.device) if want_nodes else None
+        self._stream()
+        _chk(_lib.dsmc_build_chi_table_lj(self._h, C.c_int32(nE), C.c_int32(nB), C.c_float(lnE_min), C.c_float(lnE_max),
+                                          C.c_float(b_max), C.c_float(eps_over_k), C.c_float(sigma),
+                                          _ptr(out, torch.float32) if out is not None else C.c_void_p(0)),
+             "dsmc_build_chi_table_lj")
         return out
 
     def chi_exact_batch(self, E_over_k, b, eps_over_k: float = 119.8, sigma: float = 3.405e-10, flags: int = 0,

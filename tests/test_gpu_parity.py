@@ -523,3 +523,55 @@ def test_chi_exact_batch_golden_and_oracle(dsmc):
     absd = ctx.chi_exact_batch(dev(E32), dev(b32), eps_k, sig, flags=dsmc.F_CHI_ABS).cpu().numpy()
     assert np.array_equal(absd, np.abs(got.astype(np.float32)))
     ctx.close()
+
+
+def test_build_chi_table_on_device(dsmc):
+    """(f2) the chi table generated on the GPU by the quadrature kernel against the oracle's table builder, node by
+    node outside the orbiting band (Q23), and lookups through the installed table against the oracle's bilinear."""
+    nE = nB = 128
+    lo, hi = float(np.float32(np.log(5.0))), float(np.float32(np.log(6.0e4)))
+    ctx = dsmc.Context(1 << 16, 1)
+    got = ctx.build_chi_table_lj(nE, nB, lo, hi, 1e-9, want_nodes=True).cpu().numpy().astype(np.float64)
+    ctx.check()
+    tab = oracle.build_chi_table(oracle.lj_argon(), nE, nB, lnE_min=lo, lnE_max=hi, b_max=1e-9, n_panels=2)
+    want = tab.chi.astype(np.float64)
+    d = np.abs(got - want)
+    # orbiting band: rows with E* < 0.8 near the orbiting impact parameter are ill-conditioned (chi -> infinity);
+    # compare where the table is smooth (neighbouring nodes within 0.5 rad)
+    smooth = np.ones_like(d, bool)
+    smooth[:, 1:] &= np.abs(np.diff(want, axis=1)) < 0.5
+    smooth[:, :-1] &= np.abs(np.diff(want, axis=1)) < 0.5
+    print("device-built chi table: max diff on smooth nodes %.2e (%.1f%% of nodes), elsewhere median %.2e"
+          % (d[smooth].max(), 100 * smooth.mean(), np.median(d[~smooth]) if (~smooth).any() else 0.0))
+    assert smooth.mean() > 0.97
+    assert d[smooth].max() < 5e-6
+    assert got[:, 0].min() == np.float32(np.pi) and got[:, 0].max() == np.float32(np.pi)  # b = 0: head-on
+    # the installed table serves lookups
+    E, b = wl.abinitio_pair_batch(seed=9, n=50_000)
+    chi = ctx.chi_batch(dev(E), dev(b), 0, 1e-9).cpu().numpy().astype(np.float64)
+    ref = oracle.chi_batch(E, b, 0, 1e-9, table=oracle.ChiTable(got.astype(np.float32), lo, hi))
+    sl = _table_slope(oracle.ChiTable(got.astype(np.float32), lo, hi), np.log(E.astype(np.float64)), b.astype(np.float64) / 1e-9)
+    assert np.all(np.abs(chi - ref) <= 1e-5 * np.maximum(np.abs(ref), 1) + 2e-4 * sl + 1e-6)
+    ctx.close()
+
+
+def test_chapman_enskog_from_the_gpu_quadrature(dsmc):
+    """(f2) physics check that does not involve the oracle: Omega^(2,2)*(T*) of the LJ gas from the GPU's own
+    deflection angles (eqs. 18-19, standard Chapman-Enskog form) against the textbook table."""
+    import os
+    eps_k, sig = 119.8, 3.405e-10
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "lj_omega22_textbook.txt"))
+            if l.strip() and not l.startswith("#")]
+    xs, ws = np.polynomial.laguerre.laggauss(20)
+    nb, bmax = 2000, 4.0
+    bs = (np.arange(nb) + 0.5) * bmax / nb
+    ctx = dsmc.Context(1 << 18, 1)
+    for Ts, want in ((float(r[0]), float(r[1])) for r in rows):
+        E = np.repeat(xs * Ts * eps_k, nb).astype(np.float32)
+        b = np.tile(bs * sig, len(xs)).astype(np.float32)
+        chi = ctx.chi_exact_batch(dev(E), dev(b), eps_k, sig).cpu().numpy().astype(np.float64).reshape(len(xs), nb)
+        q2 = 3.0 * ((1.0 - np.cos(chi) ** 2) * bs[None, :]).sum(axis=1) * bmax / nb
+        got = float((ws * xs ** 3 * q2).sum() / 6.0)
+        print("Omega22*(T* = %g) = %.4f (textbook %.4f)" % (Ts, got, want))
+        assert abs(got / want - 1.0) < 5e-3
+    ctx.close()
