@@ -26,6 +26,7 @@ _LIB = os.path.join(_DIR, "liboracle.so")
 KB = 1.380649e-23
 
 F_NOISE, F_ENERGY_SHELL, F_MOMENT_MATCH, F_ACCEPT, F_MATCH_ENERGY_ONLY = 1, 2, 4, 8, 32
+F_PAIR_REPLACE = 128
 ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 POT_LJ, POT_HARD_SPHERE, POT_INV_R, POT_INV_R2 = 0, 1, 2, 3
 
@@ -208,6 +209,12 @@ def pair_uniforms(seed, step, cell, s):
     u = (C.c_double * 3)()
     lib().orc_pair_uniforms(C.c_uint64(seed), C.c_uint32(step), C.c_uint32(cell), C.c_uint32(s), u)
     return np.array(list(u))
+
+
+def pair_draw(seed, step, cell, s, N):
+    i, j = C.c_int32(0), C.c_int32(0)
+    lib().orc_pair_draw(C.c_uint64(seed), C.c_uint32(step), C.c_uint32(cell), C.c_uint32(s), C.c_int32(N), C.byref(i), C.byref(j))
+    return i.value, j.value
 
 
 def pair_normals(seed, step, cell, s):

@@ -65,6 +65,17 @@ void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, 
   u[2] = orc_u01(r[2u * (s & 1u) + 1u]);
 }
 
+/* stream 4: with-replacement pair draw ("two particles i, j in C_k are selected uniformly at random") */
+void orc_pair_draw(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, int32_t N, int32_t *i, int32_t *j) {
+  uint32_t r[4];
+  philox_at(seed, s, cell, step, 4u, r);
+  int32_t ii = (int32_t)(((uint64_t)r[0] * (uint64_t)(uint32_t)N) >> 32);
+  int32_t jj = (int32_t)(((uint64_t)r[1] * (uint64_t)(uint32_t)(N - 1)) >> 32);
+  if (jj >= ii) jj++;
+  *i = ii;
+  *j = jj;
+}
+
 /* stream 2: xi ~ N(0,I3), eq. 2, by Box-Muller on four uniforms */
 void orc_pair_normals(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double xi[3]) {
   uint32_t r[4];
@@ -402,11 +413,25 @@ int orc_collide_abinitio(int64_t n, int32_t n_cells, const int32_t *cell_start, 
     double ubar[3], Theta, Tk, E_pre = 0.0;
     orc_cell_state(N, cx, cy, cz, prm->mass, ubar, &Theta, &Tk);
     for (int32_t p = 0; p < N; ++p) E_pre += cx[p] * cx[p] + cy[p] * cy[p] + cz[p] * cz[p];
+    /* with replacement, every pair of the cell is evaluated on the PRE-collision velocities
+     * ("all collision pairs in a cell are evaluated in a single forward pass") and the velocity changes
+     * of a particle that appears in several pairs add up; momentum is conserved exactly, energy is restored by
+     * the cell-wise correction. */
+    const int replace = (prm->flags & ORC_F_PAIR_REPLACE) != 0;
     int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
-    int32_t M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, prm->pairs_per_cell, pi);
+    double *dv = replace ? (double *)calloc((size_t)(3 * N), sizeof(double)) : NULL;
+    int32_t M;
+    if (replace) {
+      M = N / 2;
+      if (prm->pairs_per_cell >= 0 && prm->pairs_per_cell < M) M = prm->pairs_per_cell;
+    } else {
+      M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, prm->pairs_per_cell, pi);
+    }
     int32_t n_collided = 0;
     for (int32_t s = 0; s < M; ++s) {
-      int32_t i = pi[2 * s], j = pi[2 * s + 1];
+      int32_t i, j;
+      if (replace) orc_pair_draw(seed, step, (uint32_t)(k + prm->cell_base), (uint32_t)s, N, &i, &j);
+      else { i = pi[2 * s]; j = pi[2 * s + 1]; }
       double g[3] = {cx[i] - cx[j], cy[i] - cy[j], cz[i] - cz[j]};
       double g2 = g[0] * g[0] + g[1] * g[1] + g[2] * g[2];
       double gn = sqrt(g2);
@@ -426,15 +451,26 @@ int orc_collide_abinitio(int64_t n, int32_t n_cells, const int32_t *cell_start, 
                                    : orc_chi_mlp(net, prm->lnE_min, prm->lnE_max, lnE, btilde);
         double eps = 2.0 * PI * U[2];
         if (gn > 0.0) orc_rotate(g, chi, eps, gp);
-        double cm[3] = {0.5 * (cx[i] + cx[j]), 0.5 * (cy[i] + cy[j]), 0.5 * (cz[i] + cz[j])};
-        cx[i] = cm[0] + 0.5 * gp[0]; cy[i] = cm[1] + 0.5 * gp[1]; cz[i] = cm[2] + 0.5 * gp[2];
-        cx[j] = cm[0] - 0.5 * gp[0]; cy[j] = cm[1] - 0.5 * gp[1]; cz[j] = cm[2] - 0.5 * gp[2];
+        if (replace) { /* v_i' - v_i = (g' - g) / 2 = -(v_j' - v_j), eqs. 6-8 */
+          for (int d = 0; d < 3; ++d) {
+            dv[3 * i + d] += 0.5 * (gp[d] - g[d]);
+            dv[3 * j + d] -= 0.5 * (gp[d] - g[d]);
+          }
+        } else {
+          double cm[3] = {0.5 * (cx[i] + cx[j]), 0.5 * (cy[i] + cy[j]), 0.5 * (cz[i] + cz[j])};
+          cx[i] = cm[0] + 0.5 * gp[0]; cy[i] = cm[1] + 0.5 * gp[1]; cz[i] = cm[2] + 0.5 * gp[2];
+          cx[j] = cm[0] - 0.5 * gp[0]; cy[j] = cm[1] - 0.5 * gp[1]; cz[j] = cm[2] - 0.5 * gp[2];
+        }
         n_collided++;
       }
       if (gprime_out) { gprime_out[3 * (a + s)] = gp[0]; gprime_out[3 * (a + s) + 1] = gp[1]; gprime_out[3 * (a + s) + 2] = gp[2]; }
       if (chi_out) chi_out[a + s] = chi;
     }
     free(pi);
+    if (replace) {
+      for (int32_t p = 0; p < N; ++p) { cx[p] += dv[3 * p]; cy[p] += dv[3 * p + 1]; cz[p] += dv[3 * p + 2]; }
+      free(dv);
+    }
     if ((prm->flags & ORC_F_MOMENT_MATCH) && n_collided > 0)
       match_cell(N, cx, cy, cz, ubar, Theta, E_pre, prm->flags);
   }

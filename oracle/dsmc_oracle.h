@@ -30,6 +30,7 @@ extern "C" {
 #define ORC_F_MOMENT_MATCH 4u       /* cell-wise correction, eqs. 10-11 P:L126-131 + P:L46 */
 #define ORC_F_ACCEPT 8u             /* NTC acceptance test */
 #define ORC_F_MATCH_ENERGY_ONLY 32u /* literal eq. 11 (scale raw velocities) */
+#define ORC_F_PAIR_REPLACE 128u     /* NTC-style selection WITH replacement, batch semantics */
 
 #define ORC_ACT_TANH 0
 #define ORC_ACT_RELU 1
@@ -89,6 +90,9 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 double orc_u01(uint32_t x); /* ((x>>9)+0.5)*2^-23 in (0,1), exact in fp32 */
 /* pairing key of slot p in cell k at step t (stream 0) */
 uint32_t orc_pair_key(uint64_t seed, uint32_t step, uint32_t cell, uint32_t slot);
+/* with-replacement selection (stream 4): i = mulhi(R0, N), j = mulhi(R1, N-1) + (j >= i), uniform over ordered
+ * pairs i != j */
+void orc_pair_draw(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, int32_t N, int32_t *i, int32_t *j);
 /* per-pair uniforms: U_acc (stream 3, word s&3 of block s>>2), U_b, U_eps (stream 1, words 2(s&1), 2(s&1)+1
  * of block s>>1) */
 void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double u[3]);

@@ -578,3 +578,66 @@ def test_chapman_enskog_collision_integral_of_lj_matches_textbook():
     for Ts, want in ((float(r[0]), float(r[1])) for r in rows):
         got = sum(w * x ** 3 * q2_star(x * Ts) for x, w in zip(xs, ws)) / 6.0
         assert abs(got / want - 1.0) < 5e-3, (Ts, got, want)
+
+
+def test_with_replacement_selection_and_batch_semantics():
+    """NTC-style selection WITH replacement ("two particles i, j in C_k are selected uniformly
+    at random") and batch evaluation.  Pins: (a) the draw is uniform over ORDERED pairs i != j (brute
+    force, N = 3, 4, 7); (b) a brute-force re-computation of one cell from the dumped pairs: every pair is evaluated
+    on the PRE-collision velocities and the changes add up; (c) momentum is conserved exactly before matching while
+    energy is not; (d) matching restores both."""
+    for N in (3, 4, 7):
+        n = 3000 * N * (N - 1)
+        cnt = {}
+        for s in range(n):
+            ij = oracle.pair_draw(77, 5, 9, s, N)
+            assert ij[0] != ij[1] and 0 <= ij[0] < N and 0 <= ij[1] < N
+            cnt[ij] = cnt.get(ij, 0) + 1
+        assert len(cnt) == N * (N - 1)
+        p = 1.0 / (N * (N - 1))
+        for c in cnt.values():
+            assert abs(c / n - p) < 4.5 * math.sqrt(p * (1 - p) / n)
+    # the draw is what its definition says: mulhi of the first two words of stream 4
+    r = oracle.philox4x32_10([11, 9, 5, 4], [77, 0])
+    i = (r[0] * 7) >> 32
+    j = (r[1] * 6) >> 32
+    assert oracle.pair_draw(77, 5, 9, 11, 7) == (i, j + (1 if j >= i else 0))
+
+    pop = wl.tiny_box(seed=13, n_cells=6, per_cell=40, T=800.0)
+    rc, perm, cs = oracle.bin_particles(pop.cell, pop.n_cells)
+    v = [a[perm].astype(np.float64) for a in (pop.vx, pop.vy, pop.vz)]
+    lo, hi = math.log(5.0), math.log(6e4)
+    tb = oracle.ChiTable(np.full((4, 4), 1.3, np.float32), lo, hi)  # chi = 1.3 rad for every pair
+    prm = oracle.AbinitioParams(flags=oracle.F_PAIR_REPLACE)      # no matching
+    r = oracle.collide_abinitio(cs, *v, prm, 31, 2, table=tb)
+    ok = r.pair_i >= 0
+    assert ok.sum() == 6 * 20
+    # (b) brute force for every cell from the dumped (i, j, g')
+    for k in range(pop.n_cells):
+        a, N = cs[k], cs[k + 1] - cs[k]
+        loc = np.stack([x[a:a + N] for x in v], axis=1)
+        dv = np.zeros_like(loc)
+        for s in range(N // 2):
+            i, j = r.pair_i[a + s], r.pair_j[a + s]
+            assert (i, j) == oracle.pair_draw(31, 2, k, s, N)
+            g = loc[i] - loc[j]
+            gp = r.gprime[a + s]
+            assert abs(np.linalg.norm(gp) / np.linalg.norm(g) - 1) < 1e-13          # rotation keeps |g|
+            assert abs(np.dot(g, gp) / np.dot(g, g) - math.cos(1.3)) < 1e-6         # by chi (fp32 table value)
+            dv[i] += 0.5 * (gp - g)
+            dv[j] -= 0.5 * (gp - g)
+        got = np.stack([r.vx[a:a + N], r.vy[a:a + N], r.vz[a:a + N]], axis=1)
+        np.testing.assert_allclose(got, loc + dv, rtol=0, atol=1e-9)
+    # (c) momentum exact, energy not (a particle in several pairs takes all their changes)
+    pre, post = oracle.cell_moments(cs, *v), oracle.cell_moments(cs, r.vx, r.vy, r.vz)
+    np.testing.assert_allclose(post[:, :3], pre[:, :3], atol=1e-8)
+    assert np.abs(post[:, 3] / pre[:, 3] - 1).max() > 1e-3
+    # about a quarter of the particles appear in two or more pairs at M = N / 2
+    multi = np.mean([np.bincount(np.r_[r.pair_i[cs[k]:cs[k] + 20], r.pair_j[cs[k]:cs[k] + 20]], minlength=40).max() >= 2
+                     for k in range(6)])
+    assert multi == 1.0
+    # (d) with matching both are restored
+    r2 = oracle.collide_abinitio(cs, *v, oracle.AbinitioParams(flags=oracle.F_PAIR_REPLACE | oracle.F_MOMENT_MATCH), 31, 2, table=tb)
+    post2 = oracle.cell_moments(cs, r2.vx, r2.vy, r2.vz)
+    np.testing.assert_allclose(post2[:, 3], pre[:, 3], rtol=1e-12)
+    np.testing.assert_allclose(post2[:, :3], pre[:, :3], atol=1e-8)
