@@ -243,8 +243,9 @@ def run_b200(args):
            torch.empty(pop.n_cells + 1, dtype=torch.int32, device=dev))
 
     def params(chi):
-        flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi == "mlp_tc" else 0)
-        return dsmc.AbinitioParams(chi_mode=0 if chi == "table" else 1, flags=flags, b_max=B_MAX)
+        flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi == "mlp_tc" else 0) | \
+            (dsmc.F_PAIR_REPLACE if chi == "table_replace" else 0)
+        return dsmc.AbinitioParams(chi_mode=0 if chi.startswith("table") else 1, flags=flags, b_max=B_MAX)
 
     def one_step(chi, t, ev=None):
         ctx.bin(cell, *vin, pop.n_cells, out=out)
@@ -315,7 +316,8 @@ def run_b200(args):
 
     variants = {}
     if not args.no_variants and rank == 0 or (not args.no_variants and world > 1):
-        for chi in ("table", "mlp", "mlp_tc"):
+        # table_replace: the same step with pairs drawn WITH replacement (DSMC_F_PAIR_REPLACE)
+        for chi in ("table", "mlp", "mlp_tc", "table_replace"):
             if chi == args.chi:
                 variants[chi] = {"pairs_per_s": pairs / (ms_step * 1e-3), "collide_ms": coll_ms, "step_ms": ms_step}
                 continue

@@ -37,9 +37,12 @@ static_assert(sizeof(CellInfo) == 48, "CellInfo layout");
 
 enum { MI_NACT = 0, MI_NSEG = 1, MI_NPAIRS = 2, MI_SCAN = 8 /* .. +40 */ };
 
-template <int LMAX_, int AMAX_>
+// REPLACE_: pairs drawn with replacement (DSMC_F_PAIR_REPLACE) -- a compile-time variant so that the default
+// (matching) path carries none of its code.
+template <int LMAX_, int AMAX_, bool REPLACE_ = false>
 struct Chunk {
   static constexpr int LMAX = LMAX_, AMAX = AMAX_;
+  static constexpr bool REPLACE = REPLACE_;
   static constexpr int SMAX = (LMAX / kSeg + AMAX + 2 + 3) & ~3;  // multiple of 4: keeps every array 16-byte aligned
   float4 *v;        // [LMAX] velocities (x, y, z, unused)
   float4 *part;     // [SMAX] segment partial sums
@@ -243,6 +246,17 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     }
     sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
     if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
+    if (CK::REPLACE) {  // no matching to build: pair list only, and clear the change accumulators
+      for (int q = lo + lane; q < hi; q += 32) {
+        reinterpret_cast<float *>(S.key)[q] = 0.f;
+        reinterpret_cast<float *>(S.cnt)[q] = 0.f;
+        reinterpret_cast<float *>(S.ord)[q] = 0.f;
+      }
+      const int s_hi = min(M, (piece + 1) * (kSeg / 2));
+      for (int s = piece * (kSeg / 2) + lane; s < s_hi; s += 32)
+        S.pairs[pair_off + s] = (uint32_t)(start + 2 * s) | ((uint32_t)a << 16);
+      continue;
+    }
     // pairing keys: Philox block blk serves slots 4 blk .. 4 blk + 3 of the cell (stream 0)
     const int b_hi = min((piece + 1) * (kSeg / 4), (N + 3) >> 2);
     for (int blk = piece * (kSeg / 4) + lane; blk < b_hi; blk += 32) {
@@ -277,6 +291,10 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     ci.uy = (float)((double)ci.uy + dy);
     ci.uz = (float)((double)ci.uz + dz);
     ci.theta = (float)(s2 - N * (dx * dx + dy * dy + dz * dz));
+  }
+  if (CK::REPLACE) {  // pairs are drawn, not matched: nothing to sort
+    T.sync();
+    return;
   }
   block_excl_scan_coalesced(T, S.cnt, n_loc, S.misc + MI_SCAN);
   // placement, one warp per segment (cell constants in registers): cnt[bucket] ends as the bucket's end
@@ -329,9 +347,10 @@ struct PairCtx {
   float U_b, U_eps;
 };
 
-// the two members of pair t, their velocities and relative velocity (eq. 1); no random numbers
+// the two members of pair t (from the matching, or drawn with replacement), their velocities and relative
+// velocity (eq. 1)
 template <class CK>
-__device__ __forceinline__ PairCtx pair_load(const CK &S, int t) {
+__device__ __forceinline__ PairCtx pair_load(const StepParams &P, const CK &S, int t) {
   PairCtx c;
   const uint32_t e = S.pairs[t];
   const int pos = e & 0xFFFFu;
@@ -340,8 +359,18 @@ __device__ __forceinline__ PairCtx pair_load(const CK &S, int t) {
   c.start = ci.start;
   c.cell = (uint32_t)ci.cell;
   c.s = (pos - c.start) >> 1;
-  c.i = S.pi[pos];
-  c.j = S.pi[pos + 1];
+  if (CK::REPLACE) {  // stream 4: i = mulhi(R0, N), j = mulhi(R1, N - 1) + (j >= i)
+    const uint4 r = philox4x32_10((uint32_t)c.s, c.cell + P.cell_base, P.step, 4u, P.seed_lo, P.seed_hi);
+    const int N = ci.N;
+    const int i = (int)__umulhi(r.x, (uint32_t)N);
+    int j = (int)__umulhi(r.y, (uint32_t)(N - 1));
+    j += (j >= i) ? 1 : 0;
+    c.i = c.start + i;
+    c.j = c.start + j;
+  } else {
+    c.i = S.pi[pos];
+    c.j = S.pi[pos + 1];
+  }
   c.vi = S.v[c.i];
   c.vj = S.v[c.j];
   c.gx = c.vi.x - c.vj.x;  // eq. 1
@@ -356,7 +385,7 @@ __device__ __forceinline__ PairCtx pair_load(const CK &S, int t) {
 
 template <class CK>
 __device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, int t, bool need_randoms) {
-  PairCtx c = pair_load(S, t);
+  PairCtx c = pair_load(P, S, t);
   const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
   if (need_randoms || accept) {
     // stream 1: one block per two pair slots, (U_b, U_eps) = words 2(s&1), 2(s&1)+1 of block s>>1
@@ -377,7 +406,16 @@ __device__ __forceinline__ PairCtx pair_setup(const StepParams &P, const CK &S, 
 template <class CK>
 __device__ __forceinline__ void pair_commit(const StepParams &P, CK &S, const PairCtx &c, float px, float py,
                                             float pz, float aux, int q0) {
-  if (c.acc) {  // eqs. 6-8
+  if (c.acc && CK::REPLACE) {
+    // batch semantics: v_i' - v_i = (g' - g) / 2 = -(v_j' - v_j) (eqs. 6-8) is added to the particle's change;
+    // S.v keeps the pre-collision velocities until chunk_finish applies the sums
+    float *dx = reinterpret_cast<float *>(S.key), *dy = reinterpret_cast<float *>(S.cnt),
+          *dz = reinterpret_cast<float *>(S.ord);
+    const float hx = 0.5f * (px - c.gx), hy = 0.5f * (py - c.gy), hz = 0.5f * (pz - c.gz);
+    atomicAdd(dx + c.i, hx); atomicAdd(dy + c.i, hy); atomicAdd(dz + c.i, hz);
+    atomicAdd(dx + c.j, -hx); atomicAdd(dy + c.j, -hy); atomicAdd(dz + c.j, -hz);
+    if (P.flags & DSMC_F_ACCEPT) S.cells[c.a].collided = 1;
+  } else if (c.acc) {  // eqs. 6-8
     const float cx = 0.5f * (c.vi.x + c.vj.x), cy = 0.5f * (c.vi.y + c.vj.y), cz = 0.5f * (c.vi.z + c.vj.z);
     S.v[c.i] = make_float4(fmaf(0.5f, px, cx), fmaf(0.5f, py, cy), fmaf(0.5f, pz, cz), 0.f);
     S.v[c.j] = make_float4(fmaf(-0.5f, px, cx), fmaf(-0.5f, py, cy), fmaf(-0.5f, pz, cz), 0.f);
@@ -445,6 +483,7 @@ template <class TM, class CK>
 __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc, int q0) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   const int n_act = S.misc[MI_NACT], n_seg = S.misc[MI_NSEG];
+  constexpr bool replace = CK::REPLACE;
   if (P.flags & DSMC_F_MOMENT_MATCH) {
     for (int sg = warp; sg < n_seg; sg += TM::kW) {
       const uint32_t e = S.segs[sg];
@@ -455,7 +494,13 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
       const float ux = ci.ux, uy = ci.uy, uz = ci.uz;
       float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
       for (int q = lo + lane; q < hi; q += 32) {
-        const float4 v = S.v[q];
+        float4 v = S.v[q];
+        if (replace) {  // with-replacement selection: apply the accumulated changes (this thread owns slot q)
+          v.x += reinterpret_cast<const float *>(S.key)[q];
+          v.y += reinterpret_cast<const float *>(S.cnt)[q];
+          v.z += reinterpret_cast<const float *>(S.ord)[q];
+          S.v[q] = v;
+        }
         const float dx = v.x - ux, dy = v.y - uy, dz = v.z - uz;
         sx += dx; sy += dy; sz += dz;
         s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
@@ -517,7 +562,12 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
       const int piece = e >> 16;
       const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
       for (int q = lo + lane; q < hi; q += 32) {
-        const float4 v = S.v[q];
+        float4 v = S.v[q];
+        if (replace) {
+          v.x += reinterpret_cast<const float *>(S.key)[q];
+          v.y += reinterpret_cast<const float *>(S.cnt)[q];
+          v.z += reinterpret_cast<const float *>(S.ord)[q];
+        }
         P.vx[q0 + q] = v.x;
         P.vy[q0 + q] = v.y;
         P.vz[q0 + q] = v.z;

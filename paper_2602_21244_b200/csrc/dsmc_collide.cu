@@ -217,26 +217,26 @@ __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev 
   chunk_finish(T, P, S, n_loc, q0);
 }
 
-template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads>
+template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads, bool REPL = false>
 __global__ void __launch_bounds__(NT, MINB) k_collide(const StepParams P, const MlpDev net) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Chunk<LMAX, AMAX> S;
+  Chunk<LMAX, AMAX, REPL> S;
   float *mlp = reinterpret_cast<float *>(S.carve(smem_raw));
   if (SRC == 0) {
-    process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP, DST>(P, net, S, mlp, blockIdx.x);
+    process_chunk<NT, Chunk<LMAX, AMAX, REPL>, OP_TABLE, TP, DST>(P, net, S, mlp, blockIdx.x);
   } else {
     const int32_t *list = SRC == 1 ? P.big : P.big2;
     const int n_list = *reinterpret_cast<volatile const int32_t *>(list);
     for (int i = blockIdx.x; i < n_list; i += gridDim.x) {
-      process_chunk<NT, Chunk<LMAX, AMAX>, OP_TABLE, TP, DST>(P, net, S, mlp, list[1 + i]);
+      process_chunk<NT, Chunk<LMAX, AMAX, REPL>, OP_TABLE, TP, DST>(P, net, S, mlp, list[1 + i]);
       __syncthreads();
     }
   }
 }
 
-template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads>
+template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads, bool REPL = false>
 static int launch_one(dsmc_ctx *c, const StepParams &p, const MlpDev &nd, int grid, size_t mlp_bytes) {
-  auto kern = k_collide<LMAX, AMAX, OP_TABLE, TP, SRC, DST, MINB, NT>;
+  auto kern = k_collide<LMAX, AMAX, OP_TABLE, TP, SRC, DST, MINB, NT, REPL>;
   const size_t smem = Chunk<LMAX, AMAX>::bytes() + mlp_bytes;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
@@ -266,6 +266,21 @@ int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {
   if (rc != DSMC_OK) return rc;
   MlpDev nd{};
   const int big_grid = c->num_sms;
+  if (p.flags & DSMC_F_PAIR_REPLACE) {  // pairs drawn with replacement: separate instantiations
+    if (p.op == 1) {
+      rc = launch_one<704, 32, true, 64, 0, 1, 9, 128, true>(c, p, nd, p.n_chunks, 0);
+      if (rc != DSMC_OK) return rc;
+      rc = launch_one<1024, 8, true, 64, 1, 2, 7, 128, true>(c, p, nd, c->num_sms * 7, 0);
+      if (rc != DSMC_OK) return rc;
+      return launch_one<kLmaxBig, kAmaxBig, true, 64, 2, 0, 1, kThreads, true>(c, p, nd, big_grid, 0);
+    }
+    nd = *net;
+    if (nd.dmax > 128) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    const size_t mbr = sizeof(float) * 2 * nd.dmax * 64;
+    rc = launch_one<kLmaxSmall, kAmaxSmall, false, 64, 0, 1, 1, kThreads, true>(c, p, nd, p.n_chunks, mbr);
+    if (rc != DSMC_OK) return rc;
+    return launch_one<kLmaxBig, kAmaxBig, false, 64, 1, 0, 1, kThreads, true>(c, p, nd, big_grid, mbr);
+  }
   if (p.op == 1) {
     // three footprints: 704 slots and 32 cells at 9 CTAs/SM (chunks of cells up to ~230 particles), 1024 slots / 8 cells at 7 CTAs/SM
     // (one ~1000-particle cell), then anything legal on one CTA per SM

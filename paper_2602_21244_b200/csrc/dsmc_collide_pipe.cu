@@ -95,7 +95,7 @@ __device__ __forceinline__ void finish_pairs(const TM &T, const StepParams &P, C
     while (ld_volatile(tiles_done) < n_tiles) __nanosleep(64);
   T.sync();
   for (int t = T.tid; t < n_pairs; t += TM::kN) {
-    PairCtx c = pair_load(S, t);
+    PairCtx c = pair_load(P, S, t);
     const float ue = __int_as_float(S.cnt[t]);
     c.acc = ue > 0.f;
     c.U_eps = fabsf(ue);

@@ -575,3 +575,51 @@ def test_chapman_enskog_from_the_gpu_quadrature(dsmc):
         print("Omega22*(T* = %g) = %.4f (textbook %.4f)" % (Ts, got, want))
         assert abs(got / want - 1.0) < 5e-3
     ctx.close()
+
+
+# --------------------------------------------------------------------------------------- (f1) with replacement
+@pytest.mark.parametrize("mode,match", [("table", True), ("table", False), ("mlp", True)])
+def test_collide_abinitio_with_replacement(dsmc, mode, match):
+    """pairs drawn with replacement, batch semantics.  Pair indices bit-exact, per-pair g' to the FP32
+    tolerance, final velocities to 1e-5 of the thermal scale (the changes of a particle are summed by shared-memory
+    atomics in no fixed order), conserved moments to 1e-6 with matching; momentum exact without."""
+    pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    tab = _lj_table()
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    net = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    cm = 0 if mode == "table" else 1
+    flags = dsmc.F_PAIR_REPLACE | (dsmc.F_MOMENT_MATCH if match else 0)
+    oflags = oracle.F_PAIR_REPLACE | (oracle.F_MOMENT_MATCH if match else 0)
+    prm = dsmc.AbinitioParams(chi_mode=cm, flags=flags)
+    oprm = oracle.AbinitioParams(chi_mode=cm, flags=oflags, lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
+    otab = oracle.ChiTable(tab.chi, float(np.float32(tab.lnE_min)), float(np.float32(tab.lnE_max)))
+    v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+    dump = dsmc.PairDump(pop.n, "cuda")
+    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=6, step=1, dump=dump)
+    ctx.check()
+    ref = oracle.collide_abinitio(cs_h, *v_in, oprm, 6, 1, net=net, table=otab)
+    np.testing.assert_array_equal(dump.pair_i.cpu().numpy(), ref.pair_i)
+    np.testing.assert_array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
+    sel = ref.pair_i >= 0
+    dchi = np.abs(dump.aux.cpu().numpy().astype(np.float64) - ref.aux)
+    slope = 1.01 * dchi if mode == "table" else None
+    _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5 if mode == "table" else 3e-5, 1e-6, slope=slope)
+    N = np.diff(cs_h)
+    pre = oracle.cell_moments(cs_h, *v_in)
+    got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+    ok = N >= 2
+    scale = np.repeat(np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1)), N)
+    tol_v = 1e-5 + (2.1 * dchi[sel].max() if mode == "table" else 1e-4)
+    for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
+        assert (np.abs(a.cpu().numpy().astype(np.float64) - want) / scale).max() < tol_v
+    assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    if match:
+        assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+    else:
+        assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() > 1e-3  # energy is NOT conserved without the correction
+    ctx.close()
