@@ -26,7 +26,7 @@ constexpr int kSeg = 128;  // particles per segment = one warp pass of 32 Philox
 constexpr int kWarps = kThreads / 32;
 
 struct __align__(16) CellInfo {
-  float ux, uy, uz, theta;  // pre-collision mean, sum |v-u|^2; finish_post overwrites: Bx,By,Bz,alpha
+  float ux, uy, uz, theta;  // pre-collision mean, sum |v-u|^2; chunk_finish overwrites: Bx, By, Bz, alpha - 1
   int32_t cell;             // global cell id
   int32_t pair_off;         // first entry of this cell in pairs[]
   uint16_t start, N, M, seg0;
@@ -535,10 +535,12 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
           bz = uz - alpha * (uz + dz);
         }
       }
-      ci.ux = (float)bx; ci.uy = (float)by; ci.uz = (float)bz; ci.theta = (float)alpha;
+      // alpha is 1 + O(1e-7): FP32 cannot resolve it (spacing 6e-8 .. 1.2e-7 around 1, a biased correction that
+      // showed as a -2.6e-8 per step energy drift), so the store applies v + (alpha - 1) v + B with alpha - 1 in FP32
+      ci.ux = (float)bx; ci.uy = (float)by; ci.uz = (float)bz; ci.theta = (float)(alpha - 1.0);
     }
     T.sync();
-    // store, one warp per segment: v <- alpha v + B with the cell's coefficients in registers.  Cells in
+    // store, one warp per segment: v <- v + (alpha - 1) v + B with the cell's coefficients in registers.  Cells in
     // which nothing collided (and particles of cells with N < 2) are unchanged and not written.
     for (int sg = warp; sg < n_seg; sg += TM::kW) {
       const uint32_t e = S.segs[sg];
@@ -549,9 +551,9 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
       const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
       for (int q = lo + lane; q < hi; q += 32) {
         const float4 v = S.v[q];
-        P.vx[q0 + q] = fmaf(co.w, v.x, co.x);
-        P.vy[q0 + q] = fmaf(co.w, v.y, co.y);
-        P.vz[q0 + q] = fmaf(co.w, v.z, co.z);
+        P.vx[q0 + q] = fmaf(co.w, v.x, v.x + co.x);
+        P.vy[q0 + q] = fmaf(co.w, v.y, v.y + co.y);
+        P.vz[q0 + q] = fmaf(co.w, v.z, v.z + co.z);
       }
     }
   } else {
