@@ -51,8 +51,12 @@ __global__ void __launch_bounds__(kThreads) k_moment_match(int32_t K, const int3
       }
       e = warp_sum(e);
       if (e > 0.0) {
-        const float alpha = (float)sqrt(Et / e);
-        for (int p = a + lane; p < b; p += 32) { vx[p] *= alpha; vy[p] *= alpha; vz[p] *= alpha; }
+        const double alpha = sqrt(Et / e);  // FP64: alpha = 1 + O(1e-7) is not resolvable in FP32
+        for (int p = a + lane; p < b; p += 32) {
+          vx[p] = (float)(alpha * vx[p]);
+          vy[p] = (float)(alpha * vy[p]);
+          vz[p] = (float)(alpha * vz[p]);
+        }
       }
       continue;
     }
