@@ -398,3 +398,51 @@ def build_chi_table(pot: Potential, nE, nB, lnE_min=float(np.log(5.0)),
                               C.c_double(lnE_max), C.c_double(b_max), C.c_int32(n_panels),
                               _p(chi, C.c_float))
     return ChiTable(chi, lnE_min, lnE_max)
+
+
+# ------------------------------------------------------------- f4: move + walls + sampling (Q30)
+class _Couette(C.Structure):
+    _fields_ = [("L", C.c_double), ("dt", C.c_double), ("u_wall", C.c_double), ("rt_wall", C.c_double),
+                ("accommodation", C.c_double), ("n_cells", C.c_int32)]
+
+
+MAX_BOUNCES = 4
+
+
+@dataclass
+class CouetteParams:
+    L: float
+    dt: float
+    u_wall: float
+    rt_wall: float
+    accommodation: float
+    n_cells: int
+
+    def c(self):
+        return _Couette(self.L, self.dt, self.u_wall, self.rt_wall, self.accommodation, self.n_cells)
+
+
+def move_couette(x, vx, vy, vz, prm: CouetteParams, seed, step):
+    """Free flight for dt between Maxwell walls (Q30).  Returns (x, vx, vy, vz, cell, bounces, margin)."""
+    x, vx, vy, vz = (_f64(a).copy() for a in (x, vx, vy, vz))
+    n = x.shape[0]
+    cell = np.empty(n, np.int32)
+    nb = np.empty(n, np.int32)
+    mg = np.empty(n, np.float64)
+    c = prm.c()
+    lib().orc_move_couette(C.c_int64(n), _p(x, C.c_double), _p(vx, C.c_double), _p(vy, C.c_double),
+                           _p(vz, C.c_double), _p(cell, C.c_int32), _p(nb, C.c_int32), _p(mg, C.c_double),
+                           C.byref(c), C.c_uint64(seed), C.c_uint32(step))
+    return x, vx, vy, vz, cell, nb, mg
+
+
+def sample_cells(cell_start, vx, vy, vz, acc=None):
+    """acc[n_cells, 8] += (count, sums of vx, vy, vz, vx^2, vy^2, vz^2, vx vy) per cell."""
+    cs = _i32(cell_start)
+    K = cs.shape[0] - 1
+    if acc is None:
+        acc = np.zeros((K, 8), np.float64)
+    vx, vy, vz = _f64(vx), _f64(vy), _f64(vz)
+    lib().orc_sample_cells(C.c_int32(K), _p(cs, C.c_int32), _p(vx, C.c_double), _p(vy, C.c_double),
+                           _p(vz, C.c_double), _p(acc, C.c_double))
+    return acc

@@ -594,3 +594,86 @@ void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, doubl
     }
   }
 }
+
+
+/* ------------------------------------------------------------------------------------------
+ * f4.  Free flight + Maxwell walls for the 1-D Couette layout (Q30), and the
+ * per-cell sampling sums.
+ * ---------------------------------------------------------------------------------------- */
+void orc_move_couette(int64_t n, double *x, double *vx, double *vy, double *vz, int32_t *cell, int32_t *bounces,
+                      double *margin, const orc_couette_params *p, uint64_t seed, uint32_t step) {
+  const double L = p->L, srt = sqrt(p->rt_wall);
+  for (int64_t q = 0; q < n; ++q) {
+    double xx = x[q], t_left = p->dt, mg = 1e300;
+    int nb = 0;
+    for (;;) {
+      double xn = xx + vx[q] * t_left;
+      if (xn >= 0.0 && xn <= L) { /* no (further) wall hit */
+        double d0 = fabs(xn) / L, d1 = fabs(L - xn) / L;
+        if (d0 < mg) mg = d0;
+        if (d1 < mg) mg = d1;
+        xx = xn;
+        break;
+      }
+      {
+        double d = (xn < 0.0 ? -xn : xn - L) / L;
+        if (d < mg) mg = d;
+      }
+      if (nb == ORC_MAX_BOUNCES) { /* give up: clamp into the gap */
+        xx = xn < 0.0 ? 0.0 : L;
+        break;
+      }
+      {
+        const int upper = xn > L;
+        const double wall = upper ? L : 0.0;
+        uint32_t r[4];
+        t_left -= (wall - xx) / vx[q]; /* time of the hit */
+        xx = wall;
+        philox_at(seed, (uint32_t)q, (uint32_t)nb, step, 5u, r);
+        {
+          double u0 = orc_u01(r[0]), da = fabs(u0 - p->accommodation);
+          if (da < mg) mg = da;
+          if (u0 < p->accommodation) { /* diffuse re-emission from the wall Maxwellian */
+            double vn = sqrt(-2.0 * p->rt_wall * log(orc_u01(r[1])));
+            double rad = sqrt(-2.0 * log(orc_u01(r[2]))), ang = 2.0 * PI * orc_u01(r[3]);
+            vx[q] = upper ? -vn : vn;
+            vy[q] = srt * rad * cos(ang) + (upper ? p->u_wall : -p->u_wall);
+            vz[q] = srt * rad * sin(ang);
+          } else { /* specular */
+            vx[q] = -vx[q];
+          }
+        }
+        nb++;
+      }
+    }
+    x[q] = xx;
+    {
+      double s = xx * (double)p->n_cells / L;
+      int32_t k = (int32_t)floor(s);
+      double f = fabs(s - floor(s + 0.5)) / (double)p->n_cells; /* distance to the nearest cell boundary / L */
+      if (k > p->n_cells - 1) k = p->n_cells - 1;
+      if (k < 0) k = 0;
+      if (f < mg) mg = f;
+      cell[q] = k;
+    }
+    if (bounces) bounces[q] = nb;
+    if (margin) margin[q] = mg;
+  }
+}
+
+void orc_sample_cells(int32_t n_cells, const int32_t *cell_start, const double *vx, const double *vy,
+                      const double *vz, double *acc) {
+  for (int32_t k = 0; k < n_cells; ++k) {
+    double *a = acc + 8 * (size_t)k;
+    for (int32_t s = cell_start[k]; s < cell_start[k + 1]; ++s) {
+      a[0] += 1.0;
+      a[1] += vx[s];
+      a[2] += vy[s];
+      a[3] += vz[s];
+      a[4] += vx[s] * vx[s];
+      a[5] += vy[s] * vy[s];
+      a[6] += vz[s] * vz[s];
+      a[7] += vx[s] * vy[s];
+    }
+  }
+}

@@ -152,6 +152,31 @@ double orc_chi_exact(const orc_potential *pot, double E, double b, int32_t n_pan
 void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, double lnE_min,
                          double lnE_max, double b_max, int32_t n_panels, float *chi);
 
+/* ---- f4: the minimal DSMC loop around the collision step, 1-D Couette layout (Q30) ----
+ * Walls at x = 0 (moving with y-velocity -u_wall) and x = L (+u_wall), "U_wall = +-500 m/s".  The paper
+ * only says "a standard DSMC simulation of Couette flow"; the standard is taken to be: free flight for dt, Maxwell
+ * wall model (a fraction `accommodation` of the wall hits is re-emitted diffusely from the wall Maxwellian at
+ * rt_wall = k_B T_w / m, the rest reflects specularly), the flight continues for the rest of dt with the new
+ * velocity (at most ORC_MAX_BOUNCES wall hits, then the position is clamped into the gap), and the cell index is
+ * floor(x n_cells / L).  Random numbers: Philox stream 5, counter (particle index, bounce number, step, 5):
+ * word 0 decides diffuse (u < accommodation), word 1 the wall-normal speed sqrt(-2 rt ln u) (flux-weighted),
+ * words 2, 3 the Box-Muller pair for the tangential components. */
+#define ORC_MAX_BOUNCES 4
+typedef struct {
+  double L, dt, u_wall, rt_wall, accommodation;
+  int32_t n_cells;
+} orc_couette_params;
+/* x, vx, vy, vz in/out; cell[n], bounces[n] (may be NULL) out; margin[n] (may be NULL) out = the smallest distance
+ * of any floating-point decision taken for the particle from its threshold (wall crossing and cell boundary as a
+ * fraction of L, diffuse/specular draw as |u - accommodation|): a parity test compares decisions only where the
+ * margin exceeds the FP32 resolution. */
+void orc_move_couette(int64_t n, double *x, double *vx, double *vy, double *vz, int32_t *cell, int32_t *bounces,
+                      double *margin, const orc_couette_params *p, uint64_t seed, uint32_t step);
+/* acc[n_cells][8] += (count, sum vx, vy, vz, vx^2, vy^2, vz^2, vx vy) of every cell (time-averaged sampling of the
+ * macroscopic fields U, T, tau_xy: P:L187) */
+void orc_sample_cells(int32_t n_cells, const int32_t *cell_start, const double *vx, const double *vy,
+                      const double *vz, double *acc);
+
 #ifdef __cplusplus
 }
 #endif
