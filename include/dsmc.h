@@ -15,6 +15,8 @@
  *   dsmc_chi_exact_batch   chi by the deflection-integral quadrature itself (eq. 16), LJ 12-6
  *   dsmc_build_chi_table_lj  the chi table generated on the device by that quadrature
  *   dsmc_step_host         bin + fused step on HOST buffers (copies inside), for end-to-end timing
+ *   dsmc_move_couette, dsmc_gather_f32, dsmc_sample_cells, dsmc_couette_run
+ *                          the minimal DSMC loop around the step for the 1-D Couette layout
  *
  * Conventions
  *   - Plain C, no C++/torch types.  Every function returns an int status (0 = DSMC_OK).
@@ -212,6 +214,47 @@ int dsmc_step_host(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cel
                    float *vy_out_h, float *vz_out_h, int32_t *perm_h, int32_t *cell_start_h,
                    const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi, uint64_t seed,
                    uint32_t step);
+
+/* ---- f4: the minimal DSMC loop around the step, 1-D Couette layout (Q30) -------
+ * Walls normal to x at x = 0 (moving with y-velocity -u_wall) and x = L (+u_wall); "U_wall = +-500 m/s".
+ * The paper says only "a standard DSMC simulation of Couette flow"; standard is read as (Q30): free flight for dt;
+ * Maxwell wall model (a fraction `accommodation` of the wall hits is re-emitted diffusely from the wall Maxwellian
+ * at rt_wall = k_B T_w / m [m^2/s^2], normal speed sqrt(-2 rt ln u), the rest reflects specularly); the flight
+ * continues with the new velocity for the rest of dt (at most DSMC_MAX_BOUNCES wall hits per step, then the
+ * particle is parked on the wall); cell = floor(x n_cells / L) clamped to [0, n_cells).
+ * Random numbers: Philox stream 5, counter (particle index, bounce number, step, 5): word 0 decides diffuse
+ * (u < accommodation), word 1 the normal speed, words 2, 3 the Box-Muller pair of the tangential components. */
+#define DSMC_MAX_BOUNCES 4
+typedef struct {
+  float L;             /* gap [m] */
+  float dt;            /* time step [s] */
+  float u_wall;        /* wall speed [m/s] */
+  float rt_wall;       /* k_B T_wall / m [m^2/s^2] */
+  float accommodation; /* in [0, 1]: 1 = fully diffuse walls, 0 = specular */
+  int32_t n_cells;
+} dsmc_couette_params;
+
+/* x, vx, vy, vz [n] in/out (vy, vz are written only for re-emitted particles); cell [n] out; bounces [n] out or
+ * NULL (wall hits of the particle in this step). */
+int dsmc_move_couette(dsmc_ctx *ctx, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,
+                      int32_t *bounces, const dsmc_couette_params *geo, uint64_t seed, uint32_t step);
+
+/* dst[s] = src[perm[s]], s < n: carries a per-particle array (the position) into the order dsmc_bin produced.
+ * perm values must lie in [0, n); src and dst must not overlap. */
+int dsmc_gather_f32(dsmc_ctx *ctx, int64_t n, const int32_t *perm, const float *src, float *dst);
+
+/* acc [n_cells][8] (FP64, device) += per cell (count, sum vx, vy, vz, vx^2, vy^2, vz^2, vx vy) of the sorted
+ * arrays: the time-averaged sums behind U, T, rho, tau_xy.  The caller zeroes acc. */
+int dsmc_sample_cells(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_start, const float *vx,
+                      const float *vy, const float *vz, double *acc);
+
+/* n_steps of  move -> bin -> gather x -> fused collision step (vhs or abi, exactly one non-NULL; step index
+ * step0 + k for the random numbers of both move and collide) -> sample (steps k >= sample_from, into acc if
+ * non-NULL), entirely on the device in context-owned scratch.  x, vx, vy, vz [n] in/out: on return they hold the
+ * state after the last step, in that step's cell-sorted order.  Synchronises and returns the sticky status. */
+int dsmc_couette_run(dsmc_ctx *ctx, int64_t n, float *x, float *vx, float *vy, float *vz,
+                     const dsmc_couette_params *geo, const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi,
+                     uint64_t seed, uint32_t step0, int32_t n_steps, int32_t sample_from, double *acc);
 
 #ifdef __cplusplus
 }

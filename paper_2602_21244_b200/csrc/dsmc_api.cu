@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "dsmc_internal.h"
@@ -77,6 +78,8 @@ int dsmc_destroy(dsmc_ctx *c) {
   for (int a = 0; a < 3; ++a) { cudaFree(c->h_v[a]); cudaFree(c->h_vs[a]); }
   cudaFree(c->h_perm);
   cudaFree(c->h_cell_start);
+  cudaFree(c->h_x[0]);
+  cudaFree(c->h_x[1]);
   delete c;
   return DSMC_OK;
 }
@@ -331,6 +334,9 @@ static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
   for (int a = 0; a < 3; ++a) { cudaFree(c->h_v[a]); cudaFree(c->h_vs[a]); }
   cudaFree(c->h_perm);
   cudaFree(c->h_cell_start);
+  cudaFree(c->h_x[0]);
+  cudaFree(c->h_x[1]);
+  c->h_x[0] = c->h_x[1] = nullptr;
   c->host_cap_n = 0;
   CK(cudaMalloc(&c->h_cell, sizeof(int32_t) * (size_t)n));
   for (int a = 0; a < 3; ++a) {
@@ -338,6 +344,7 @@ static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
     CK(cudaMalloc(&c->h_vs[a], sizeof(float) * (size_t)n));
   }
   CK(cudaMalloc(&c->h_perm, sizeof(int32_t) * (size_t)n));
+  for (int a = 0; a < 2; ++a) CK(cudaMalloc(&c->h_x[a], sizeof(float) * (size_t)n));
   CK(cudaMalloc(&c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1)));
   c->host_cap_n = n;
   c->host_cap_cells = K;
@@ -414,6 +421,78 @@ int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, con
   if (perm_h) CK(cudaMemcpyAsync(perm_h, c->h_perm, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost, s));
   if (cell_start_h)
     CK(cudaMemcpyAsync(cell_start_h, c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1), cudaMemcpyDeviceToHost, s));
+  return dsmc_sync_status(c);
+}
+
+int dsmc_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,
+                      int32_t *bounces, const dsmc_couette_params *g, uint64_t seed, uint32_t step) {
+  if (!c || n < 0 || !g || !(g->L > 0.f) || !(g->dt >= 0.f) || !(g->rt_wall > 0.f) || g->n_cells <= 0 ||
+      !(g->accommodation >= 0.f && g->accommodation <= 1.f))
+    return DSMC_ERR_INVALID_ARG;
+  if (n == 0) return DSMC_OK;
+  if (!x || !vx || !vy || !vz || !cell) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_move_couette(c, n, x, vx, vy, vz, cell, bounces, g, seed, step);
+}
+
+int dsmc_gather_f32(dsmc_ctx *c, int64_t n, const int32_t *perm, const float *src, float *dst) {
+  if (!c || n < 0) return DSMC_ERR_INVALID_ARG;
+  if (n == 0) return DSMC_OK;
+  if (!perm || !src || !dst || src == dst) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_gather_f32(c, n, perm, src, dst);
+}
+
+int dsmc_sample_cells(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, const float *vx, const float *vy,
+                      const float *vz, double *acc) {
+  if (!c || n < 0 || K < 0) return DSMC_ERR_INVALID_ARG;
+  if (K == 0) return DSMC_OK;
+  if (!cs || !acc || (n > 0 && (!vx || !vy || !vz))) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_sample_cells(c, K, cs, vx, vy, vz, acc);
+}
+
+int dsmc_couette_run(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz,
+                     const dsmc_couette_params *g, const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi,
+                     uint64_t seed, uint32_t step0, int32_t n_steps, int32_t sample_from, double *acc) {
+  if (!c || n <= 0 || n > c->max_particles || !g || g->n_cells <= 0 || g->n_cells > c->max_cells || n_steps < 0 ||
+      (!vhs && !abi) || (vhs && abi) || !x || !vx || !vy || !vz)
+    return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  const int32_t K = g->n_cells;
+  int rc = ensure_host_staging(c, n, K);
+  if (rc != DSMC_OK) return rc;
+  cudaStream_t s = c->stream;
+  const size_t bytes = sizeof(float) * (size_t)n;
+  // state lives in (h_x[0], h_v) before the move / bin and in (h_x[1], h_vs) after it
+  float *user[4] = {x, vx, vy, vz};
+  float *sorted[4] = {c->h_x[1], c->h_vs[0], c->h_vs[1], c->h_vs[2]};
+  float *unsorted[4] = {c->h_x[0], c->h_v[0], c->h_v[1], c->h_v[2]};
+  for (int a = 0; a < 4; ++a) CK(cudaMemcpyAsync(unsorted[a], user[a], bytes, cudaMemcpyDeviceToDevice, s));
+  for (int32_t k = 0; k < n_steps; ++k) {
+    const uint32_t step = step0 + (uint32_t)k;
+    rc = dsmc_move_couette(c, n, unsorted[0], unsorted[1], unsorted[2], unsorted[3], c->h_cell, nullptr, g, seed,
+                           step);
+    if (rc != DSMC_OK) return rc;
+    rc = dsmc_bin(c, n, K, c->h_cell, unsorted[1], unsorted[2], unsorted[3], sorted[1], sorted[2], sorted[3],
+                  c->h_perm, c->h_cell_start);
+    if (rc != DSMC_OK) return rc;
+    rc = dsmc_gather_f32(c, n, c->h_perm, unsorted[0], sorted[0]);
+    if (rc != DSMC_OK) return rc;
+    if (vhs)
+      rc = dsmc_collide_vhs_nn(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], nullptr, vhs, seed, step,
+                               nullptr);
+    else
+      rc = dsmc_collide_abinitio(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], nullptr, abi, seed, step,
+                                 nullptr);
+    if (rc != DSMC_OK) return rc;
+    if (acc && k >= sample_from) {
+      rc = dsmc_sample_cells(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], acc);
+      if (rc != DSMC_OK) return rc;
+    }
+    for (int a = 0; a < 4; ++a) std::swap(sorted[a], unsorted[a]);  // this step's output is the next step's input
+  }
+  for (int a = 0; a < 4; ++a) CK(cudaMemcpyAsync(user[a], unsorted[a], bytes, cudaMemcpyDeviceToDevice, s));
   return dsmc_sync_status(c);
 }
 

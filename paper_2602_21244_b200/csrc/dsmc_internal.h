@@ -109,6 +109,7 @@ struct dsmc_ctx {
   int32_t *h_cell;
   float *h_v[3], *h_vs[3];
   int32_t *h_perm, *h_cell_start;
+  float *h_x[2];  // dsmc_couette_run: positions (unsorted / sorted)
   int64_t host_cap_n;
   int32_t host_cap_cells;
 };
@@ -134,6 +135,11 @@ int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float 
                      double sigma, int take_abs);
 int launch_chi_table_lj(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_max, double b_max, double eps_over_k,
                         double sigma, float *table_dev, float4 *quad_dev);
+int launch_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,
+                        int32_t *bounces, const dsmc_couette_params *g, uint64_t seed, uint32_t step);
+int launch_gather_f32(dsmc_ctx *c, int64_t n, const int32_t *perm, const float *src, float *dst);
+int launch_sample_cells(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *vx, const float *vy, const float *vz,
+                        double *acc);
 // host-side packing of the tensor-core weight image (dsmc_collide_tc.cu)
 int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStream_t s);
 }  // namespace dsmc

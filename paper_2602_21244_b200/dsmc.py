@@ -28,7 +28,8 @@ ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
-           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host"]
+           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host", "dsmc_move_couette",
+           "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run"]
 
 
 class DsmcError(RuntimeError):
@@ -53,6 +54,11 @@ class _AbiParams(C.Structure):
     _fields_ = [("mass", C.c_float), ("b_max", C.c_float), ("lnE_min", C.c_float), ("lnE_max", C.c_float),
                 ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32), ("flags", C.c_uint32),
                 ("cell_base", C.c_int32)]
+
+
+class _CouetteParams(C.Structure):
+    _fields_ = [("L", C.c_float), ("dt", C.c_float), ("u_wall", C.c_float), ("rt_wall", C.c_float),
+                ("accommodation", C.c_float), ("n_cells", C.c_int32)]
 
 
 class _PairDump(C.Structure):
@@ -126,6 +132,20 @@ class AbinitioParams:
     def c(self):
         return _AbiParams(self.mass, self.b_max, self.lnE_min, self.lnE_max, self.chi_mode, self.pairs_per_cell,
                           self.flags, self.cell_base)
+
+
+@dataclass
+class CouetteParams:
+    """1-D Couette layout (Q30): walls at x = 0 (-u_wall) and x = L (+u_wall), Maxwell wall model."""
+    L: float
+    dt: float
+    u_wall: float
+    rt_wall: float
+    accommodation: float
+    n_cells: int
+
+    def c(self):
+        return _CouetteParams(self.L, self.dt, self.u_wall, self.rt_wall, self.accommodation, self.n_cells)
 
 
 class PairDump:
@@ -290,6 +310,50 @@ class Context:
                                        _ptr(b, torch.float32), _ptr(out, torch.float32), C.c_float(eps_over_k),
                                        C.c_float(sigma), C.c_uint32(flags)), "dsmc_chi_exact_batch")
         return out
+
+    # ---- f4: the minimal DSMC loop around the step (1-D Couette layout)
+    def move_couette(self, x, vx, vy, vz, geo: "CouetteParams", seed: int, step: int, cell=None, bounces=None):
+        """Free flight + Maxwell walls in place; returns the cell index array."""
+        g = geo.c()
+        if cell is None:
+            cell = torch.empty(x.shape[0], dtype=torch.int32, device=x.device)
+        self._stream()
+        _chk(_lib.dsmc_move_couette(self._h, C.c_int64(x.shape[0]), _ptr(x, torch.float32), _ptr(vx, torch.float32),
+                                    _ptr(vy, torch.float32), _ptr(vz, torch.float32), _ptr(cell, torch.int32),
+                                    _ptr(bounces, torch.int32) if bounces is not None else C.c_void_p(0),
+                                    C.byref(g), C.c_uint64(seed), C.c_uint32(step)), "dsmc_move_couette")
+        return cell
+
+    def gather_f32(self, perm, src, out=None):
+        if out is None:
+            out = torch.empty_like(src)
+        self._stream()
+        _chk(_lib.dsmc_gather_f32(self._h, C.c_int64(src.shape[0]), _ptr(perm, torch.int32),
+                                  _ptr(src, torch.float32), _ptr(out, torch.float32)), "dsmc_gather_f32")
+        return out
+
+    def sample_cells(self, cell_start, vx_s, vy_s, vz_s, acc):
+        self._stream()
+        _chk(_lib.dsmc_sample_cells(self._h, C.c_int64(vx_s.shape[0]), C.c_int32(cell_start.shape[0] - 1),
+                                    _ptr(cell_start, torch.int32), _ptr(vx_s, torch.float32),
+                                    _ptr(vy_s, torch.float32), _ptr(vz_s, torch.float32),
+                                    _ptr(acc, torch.float64)), "dsmc_sample_cells")
+        return acc
+
+    def couette_run(self, x, vx, vy, vz, geo: "CouetteParams", n_steps: int, vhs: VhsParams = None,
+                    abi: AbinitioParams = None, seed: int = 0, step0: int = 0, sample_from: int = 0, acc=None):
+        """n_steps of move -> bin -> gather -> collide -> sample on the device; x, v updated in place."""
+        g = geo.c()
+        pv = vhs.c() if vhs is not None else None
+        pa = abi.c() if abi is not None else None
+        self._stream()
+        _chk(_lib.dsmc_couette_run(
+            self._h, C.c_int64(x.shape[0]), _ptr(x, torch.float32), _ptr(vx, torch.float32),
+            _ptr(vy, torch.float32), _ptr(vz, torch.float32), C.byref(g),
+            C.byref(pv) if pv is not None else None, C.byref(pa) if pa is not None else None, C.c_uint64(seed),
+            C.c_uint32(step0), C.c_int32(n_steps), C.c_int32(sample_from),
+            _ptr(acc, torch.float64) if acc is not None else C.c_void_p(0)), "dsmc_couette_run")
+        return acc
 
     # ---- end to end on host buffers (pinned CPU tensors)
     def step_host(self, cell_h, vx_h, vy_h, vz_h, n_cells, out_h, vhs: VhsParams = None,

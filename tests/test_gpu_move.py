@@ -1,0 +1,226 @@
+"""GPU parity tests (-m gpu) of the minimal DSMC loop around the collision step: free flight +
+Maxwell walls (dsmc_move_couette), the gather into sorted order, the per-cell sampling sums and the device-side
+loop (dsmc_couette_run), against the CPU oracle on the same seeded inputs.
+
+Decisions taken in floating point (wall hit, diffuse or specular, cell index) are compared wherever the oracle
+reports a margin above the FP32 resolution (1e-5 of the gap); elsewhere either answer is right and the test checks
+that the GPU's own outputs are consistent (position inside the gap, cell = floor(x n_cells / L))."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_21244_b200 import workloads as wl
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+RT = 208.13 * 273.0
+
+
+@pytest.fixture(scope="module")
+def dsmc():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2602_21244_b200 import dsmc as mod
+    return mod
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _gas(n, seed, L, rt=RT):
+    rng = np.random.default_rng(seed)
+    x = (rng.random(n) * L).astype(np.float32)
+    v = rng.normal(0.0, math.sqrt(rt), (3, n)).astype(np.float32)
+    return np.minimum(x, np.float32(L)), v
+
+
+@pytest.mark.parametrize("case", ["typical", "many_bounces", "specular", "empty"])
+def test_move_couette_matches_oracle(dsmc, case):
+    L, K, U = 0.05, 200, 500.0
+    n = 300_007
+    dt = 0.5 * (L / K) / math.sqrt(RT)
+    acc = 0.8
+    if case == "many_bounces":
+        dt = 0.9 * L / math.sqrt(RT)  # a thermal particle crosses the gap in a step: up to > DSMC_MAX_BOUNCES hits
+    if case == "specular":
+        acc, dt = 0.0, 0.4 * L / math.sqrt(RT)
+    if case == "empty":
+        n = 0
+    x, v = _gas(n, 3, L)
+    geo_o = oracle.CouetteParams(float(np.float32(L)), float(np.float32(dt)), U, float(np.float32(RT)),
+                                 float(np.float32(acc)), K)
+    geo = dsmc.CouetteParams(L, dt, U, RT, acc, K)
+    ctx = dsmc.Context(max(n, 1), K)
+    xd, vxd, vyd, vzd = dev(x), dev(v[0]), dev(v[1]), dev(v[2])
+    nb_d = torch.zeros(n, dtype=torch.int32, device="cuda")
+    cell_d = ctx.move_couette(xd, vxd, vyd, vzd, geo, seed=77, step=5, bounces=nb_d)
+    ctx.check()
+    if n == 0:
+        ctx.close()
+        return
+    xo, vxo, vyo, vzo, cell_o, nb_o, mg = oracle.move_couette(x, v[0], v[1], v[2], geo_o, 77, 5)
+    xg, vxg, vyg, vzg = (t.cpu().numpy() for t in (xd, vxd, vyd, vzd))
+    cell_g, nb_g = cell_d.cpu().numpy(), nb_d.cpu().numpy()
+    # validity, every particle
+    Lf = np.float32(L)
+    assert np.all((xg >= 0) & (xg <= Lf))
+    cpl = np.float32(K / float(Lf))
+    assert np.array_equal(cell_g, np.clip(np.floor(xg * cpl).astype(np.int64), 0, K - 1))
+    # decisions and values where the oracle's decisions are resolvable in FP32
+    sure = mg > 1e-5
+    print("%s: %.4f%% of particles within 1e-5 of a decision threshold; bounces up to %d; %.1f%% hit a wall"
+          % (case, 100 * (1 - sure.mean()), nb_o.max(), 100 * (nb_o > 0).mean()))
+    assert sure.mean() > 0.995
+    assert np.array_equal(nb_g[sure], nb_o[sure])
+    assert np.array_equal(cell_g[sure], cell_o[sure])
+    assert np.abs(xg[sure] - xo[sure]).max() <= 4e-6 * L
+    for got, want, raw in ((vxg, vxo, v[0]), (vyg, vyo, v[1]), (vzg, vzo, v[2])):
+        assert np.abs(got[sure] - want[sure]).max() <= 2e-5 * math.sqrt(RT + U * U)
+        untouched = sure & (nb_o == 0)
+        assert np.array_equal(got[untouched], raw[untouched])  # bit-exact where no wall was met
+    if case == "many_bounces":
+        assert nb_o.max() == oracle.MAX_BOUNCES and (nb_o >= 2).mean() > 0.05
+    if case == "specular":
+        assert np.array_equal(vyg, v[1]) and np.array_equal(vzg, v[2])
+    ctx.close()
+
+
+def test_gather_bit_exact(dsmc):
+    rng = np.random.default_rng(1)
+    n = 200_003
+    perm = rng.permutation(n).astype(np.int32)
+    src = rng.normal(size=n).astype(np.float32)
+    ctx = dsmc.Context(n, 1)
+    got = ctx.gather_f32(dev(perm), dev(src)).cpu().numpy()
+    ctx.check()
+    assert np.array_equal(got, src[perm])
+    ctx.close()
+
+
+def test_sample_cells_matches_oracle_and_accumulates(dsmc):
+    pop = wl.mach10_cylinder(nx=60, ny=30, n_total=200_000)  # ragged cells, some empty, some large
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    vx_s, vy_s, vz_s, perm, cs = ctx.bin(dev(pop.cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), pop.n_cells)
+    acc = torch.zeros((pop.n_cells, 8), dtype=torch.float64, device="cuda")
+    ctx.sample_cells(cs, vx_s, vy_s, vz_s, acc)
+    ctx.check()
+    cs_h = cs.cpu().numpy()
+    v = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+    want = oracle.sample_cells(cs_h, *v)
+    got = acc.cpu().numpy()
+    assert np.array_equal(got[:, 0], want[:, 0])
+    scale = np.maximum(want[:, 4:7].sum(axis=1, keepdims=True), 1.0)  # sum of squares bounds every term
+    assert np.abs(got - want).max() <= 1e-12 * scale.max()
+    assert (np.abs(got - want) / scale).max() <= 1e-13
+    ctx.sample_cells(cs, vx_s, vy_s, vz_s, acc)
+    ctx.check()
+    assert np.allclose(acc.cpu().numpy(), 2 * want, rtol=1e-13, atol=1e-9)
+    ctx.close()
+
+
+def _lj_table(nE=128, nB=128):
+    return oracle.build_chi_table(oracle.lj_argon(), nE, nB, n_panels=2)
+
+
+def test_couette_run_equals_the_staged_calls(dsmc):
+    """dsmc_couette_run is plumbing: three steps of it must give, bit for bit, what the individual entry points give
+    when called in the same order (move -> bin -> gather -> collide -> sample)."""
+    L, K, U = 0.02, 64, 500.0
+    n = 64 * 300 + 11
+    dt = 0.5 * (L / K) / math.sqrt(RT)
+    x, v = _gas(n, 8, L)
+    geo = dsmc.CouetteParams(L, dt, U, RT, 1.0, K)
+    prm = dsmc.AbinitioParams(pairs_per_cell=40, flags=dsmc.F_MOMENT_MATCH)
+    tab = _lj_table(64, 64)
+    ctx = dsmc.Context(n, K)
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    # staged
+    xs, vxs, vys, vzs = dev(x), dev(v[0]), dev(v[1]), dev(v[2])
+    acc_s = torch.zeros((K, 8), dtype=torch.float64, device="cuda")
+    for k in range(3):
+        cell = ctx.move_couette(xs, vxs, vys, vzs, geo, seed=5, step=10 + k)
+        vxs, vys, vzs, perm, cs = ctx.bin(cell, vxs, vys, vzs, K)
+        xs = ctx.gather_f32(perm, xs)
+        ctx.collide_abinitio(cs, vxs, vys, vzs, prm, seed=5, step=10 + k)
+        if k >= 1:
+            ctx.sample_cells(cs, vxs, vys, vzs, acc_s)
+    ctx.check()
+    # one call
+    xr, vxr, vyr, vzr = dev(x), dev(v[0]), dev(v[1]), dev(v[2])
+    acc_r = torch.zeros((K, 8), dtype=torch.float64, device="cuda")
+    ctx.couette_run(xr, vxr, vyr, vzr, geo, 3, abi=prm, seed=5, step0=10, sample_from=1, acc=acc_r)
+    for a, b in ((xs, xr), (vxs, vxr), (vys, vyr), (vzs, vzr), (acc_s, acc_r)):
+        assert torch.equal(a, b)
+    assert float(acc_r[:, 0].sum()) == 2 * n
+    ctx.close()
+
+
+def test_couette_flow_profiles_against_the_oracle_loop(dsmc):
+    """A physical run (P:L183-187 setting in miniature): gas between diffuse walls moving at +-U, ab initio table
+    operator with a fixed number of collision pairs per cell and step.  The GPU loop and the oracle loop (same
+    stages, FP64) are chaotic, so they are compared through their time-averaged profiles: wall-parallel velocity
+    u_y(x), shear stress <vx vy> and temperature.  Physics checks on the GPU result: the shear stress is uniform
+    across the gap (momentum conservation), below the free-molecular value U sqrt(2RT/pi), the velocity profile is
+    antisymmetric with slip at the walls (|u| < U), viscous heating raises T above the wall temperature."""
+    L, K, U = 0.02, 20, 500.0
+    per = 400
+    n = K * per
+    dt = 0.4 * (L / K) / math.sqrt(RT)
+    n_steps, sample_from = 500, 250
+    x, v = _gas(n, 12, L)
+    geo = dsmc.CouetteParams(L, dt, U, RT, 1.0, K)
+    geo_o = oracle.CouetteParams(float(np.float32(L)), float(np.float32(dt)), U, float(np.float32(RT)), 1.0, K)
+    m_pairs = 60
+    tab = _lj_table(64, 64)
+    ctx = dsmc.Context(n, K)
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    prm = dsmc.AbinitioParams(pairs_per_cell=m_pairs, flags=dsmc.F_MOMENT_MATCH)
+    xd, vxd, vyd, vzd = dev(x), dev(v[0]), dev(v[1]), dev(v[2])
+    acc = torch.zeros((K, 8), dtype=torch.float64, device="cuda")
+    ctx.couette_run(xd, vxd, vyd, vzd, geo, n_steps, abi=prm, seed=1, step0=0, sample_from=sample_from, acc=acc)
+    G = acc.cpu().numpy()
+    # oracle loop
+    prm_o = oracle.AbinitioParams(pairs_per_cell=m_pairs, flags=oracle.F_MOMENT_MATCH)
+    xo = x.astype(np.float64)
+    vo = [a.astype(np.float64) for a in v]
+    O = np.zeros((K, 8))
+    for k in range(n_steps):
+        xo, vo[0], vo[1], vo[2], cell, nb, mg = oracle.move_couette(xo, vo[0], vo[1], vo[2], geo_o, 1, k)
+        rc, perm, cs = oracle.bin_particles(cell, K)
+        xo = xo[perm]
+        vo = [a[perm] for a in vo]
+        res = oracle.collide_abinitio(cs, vo[0], vo[1], vo[2], prm_o, 1, k, table=tab)
+        vo = [res.vx, res.vy, res.vz]
+        if k >= sample_from:
+            oracle.sample_cells(cs, vo[0], vo[1], vo[2], O)
+
+    def fields(A):
+        cnt = A[:, 0]
+        uy = A[:, 2] / cnt
+        txy = (A[:, 7] - A[:, 1] * uy) / cnt.mean()   # momentum flux per mean density: n <c_x c_y> / n_0
+        T = ((A[:, 4] + A[:, 5] + A[:, 6]) / cnt - (A[:, 1] ** 2 + A[:, 2] ** 2 + A[:, 3] ** 2) / cnt ** 2) / 3.0
+        return cnt, uy, txy, T
+
+    cg, uyg, tg, Tg = fields(G)
+    co, uyo, to, To = fields(O)
+    fm = U * math.sqrt(2 * RT / math.pi)
+    print("Couette loop: u_y(wall cells) GPU %.1f / %.1f, oracle %.1f / %.1f; <vx vy> GPU %.0f oracle %.0f "
+          "(free-molecular %.0f); T/T_w GPU %.3f oracle %.3f"
+          % (uyg[0], uyg[-1], uyo[0], uyo[-1], tg.mean(), to.mean(), -fm, Tg.mean() / RT, To.mean() / RT))
+    assert cg.sum() == co.sum() == (n_steps - sample_from) * n
+    assert np.abs(cg / cg.sum() - 1.0 / K).max() < 0.1 / K and np.abs(co / co.sum() - 1.0 / K).max() < 0.1 / K
+    assert np.abs(uyg - uyo).max() < 0.05 * U             # profiles agree within the statistical scatter
+    assert abs(tg.mean() / to.mean() - 1) < 0.04
+    assert abs(Tg.mean() / To.mean() - 1) < 0.03
+    # physics of the GPU result
+    assert np.abs(tg / tg.mean() - 1).max() < 0.06        # uniform momentum flux
+    assert -fm < tg.mean() < -0.2 * fm
+    assert np.all(np.diff(uyg[2:-2]) > -0.05 * U) and uyg[0] < -0.3 * U and uyg[-1] > 0.3 * U
+    assert abs(uyg[0]) < U and abs(uyg[-1]) < U           # velocity slip
+    assert np.abs(uyg + uyg[::-1]).max() < 0.06 * U       # antisymmetry
+    assert Tg.mean() > 1.02 * RT                          # viscous heating
+    ctx.close()
