@@ -13,6 +13,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -376,6 +377,45 @@ def run_b200(args):
         cfg4["table"]["hbm_frac"] = n4 * 12 / (cfg4["table"]["ms"] * 1e-3) / 1e9 / hbm_peak
         del E4d, b4d, o4
 
+    # (f4) the whole DSMC loop around the step on the same population laid out as a 1-D channel: move + Maxwell walls
+    # -> bin -> gather x -> fused collide (table) -> sample, on the device (dsmc_couette_run); the input of every
+    # bin is the previous step's sorted order after one free flight, as in a running simulation
+    loop = {}
+    if not args.no_variants and rank == 0:
+        rng = np.random.default_rng(11)
+        rt = float((pop.vx.astype(np.float64) ** 2 + pop.vy.astype(np.float64) ** 2 + pop.vz.astype(np.float64) ** 2).mean() / 3)
+        dx = 1.0e-4
+        geo = dsmc.CouetteParams(L=dx * pop.n_cells, dt=0.3 * dx / math.sqrt(rt), u_wall=500.0, rt_wall=rt,
+                                 accommodation=1.0, n_cells=pop.n_cells)
+        xs = torch.from_numpy(((pop.cell + rng.random(pop.n)) * dx).astype(np.float32)).to(dev)
+        vs = [v.clone() for v in vin]
+        acc = torch.zeros((pop.n_cells, 8), dtype=torch.float64, device=dev)
+        n_loop = max(5, args.steps // 2)
+        ctx.couette_run(xs, *vs, geo, 3, abi=params("table"), seed=4, step0=0, sample_from=0, acc=acc)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        l0 = ctx.launch_count()
+        a0.record()
+        ctx.couette_run(xs, *vs, geo, n_loop, abi=params("table"), seed=4, step0=3, sample_from=0, acc=acc)
+        a1.record()
+        torch.cuda.synchronize()
+        loop = {"ms_per_step": a0.elapsed_time(a1) / n_loop, "steps": n_loop,
+                "launches_per_step": (ctx.launch_count() - l0) / n_loop}
+        cellb = torch.empty(pop.n, dtype=torch.int32, device=dev)
+        for name, fn in (("move_ms", lambda t: ctx.move_couette(xs, *vs, geo, seed=4, step=100 + t, cell=cellb)),
+                         ("gather_ms", lambda t: ctx.gather_f32(out[3], xs, out=out[0])),
+                         ("sample_ms", lambda t: ctx.sample_cells(out[4], out[0], out[1], out[2], acc))):
+            fn(0)
+            torch.cuda.synchronize()
+            a0.record()
+            for t in range(5):
+                fn(1 + t)
+            a1.record()
+            torch.cuda.synchronize()
+            loop[name] = a0.elapsed_time(a1) / 5
+        loop["pairs_per_s"] = pairs / (loop["ms_per_step"] * 1e-3)
+        del xs, vs, acc, cellb
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -412,7 +452,7 @@ def run_b200(args):
             "config": config_dict(args, pop, pairs), "clocks": sampler.summary(),
             "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "api": "dsmc_step_host (pinned host buffers)"},
-            "gpu_launches": int(launches), "roofline": roof, "variants": variants, "cfg4_chi_batch": cfg4,
+            "gpu_launches": int(launches), "roofline": roof, "variants": variants, "cfg4_chi_batch": cfg4, "couette_loop": loop,
             "table_build_s": t_table}
     if not args.no_cpu_baseline and world >= 1:
         chi = "table" if args.chi == "table" else "mlp"
