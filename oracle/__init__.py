@@ -52,13 +52,13 @@ class _Vhs(C.Structure):
     _fields_ = [("mass", C.c_double), ("sigma_v", C.c_double), ("T_scale", C.c_double),
                 ("noise_sigma", C.c_double), ("shell_eps", C.c_double), ("d_ref", C.c_double),
                 ("omega", C.c_double), ("T_ref", C.c_double), ("pairs_per_cell", C.c_int32),
-                ("flags", C.c_uint32), ("cell_base", C.c_int32)]
+                ("flags", C.c_uint32), ("cell_base", C.c_int32), ("pairs_count", C.POINTER(C.c_int32))]
 
 
 class _Abi(C.Structure):
     _fields_ = [("mass", C.c_double), ("b_max", C.c_double), ("lnE_min", C.c_double),
                 ("lnE_max", C.c_double), ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32),
-                ("flags", C.c_uint32), ("cell_base", C.c_int32)]
+                ("flags", C.c_uint32), ("cell_base", C.c_int32), ("pairs_count", C.POINTER(C.c_int32))]
 
 
 class _Table(C.Structure):
@@ -138,10 +138,15 @@ class VhsParams:
     pairs_per_cell: int = -1
     flags: int = F_NOISE | F_ENERGY_SHELL | F_MOMENT_MATCH
     cell_base: int = 0
+    pairs_count: np.ndarray = None  # per-cell request (int32), overrides pairs_per_cell
 
     def c(self):
+        pc = None
+        if self.pairs_count is not None:
+            self.pairs_count = _i32(self.pairs_count)
+            pc = _p(self.pairs_count, C.c_int32)
         return _Vhs(self.mass, self.sigma_v, self.T_scale, self.noise_sigma, self.shell_eps,
-                    self.d_ref, self.omega, self.T_ref, self.pairs_per_cell, self.flags, self.cell_base)
+                    self.d_ref, self.omega, self.T_ref, self.pairs_per_cell, self.flags, self.cell_base, pc)
 
 
 @dataclass
@@ -154,10 +159,15 @@ class AbinitioParams:
     pairs_per_cell: int = -1
     flags: int = F_MOMENT_MATCH
     cell_base: int = 0
+    pairs_count: np.ndarray = None  # per-cell request (int32), overrides pairs_per_cell
 
     def c(self):
+        pc = None
+        if self.pairs_count is not None:
+            self.pairs_count = _i32(self.pairs_count)
+            pc = _p(self.pairs_count, C.c_int32)
         return _Abi(self.mass, self.b_max, self.lnE_min, self.lnE_max, self.chi_mode,
-                    self.pairs_per_cell, self.flags, self.cell_base)
+                    self.pairs_per_cell, self.flags, self.cell_base, pc)
 
 
 @dataclass
@@ -446,3 +456,15 @@ def sample_cells(cell_start, vx, vy, vz, acc=None):
     lib().orc_sample_cells(C.c_int32(K), _p(cs, C.c_int32), _p(vx, C.c_double), _p(vy, C.c_double),
                            _p(vz, C.c_double), _p(acc, C.c_double))
     return acc
+
+
+def ntc_counts(cell_start, sigma_cr_max, coef, remainder):
+    """NTC candidate counts with carried remainder (Q31); `remainder` (float64) is updated in place."""
+    cs = _i32(cell_start)
+    K = cs.shape[0] - 1
+    scm = np.ascontiguousarray(sigma_cr_max, np.float32)
+    assert remainder.dtype == np.float64 and remainder.flags.c_contiguous and remainder.shape[0] == K
+    counts = np.empty(K, np.int32)
+    lib().orc_ntc_counts(C.c_int32(K), _p(cs, C.c_int32), _p(scm, C.c_float), C.c_double(coef),
+                         _p(remainder, C.c_double), _p(counts, C.c_int32))
+    return counts

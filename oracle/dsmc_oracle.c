@@ -342,7 +342,8 @@ int orc_collide_vhs_nn(int64_t n, int32_t n_cells, const int32_t *cell_start, do
     orc_cell_state(N, cx, cy, cz, prm->mass, ubar, &Theta, &Tk);
     for (int32_t p = 0; p < N; ++p) E_pre += cx[p] * cx[p] + cy[p] * cy[p] + cz[p] * cz[p];
     int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
-    int32_t M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, prm->pairs_per_cell, pi);
+    int32_t M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N,
+                            prm->pairs_count ? prm->pairs_count[k] : prm->pairs_per_cell, pi);
     int32_t n_collided = 0;
     for (int32_t s = 0; s < M; ++s) {
       int32_t i = pi[2 * s], j = pi[2 * s + 1];
@@ -421,11 +422,12 @@ int orc_collide_abinitio(int64_t n, int32_t n_cells, const int32_t *cell_start, 
     int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
     double *dv = replace ? (double *)calloc((size_t)(3 * N), sizeof(double)) : NULL;
     int32_t M;
+    const int32_t M_req = prm->pairs_count ? prm->pairs_count[k] : prm->pairs_per_cell;
     if (replace) {
       M = N / 2;
-      if (prm->pairs_per_cell >= 0 && prm->pairs_per_cell < M) M = prm->pairs_per_cell;
+      if (M_req >= 0 && M_req < M) M = M_req;
     } else {
-      M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, prm->pairs_per_cell, pi);
+      M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, M_req, pi);
     }
     int32_t n_collided = 0;
     for (int32_t s = 0; s < M; ++s) {
@@ -674,6 +676,31 @@ void orc_sample_cells(int32_t n_cells, const int32_t *cell_start, const double *
       a[5] += vy[s] * vy[s];
       a[6] += vz[s] * vz[s];
       a[7] += vx[s] * vy[s];
+    }
+  }
+}
+
+
+/* f1: NTC candidate count with carried remainder (Q31) */
+void orc_ntc_counts(int32_t n_cells, const int32_t *cell_start, const float *sigma_cr_max, double coef,
+                    double *remainder, int32_t *counts) {
+  for (int32_t k = 0; k < n_cells; ++k) {
+    int32_t N = cell_start[k + 1] - cell_start[k];
+    if (N < 2) {
+      counts[k] = 0;
+      continue;
+    }
+    {
+      double pairs = (double)N * (double)(N - 1);
+      double m = 0.5 * pairs;
+      m = m * coef;
+      m = m * (double)sigma_cr_max[k];
+      m = m + remainder[k];
+      {
+        double f = floor(m);
+        counts[k] = (int32_t)f;
+        remainder[k] = m - f;
+      }
     }
   }
 }

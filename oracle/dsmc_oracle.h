@@ -57,6 +57,8 @@ typedef struct {
   int32_t pairs_per_cell;     /* >0 request per cell, -1 = floor(N_k/2) */
   uint32_t flags;
   int32_t cell_base;          /* RNG cell coordinate of local cell 0 (cell-range shards) */
+  const int32_t *pairs_count; /* NULL, or the request of every cell (overrides pairs_per_cell): the NTC candidate
+                                 count of orc_ntc_counts, "proportional to N_k (N_k - 1) and ... (sigma v_r)max,k" */
 } orc_vhs_params;
 
 typedef struct {
@@ -66,6 +68,7 @@ typedef struct {
   int32_t pairs_per_cell;
   uint32_t flags;
   int32_t cell_base; /* RNG cell coordinate of local cell 0 */
+  const int32_t *pairs_count; /* as in orc_vhs_params */
 } orc_abinitio_params;
 
 typedef struct { /* chi[iE*nB + iB], node (lnE_min + iE*dE, iB/(nB-1)), Q13 */
@@ -151,6 +154,14 @@ double orc_chi_exact(const orc_potential *pot, double E, double b, int32_t n_pan
 /* fills chi[nE*nB] with |chi| rounded to fp32 (Q14) */
 void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, double lnE_min,
                          double lnE_max, double b_max, int32_t n_panels, float *chi);
+
+/* ---- f1: NTC candidate count with a carried remainder (Bird 1994 eq. 11.3; Q31) ----
+ * "a number of candidate pairs is drawn proportional to N_k (N_k - 1) and a cell-wise upper bound (sigma v_r)max,k":
+ * m = 1/2 N_k (N_k - 1) coef (sigma v_r)max,k + R_k, count_k = floor(m), R_k <- m - count_k, with
+ * coef = F_N dt / V_c (the paper does not give the constant: an input).  Evaluated in fp64 in exactly this order
+ * (((0.5 * (N (N-1))) * coef) * max) + R.  Cells with N_k < 2 get 0 and keep their remainder. */
+void orc_ntc_counts(int32_t n_cells, const int32_t *cell_start, const float *sigma_cr_max, double coef,
+                    double *remainder, int32_t *counts);
 
 /* ---- f4: the minimal DSMC loop around the collision step, 1-D Couette layout (Q30) ----
  * Walls at x = 0 (moving with y-velocity -u_wall) and x = L (+u_wall), "U_wall = +-500 m/s".  The paper

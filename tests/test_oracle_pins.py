@@ -641,3 +641,58 @@ def test_with_replacement_selection_and_batch_semantics():
     post2 = oracle.cell_moments(cs, r2.vx, r2.vy, r2.vz)
     np.testing.assert_allclose(post2[:, 3], pre[:, 3], rtol=1e-12)
     np.testing.assert_allclose(post2[:, :3], pre[:, :3], atol=1e-8)
+
+
+# --------------------------------------------------------------- f1: NTC candidate count, carried remainder
+def test_ntc_counts_formula_remainder_and_time_average():
+    """count = floor(1/2 N (N-1) coef max + R) ("proportional to N_k (N_k - 1) and ... (sigma v_r)max,k"),
+    the fraction is carried: over T steps the counts add up to floor(T m) and never differ from m by one or more."""
+    cs = np.array([0, 10, 11, 11, 31, 131], np.int32)
+    cap = np.array([1.0, 5.0, 7.0, 2.0, 0.37], np.float32)
+    coef = 0.0123
+    R = np.zeros(5)
+    N = np.diff(cs).astype(np.float64)
+    m = 0.5 * N * (N - 1) * coef * cap.astype(np.float64)
+    total = np.zeros(5, np.int64)
+    for t in range(1, 401):
+        c = oracle.ntc_counts(cs, cap, coef, R)
+        total += c
+        assert np.all(c >= np.floor(m)) and np.all(c <= np.floor(m) + 1)
+        assert np.all((R >= 0) & (R < 1))
+        assert np.all(np.abs(total - t * m) < 1.0)          # the running total tracks t m to within one pair
+    assert list(total[1:3]) == [0, 0]                       # N = 1 and N = 0: no candidates
+    assert abs(R[0] - (400 * m[0] - total[0])) < 1e-9
+    # a remainder handed in is honoured
+    R = np.array([0.75, 0, 0, 0, 0])
+    c = oracle.ntc_counts(cs, cap, coef, R)
+    assert c[0] == math.floor(m[0] + 0.75) and abs(R[0] - (m[0] + 0.75 - c[0])) < 1e-12
+
+
+def test_ntc_equilibrium_collision_frequency_closed_form():
+    """NTC candidates x acceptance reproduce the equilibrium VHS collision rate (Bird 1994 eq. 4.64):
+    accepted collisions per cell and step = 1/2 N (N-1) coef <sigma_T c_r>, <sigma_T c_r> = nu / n =
+    4 d_ref^2 sqrt(pi kB T_ref / m) (T / T_ref)^(1 - omega); checked at T = 400 K so the exponent matters."""
+    T = 400.0
+    K, N, steps = 200, 200, 6
+    pop = wl.tiny_box(seed=21, n_cells=K, per_cell=N, T=T)
+    rc, perm, cs = oracle.bin_particles(pop.cell, K)
+    v = [a[perm].astype(np.float64) for a in (pop.vx, pop.vy, pop.vz)]
+    base = oracle.VhsParams(flags=oracle.F_ACCEPT | oracle.F_ENERGY_SHELL | oracle.F_NOISE, sigma_v=wl.SIGMA_V)
+    cap = np.full(K, oracle.vhs_sigma_g(8 * wl.SIGMA_V, base), np.float32)
+    rate = 4 * base.d_ref ** 2 * math.sqrt(math.pi * KB * base.T_ref / M) * (T / base.T_ref) ** (1 - base.omega)
+    coef = 24.3 / (0.5 * N * (N - 1) * float(cap[0]))       # 24.3 candidates per cell and step
+    Ws, bs = wl.random_mlp(0, [8, 8, 8, 3])
+    R = np.zeros(K)
+    cand = acc = 0
+    for t in range(steps):
+        counts = oracle.ntc_counts(cs, cap, coef, R)
+        prm = oracle.VhsParams(flags=base.flags, sigma_v=wl.SIGMA_V, pairs_count=counts)
+        r = oracle.collide_vhs_nn(cs, *v, oracle.Mlp(Ws, bs), prm, 4, t, sigma_cr_max=cap)
+        ok = r.pair_i >= 0
+        assert ok.sum() == counts.sum()                      # every cell ran exactly its own count
+        cand += ok.sum()
+        acc += r.accepted[ok].sum()
+        v = [r.vx, r.vy, r.vz]                               # energy-shell collisions keep the gas at T
+    assert abs(cand - steps * K * 24.3) < K                  # carried remainders: within one pair per cell
+    want = steps * K * 0.5 * N * (N - 1) * coef * rate
+    assert abs(acc - want) < 4 * math.sqrt(want)             # Poisson scatter of the accepted count
