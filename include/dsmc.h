@@ -15,6 +15,7 @@
  *   dsmc_chi_exact_batch   chi by the deflection-integral quadrature itself (eq. 16), LJ 12-6
  *   dsmc_build_chi_table_lj  the chi table generated on the device by that quadrature
  *   dsmc_step_host         bin + fused step on HOST buffers (copies inside), for end-to-end timing
+ *   dsmc_ntc_counts        NTC candidate counts with carried remainder
  *   dsmc_move_couette, dsmc_gather_f32, dsmc_sample_cells, dsmc_couette_run
  *                          the minimal DSMC loop around the step for the 1-D Couette layout
  *
@@ -134,6 +135,9 @@ typedef struct {
   uint32_t flags;
   int32_t cell_base;         /* RNG cell coordinate of local cell 0: a rank that owns the global cell range
                                 [c0, c1) passes c0 and draws exactly the randoms of the unsharded run */
+  const int32_t *pairs_count; /* NULL, or DEVICE array [n_cells]: the request of every cell, overriding
+                                pairs_per_cell (e.g. the NTC candidate counts of dsmc_ntc_counts).
+                                M_k = min(pairs_count[k], N_k/2); negative entries mean N_k/2 */
 } dsmc_vhs_params;
 
 typedef struct {
@@ -144,6 +148,7 @@ typedef struct {
   int32_t pairs_per_cell;
   uint32_t flags;         /* NOISE / ENERGY_SHELL are ignored here */
   int32_t cell_base;      /* as in dsmc_vhs_params */
+  const int32_t *pairs_count; /* as in dsmc_vhs_params */
 } dsmc_abinitio_params;
 
 /* Optional debug output (any member may be NULL).  All arrays have n entries; pair slot s of
@@ -214,6 +219,16 @@ int dsmc_step_host(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cel
                    float *vy_out_h, float *vz_out_h, int32_t *perm_h, int32_t *cell_start_h,
                    const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi, uint64_t seed,
                    uint32_t step);
+
+/* ---- f1: NTC candidate count with a carried remainder (Q31) ---------------------------
+ * "a number of candidate pairs is drawn proportional to N_k (N_k - 1) and a cell-wise upper bound (sigma v_r)max,k":
+ * m = 1/2 N_k (N_k - 1) coef sigma_cr_max[k] + remainder[k]; counts[k] = floor(m); remainder[k] = m - counts[k],
+ * evaluated in FP64 in that order, coef = F_N dt / V_c (not given by the paper: an input).  Cells with N_k < 2 get
+ * 0 and keep their remainder.  sigma_cr_max [n_cells] float, remainder [n_cells] double in/out (the caller zeroes
+ * it once), counts [n_cells] int32 out: pass it as pairs_count of the next fused step (with DSMC_F_ACCEPT and the
+ * same sigma_cr_max this is the NTC scheme; the disjoint matching caps the count at N_k/2). */
+int dsmc_ntc_counts(dsmc_ctx *ctx, int32_t n_cells, const int32_t *cell_start, const float *sigma_cr_max,
+                    double coef, double *remainder, int32_t *counts);
 
 /* ---- f4: the minimal DSMC loop around the step, 1-D Couette layout (Q30) -------
  * Walls normal to x at x = 0 (moving with y-velocity -u_wall) and x = L (+u_wall); "U_wall = +-500 m/s".

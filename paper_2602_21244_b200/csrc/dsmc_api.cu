@@ -257,6 +257,7 @@ int dsmc_collide_vhs_nn(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
   fill_common(p, c, n, K, cs, vx, vy, vz, sigma_cr_max, seed, step, dump);
   p.flags = prm->flags;
   p.pairs_per_cell = prm->pairs_per_cell;
+  p.pairs_count = prm->pairs_count;
   p.op = 0;
   p.cell_base = (uint32_t)prm->cell_base;
   p.mass = prm->mass;
@@ -297,6 +298,7 @@ int dsmc_collide_abinitio(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, 
   fill_common(p, c, n, K, cs, vx, vy, vz, cr_max, seed, step, dump);
   p.flags = prm->flags & ~(uint32_t)(DSMC_F_NOISE | DSMC_F_ENERGY_SHELL);
   p.pairs_per_cell = prm->pairs_per_cell;
+  p.pairs_count = prm->pairs_count;
   p.op = prm->chi_mode == 0 ? 1 : 2;
   p.cell_base = (uint32_t)prm->cell_base;
   p.mass = prm->mass;
@@ -422,6 +424,15 @@ int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, con
   if (cell_start_h)
     CK(cudaMemcpyAsync(cell_start_h, c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1), cudaMemcpyDeviceToHost, s));
   return dsmc_sync_status(c);
+}
+
+int dsmc_ntc_counts(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *sigma_cr_max, double coef,
+                    double *remainder, int32_t *counts) {
+  if (!c || K < 0 || !(coef >= 0.0)) return DSMC_ERR_INVALID_ARG;
+  if (K == 0) return DSMC_OK;
+  if (!cs || !sigma_cr_max || !remainder || !counts) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(c->device));
+  return launch_ntc_counts(c, K, cs, sigma_cr_max, coef, remainder, counts);
 }
 
 int dsmc_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,

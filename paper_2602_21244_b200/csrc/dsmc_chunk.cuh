@@ -185,7 +185,8 @@ __device__ int chunk_begin(const TM &T, const StepParams &P, CK &S, int chunk, i
     const int a = atomicAdd(&S.misc[MI_NACT], 1);
     if (a >= CK::AMAX) continue;
     int M = N >> 1;
-    if (P.pairs_per_cell >= 0 && P.pairs_per_cell < M) M = P.pairs_per_cell;
+    const int req = P.pairs_count ? __ldg(P.pairs_count + c) : P.pairs_per_cell;
+    if (req >= 0 && req < M) M = req;
     const int nseg = (N + kSeg - 1) / kSeg;
     const int seg0 = atomicAdd(&S.misc[MI_NSEG], nseg);
     CellInfo ci;

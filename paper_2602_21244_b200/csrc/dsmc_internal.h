@@ -54,6 +54,7 @@ struct StepParams {
   uint32_t cell_base;  // RNG cell coordinate of local cell 0
   uint32_t flags;
   int32_t pairs_per_cell;
+  const int32_t *pairs_count;  // per-cell request or nullptr
   int32_t op;  // 0 = VHS-NN, 1 = ab initio table, 2 = ab initio MLP
   float mass;
   // VHS-NN
@@ -137,6 +138,8 @@ int launch_chi_table_lj(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_
                         double sigma, float *table_dev, float4 *quad_dev);
 int launch_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,
                         int32_t *bounces, const dsmc_couette_params *g, uint64_t seed, uint32_t step);
+int launch_ntc_counts(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *cap, double coef, double *remainder,
+                      int32_t *counts);
 int launch_gather_f32(dsmc_ctx *c, int64_t n, const int32_t *perm, const float *src, float *dst);
 int launch_sample_cells(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *vx, const float *vy, const float *vz,
                         double *acc);

@@ -101,6 +101,35 @@ __global__ void __launch_bounds__(256) k_sample_cells(int32_t K, const int32_t *
   }
 }
 
+// f1: NTC candidate counts with carried remainder (Q31).  FP64, one thread per cell; the products are
+// rounded one by one (no FMA contraction) so that the floor is taken of the same number on every machine.
+__global__ void __launch_bounds__(256) k_ntc_counts(int32_t K, const int32_t *__restrict__ cs,
+                                                   const float *__restrict__ cap, double coef,
+                                                   double *__restrict__ remainder, int32_t *__restrict__ counts) {
+  for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < K; k += (int64_t)gridDim.x * blockDim.x) {
+    const int N = __ldg(cs + k + 1) - __ldg(cs + k);
+    if (N < 2) {
+      counts[k] = 0;
+      continue;
+    }
+    double m = __dmul_rn(0.5, (double)N * (double)(N - 1));
+    m = __dmul_rn(m, coef);
+    m = __dmul_rn(m, (double)__ldg(cap + k));
+    m = __dadd_rn(m, remainder[k]);
+    const double f = floor(m);
+    counts[k] = (int32_t)f;
+    remainder[k] = __dsub_rn(m, f);
+  }
+}
+
+int launch_ntc_counts(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *cap, double coef, double *remainder,
+                      int32_t *counts) {
+  const int grid = (int)std::min<int64_t>(((int64_t)K + 255) / 256, (int64_t)c->num_sms * 8);
+  k_ntc_counts<<<grid, 256, 0, c->stream>>>(K, cs, cap, coef, remainder, counts);
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
 int launch_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,
                         int32_t *bounces, const dsmc_couette_params *g, uint64_t seed, uint32_t step) {
   MoveParams P;

@@ -29,7 +29,7 @@ EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
            "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host", "dsmc_move_couette",
-           "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run"]
+           "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run", "dsmc_ntc_counts"]
 
 
 class DsmcError(RuntimeError):
@@ -47,13 +47,13 @@ class _VhsParams(C.Structure):
     _fields_ = [("mass", C.c_float), ("sigma_v", C.c_float), ("T_scale", C.c_float),
                 ("noise_sigma", C.c_float), ("shell_eps", C.c_float), ("d_ref", C.c_float),
                 ("omega", C.c_float), ("T_ref", C.c_float), ("pairs_per_cell", C.c_int32),
-                ("flags", C.c_uint32), ("cell_base", C.c_int32)]
+                ("flags", C.c_uint32), ("cell_base", C.c_int32), ("pairs_count", C.c_void_p)]
 
 
 class _AbiParams(C.Structure):
     _fields_ = [("mass", C.c_float), ("b_max", C.c_float), ("lnE_min", C.c_float), ("lnE_max", C.c_float),
                 ("chi_mode", C.c_int32), ("pairs_per_cell", C.c_int32), ("flags", C.c_uint32),
-                ("cell_base", C.c_int32)]
+                ("cell_base", C.c_int32), ("pairs_count", C.c_void_p)]
 
 
 class _CouetteParams(C.Structure):
@@ -112,10 +112,12 @@ class VhsParams:
     pairs_per_cell: int = -1
     flags: int = F_NOISE | F_ENERGY_SHELL | F_MOMENT_MATCH
     cell_base: int = 0
+    pairs_count: "torch.Tensor" = None  # device int32 [n_cells]: per-cell request, overrides pairs_per_cell
 
     def c(self):
         return _VhsParams(self.mass, self.sigma_v, self.T_scale, self.noise_sigma, self.shell_eps, self.d_ref,
-                          self.omega, self.T_ref, self.pairs_per_cell, self.flags, self.cell_base)
+                          self.omega, self.T_ref, self.pairs_per_cell, self.flags, self.cell_base,
+                          _ptr(self.pairs_count, torch.int32) if self.pairs_count is not None else None)
 
 
 @dataclass
@@ -128,10 +130,12 @@ class AbinitioParams:
     pairs_per_cell: int = -1
     flags: int = F_MOMENT_MATCH
     cell_base: int = 0
+    pairs_count: "torch.Tensor" = None  # device int32 [n_cells]: per-cell request, overrides pairs_per_cell
 
     def c(self):
         return _AbiParams(self.mass, self.b_max, self.lnE_min, self.lnE_max, self.chi_mode, self.pairs_per_cell,
-                          self.flags, self.cell_base)
+                          self.flags, self.cell_base,
+                          _ptr(self.pairs_count, torch.int32) if self.pairs_count is not None else None)
 
 
 @dataclass
@@ -309,6 +313,18 @@ class Context:
         _chk(_lib.dsmc_chi_exact_batch(self._h, C.c_int64(E_over_k.shape[0]), _ptr(E_over_k, torch.float32),
                                        _ptr(b, torch.float32), _ptr(out, torch.float32), C.c_float(eps_over_k),
                                        C.c_float(sigma), C.c_uint32(flags)), "dsmc_chi_exact_batch")
+        return out
+
+    # ---- f1: NTC candidate counts with carried remainder
+    def ntc_counts(self, cell_start, sigma_cr_max, coef: float, remainder, out=None):
+        """counts[k] = floor(1/2 N (N-1) coef sigma_cr_max[k] + remainder[k]); remainder (float64) updated in place."""
+        K = cell_start.shape[0] - 1
+        if out is None:
+            out = torch.empty(K, dtype=torch.int32, device=cell_start.device)
+        self._stream()
+        _chk(_lib.dsmc_ntc_counts(self._h, C.c_int32(K), _ptr(cell_start, torch.int32),
+                                  _ptr(sigma_cr_max, torch.float32), C.c_double(coef),
+                                  _ptr(remainder, torch.float64), _ptr(out, torch.int32)), "dsmc_ntc_counts")
         return out
 
     # ---- f4: the minimal DSMC loop around the step (1-D Couette layout)

@@ -224,3 +224,63 @@ def test_couette_flow_profiles_against_the_oracle_loop(dsmc):
     assert np.abs(uyg + uyg[::-1]).max() < 0.06 * U       # antisymmetry
     assert Tg.mean() > 1.02 * RT                          # viscous heating
     ctx.close()
+
+
+# ------------------------------------------------------------------ f1: NTC candidate counts (Q31)
+def test_ntc_counts_bit_exact_and_per_cell_requests(dsmc):
+    """dsmc_ntc_counts against the oracle over several steps (counts and FP64 remainders bit-exact), then one fused
+    step of each operator driven by the per-cell counts: pair indices bit-exact against the oracle, every cell ran
+    min(count, N/2) pairs."""
+    rng = np.random.default_rng(4)
+    counts = rng.integers(0, 120, 900)
+    counts[3], counts[4], counts[5], counts[6] = 0, 1, 2, 2048
+    pop = wl._populate("ragged", counts, np.full(900, 300.0), np.zeros(900), np.zeros(900), 4)
+    K = pop.n_cells
+    ctx = dsmc.Context(pop.n, K)
+    vx_s, vy_s, vz_s, perm, cs = ctx.bin(dev(pop.cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), K)
+    cs_h = cs.cpu().numpy()
+    cap = (rng.random(K) * 2e-16 + 1e-16).astype(np.float32)
+    coef = 0.37 / (60 * float(cap.mean()))     # about 0.37 N candidates in a 120-particle cell
+    R_o = np.zeros(K)
+    R_d = torch.zeros(K, dtype=torch.float64, device="cuda")
+    cap_d = dev(cap)
+    for t in range(5):
+        want = oracle.ntc_counts(cs_h, cap, coef, R_o)
+        got = ctx.ntc_counts(cs, cap_d, coef, R_d)
+        ctx.check()
+        assert np.array_equal(got.cpu().numpy(), want)
+        assert np.array_equal(R_d.cpu().numpy(), R_o)
+    assert want.max() > 60 and (want == 0).sum() > 3 and want[6] > 1024   # some above N/2, some zero
+    N = np.diff(cs_h)
+    M_want = np.where(N >= 2, np.minimum(want, N // 2), 0)
+    # ab initio table operator with the per-cell counts
+    tab = _lj_table(64, 64)
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    v_in = [a.cpu().numpy().astype(np.float64) for a in (vx_s, vy_s, vz_s)]
+    dump = dsmc.PairDump(pop.n, "cuda")
+    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, dsmc.AbinitioParams(pairs_count=got), seed=9, step=1, dump=dump)
+    ctx.check()
+    ref = oracle.collide_abinitio(cs_h, *v_in, oracle.AbinitioParams(pairs_count=want), 9, 1, table=tab)
+    pi = dump.pair_i.cpu().numpy()
+    assert np.array_equal(pi, ref.pair_i) and np.array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
+    per_cell = np.add.reduceat((pi >= 0).astype(np.int64), cs_h[:-1][N > 0])
+    assert np.array_equal(per_cell, M_want[N > 0])
+    for a, w in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
+        assert np.abs(a.cpu().numpy() - w).max() < 2e-4 * 400
+    # VHS-NN with NTC acceptance on the same counts
+    Ws, bs = wl.random_mlp(2, [8, 64, 64, 3])
+    ctx.set_mlp(0, Ws, bs, dsmc.ACT_TANH)
+    net = oracle.Mlp(Ws, bs, oracle.ACT_TANH)
+    flags = dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | dsmc.F_ACCEPT
+    oprm = oracle.VhsParams(sigma_v=float(np.float32(wl.SIGMA_V)), flags=flags, pairs_count=want)
+    cap_v = np.full(K, oracle.vhs_sigma_g(6 * wl.SIGMA_V, oprm), np.float32)
+    v_in = [a.cpu().numpy().astype(np.float64) for a in (vx_s, vy_s, vz_s)]
+    dump = dsmc.PairDump(pop.n, "cuda")
+    ctx.collide_vhs_nn(cs, vx_s, vy_s, vz_s, dsmc.VhsParams(sigma_v=wl.SIGMA_V, flags=flags, pairs_count=got),
+                       seed=9, step=2, sigma_cr_max=dev(cap_v), dump=dump)
+    ctx.check()
+    ref = oracle.collide_vhs_nn(cs_h, *v_in, net, oprm, 9, 2, sigma_cr_max=cap_v)
+    assert np.array_equal(dump.pair_i.cpu().numpy(), ref.pair_i)
+    assert np.array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
+    assert (dump.accepted.cpu().numpy() != ref.accepted).sum() <= 2      # Q22: decisions at the threshold
+    ctx.close()
