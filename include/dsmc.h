@@ -95,7 +95,8 @@ int dsmc_set_mlp(dsmc_ctx *ctx, int slot, const dsmc_mlp_desc *desc);
 
 /* chi table: chi_host HOST fp32 [nE][nB] row-major, node (iE,iB) at
  * E~ = lnE_min + iE (lnE_max-lnE_min)/(nE-1) with E~ = ln(E_r/k_B [K]), b~ = iB/(nB-1).
- * Lookups clamp both coordinates to the grid (Q13).  Copied during the call. */
+ * Lookups clamp both coordinates to the grid (Q13).  Copied during the call.  Every node must be finite
+ * (DSMC_ERR_INVALID_ARG otherwise): cap nodes on the orbiting singularity as dsmc_build_chi_table_lj does (64 pi, Q23). */
 int dsmc_set_chi_table(dsmc_ctx *ctx, const float *chi_host, int32_t nE, int32_t nB, float lnE_min,
                        float lnE_max);
 
@@ -247,6 +248,13 @@ typedef struct {
   float rt_wall;       /* k_B T_wall / m [m^2/s^2] */
   float accommodation; /* in [0, 1]: 1 = fully diffuse walls, 0 = specular */
   int32_t n_cells;
+  /* used by dsmc_couette_run only: NTC rate control.  ntc_coef = F_N dt / V_c > 0 makes every step draw
+   * dsmc_ntc_counts candidates per cell (remainders start at 0 and are carried through the run) against the uniform
+   * bound sigma_cr_max [m^3/s]; with DSMC_F_ACCEPT the same bound caps the acceptance test (VHS-NN: sigma_T(g) g /
+   * sigma_cr_max; ab initio, constant cross-section pi b_max^2: g / (sigma_cr_max / (pi b_max^2))).
+   * ntc_coef = 0: the pair request of the operator's parameter struct is used as is. */
+  float ntc_coef;
+  float sigma_cr_max;
 } dsmc_couette_params;
 
 /* x, vx, vy, vz [n] in/out (vy, vz are written only for re-emitted particles); cell [n] out; bounces [n] out or

@@ -592,7 +592,11 @@ void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, doubl
     double E = ORC_KB * exp(lnE);
     for (int32_t iB = 0; iB < nB; ++iB) {
       double b = b_max * (double)iB / (double)(nB - 1);
-      chi[(size_t)iE * nB + iB] = (float)fabs(orc_chi_exact(pot, E, b, n_panels)); /* Q14 */
+      double c = fabs(orc_chi_exact(pot, E, b, n_panels)); /* Q14 */
+      /* Q23: a node that falls on the orbiting singularity (chi -> infinity: the pair spirals) is capped at 32
+       * revolutions so that the fp32 table stays finite; any such angle is as good as another */
+      if (!(c <= 64.0 * PI)) c = 64.0 * PI;
+      chi[(size_t)iE * nB + iB] = (float)c;
     }
   }
 }

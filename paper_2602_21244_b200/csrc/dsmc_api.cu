@@ -80,6 +80,10 @@ int dsmc_destroy(dsmc_ctx *c) {
   cudaFree(c->h_cell_start);
   cudaFree(c->h_x[0]);
   cudaFree(c->h_x[1]);
+  cudaFree(c->h_counts);
+  cudaFree(c->h_rem);
+  cudaFree(c->h_cap[0]);
+  cudaFree(c->h_cap[1]);
   delete c;
   return DSMC_OK;
 }
@@ -166,6 +170,8 @@ int dsmc_set_mlp(dsmc_ctx *c, int slot, const dsmc_mlp_desc *d) {
 
 int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t nB, float lnE_min, float lnE_max) {
   if (!c || !chi_host || nE < 2 || nB < 2 || !(lnE_max > lnE_min)) return DSMC_ERR_INVALID_ARG;
+  for (size_t i = 0; i < (size_t)nE * nB; ++i)
+    if (!isfinite(chi_host[i])) return DSMC_ERR_INVALID_ARG;  // a non-finite node would poison every pair near it
   CK(cudaSetDevice(c->device));
   CK(cudaStreamSynchronize(c->stream));
   cudaFree(c->d_table);
@@ -339,6 +345,13 @@ static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
   cudaFree(c->h_x[0]);
   cudaFree(c->h_x[1]);
   c->h_x[0] = c->h_x[1] = nullptr;
+  cudaFree(c->h_counts);
+  cudaFree(c->h_rem);
+  cudaFree(c->h_cap[0]);
+  cudaFree(c->h_cap[1]);
+  c->h_counts = nullptr;
+  c->h_rem = nullptr;
+  c->h_cap[0] = c->h_cap[1] = nullptr;
   c->host_cap_n = 0;
   CK(cudaMalloc(&c->h_cell, sizeof(int32_t) * (size_t)n));
   for (int a = 0; a < 3; ++a) {
@@ -348,6 +361,9 @@ static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
   CK(cudaMalloc(&c->h_perm, sizeof(int32_t) * (size_t)n));
   for (int a = 0; a < 2; ++a) CK(cudaMalloc(&c->h_x[a], sizeof(float) * (size_t)n));
   CK(cudaMalloc(&c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1)));
+  CK(cudaMalloc(&c->h_counts, sizeof(int32_t) * (size_t)K));
+  CK(cudaMalloc(&c->h_rem, sizeof(double) * (size_t)K));
+  for (int a = 0; a < 2; ++a) CK(cudaMalloc(&c->h_cap[a], sizeof(float) * (size_t)K));
   c->host_cap_n = n;
   c->host_cap_cells = K;
   return DSMC_OK;
@@ -480,6 +496,24 @@ int dsmc_couette_run(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, flo
   float *sorted[4] = {c->h_x[1], c->h_vs[0], c->h_vs[1], c->h_vs[2]};
   float *unsorted[4] = {c->h_x[0], c->h_v[0], c->h_v[1], c->h_v[2]};
   for (int a = 0; a < 4; ++a) CK(cudaMemcpyAsync(unsorted[a], user[a], bytes, cudaMemcpyDeviceToDevice, s));
+  // NTC rate control: per-cell candidate counts every step, uniform caps
+  const bool ntc = g->ntc_coef > 0.f;
+  dsmc_vhs_params pv;
+  dsmc_abinitio_params pa;
+  const float *cap = nullptr;
+  if (vhs) pv = *vhs;
+  if (abi) pa = *abi;
+  if (ntc) {
+    if (!(g->sigma_cr_max > 0.f)) return DSMC_ERR_INVALID_ARG;
+    const float cap_accept =
+        vhs ? g->sigma_cr_max : (float)((double)g->sigma_cr_max / (M_PI * (double)abi->b_max * (double)abi->b_max));
+    rc = launch_fill_f32(c, K, c->h_cap[0], g->sigma_cr_max);
+    if (rc == DSMC_OK) rc = launch_fill_f32(c, K, c->h_cap[1], cap_accept);
+    if (rc != DSMC_OK) return rc;
+    CK(cudaMemsetAsync(c->h_rem, 0, sizeof(double) * (size_t)K, s));
+    pv.pairs_count = pa.pairs_count = c->h_counts;
+    if ((vhs ? vhs->flags : abi->flags) & DSMC_F_ACCEPT) cap = c->h_cap[1];
+  }
   for (int32_t k = 0; k < n_steps; ++k) {
     const uint32_t step = step0 + (uint32_t)k;
     rc = dsmc_move_couette(c, n, unsorted[0], unsorted[1], unsorted[2], unsorted[3], c->h_cell, nullptr, g, seed,
@@ -490,11 +524,15 @@ int dsmc_couette_run(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, flo
     if (rc != DSMC_OK) return rc;
     rc = dsmc_gather_f32(c, n, c->h_perm, unsorted[0], sorted[0]);
     if (rc != DSMC_OK) return rc;
+    if (ntc) {
+      rc = dsmc_ntc_counts(c, K, c->h_cell_start, c->h_cap[0], (double)g->ntc_coef, c->h_rem, c->h_counts);
+      if (rc != DSMC_OK) return rc;
+    }
     if (vhs)
-      rc = dsmc_collide_vhs_nn(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], nullptr, vhs, seed, step,
+      rc = dsmc_collide_vhs_nn(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], cap, &pv, seed, step,
                                nullptr);
     else
-      rc = dsmc_collide_abinitio(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], nullptr, abi, seed, step,
+      rc = dsmc_collide_abinitio(c, n, K, c->h_cell_start, sorted[1], sorted[2], sorted[3], cap, &pa, seed, step,
                                  nullptr);
     if (rc != DSMC_OK) return rc;
     if (acc && k >= sample_from) {

@@ -101,7 +101,8 @@ __global__ void __launch_bounds__(128) k_chi_table_lj(int nE, int nB, double lnE
     const int iE = (int)(p / nB), iB = (int)(p % nB);
     const double Es = exp(lnE_min + iE * dlnE) * inv_eps_k;
     const double bs = bmax_star * ((double)iB / (double)(nB - 1));
-    table[p] = (float)fabs(chi_exact_lj(Es, bs));
+    // Q23: a node on the orbiting singularity (chi -> infinity) is capped at 32 revolutions: the table stays finite
+    table[p] = (float)fmin(fabs(chi_exact_lj(Es, bs)), 64.0 * 3.141592653589793);
   }
 }
 

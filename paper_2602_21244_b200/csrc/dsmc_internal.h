@@ -111,6 +111,9 @@ struct dsmc_ctx {
   float *h_v[3], *h_vs[3];
   int32_t *h_perm, *h_cell_start;
   float *h_x[2];  // dsmc_couette_run: positions (unsorted / sorted)
+  int32_t *h_counts;  // dsmc_couette_run, NTC: candidate counts, remainders, count / acceptance caps [cells]
+  double *h_rem;
+  float *h_cap[2];
   int64_t host_cap_n;
   int32_t host_cap_cells;
 };
@@ -140,6 +143,7 @@ int launch_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, 
                         int32_t *bounces, const dsmc_couette_params *g, uint64_t seed, uint32_t step);
 int launch_ntc_counts(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *cap, double coef, double *remainder,
                       int32_t *counts);
+int launch_fill_f32(dsmc_ctx *c, int64_t n, float *dst, float value);
 int launch_gather_f32(dsmc_ctx *c, int64_t n, const int32_t *perm, const float *src, float *dst);
 int launch_sample_cells(dsmc_ctx *c, int32_t K, const int32_t *cs, const float *vx, const float *vy, const float *vz,
                         double *acc);

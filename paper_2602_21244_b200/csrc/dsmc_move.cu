@@ -150,6 +150,18 @@ int launch_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, 
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
 
+__global__ void __launch_bounds__(256) k_fill_f32(int64_t n, float *__restrict__ dst, float value) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    dst[i] = value;
+}
+
+int launch_fill_f32(dsmc_ctx *c, int64_t n, float *dst, float value) {
+  const int grid = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 8);
+  k_fill_f32<<<grid, 256, 0, c->stream>>>(n, dst, value);
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
 int launch_gather_f32(dsmc_ctx *c, int64_t n, const int32_t *perm, const float *src, float *dst) {
   const int grid = (int)std::min<int64_t>((n + 255) / 256, (int64_t)c->num_sms * 16);
   k_gather_f32<<<grid, 256, 0, c->stream>>>(n, perm, src, dst);

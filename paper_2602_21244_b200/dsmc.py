@@ -58,7 +58,8 @@ class _AbiParams(C.Structure):
 
 class _CouetteParams(C.Structure):
     _fields_ = [("L", C.c_float), ("dt", C.c_float), ("u_wall", C.c_float), ("rt_wall", C.c_float),
-                ("accommodation", C.c_float), ("n_cells", C.c_int32)]
+                ("accommodation", C.c_float), ("n_cells", C.c_int32), ("ntc_coef", C.c_float),
+                ("sigma_cr_max", C.c_float)]
 
 
 class _PairDump(C.Structure):
@@ -147,9 +148,12 @@ class CouetteParams:
     rt_wall: float
     accommodation: float
     n_cells: int
+    ntc_coef: float = 0.0      # F_N dt / V_c; > 0: NTC candidate counts every step of couette_run
+    sigma_cr_max: float = 0.0  # uniform (sigma c_r)max bound of the NTC count and acceptance
 
     def c(self):
-        return _CouetteParams(self.L, self.dt, self.u_wall, self.rt_wall, self.accommodation, self.n_cells)
+        return _CouetteParams(self.L, self.dt, self.u_wall, self.rt_wall, self.accommodation, self.n_cells,
+                              self.ntc_coef, self.sigma_cr_max)
 
 
 class PairDump:

@@ -284,3 +284,68 @@ def test_ntc_counts_bit_exact_and_per_cell_requests(dsmc):
     assert np.array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
     assert (dump.accepted.cpu().numpy() != ref.accepted).sum() <= 2      # Q22: decisions at the threshold
     ctx.close()
+
+
+def test_couette_viscosity_matches_chapman_enskog(dsmc):
+    """End-to-end physics of the whole device-side loop with NTC rate control and the ab initio table
+    operator: argon (LJ 12-6) between diffuse walls at Kn = 0.05.  In the bulk the momentum flux must equal
+    mu(T) du_y/dx with the Chapman-Enskog viscosity of the SAME potential, mu = 5/16 sqrt(pi m k T) / (pi sigma^2
+    Omega22*(T*)) (the paper's eqs. 17-19 in standard form, Q28), Omega22* evaluated here from the oracle's
+    deflection angles (pinned to the textbook table by P14).  Nothing in the collision path knows about viscosity:
+    pairing, NTC counts, acceptance, the chi table, the rotation and the cell-wise matching all have to be right
+    for this number to come out."""
+    KB, m = 1.380649e-23, 6.63e-26
+    eps_k, sig = 119.8, 3.405e-10
+    Tw, U = 273.0, 150.0
+    rt = KB * Tw / m
+    b_max = 1.0e-9
+    n_dens = 1.0e20
+    K, per = 60, 150
+    L = 0.345                                   # Kn = 0.05 on the viscosity-based mean free path (17 mm)
+    dt = 1.0e-6
+    g_max = 2000.0
+    sigma_T = math.pi * b_max ** 2
+    geo = dsmc.CouetteParams(L, dt, U, rt, 1.0, K, ntc_coef=n_dens * dt / per, sigma_cr_max=sigma_T * g_max)
+    n = K * per
+    rng = np.random.default_rng(31)
+    x = (rng.random(n) * L).astype(np.float32)
+    v = rng.normal(0.0, math.sqrt(rt), (3, n))
+    v[1] += 0.85 * U * (2 * x / L - 1)          # start near the steady shear profile: short transient
+    v = v.astype(np.float32)
+    ctx = dsmc.Context(n, K)
+    ctx.build_chi_table_lj(512, 512, b_max=b_max, eps_over_k=eps_k, sigma=sig)
+    prm = dsmc.AbinitioParams(mass=m, b_max=b_max, flags=dsmc.F_MOMENT_MATCH | dsmc.F_ACCEPT)
+    xd, vxd, vyd, vzd = dev(x), dev(v[0]), dev(v[1]), dev(v[2])
+    acc = torch.zeros((K, 8), dtype=torch.float64, device="cuda")
+    n_steps, sample_from = 30000, 6000
+    ctx.couette_run(xd, vxd, vyd, vzd, geo, n_steps, abi=prm, seed=2, step0=0, sample_from=sample_from, acc=acc)
+    A = acc.cpu().numpy()
+    cnt = A[:, 0]
+    uy = A[:, 2] / cnt
+    flux = (A[:, 7] - A[:, 1] * uy).sum() / cnt.sum()            # <n c_x c_y> / n_0, uniform across the gap
+    T = m * ((A[:, 4] + A[:, 5] + A[:, 6]) / cnt - (A[:, 1] ** 2 + A[:, 2] ** 2 + A[:, 3] ** 2) / cnt ** 2) / (3 * KB)
+    xc = (np.arange(K) + 0.5) * L / K
+    bulk = slice(10, K - 10)                                     # outside the Knudsen layers (3 mean free paths)
+    slope = np.polyfit(xc[bulk], uy[bulk], 1)[0]
+    rho0 = n_dens * m
+    mu_meas = -rho0 * flux / slope
+    T_bulk = T[bulk].mean()
+    # Chapman-Enskog viscosity of LJ argon at T_bulk from the oracle's deflection angles
+    pot = oracle.lj_argon()
+    xs, ws = np.polynomial.laguerre.laggauss(20)
+    nb, bm = 400, 4.0
+    bs = (np.arange(nb) + 0.5) * bm / nb
+
+    def q2_star(Es):
+        chi = np.array([oracle.chi_exact(pot, Es * eps_k * KB, b * sig) for b in bs])
+        return 3.0 * np.sum((1.0 - np.cos(chi) ** 2) * bs) * bm / nb
+
+    Ts = T_bulk / eps_k
+    omega = sum(w * xx ** 3 * q2_star(xx * Ts) for xx, w in zip(xs, ws)) / 6.0
+    mu_ce = 5.0 / 16.0 * math.sqrt(math.pi * m * KB * T_bulk) / (math.pi * sig ** 2 * omega)
+    print("Couette, LJ argon, Kn 0.05: mu = %.4e Pa s measured, %.4e Chapman-Enskog (Omega22* = %.4f at T = %.1f K);"
+          " slope %.1f 1/s of %.1f no-slip; T_max %.1f K" % (mu_meas, mu_ce, omega, T_bulk, slope, 2 * U / L, T.max()))
+    assert 0.75 * 2 * U / L < slope < 2 * U / L                  # velocity slip
+    assert Tw < T_bulk < Tw + 20 and T.argmax() in range(K // 2 - 12, K // 2 + 12)   # viscous heating, centred
+    assert abs(mu_meas / mu_ce - 1) < 0.06
+    ctx.close()
