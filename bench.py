@@ -42,6 +42,7 @@ def parse():
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the population (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--no-loop", action="store_true", help="skip the couette_loop section (SURVEY 8(f4))")
     return ap.parse_args()
 
 
@@ -381,7 +382,7 @@ def run_b200(args):
     # -> bin -> gather x -> fused collide (table) -> sample, on the device (dsmc_couette_run); the input of every
     # bin is the previous step's sorted order after one free flight, as in a running simulation
     loop = {}
-    if not args.no_variants and rank == 0:
+    if not args.no_loop and rank == 0:
         rng = np.random.default_rng(11)
         rt = float((pop.vx.astype(np.float64) ** 2 + pop.vy.astype(np.float64) ** 2 + pop.vz.astype(np.float64) ** 2).mean() / 3)
         dx = 1.0e-4
