@@ -149,6 +149,23 @@ __device__ __forceinline__ float warp_sum_f(float v) {
   return v;
 }
 
+// Four warp sums for the price of six shuffles (instead of twenty): the butterfly halves the number of values a
+// lane carries in each of its first two steps.  Returns the total of a in lanes 0-7, b in 8-15, c in 16-23, d in
+// 24-31 (lane >> 3 selects the component).
+__device__ __forceinline__ float warp_sum4_t(float a, float b, float c, float d, int lane) {
+  const bool up = lane & 16;
+  float k0 = up ? c : a, k1 = up ? d : b;
+  k0 += __shfl_xor_sync(0xffffffffu, up ? a : c, 16);
+  k1 += __shfl_xor_sync(0xffffffffu, up ? b : d, 16);
+  const bool up2 = lane & 8;
+  float k = up2 ? k1 : k0;
+  k += __shfl_xor_sync(0xffffffffu, up2 ? k0 : k1, 8);
+  k += __shfl_xor_sync(0xffffffffu, k, 4);
+  k += __shfl_xor_sync(0xffffffffu, k, 2);
+  k += __shfl_xor_sync(0xffffffffu, k, 1);
+  return k;
+}
+
 // ---------------------------------------------------------------------------------------------
 // begin: returns n_loc > 0 when there is work, 0 when the chunk has nothing to collide (nothing
 // to store either), -1 when the chunk does not fit this variant (caller defers it).
@@ -174,7 +191,7 @@ __device__ int chunk_begin(const TM &T, const StepParams &P, CK &S, int chunk, i
       asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d + 8u), "l"(P.vz + q0 + q) : "memory");
     }
   }
-  for (int q = tid; q < n_loc; q += TM::kN) S.cnt[q] = 0;
+  for (int q = 4 * tid; q < n_loc; q += 4 * TM::kN) *reinterpret_cast<int4 *>(S.cnt + q) = make_int4(0, 0, 0, 0);
   if (tid < 8) S.misc[tid] = 0;
   T.sync();
   // cell discovery (order of the active list is irrelevant to the results)
@@ -228,9 +245,10 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
       const int m = min(N, 32);
       const float4 f = lane < m ? S.v[start + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
       const float im = 1.0f / (float)m;
-      pv.x = warp_sum_f(f.x) * im;
-      pv.y = warp_sum_f(f.y) * im;
-      pv.z = warp_sum_f(f.z) * im;
+      const float t = warp_sum4_t(f.x, f.y, f.z, 0.f, lane) * im;
+      pv.x = __shfl_sync(0xffffffffu, t, 0);
+      pv.y = __shfl_sync(0xffffffffu, t, 8);
+      pv.z = __shfl_sync(0xffffffffu, t, 16);
       pv.w = 0.f;
       if (lane == 0 && piece == 0) {  // parked in the cell record until the finalisation below replaces it by u
         S.cells[a].ux = pv.x;
@@ -245,8 +263,10 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
       sx += dx; sy += dy; sz += dz;
       s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
     }
-    sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
-    if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
+    {
+      const float t = warp_sum4_t(sx, sy, sz, s2, lane);
+      if ((lane & 7) == 0) reinterpret_cast<float *>(&S.part[sg])[lane >> 3] = t;
+    }
     if (CK::REPLACE) {  // no matching to build: pair list only, and clear the change accumulators
       for (int q = lo + lane; q < hi; q += 32) {
         reinterpret_cast<float *>(S.key)[q] = 0.f;
@@ -506,8 +526,8 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
         sx += dx; sy += dy; sz += dz;
         s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
       }
-      sx = warp_sum_f(sx); sy = warp_sum_f(sy); sz = warp_sum_f(sz); s2 = warp_sum_f(s2);
-      if (lane == 0) S.part[sg] = make_float4(sx, sy, sz, s2);
+      const float t = warp_sum4_t(sx, sy, sz, s2, lane);
+      if ((lane & 7) == 0) reinterpret_cast<float *>(&S.part[sg])[lane >> 3] = t;
     }
     T.sync();
     for (int a = tid; a < n_act; a += TM::kN) {
