@@ -341,12 +341,24 @@ int orc_collide_vhs_nn(int64_t n, int32_t n_cells, const int32_t *cell_start, do
     double ubar[3], Theta, Tk, E_pre = 0.0;
     orc_cell_state(N, cx, cy, cz, prm->mass, ubar, &Theta, &Tk);
     for (int32_t p = 0; p < N; ++p) E_pre += cx[p] * cx[p] + cy[p] * cy[p] + cz[p] * cz[p];
+    /* with replacement (the paper's literal NTC text), batch semantics as in
+     * orc_collide_abinitio below: every pair sees the PRE-collision velocities, changes add up (Q29) */
+    const int replace = (prm->flags & ORC_F_PAIR_REPLACE) != 0;
+    const int32_t M_req = prm->pairs_count ? prm->pairs_count[k] : prm->pairs_per_cell;
     int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
-    int32_t M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N,
-                            prm->pairs_count ? prm->pairs_count[k] : prm->pairs_per_cell, pi);
+    double *dv = replace ? (double *)calloc((size_t)(3 * N), sizeof(double)) : NULL;
+    int32_t M;
+    if (replace) {
+      M = N / 2;
+      if (M_req >= 0 && M_req < M) M = M_req;
+    } else {
+      M = orc_pairing(seed, step, (uint32_t)(k + prm->cell_base), N, M_req, pi);
+    }
     int32_t n_collided = 0;
     for (int32_t s = 0; s < M; ++s) {
-      int32_t i = pi[2 * s], j = pi[2 * s + 1];
+      int32_t i, j;
+      if (replace) orc_pair_draw(seed, step, (uint32_t)(k + prm->cell_base), (uint32_t)s, N, &i, &j);
+      else { i = pi[2 * s]; j = pi[2 * s + 1]; }
       double g[3] = {cx[i] - cx[j], cy[i] - cy[j], cz[i] - cz[j]}; /* eq. 1 */
       double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
       double U[3], xi[3];
@@ -379,15 +391,26 @@ int orc_collide_vhs_nn(int64_t n, int32_t n_cells, const int32_t *cell_start, do
         } else {
           gp[0] = prm->sigma_v * h[0]; gp[1] = prm->sigma_v * h[1]; gp[2] = prm->sigma_v * h[2];
         }
-        double cm[3] = {0.5 * (cx[i] + cx[j]), 0.5 * (cy[i] + cy[j]), 0.5 * (cz[i] + cz[j])};
-        cx[i] = cm[0] + 0.5 * gp[0]; cy[i] = cm[1] + 0.5 * gp[1]; cz[i] = cm[2] + 0.5 * gp[2];
-        cx[j] = cm[0] - 0.5 * gp[0]; cy[j] = cm[1] - 0.5 * gp[1]; cz[j] = cm[2] - 0.5 * gp[2];
+        if (replace) { /* v_i' - v_i = (g' - g) / 2 = -(v_j' - v_j), eqs. 6-8 */
+          for (int d = 0; d < 3; ++d) {
+            dv[3 * i + d] += 0.5 * (gp[d] - g[d]);
+            dv[3 * j + d] -= 0.5 * (gp[d] - g[d]);
+          }
+        } else {
+          double cm[3] = {0.5 * (cx[i] + cx[j]), 0.5 * (cy[i] + cy[j]), 0.5 * (cz[i] + cz[j])};
+          cx[i] = cm[0] + 0.5 * gp[0]; cy[i] = cm[1] + 0.5 * gp[1]; cz[i] = cm[2] + 0.5 * gp[2];
+          cx[j] = cm[0] - 0.5 * gp[0]; cy[j] = cm[1] - 0.5 * gp[1]; cz[j] = cm[2] - 0.5 * gp[2];
+        }
         n_collided++;
       }
       if (gprime_out) { gprime_out[3 * (a + s)] = gp[0]; gprime_out[3 * (a + s) + 1] = gp[1]; gprime_out[3 * (a + s) + 2] = gp[2]; }
       if (hnorm_out) hnorm_out[a + s] = hn;
     }
     free(pi);
+    if (replace) {
+      for (int32_t p = 0; p < N; ++p) { cx[p] += dv[3 * p]; cy[p] += dv[3 * p + 1]; cz[p] += dv[3 * p + 2]; }
+      free(dv);
+    }
     if ((prm->flags & ORC_F_MOMENT_MATCH) && n_collided > 0)
       match_cell(N, cx, cy, cz, ubar, Theta, E_pre, prm->flags);
   }

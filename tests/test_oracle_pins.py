@@ -696,3 +696,48 @@ def test_ntc_equilibrium_collision_frequency_closed_form():
     assert abs(cand - steps * K * 24.3) < K                  # carried remainders: within one pair per cell
     want = steps * K * 0.5 * N * (N - 1) * coef * rate
     assert abs(acc - want) < 4 * math.sqrt(want)             # Poisson scatter of the accepted count
+
+
+def test_with_replacement_vhs_nn_batch_semantics():
+    """SURVEY 8(f1) for the VHS-surrogate operator: the same with-replacement draw and batch semantics as the ab
+    initio step.  Brute force from the dumped pairs: g' recomputed with the MLP evaluated by numpy on the
+    PRE-collision relative velocity (features of Q2/Q3, energy-shell projection eq. 5), changes added up; momentum
+    exact, energy restored only by the matching."""
+    pop = wl.tiny_box(seed=17, n_cells=5, per_cell=36, T=300.0)
+    rc, perm, cs = oracle.bin_particles(pop.cell, pop.n_cells)
+    v = [a[perm].astype(np.float64) for a in (pop.vx, pop.vy, pop.vz)]
+    Ws, bs = wl.random_mlp(6, [8, 16, 16, 3])
+    net = oracle.Mlp(Ws, bs, oracle.ACT_TANH)
+    flags = oracle.F_PAIR_REPLACE | oracle.F_ENERGY_SHELL          # no noise: the features are deterministic
+    prm = oracle.VhsParams(sigma_v=wl.SIGMA_V, flags=flags)
+    r = oracle.collide_vhs_nn(cs, *v, net, prm, 5, 3)
+    assert (r.pair_i >= 0).sum() == 5 * 18
+    for k in range(pop.n_cells):
+        a, N = cs[k], cs[k + 1] - cs[k]
+        loc = np.stack([x[a:a + N] for x in v], axis=1)
+        ubar = loc.mean(axis=0)
+        Tk = M * ((loc - ubar) ** 2).sum() / (3 * KB * N)           # eq. 10 cell temperature (Q3)
+        dv = np.zeros_like(loc)
+        for s in range(N // 2):
+            i, j = r.pair_i[a + s], r.pair_j[a + s]
+            assert (i, j) == oracle.pair_draw(5, 3, k, s, N)
+            g = loc[i] - loc[j]
+            gn = np.linalg.norm(g)
+            h = np.concatenate([g / wl.SIGMA_V, [gn / wl.SIGMA_V, Tk / 273.0, 0.0, 0.0, 0.0]])
+            for l, (W, b) in enumerate(zip(Ws, bs)):
+                h = W.astype(np.float64) @ h + b.astype(np.float64)
+                if l < len(Ws) - 1:
+                    h = np.tanh(h)
+            gp = gn * h / np.linalg.norm(h)
+            np.testing.assert_allclose(r.gprime[a + s], gp, rtol=1e-10, atol=1e-9)
+            dv[i] += 0.5 * (gp - g)
+            dv[j] -= 0.5 * (gp - g)
+        got = np.stack([r.vx[a:a + N], r.vy[a:a + N], r.vz[a:a + N]], axis=1)
+        np.testing.assert_allclose(got, loc + dv, rtol=0, atol=1e-9)
+    pre, post = oracle.cell_moments(cs, *v), oracle.cell_moments(cs, r.vx, r.vy, r.vz)
+    np.testing.assert_allclose(post[:, :3], pre[:, :3], atol=1e-8)
+    assert np.abs(post[:, 3] / pre[:, 3] - 1).max() > 1e-3
+    r2 = oracle.collide_vhs_nn(cs, *v, net, oracle.VhsParams(sigma_v=wl.SIGMA_V, flags=flags | oracle.F_MOMENT_MATCH), 5, 3)
+    post2 = oracle.cell_moments(cs, r2.vx, r2.vy, r2.vz)
+    np.testing.assert_allclose(post2[:, 3], pre[:, 3], rtol=1e-12)
+    np.testing.assert_allclose(post2[:, :3], pre[:, :3], atol=1e-8)
