@@ -121,7 +121,7 @@ enum {
                                    + (j >= i) from Philox stream 4; every pair of a cell is evaluated on the
                                    pre-collision velocities (one batch) and the velocity changes of a
                                    particle that appears in several pairs add up.  Momentum is conserved exactly,
-                                   energy is restored by DSMC_F_MOMENT_MATCH.  Ab initio operator, FP32 / table paths
+                                   energy is restored by DSMC_F_MOMENT_MATCH.  Both operators, FP32 / table paths
                                    (not with DSMC_F_BF16_TC).  No key sort: the cheapest selection. */
 };
 

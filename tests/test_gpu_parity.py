@@ -625,6 +625,54 @@ def test_collide_abinitio_with_replacement(dsmc, mode, match):
     ctx.close()
 
 
+def test_collide_vhs_nn_with_replacement(dsmc):
+    """SURVEY 8(f1) for the VHS-surrogate operator with NTC acceptance: pairs drawn with replacement, batch
+    semantics.  Pair indices and acceptance bit-exact, g' to the FP32 tolerance on the gated set (Q21), velocities
+    to 1e-4 of the thermal scale, conserved moments to 1e-6."""
+    pop = wl.cavity(nx=16, ny=16)
+    ctx, net = _setup_vhs(dsmc, pop, 64, 5)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    flags = dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | dsmc.F_ACCEPT | dsmc.F_PAIR_REPLACE
+    prm = dsmc.VhsParams(sigma_v=wl.SIGMA_V, flags=flags)
+    oprm = oracle.VhsParams(sigma_v=float(np.float32(wl.SIGMA_V)), flags=flags)
+    cap = np.full(pop.n_cells, oracle.vhs_sigma_g(6 * wl.SIGMA_V, oprm), np.float32)
+    v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+    dump = dsmc.PairDump(pop.n, "cuda")
+    ctx.collide_vhs_nn(cs, vx_s, vy_s, vz_s, prm, seed=8, step=4, sigma_cr_max=dev(cap), dump=dump)
+    ctx.check()
+    ref = oracle.collide_vhs_nn(cs_h, *v_in, net, oprm, 8, 4, sigma_cr_max=cap)
+    np.testing.assert_array_equal(dump.pair_i.cpu().numpy(), ref.pair_i)
+    np.testing.assert_array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
+    diff = dump.accepted.cpu().numpy() != ref.accepted
+    assert diff.sum() <= 2                                   # Q22: decisions within 1e-5 of the threshold
+    N = np.diff(cs_h)
+    pre = oracle.cell_moments(cs_h, *v_in)
+    got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+    ok = N >= 2
+    assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+    sel = ref.pair_i >= 0
+    if not diff.any():
+        hn = ref.aux
+        gate = (hn >= 0.25 * np.median(hn[sel & (ref.accepted == 1)])) | (ref.accepted == 0)
+        idx = np.flatnonzero(sel & gate)
+        k = np.searchsorted(cs_h, idx, side="right") - 1
+        g = np.stack([a[cs_h[k] + ref.pair_i[idx]] - a[cs_h[k] + ref.pair_j[idx]] for a in v_in], axis=1)
+        err = np.linalg.norm(dump.gprime.cpu().numpy()[idx].astype(np.float64) - ref.gprime[idx], axis=1) / np.linalg.norm(g, axis=1)
+        assert err.max() < 2e-5
+        scale = np.repeat(np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1)), N)
+        for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
+            assert np.median(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale) < 1e-5
+    multi = np.bincount(np.r_[ref.pair_i[sel] + cs_h[k_all(cs_h, sel)], ref.pair_j[sel] + cs_h[k_all(cs_h, sel)]], minlength=pop.n)
+    assert (multi >= 2).mean() > 0.15                         # particles drawn into several pairs of one batch
+    ctx.close()
+
+
+def k_all(cs_h, sel):
+    return np.searchsorted(cs_h, np.flatnonzero(sel), side="right") - 1
+
+
 # --------------------------------------------------------------------------------------- free-running runs (Q20)
 @pytest.mark.parametrize("tc", [False, True])
 def test_free_running_100_steps_no_artificial_cooling(dsmc, tc):
