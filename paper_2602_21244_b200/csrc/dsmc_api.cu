@@ -41,6 +41,8 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
     if (passes > 3) return DSMC_ERR_INVALID_ARG;
     CK(cudaMalloc(&c->d_bin_hist, sizeof(int32_t) * tiles * kBinMaxRadix));
     CK(cudaMalloc(&c->d_bin_group, sizeof(int32_t) * (size_t)c->num_sms * kBinMaxRadix));
+    CK(cudaMalloc(&c->d_cell_count, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) + 1)));
+    CK(cudaMalloc(&c->d_cell_tile_sums, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) / 4096 + 2)));
     for (int i = 0; i < 2; ++i) {
       CK(cudaMalloc(&c->d_bin_cell[i], sizeof(int32_t) * np));
       if (i < passes - 1) CK(cudaMalloc(&c->d_bin_rec[i], sizeof(float4) * np));
@@ -63,6 +65,8 @@ int dsmc_destroy(dsmc_ctx *c) {
   cudaFree(c->d_status);
   cudaFree(c->d_bin_hist);
   cudaFree(c->d_bin_group);
+  cudaFree(c->d_cell_count);
+  cudaFree(c->d_cell_tile_sums);
   for (int i = 0; i < 2; ++i) { cudaFree(c->d_bin_rec[i]); cudaFree(c->d_bin_cell[i]); }
   cudaFree(c->d_chunk_first);
   cudaFree(c->d_big);

@@ -12,9 +12,10 @@
 //              k_prefix      exclusive prefix over (digit, tile)       in place
 //              k_downsweep   stable in-tile ranking (warp match + per-warp digit counters),
 //                            reorder in shared memory, write runs
-//   finally    k_cell_start  CSR offsets from the boundaries of the sorted cell ids
+//   finally    k_cell_tile_sums, k_cell_scan   CSR offsets = prefix sum of the per-cell counts the last down-sweep
+//                            accumulates (one atomic per run of equal cells; the sorted cell ids are never written)
 //
-// Algorithmic traffic (2 passes): 4+16+20 B and 4+20+20 B per particle, +8 B for the offsets.
+// Algorithmic traffic (2 passes): 4+16+20 B and 4+20+16 B per particle.
 #include <algorithm>
 
 #include "dsmc_device.cuh"
@@ -161,7 +162,8 @@ struct BinIo {
   int32_t *cell_out;
   // LAST pass output
   float *vx_s, *vy_s, *vz_s;
-  int32_t *perm, *cell_sorted;
+  int32_t *perm;
+  int32_t *cell_count;  // [n_cells + 1], zeroed: particles per cell, counted by the LAST pass
   int32_t bulk_ok;  // FIRST-pass inputs are 16-byte aligned
 };
 
@@ -331,7 +333,10 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
       io.vx_s[dst] = rr.y;
       io.vy_s[dst] = rr.z;
       io.vz_s[dst] = rr.w;
-      io.cell_sorted[dst] = cc;
+      // particles per cell: the 32 consecutive sorted positions of a warp hold a few runs of equal cell ids (the
+      // tile arrives ordered by the lower digits), one atomic per run
+      const uint32_t m = __match_any_sync(__activemask(), cc);
+      if (lane == __ffs(m) - 1) atomicAdd(io.cell_count + cc, __popc(m));
     } else {
       io.rec_out[dst] = rr;
       io.cell_out[dst] = cc;
@@ -339,27 +344,81 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
   }
 }
 
-// cell_start[c] = first sorted slot whose cell id is >= c (CSR offsets; covers empty cells).
-// Four consecutive slots per thread (one 16-byte load + the left neighbour).
-__global__ void __launch_bounds__(256) k_cell_start(int64_t n, int32_t K, const int32_t *__restrict__ cell_sorted,
-                                                   int32_t *__restrict__ cell_start) {
-  const int64_t s0 = 4 * (blockIdx.x * (int64_t)blockDim.x + threadIdx.x);
-  if (s0 > n) return;
-  int v[5];
-  v[0] = s0 > 0 ? __ldg(cell_sorted + s0 - 1) : -1;
-  if (s0 + 4 <= n) {
-    const int4 q = __ldg(reinterpret_cast<const int4 *>(cell_sorted + s0));
-    v[1] = q.x; v[2] = q.y; v[3] = q.z; v[4] = q.w;
-  } else {
+// cell_start = exclusive prefix sum of the per-cell counts (CSR offsets; entry n_cells = particles kept).  Two
+// launches: sums of 4096-count tiles, then every CTA adds up the tiles before its own and scans its tile.
+constexpr int kScanThreads = 256, kScanItems = 16, kScanTile = kScanThreads * kScanItems;
+
+__global__ void __launch_bounds__(kScanThreads) k_cell_tile_sums(int32_t n, const int32_t *__restrict__ count,
+                                                                int32_t *__restrict__ tile_sums) {
+  __shared__ int ws[kScanThreads / 32];
+  const int base = blockIdx.x * kScanTile;
+  int sum = 0;
 #pragma unroll
-    for (int u = 0; u < 4; ++u) v[1 + u] = s0 + u < n ? __ldg(cell_sorted + s0 + u) : K;
+  for (int r = 0; r < kScanItems; ++r) {
+    const int i = base + r * kScanThreads + threadIdx.x;
+    sum += i < n ? __ldg(count + i) : 0;
   }
 #pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    const int64_t s = s0 + u;
-    if (s > n) break;
-    const int prev = max(-1, min(v[u], K)), cur = max(-1, min(s < n ? v[u + 1] : K, K));
-    for (int cc = prev + 1; cc <= cur; ++cc) cell_start[cc] = (int32_t)s;
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = sum;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int t = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) t += ws[w];
+    tile_sums[blockIdx.x] = t;
+  }
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_cell_scan(int32_t n, const int32_t *__restrict__ count,
+                                                           const int32_t *__restrict__ tile_sums,
+                                                           int32_t *__restrict__ cell_start) {
+  __shared__ int ws[kScanThreads / 32];
+  __shared__ int sc[kScanTile];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int base = blockIdx.x * kScanTile;
+  // tiles before this one
+  int before = 0;
+  for (int t = tid; t < (int)blockIdx.x; t += kScanThreads) before += __ldg(tile_sums + t);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xffffffffu, before, o);
+  if (lane == 0) ws[warp] = before;
+  // stage the tile (coalesced), then every thread owns kScanItems consecutive counts
+#pragma unroll
+  for (int r = 0; r < kScanItems; ++r) {
+    const int i = base + r * kScanThreads + tid;
+    sc[r * kScanThreads + tid] = i < n ? __ldg(count + i) : 0;
+  }
+  __syncthreads();
+  before = 0;
+#pragma unroll
+  for (int w = 0; w < kScanThreads / 32; ++w) before += ws[w];
+  int loc[kScanItems], sum = 0;
+#pragma unroll
+  for (int r = 0; r < kScanItems; ++r) {
+    loc[r] = sum;
+    sum += sc[tid * kScanItems + r];
+  }
+  int inc = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += y;
+  }
+  __syncthreads();  // ws and sc are read by everyone above
+  if (lane == 31) ws[warp] = inc;
+  __syncthreads();
+  int woff = 0;
+#pragma unroll
+  for (int w = 0; w < kScanThreads / 32; ++w) woff += (w < warp) ? ws[w] : 0;
+  const int mine = before + woff + inc - sum;
+#pragma unroll
+  for (int r = 0; r < kScanItems; ++r) sc[tid * kScanItems + r] = mine + loc[r];
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < kScanItems; ++r) {
+    const int i = base + r * kScanThreads + tid;
+    if (i < n) cell_start[i] = sc[r * kScanThreads + tid];
   }
 }
 
@@ -386,6 +445,7 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     return cudaMemsetAsync(cell_start, 0, sizeof(int32_t) * (size_t)(K + 1), s) == cudaSuccess ? DSMC_OK
                                                                                                 : DSMC_ERR_CUDA;
   }
+  if (cudaMemsetAsync(c->d_cell_count, 0, sizeof(int32_t) * (size_t)(K + 1), s) != cudaSuccess) return DSMC_ERR_CUDA;
   int bits = 1;
   while ((int64_t(1) << bits) < (int64_t)K) ++bits;
   const int passes = (bits + 8) / 9;
@@ -409,7 +469,7 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     io.rec_out = c->d_bin_rec[p & 1];
     io.cell_out = c->d_bin_cell[p & 1];
     io.vx_s = vx_s; io.vy_s = vy_s; io.vz_s = vz_s; io.perm = perm;
-    io.cell_sorted = c->d_bin_cell[p & 1];
+    io.cell_count = c->d_cell_count;
     io.bulk_ok = ((reinterpret_cast<uintptr_t>(cell) | reinterpret_cast<uintptr_t>(vx) |
                    reinterpret_cast<uintptr_t>(vy) | reinterpret_cast<uintptr_t>(vz)) & 15) == 0;
     if (cudaMemsetAsync(c->d_bin_group, 0, sizeof(int32_t) * (size_t)groups * kBinMaxRadix, s) != cudaSuccess)
@@ -427,8 +487,10 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     else launch_downsweep<false, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
     c->launches += 3;
     if (last) {
-      k_cell_start<<<(int)((n / 4 + 1 + 255) / 256), 256, 0, s>>>(n, K, io.cell_sorted, cell_start);
-      c->launches += 1;
+      const int n_scan = K + 1, scan_tiles = (n_scan + kScanTile - 1) / kScanTile;
+      k_cell_tile_sums<<<scan_tiles, kScanThreads, 0, s>>>(n_scan, c->d_cell_count, c->d_cell_tile_sums);
+      k_cell_scan<<<scan_tiles, kScanThreads, 0, s>>>(n_scan, c->d_cell_count, c->d_cell_tile_sums, cell_start);
+      c->launches += 2;
     }
   }
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;

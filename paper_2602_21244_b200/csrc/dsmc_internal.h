@@ -90,6 +90,8 @@ struct dsmc_ctx {
   int32_t *d_bin_group;  // [num_sms][kBinMaxRadix]
   float4 *d_bin_rec[2];  // (idx, vx, vy, vz) between passes
   int32_t *d_bin_cell[2];
+  int32_t *d_cell_count;      // [max_cells + 1] particles per cell (dsmc_bin)
+  int32_t *d_cell_tile_sums;  // [(max_cells + 1) / 4096 + 1]
   int32_t *d_chunk_first;  // [max_particles / kChunk + 2]
   int4 *d_chunk_meta;      // [max_particles / kChunk + 2]
   int32_t *d_big;          // [max_particles / kChunk + 2]
