@@ -417,6 +417,50 @@ def run_b200(args):
         loop["pairs_per_s"] = pairs / (loop["ms_per_step"] * 1e-3)
         del xs, vs, acc, cellb
 
+    # the paper's other two population shapes (north_star: "Couette, cavity and Mach 10 cylinder"): cfg 2 and cfg 3
+    # with the VHS-surrogate MLP 8->128->128->3 (random init), FP32 and tensor-core paths; step = bin + fused collide.
+    # These are 1e5 / 5e5 pairs per step: launch- and latency-bound, reported for completeness (not the headline).
+    other = {}
+    if not args.no_variants and rank == 0:
+        from paper_2602_21244_b200 import workloads as wl
+        for name, popf, ppc, sw in (("cfg2_couette_200x1000", wl.couette, 500, 1), ("cfg3_cavity_100x100x100", wl.cavity, 50, 2)):
+            p2 = popf()
+            c2 = dsmc.Context(p2.n, p2.n_cells, device=local)
+            Ws, bs = wl.random_mlp(sw, [8, 128, 128, 3])
+            c2.set_mlp(0, Ws, bs, dsmc.ACT_TANH)
+            cell2 = torch.from_numpy(p2.cell).to(dev)
+            v2 = [torch.from_numpy(a).to(dev) for a in (p2.vx, p2.vy, p2.vz)]
+            o2 = (torch.empty(p2.n, dtype=torch.float32, device=dev), torch.empty(p2.n, dtype=torch.float32, device=dev),
+                  torch.empty(p2.n, dtype=torch.float32, device=dev), torch.empty(p2.n, dtype=torch.int32, device=dev),
+                  torch.empty(p2.n_cells + 1, dtype=torch.int32, device=dev))
+            pairs2 = p2.pairs_per_step(ppc)
+            other[name] = {"pairs_per_step": int(pairs2)}
+            for path, fl in (("fp32", 0), ("bf16_tc", dsmc.F_BF16_TC)):
+                prm2 = dsmc.VhsParams(sigma_v=wl.SIGMA_V, pairs_per_cell=ppc,
+                                      flags=dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | fl)
+                for t in range(3):
+                    c2.bin(cell2, *v2, p2.n_cells, out=o2)
+                    c2.collide_vhs_nn(o2[4], o2[0], o2[1], o2[2], prm2, seed=sw, step=t)
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+                a0.record()
+                for t in range(20):
+                    c2.bin(cell2, *v2, p2.n_cells, out=o2)
+                    ev2[t][0].record()
+                    c2.collide_vhs_nn(o2[4], o2[0], o2[1], o2[2], prm2, seed=sw, step=3 + t)
+                    ev2[t][1].record()
+                a1.record()
+                torch.cuda.synchronize()
+                ms2 = a0.elapsed_time(a1) / 20
+                other[name][path] = {"step_ms": ms2, "collide_ms": float(np.mean([a.elapsed_time(b) for a, b in ev2])),
+                                     "pairs_per_s": pairs2 / (ms2 * 1e-3)}
+            st2 = c2.sync_status()
+            if st2 != 0:
+                other[name]["status"] = int(st2)
+            c2.close()
+            del cell2, v2, o2
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -453,7 +497,7 @@ def run_b200(args):
             "config": config_dict(args, pop, pairs), "clocks": sampler.summary(),
             "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "api": "dsmc_step_host (pinned host buffers)"},
-            "gpu_launches": int(launches), "roofline": roof, "variants": variants, "cfg4_chi_batch": cfg4, "couette_loop": loop,
+            "gpu_launches": int(launches), "roofline": roof, "variants": variants, "cfg4_chi_batch": cfg4, "couette_loop": loop, "other_workloads": other,
             "table_build_s": t_table}
     if not args.no_cpu_baseline and world >= 1:
         chi = "table" if args.chi == "table" else "mlp"
