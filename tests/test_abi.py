@@ -32,6 +32,12 @@ def test_strerror_and_host_side_argument_errors():
     assert lib.dsmc_create(None, 0, C.c_int64(10), 4) == -1  # null out pointer: invalid argument
     assert lib.dsmc_sync_status(None) == -1
     assert lib.dsmc_set_stream(None, None) == -1
+    # the section-9 entry points reject a null context before touching anything
+    assert lib.dsmc_move_couette(None, C.c_int64(4), None, None, None, None, None, None, None, C.c_uint64(0), 0) == -1
+    assert lib.dsmc_gather_f32(None, C.c_int64(4), None, None, None) == -1
+    assert lib.dsmc_sample_cells(None, C.c_int64(4), 1, None, None, None, None, None) == -1
+    assert lib.dsmc_ntc_counts(None, 1, None, None, C.c_double(1.0), None, None) == -1
+    assert lib.dsmc_couette_run(None, C.c_int64(4), None, None, None, None, None, None, None, C.c_uint64(0), 0, 1, 0, None) == -1
 
 
 def test_product_does_not_import_the_oracle():
