@@ -349,3 +349,34 @@ def test_couette_viscosity_matches_chapman_enskog(dsmc):
     assert Tw < T_bulk < Tw + 20 and T.argmax() in range(K // 2 - 12, K // 2 + 12)   # viscous heating, centred
     assert abs(mu_meas / mu_ce - 1) < 0.06
     ctx.close()
+
+
+def test_argument_errors_of_the_loop_entry_points(dsmc):
+    """Host-detectable errors return DSMC_ERR_INVALID_ARG and launch nothing; a chi table with a non-finite node is
+    refused (Q23: such a node would turn every pair near it, and through the matching its whole cell, into NaN)."""
+    ctx = dsmc.Context(1024, 8)
+    x = torch.zeros(16, device="cuda")
+    v = [torch.zeros(16, device="cuda") for _ in range(3)]
+    good = dict(L=1.0, dt=1e-3, u_wall=1.0, rt_wall=1.0, accommodation=1.0, n_cells=8)
+    l0 = ctx.launch_count()
+    for bad in (dict(L=0.0), dict(rt_wall=0.0), dict(accommodation=1.5), dict(accommodation=-0.1), dict(n_cells=0)):
+        with pytest.raises(dsmc.DsmcError) as e:
+            ctx.move_couette(x, *v, dsmc.CouetteParams(**{**good, **bad}), seed=0, step=0)
+        assert e.value.status == -1
+    with pytest.raises(dsmc.DsmcError):   # n_cells above the context's capacity
+        ctx.couette_run(x, *v, dsmc.CouetteParams(**{**good, "n_cells": 9}), 1, abi=dsmc.AbinitioParams())
+    with pytest.raises(dsmc.DsmcError):   # neither operator
+        ctx.couette_run(x, *v, dsmc.CouetteParams(**good), 1)
+    with pytest.raises(dsmc.DsmcError):   # NTC without a bound
+        ctx.build_chi_table_lj(16, 16)
+        ctx.couette_run(x, *v, dsmc.CouetteParams(**{**good, "ntc_coef": 1.0}), 1, abi=dsmc.AbinitioParams())
+    assert ctx.launch_count() - l0 <= 2   # only the table build launched anything
+    tab = np.ones((8, 8), np.float32)
+    tab[3, 4] = np.inf
+    with pytest.raises(dsmc.DsmcError) as e:
+        ctx.set_chi_table(tab, math.log(5.0), math.log(6e4))
+    assert e.value.status == -1
+    tab[3, 4] = np.nan
+    with pytest.raises(dsmc.DsmcError):
+        ctx.set_chi_table(tab, math.log(5.0), math.log(6e4))
+    ctx.close()
