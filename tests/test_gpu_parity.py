@@ -36,7 +36,7 @@ def binned(dsmc, ctx, pop):
 
 
 # --------------------------------------------------------------------------------------- a1
-@pytest.mark.parametrize("case", ["tiny", "couette", "mach10_small", "ragged", "empty"])
+@pytest.mark.parametrize("case", ["tiny", "couette", "mach10_small", "ragged", "empty", "three_pass", "one_pass"])
 def test_bin_bit_exact(dsmc, case):
     if case == "tiny":
         pop = wl.tiny_box()
@@ -51,6 +51,14 @@ def test_bin_bit_exact(dsmc, case):
         counts[18] = 0
         counts[19] = 1
         pop = wl._populate("ragged", counts, np.full(3001, 300.0), np.zeros(3001), np.zeros(3001), 7)
+    elif case == "three_pass":   # 300 000 cells need 19 bits: three radix passes
+        rng = np.random.default_rng(11)
+        counts = rng.integers(0, 4, 300_000)
+        pop = wl._populate("three_pass", counts, np.full(300_000, 300.0), np.zeros(300_000), np.zeros(300_000), 11)
+    elif case == "one_pass":     # 300 cells: a single pass that is both first and last
+        rng = np.random.default_rng(12)
+        counts = rng.integers(0, 900, 300)
+        pop = wl._populate("one_pass", counts, np.full(300, 300.0), np.zeros(300), np.zeros(300), 12)
     else:
         pop = wl._populate("empty", np.zeros(5, np.int64), np.full(5, 300.0), np.zeros(5), np.zeros(5), 1)
     ctx = dsmc.Context(max(pop.n, 1), pop.n_cells)
