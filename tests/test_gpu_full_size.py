@@ -182,3 +182,63 @@ def test_vhs_nn_full_size(dsmc, cfg, tc):
     print("%s tc=%s: worst 99th-percentile particle deviation / thermal scale = %.3e over %d cells" % (cfg, tc, worst, len(cells)))
     assert worst < (1e-4 if not tc else 2e-2)
     ctx.close()
+
+
+def test_loop_kernels_full_size(dsmc):
+    """SURVEY 8(f4) at the size bench.py times (the cfg 5 population laid out as a 1-D channel, 2e7 particles, 80 000
+    cells): the move on a 400 000-particle prefix the oracle recomputes (the random numbers are keyed by the
+    particle index, so a prefix draws what the full run draws), validity of every particle, the gather bit-exact,
+    the sampling sums on every cell against numpy segment sums in fp64, NTC counts bit-exact on every cell."""
+    import math
+    pop = wl.mach10_cylinder()
+    n, K = pop.n, pop.n_cells
+    rng = np.random.default_rng(11)
+    rt = float((pop.vx.astype(np.float64) ** 2 + pop.vy.astype(np.float64) ** 2 + pop.vz.astype(np.float64) ** 2).mean() / 3)
+    dx = 1.0e-4
+    L, dt = dx * K, 0.3 * dx / math.sqrt(rt)
+    x = ((pop.cell + rng.random(n)) * dx).astype(np.float32)
+    geo = dsmc.CouetteParams(L, dt, 500.0, rt, 0.9, K)
+    ctx = dsmc.Context(n, K)
+    xd, vxd, vyd, vzd = dev(x), dev(pop.vx), dev(pop.vy), dev(pop.vz)
+    cell = ctx.move_couette(xd, vxd, vyd, vzd, geo, seed=3, step=7)
+    ctx.check()
+    xg, cg = xd.cpu().numpy(), cell.cpu().numpy()
+    Lf = np.float32(L)
+    assert np.all((xg >= 0) & (xg <= Lf))
+    assert np.array_equal(cg, np.clip(np.floor(xg * np.float32(K / float(Lf))).astype(np.int64), 0, K - 1))
+    m = 400_000
+    geo_o = oracle.CouetteParams(float(Lf), float(np.float32(dt)), 500.0, float(np.float32(rt)), float(np.float32(0.9)), K)
+    xo, vxo, vyo, vzo, co, nbo, mg = oracle.move_couette(x[:m], pop.vx[:m], pop.vy[:m], pop.vz[:m], geo_o, 3, 7)
+    sure = mg > 2e-6      # 80 000 cells: a cell is 1.25e-5 of the gap, FP32 resolves 6e-8 of it
+    assert sure.mean() > 0.6
+    assert np.array_equal(cg[:m][sure], co[sure])
+    assert np.abs(xg[:m][sure] - xo[sure]).max() <= 4e-7 * L
+    assert np.abs(vxd.cpu().numpy()[:m][sure] - vxo[sure]).max() <= 2e-5 * math.sqrt(rt)
+    # bin + gather + sample on the moved population
+    vxs, vys, vzs, perm, cs = ctx.bin(cell, vxd, vyd, vzd, K)
+    xs = ctx.gather_f32(perm, xd)
+    ctx.check()
+    perm_h, cs_h = perm.cpu().numpy(), cs.cpu().numpy()
+    assert np.array_equal(xs.cpu().numpy(), xg[perm_h])
+    assert np.array_equal(np.diff(cs_h), np.bincount(cg, minlength=K))
+    acc = torch.zeros((K, 8), dtype=torch.float64, device="cuda")
+    ctx.sample_cells(cs, vxs, vys, vzs, acc)
+    ctx.check()
+    v = [t.cpu().numpy().astype(np.float64) for t in (vxs, vys, vzs)]
+    N = np.diff(cs_h)
+    starts = cs_h[:-1][N > 0]            # reduceat over the non-empty cells: direct fp64 sums, no cancellation
+    want = np.zeros((K, 8))
+    for col, a in enumerate((np.ones(n), v[0], v[1], v[2], v[0] ** 2, v[1] ** 2, v[2] ** 2, v[0] * v[1])):
+        want[N > 0, col] = np.add.reduceat(a, starts)
+    got = acc.cpu().numpy()
+    assert np.array_equal(got[:, 0], want[:, 0])
+    scale = np.maximum(want[:, 4:7].sum(axis=1, keepdims=True), 1.0)
+    assert (np.abs(got - want) / scale).max() < 1e-12
+    # NTC counts on every cell
+    cap = (rng.random(K) * 2e-16 + 1e-16).astype(np.float32)
+    R_o, R_d = np.zeros(K), torch.zeros(K, dtype=torch.float64, device="cuda")
+    for t in range(2):
+        want_c = oracle.ntc_counts(cs_h, cap, 1.0e12, R_o)
+        got_c = ctx.ntc_counts(cs, dev(cap), 1.0e12, R_d)
+    assert np.array_equal(got_c.cpu().numpy(), want_c) and np.array_equal(R_d.cpu().numpy(), R_o)
+    ctx.close()
