@@ -39,10 +39,13 @@ enum { MI_NACT = 0, MI_NSEG = 1, MI_NPAIRS = 2, MI_SCAN = 8 /* .. +40 */ };
 
 // REPLACE_: pairs drawn with replacement (DSMC_F_PAIR_REPLACE) -- a compile-time variant so that the default
 // (matching) path carries none of its code.
-template <int LMAX_, int AMAX_, bool REPLACE_ = false>
+// PACK2N: the key sort uses 2 N buckets per cell, two 16-bit counters per int of cnt (shorter in-bucket ranking loops:
+// fused table step 0.476 -> 0.468 ms; the latency-bound groups of the tensor-core kernel lose 2 % to the extra
+// arithmetic, so only the table kernels switch it on)
+template <int LMAX_, int AMAX_, bool REPLACE_ = false, bool PACK2N_ = false>
 struct Chunk {
   static constexpr int LMAX = LMAX_, AMAX = AMAX_;
-  static constexpr bool REPLACE = REPLACE_;
+  static constexpr bool REPLACE = REPLACE_, PACK2N = PACK2N_;
   static constexpr int SMAX = (LMAX / kSeg + AMAX + 2 + 3) & ~3;  // multiple of 4: keeps every array 16-byte aligned
   float4 *v;        // [LMAX] velocities (x, y, z, unused)
   float4 *part;     // [SMAX] segment partial sums
@@ -91,7 +94,9 @@ using Team = TeamT<kThreads>;
 // L rounded up to 4.  Each thread owns eight consecutive elements per pass (two 16 B accesses),
 // scans it in registers, warp totals go through one shuffle scan.  `scratch` holds >= kWarps + 1 ints.
 // Ends with T.sync().
-template <class TM>
+// PACKED: every int holds two 16-bit counts (low half first); the scan runs over the 2 L halves and each half ends
+// as its own exclusive prefix (values stay below 65536).
+template <class TM, bool PACKED = false>
 __device__ __forceinline__ void block_excl_scan_coalesced(const TM &T, int *a, int L, int *scratch) {
   const int tid = T.tid, lane = tid & 31, warp = tid >> 5;
   int carry = 0;
@@ -112,9 +117,11 @@ __device__ __forceinline__ void block_excl_scan_coalesced(const TM &T, int *a, i
         if (i + u >= L) x[u] = 0;
     }
     int tot = 0;
+    int lo16[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {  // x[u] <- exclusive prefix inside the thread
-      const int t = x[u];
+      lo16[u] = PACKED ? (x[u] & 0xFFFF) : 0;
+      const int t = PACKED ? lo16[u] + (int)((uint32_t)x[u] >> 16) : x[u];
       x[u] = tot;
       tot += t;
     }
@@ -134,6 +141,10 @@ __device__ __forceinline__ void block_excl_scan_coalesced(const TM &T, int *a, i
       all += sw;
     }
     const int e0 = off + inc - tot;
+    if (PACKED) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) x[u] = ((e0 + x[u]) | ((e0 + x[u] + lo16[u]) << 16)) - e0;  // the stores below add e0 back
+    }
     if (i < L) {
       *reinterpret_cast<int4 *>(a + i) = make_int4(e0 + x[0], e0 + x[1], e0 + x[2], e0 + x[3]);
       if (i + 4 < L) *reinterpret_cast<int4 *>(a + i + 4) = make_int4(e0 + x[4], e0 + x[5], e0 + x[6], e0 + x[7]);
@@ -197,7 +208,7 @@ __device__ int chunk_begin(const TM &T, const StepParams &P, CK &S, int chunk, i
   // cell discovery (order of the active list is irrelevant to the results)
   for (int c = c_lo + tid; c < c_hi; c += TM::kN) {
     const int gs = __ldg(P.cell_start + c), N = __ldg(P.cell_start + c + 1) - gs;
-    if (N == 1) S.cnt[gs - q0] = 1;  // lone particle: keeps bucket positions aligned with slots
+    if (N == 1) S.cnt[gs - q0] = 1;  // lone particle (low half = its first bucket): keeps bucket positions aligned with slots
     if (N < 2) continue;
     const int a = atomicAdd(&S.misc[MI_NACT], 1);
     if (a >= CK::AMAX) continue;
@@ -288,7 +299,12 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
       for (int w = 0; w < 4; ++w) {
         if (p + w < N) {
           S.key[start + p + w] = k[w];
-          atomicAdd(&S.cnt[start + (int)__umulhi(k[w], (uint32_t)N)], 1);
+          if (CK::PACK2N) {
+            const int b2 = (int)__umulhi(k[w], 2u * (uint32_t)N);  // 2 N buckets per cell, two 16-bit counters per int
+            atomicAdd(&S.cnt[start + (b2 >> 1)], (b2 & 1) ? 0x10000 : 1);
+          } else {
+            atomicAdd(&S.cnt[start + (int)__umulhi(k[w], (uint32_t)N)], 1);
+          }
         }
       }
       const int s = p >> 1;
@@ -317,7 +333,7 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     T.sync();
     return;
   }
-  block_excl_scan_coalesced(T, S.cnt, n_loc, S.misc + MI_SCAN);
+  block_excl_scan_coalesced<TM, CK::PACK2N>(T, S.cnt, n_loc, S.misc + MI_SCAN);
   // placement, one warp per segment (cell constants in registers): cnt[bucket] ends as the bucket's end
   for (int sg = warp; sg < n_seg; sg += TM::kW) {
     const uint32_t e = S.segs[sg];
@@ -325,12 +341,18 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     const int start = ci.start, N = ci.N, piece = e >> 16;
     const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
     for (int q = lo + lane; q < hi; q += 32) {
-      const int bkt = start + (int)__umulhi(S.key[q], (uint32_t)N);
-      S.ord[atomicAdd(&S.cnt[bkt], 1)] = (uint16_t)q;
+      if (CK::PACK2N) {
+        const int b2 = (int)__umulhi(S.key[q], 2u * (uint32_t)N);
+        const uint32_t old = (uint32_t)atomicAdd(&S.cnt[start + (b2 >> 1)], (b2 & 1) ? 0x10000 : 1);
+        S.ord[(b2 & 1) ? (old >> 16) : (old & 0xFFFFu)] = (uint16_t)q;
+      } else {
+        const int bkt = start + (int)__umulhi(S.key[q], (uint32_t)N);
+        S.ord[atomicAdd(&S.cnt[bkt], 1)] = (uint16_t)q;
+      }
     }
   }
   T.sync();
-  // in-bucket ranking by (key, slot): buckets hold ~1 particle on average.  The first bucket of a cell
+  // in-bucket ranking by (key, slot): buckets hold ~1 particle on average (~0.5 with PACK2N).  The first bucket of a cell
   // begins at the cell's first slot, every other one where the previous bucket ends.
   for (int sg = warp; sg < n_seg; sg += TM::kW) {
     const uint32_t e = S.segs[sg];
@@ -339,8 +361,17 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
     for (int q = lo + lane; q < hi; q += 32) {
       const uint32_t k = S.key[q];
-      const int bkt = start + (int)__umulhi(k, (uint32_t)N);
-      const int b0 = bkt > start ? S.cnt[bkt - 1] : start, b1 = S.cnt[bkt];
+      int b0, b1;
+      if (CK::PACK2N) {
+        const int b2 = 2 * start + (int)__umulhi(k, 2u * (uint32_t)N);  // bucket index in 16-bit units
+        const uint16_t *c16 = reinterpret_cast<const uint16_t *>(S.cnt);
+        b0 = b2 > 2 * start ? c16[b2 - 1] : start;
+        b1 = c16[b2];
+      } else {
+        const int bkt = start + (int)__umulhi(k, (uint32_t)N);
+        b0 = bkt > start ? S.cnt[bkt - 1] : start;
+        b1 = S.cnt[bkt];
+      }
       int rank = 0;
       if (b1 - b0 > 1) {
 #pragma unroll 1

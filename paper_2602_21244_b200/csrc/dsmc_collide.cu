@@ -220,15 +220,15 @@ __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev 
 template <int LMAX, int AMAX, bool OP_TABLE, int TP, int SRC, int DST, int MINB, int NT = kThreads, bool REPL = false>
 __global__ void __launch_bounds__(NT, MINB) k_collide(const StepParams P, const MlpDev net) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Chunk<LMAX, AMAX, REPL> S;
+  Chunk<LMAX, AMAX, REPL, OP_TABLE> S;
   float *mlp = reinterpret_cast<float *>(S.carve(smem_raw));
   if (SRC == 0) {
-    process_chunk<NT, Chunk<LMAX, AMAX, REPL>, OP_TABLE, TP, DST>(P, net, S, mlp, blockIdx.x);
+    process_chunk<NT, Chunk<LMAX, AMAX, REPL, OP_TABLE>, OP_TABLE, TP, DST>(P, net, S, mlp, blockIdx.x);
   } else {
     const int32_t *list = SRC == 1 ? P.big : P.big2;
     const int n_list = *reinterpret_cast<volatile const int32_t *>(list);
     for (int i = blockIdx.x; i < n_list; i += gridDim.x) {
-      process_chunk<NT, Chunk<LMAX, AMAX, REPL>, OP_TABLE, TP, DST>(P, net, S, mlp, list[1 + i]);
+      process_chunk<NT, Chunk<LMAX, AMAX, REPL, OP_TABLE>, OP_TABLE, TP, DST>(P, net, S, mlp, list[1 + i]);
       __syncthreads();
     }
   }
