@@ -268,11 +268,15 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
       }
     }
     float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
-    for (int q = lo + lane; q < hi; q += 32) {
-      const float4 v = S.v[q];
-      const float dx = v.x - pv.x, dy = v.y - pv.y, dz = v.z - pv.z;
-      sx += dx; sy += dy; sz += dz;
-      s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
+#pragma unroll
+    for (int r = 0; r < kSeg / 32; ++r) {  // the segment's four rows: loads issued together
+      const int q = lo + lane + 32 * r;
+      if (q < hi) {
+        const float4 v = S.v[q];
+        const float dx = v.x - pv.x, dy = v.y - pv.y, dz = v.z - pv.z;
+        sx += dx; sy += dy; sz += dz;
+        s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
+      }
     }
     {
       const float t = warp_sum4_t(sx, sy, sz, s2, lane);
@@ -545,17 +549,21 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
       const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
       const float ux = ci.ux, uy = ci.uy, uz = ci.uz;
       float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
-      for (int q = lo + lane; q < hi; q += 32) {
-        float4 v = S.v[q];
-        if (replace) {  // with-replacement selection: apply the accumulated changes (this thread owns slot q)
-          v.x += reinterpret_cast<const float *>(S.key)[q];
-          v.y += reinterpret_cast<const float *>(S.cnt)[q];
-          v.z += reinterpret_cast<const float *>(S.ord)[q];
-          S.v[q] = v;
+#pragma unroll
+      for (int r = 0; r < kSeg / 32; ++r) {
+        const int q = lo + lane + 32 * r;
+        if (q < hi) {
+          float4 v = S.v[q];
+          if (replace) {  // with-replacement selection: apply the accumulated changes (this thread owns slot q)
+            v.x += reinterpret_cast<const float *>(S.key)[q];
+            v.y += reinterpret_cast<const float *>(S.cnt)[q];
+            v.z += reinterpret_cast<const float *>(S.ord)[q];
+            S.v[q] = v;
+          }
+          const float dx = v.x - ux, dy = v.y - uy, dz = v.z - uz;
+          sx += dx; sy += dy; sz += dz;
+          s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
         }
-        const float dx = v.x - ux, dy = v.y - uy, dz = v.z - uz;
-        sx += dx; sy += dy; sz += dz;
-        s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
       }
       const float t = warp_sum4_t(sx, sy, sz, s2, lane);
       if ((lane & 7) == 0) reinterpret_cast<float *>(&S.part[sg])[lane >> 3] = t;
@@ -601,11 +609,15 @@ __device__ void chunk_finish(const TM &T, const StepParams &P, CK &S, int n_loc,
       const float4 co = *reinterpret_cast<const float4 *>(&ci);
       const int piece = e >> 16;
       const int lo = ci.start + piece * kSeg, hi = min(lo + kSeg, (int)ci.start + (int)ci.N);
-      for (int q = lo + lane; q < hi; q += 32) {
-        const float4 v = S.v[q];
-        P.vx[q0 + q] = fmaf(co.w, v.x, v.x + co.x);
-        P.vy[q0 + q] = fmaf(co.w, v.y, v.y + co.y);
-        P.vz[q0 + q] = fmaf(co.w, v.z, v.z + co.z);
+#pragma unroll
+      for (int r = 0; r < kSeg / 32; ++r) {
+        const int q = lo + lane + 32 * r;
+        if (q < hi) {
+          const float4 v = S.v[q];
+          P.vx[q0 + q] = fmaf(co.w, v.x, v.x + co.x);
+          P.vy[q0 + q] = fmaf(co.w, v.y, v.y + co.y);
+          P.vz[q0 + q] = fmaf(co.w, v.z, v.z + co.z);
+        }
       }
     }
   } else {
