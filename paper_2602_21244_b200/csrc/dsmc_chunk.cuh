@@ -344,7 +344,10 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     const CellInfo &ci = S.cells[e & 0xFFFFu];
     const int start = ci.start, N = ci.N, piece = e >> 16;
     const int lo = start + piece * kSeg, hi = min(lo + kSeg, start + N);
-    for (int q = lo + lane; q < hi; q += 32) {
+#pragma unroll
+    for (int r = 0; r < kSeg / 32; ++r) {
+      const int q = lo + lane + 32 * r;
+      if (q >= hi) continue;
       if (CK::PACK2N) {
         const int b2 = (int)__umulhi(S.key[q], 2u * (uint32_t)N);
         const uint32_t old = (uint32_t)atomicAdd(&S.cnt[start + (b2 >> 1)], (b2 & 1) ? 0x10000 : 1);
