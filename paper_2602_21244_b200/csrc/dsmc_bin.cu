@@ -318,6 +318,9 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
   __syncthreads();
   mbar_wait(&bar[1], 0);
   const int kept = scratch[kBinWarps];
+  // two positions per trip: their (inv -> staged record) load chains overlap (four need more than the 64
+  // registers two CTAs per SM leave: measured no better than one)
+#pragma unroll 2
   for (int pos = tid; pos < kept; pos += kBinThreads) {
     const int j = inv[pos];
     const int cc = scell[j];
