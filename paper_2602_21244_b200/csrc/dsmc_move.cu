@@ -132,11 +132,11 @@ __global__ void __launch_bounds__(256) k_sample_cells(int32_t K, const int32_t *
       bn = __ldg(cs + kn + 1);
     }
     double s[7] = {0, 0, 0, 0, 0, 0, 0};
-    // four rows of 32 particles per trip: 12 loads in flight per lane (the kernel is latency-bound otherwise)
-    for (int p0 = a + lane; p0 < b; p0 += 128) {
-      float X[4], Y[4], Z[4];
+    // eight rows of 32 particles per trip: 24 loads in flight per lane (the kernel is latency-bound otherwise)
+    for (int p0 = a + lane; p0 < b; p0 += 256) {
+      float X[8], Y[8], Z[8];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < 8; ++u) {
         const int p = p0 + 32 * u;
         const bool in = p < b;
         X[u] = in ? __ldg(vx + p) : 0.f;
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256) k_sample_cells(int32_t K, const int32_t *
         Z[u] = in ? __ldg(vz + p) : 0.f;
       }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < 8; ++u) {
         const double x = X[u], y = Y[u], z = Z[u];
         s[0] += x; s[1] += y; s[2] += z;
         s[3] += x * x; s[4] += y * y; s[5] += z * z;
