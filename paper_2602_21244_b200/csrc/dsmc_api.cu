@@ -88,6 +88,11 @@ int dsmc_destroy(dsmc_ctx *c) {
   cudaFree(c->h_rem);
   cudaFree(c->h_cap[0]);
   cudaFree(c->h_cap[1]);
+  if (c->side_stream) {
+    cudaStreamDestroy(c->side_stream);
+    cudaEventDestroy(c->ev_bin);
+    cudaEventDestroy(c->ev_side);
+  }
   delete c;
   return DSMC_OK;
 }
@@ -431,6 +436,22 @@ int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, con
   rc = dsmc_bin(c, n, K, c->h_cell, c->h_v[0], c->h_v[1], c->h_v[2], c->h_vs[0], c->h_vs[1], c->h_vs[2], c->h_perm,
                 c->h_cell_start);
   if (rc != DSMC_OK) return rc;
+  // perm and cell_start are final once the bin is done: they travel back on a side stream under the collide kernels
+  const bool side = perm_h || cell_start_h;
+  if (side) {
+    if (!c->side_stream) {
+      CK(cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking));
+      CK(cudaEventCreateWithFlags(&c->ev_bin, cudaEventDisableTiming));
+      CK(cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming));
+    }
+    CK(cudaEventRecord(c->ev_bin, s));
+    CK(cudaStreamWaitEvent(c->side_stream, c->ev_bin, 0));
+    if (perm_h)
+      CK(cudaMemcpyAsync(perm_h, c->h_perm, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost, c->side_stream));
+    if (cell_start_h)
+      CK(cudaMemcpyAsync(cell_start_h, c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1), cudaMemcpyDeviceToHost,
+                         c->side_stream));
+  }
   if (vhs)
     rc = dsmc_collide_vhs_nn(c, n, K, c->h_cell_start, c->h_vs[0], c->h_vs[1], c->h_vs[2], nullptr, vhs, seed, step,
                              nullptr);
@@ -439,9 +460,10 @@ int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, con
                                step, nullptr);
   if (rc != DSMC_OK) return rc;
   for (int a = 0; a < 3; ++a) CK(cudaMemcpyAsync(dst[a], c->h_vs[a], sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, s));
-  if (perm_h) CK(cudaMemcpyAsync(perm_h, c->h_perm, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToHost, s));
-  if (cell_start_h)
-    CK(cudaMemcpyAsync(cell_start_h, c->h_cell_start, sizeof(int32_t) * (size_t)(K + 1), cudaMemcpyDeviceToHost, s));
+  if (side) {  // join the side stream before the final synchronisation
+    CK(cudaEventRecord(c->ev_side, c->side_stream));
+    CK(cudaStreamWaitEvent(s, c->ev_side, 0));
+  }
   return dsmc_sync_status(c);
 }
 

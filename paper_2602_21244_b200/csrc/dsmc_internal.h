@@ -82,6 +82,8 @@ struct StepParams {
 struct dsmc_ctx {
   int device;
   cudaStream_t stream;
+  cudaStream_t side_stream;  // dsmc_step_host: perm / cell_start go back to the host while the collide kernels run
+  cudaEvent_t ev_bin, ev_side;
   int64_t max_particles;
   int32_t max_cells;
   int32_t *d_status;

@@ -745,3 +745,28 @@ def test_relaxation_to_isotropy_with_the_ab_initio_operator(dsmc):
     kurt = float(((x - x.mean()) ** 4).mean() / x.var() ** 2)
     assert abs(kurt - 3.0) < 0.05
     ctx.close()
+
+
+def test_step_host_equals_the_device_path(dsmc):
+    """dsmc_step_host (the end-to-end entry point bench.py times: pinned host buffers in, host buffers out, perm and
+    cell_start returned on a side stream under the collide kernels) must give, bit for bit, what dsmc_bin +
+    dsmc_collide_abinitio give on device buffers; twice in a row (buffer reuse)."""
+    pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    tab = _lj_table()
+    ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    prm = dsmc.AbinitioParams(chi_mode=0, flags=dsmc.F_MOMENT_MATCH)
+    hcell = torch.from_numpy(pop.cell).pin_memory()
+    hv = [torch.from_numpy(a).pin_memory() for a in (pop.vx, pop.vy, pop.vz)]
+    hout = [torch.empty(pop.n, dtype=torch.float32).pin_memory() for _ in range(3)] + \
+           [torch.empty(pop.n, dtype=torch.int32).pin_memory(), torch.empty(pop.n_cells + 1, dtype=torch.int32).pin_memory()]
+    for step in (3, 4):
+        for t in hout:
+            t.fill_(-7)
+        ctx.step_host(hcell, *hv, pop.n_cells, hout, abi=prm, seed=9, step=step)
+        vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+        ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=9, step=step)
+        ctx.check()
+        for got, want in zip(hout, (vx_s, vy_s, vz_s, perm, cs)):
+            assert torch.equal(got, want.cpu())
+    ctx.close()
