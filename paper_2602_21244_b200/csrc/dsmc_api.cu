@@ -54,6 +54,9 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
   CK(cudaMalloc(&c->d_chunk_meta, sizeof(int4) * n_chunks));
   CK(cudaMalloc(&c->d_big2, sizeof(int32_t) * (n_chunks + 1)));
   CK(cudaMalloc(&c->d_work, sizeof(int32_t) * 4));
+  CK(cudaMalloc(&c->d_cell_list, sizeof(int4) * 3 * (size_t)(max_cells > 0 ? max_cells : 1)));
+  CK(cudaMalloc(&c->d_list_ctr, sizeof(int32_t) * 16));
+  CK(cudaMemset(c->d_list_ctr, 0, sizeof(int32_t) * 16));
   *out = c;
   return DSMC_OK;
 }
@@ -73,6 +76,8 @@ int dsmc_destroy(dsmc_ctx *c) {
   cudaFree(c->d_chunk_meta);
   cudaFree(c->d_big2);
   cudaFree(c->d_work);
+  cudaFree(c->d_cell_list);
+  cudaFree(c->d_list_ctr);
   for (int s = 0; s < 2; ++s) {
     cudaFree(c->d_weights[s]);
     cudaFree(c->d_tc_blob[s]);

@@ -1,0 +1,134 @@
+// Fused collision step, chi-table operator, "cell team" form (the north_star kernel).
+//
+// One TEAM owns one cell from its first HBM read to its last HBM write: a warp for cells of up to 256 particles,
+// the 128 threads of a CTA for up to 1024, a 256-thread CTA for up to DSMC_MAX_CELL_PARTICLES = 2048.  A thread
+// holds at most 8 particles and 8 pairing keys in registers, so every phase is a short, fully unrolled loop whose
+// trip count is uniform over the team, and the warp teams synchronise with __syncwarp only (no CTA barrier on the
+// path of a small cell).
+//
+//   load      12 B / particle, coalesced, straight into registers; the pre-collision sums (eq. 10) are
+//             taken from those registers about a pivot (mean of the cell's first 32 particles), then the
+//             velocities go to shared memory (SoA)
+//   keys      one Philox block per 4 slots (stream 0, DESIGN "RNG addressing"); bucket = top L bits of the key,
+//             L = ceil(log2 N) (+1 with XB); one shared-memory atomic per key returns its arrival index
+//   scan      exclusive prefix of the bucket counts; every counter becomes (bucket start | members << 16)
+//   place     a key alone in its bucket has its final rank (56-61 % of them); the others write their
+//             COMPOSITE (key << L | slot: the order of (key, slot) inside a bucket, in 32 bits) at bucket start
+//             + arrival index
+//   rank      ... and count the smaller composites of their bucket: pi = the unique ascending order of
+//             (key << 32 | slot) (Q7); pairs are (pi[2s], pi[2s+1])
+//   pairs     two pair slots per thread (they share one Philox block of stream 1): gather, table lookup
+//             (one 16 B load from the L2-resident quad table), rotation by (chi, eps) (Q16),
+//             centre-of-mass update (eqs. 6-8) written back to shared memory
+//   finish    post-collision sums from shared memory into registers, matching coefficients (eqs. 10-11, P:L46,
+//             Q5) in FP64, v <- v + (alpha - 1) v + B applied to the registers, 12 B / particle stored
+//
+// Work distribution: k_cell_lists sorts the cells that have pairs to collide into three lists by size; the
+// CTAs of k_cells are persistent and draw list entries from a counter (the next entry is fetched while the
+// current cell is processed).  Results depend only on (seed, step, cell, slot).
+#include <algorithm>
+
+#include "dsmc_cells.cuh"
+
+namespace dsmc {
+
+// ---------------------------------------------------------------------------------------------
+// cell lists: (cell, first slot, N, M) of every cell with M > 0, by size class
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_cell_lists(int32_t K, const int32_t *__restrict__ cs,
+                                                    const int32_t *__restrict__ pairs_count, int32_t pairs_per_cell,
+                                                    int4 *__restrict__ list0, int4 *__restrict__ list1,
+                                                    int4 *__restrict__ list2, int32_t *__restrict__ ctr,
+                                                    int32_t *__restrict__ ctr_other, int32_t *__restrict__ status) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < 8) ctr_other[c] = 0;  // the counters of the next step (this step's were zeroed by the previous one)
+  int cls = -1;
+  int4 item = make_int4(0, 0, 0, 0);
+  if (c < K) {
+    const int gs = __ldg(cs + c), N = __ldg(cs + c + 1) - gs;
+    int M = N >> 1;
+    const int req = pairs_count ? __ldg(pairs_count + c) : pairs_per_cell;
+    if (req >= 0 && req < M) M = req;
+    if (N > kMaxCell) {
+      *status = DSMC_ERR_CELL_TOO_LARGE;
+    } else if (N >= 2 && M > 0) {
+      cls = N <= 256 ? 0 : (N <= 1024 ? 1 : 2);
+      item = make_int4(c, gs, N, M);
+    }
+  }
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const unsigned m = __ballot_sync(0xffffffffu, cls == k);
+    if (m == 0) continue;
+    int base = 0;
+    if (lane == __ffs(m) - 1) base = atomicAdd(ctr + k, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+    if (cls == k) {
+      int4 *list = k == 0 ? list0 : (k == 1 ? list1 : list2);
+      list[base + __popc(m & ((1u << lane) - 1u))] = item;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernels
+// ---------------------------------------------------------------------------------------------
+// main kernel: 128-thread CTAs.  First the cells of 257..1024 particles, one per CTA at a time; then the cells of
+// up to 256 particles, one per warp at a time.  Both forms use the same shared-memory footprint.
+template <int XB>
+__global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const CellLists Lst) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  {
+    CellTeam<128, XB> T;
+    T.init(smem_raw, threadIdx.x, 0);
+    T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
+  }
+  __syncthreads();
+  {
+    CellTeam<32, XB> T;
+    T.init(smem_raw + (threadIdx.x >> 5) * CellTeam<32, XB>::bytes(), threadIdx.x & 31, 0);
+    T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
+  }
+}
+
+// cells of 1025..2048 particles: one 256-thread CTA per cell at a time
+template <int XB>
+__global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const CellLists Lst) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  CellTeam<256, XB> T;
+  T.init(smem_raw, threadIdx.x, 0);
+  T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
+}
+
+int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
+  constexpr int XB = kCellsXB;
+  CellLists L;
+  const size_t K = (size_t)c->max_cells;
+  for (int k = 0; k < 3; ++k) L.list[k] = c->d_cell_list + k * K;
+  const int e = (int)(c->list_epoch & 1);
+  c->list_epoch += 1;
+  L.ctr = c->d_list_ctr + 8 * e;
+  k_cell_lists<<<(p.n_cells + 255) / 256, 256, 0, c->stream>>>(p.n_cells, p.cell_start, p.pairs_count,
+                                                                p.pairs_per_cell, L.list[0], L.list[1], L.list[2],
+                                                                L.ctr, c->d_list_ctr + 8 * (1 - e), p.status);
+  {
+    auto kern = k_cells<XB>;
+    const size_t smem = CellTeam<128, XB>::bytes();
+    static_assert(CellTeam<128, XB>::bytes() == 4 * CellTeam<32, XB>::bytes(), "the two team forms share one footprint");
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      return DSMC_ERR_CUDA;
+    kern<<<c->num_sms * 8, 128, smem, c->stream>>>(p, L);
+  }
+  {
+    auto kern = k_cells_big<XB>;
+    const size_t smem = CellTeam<256, XB>::bytes();
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      return DSMC_ERR_CUDA;
+    kern<<<c->num_sms * 2, 256, smem, c->stream>>>(p, L);
+  }
+  c->launches += 3;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+}  // namespace dsmc

@@ -261,6 +261,7 @@ int launch_chunk_map(dsmc_ctx *c, StepParams &p) {
 }
 
 int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {
+  if (p_in.op == 1 && !(p_in.flags & DSMC_F_PAIR_REPLACE)) return launch_collide_cells(c, p_in);  // dsmc_cells.cu
   StepParams p = p_in;
   int rc = launch_chunk_map(c, p);
   if (rc != DSMC_OK) return rc;

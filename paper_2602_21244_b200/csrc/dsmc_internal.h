@@ -99,6 +99,9 @@ struct dsmc_ctx {
   int32_t *d_big;          // [max_particles / kChunk + 2]
   int32_t *d_big2;         // [max_particles / kChunk + 2]
   int32_t *d_work;         // [4] work counters of the persistent kernels ([0] main pass, [1] deferred pass)
+  int4 *d_cell_list;       // [3][max_cells] cell lists of the cell-team kernels (dsmc_cells.cu)
+  int32_t *d_list_ctr;     // [2][8] list lengths and work counters, alternating between steps
+  int64_t list_epoch;
   int64_t launches;
   int num_sms;
   // operators
@@ -133,6 +136,7 @@ int launch_moment_match(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
                         const double *target, uint32_t flags);
 int launch_chunk_map(dsmc_ctx *c, StepParams &p);
 int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
+int launch_collide_cells(dsmc_ctx *c, const StepParams &p);  // cell-team form, chi-table operator (dsmc_cells.cu)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_collide_pipe(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // warp-specialised, op 2
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
