@@ -260,6 +260,10 @@ static void fill_common(StepParams &p, dsmc_ctx *c, int64_t n, int32_t K, const 
   p.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu);
   p.seed_hi = (uint32_t)(seed >> 32);
   p.step = step;
+  for (uint32_t r = 0; r < 10; ++r) {
+    p.rk[2 * r] = p.seed_lo + r * 0x9E3779B9u;
+    p.rk[2 * r + 1] = p.seed_hi + r * 0xBB67AE85u;
+  }
   if (dump) p.dump = *dump;
   p.dump_any = (dump && (dump->pair_i || dump->pair_j || dump->accepted || dump->gprime || dump->aux)) ? 1 : 0;
   p.status = c->d_status;

@@ -10,7 +10,7 @@
 //             taken from those registers about a pivot (mean of the cell's first 32 particles), then the
 //             velocities go to shared memory (SoA)
 //   keys      one Philox block per 4 slots (stream 0, DESIGN "RNG addressing"); bucket = top L bits of the key,
-//             L = ceil(log2 N) (+1 with XB); one shared-memory atomic per key returns its arrival index
+//             L = ceil(log2 N); one shared-memory atomic per key returns its arrival index
 //   scan      exclusive prefix of the bucket counts; every counter becomes (bucket start | members << 16)
 //   place     a key alone in its bucket has its final rank (56-61 % of them); the others write their
 //             COMPOSITE (key << L | slot: the order of (key, slot) inside a bucket, in 32 bits) at bucket start
@@ -76,33 +76,30 @@ __global__ void __launch_bounds__(256) k_cell_lists(int32_t K, const int32_t *__
 // ---------------------------------------------------------------------------------------------
 // main kernel: 128-thread CTAs.  First the cells of 257..1024 particles, one per CTA at a time; then the cells of
 // up to 256 particles, one per warp at a time.  Both forms use the same shared-memory footprint.
-template <int XB>
 __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   {
-    CellTeam<128, XB> T;
+    CellTeam<128> T;
     T.init(smem_raw, threadIdx.x, 0);
     T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
   }
   __syncthreads();
   {
-    CellTeam<32, XB> T;
-    T.init(smem_raw + (threadIdx.x >> 5) * CellTeam<32, XB>::bytes(), threadIdx.x & 31, 0);
+    CellTeam<32> T;
+    T.init(smem_raw + (threadIdx.x >> 5) * CellTeam<32>::bytes(), threadIdx.x & 31, 0);
     T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
   }
 }
 
 // cells of 1025..2048 particles: one 256-thread CTA per cell at a time
-template <int XB>
 __global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  CellTeam<256, XB> T;
+  CellTeam<256> T;
   T.init(smem_raw, threadIdx.x, 0);
   T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
 }
 
 int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
-  constexpr int XB = kCellsXB;
   CellLists L;
   const size_t K = (size_t)c->max_cells;
   for (int k = 0; k < 3; ++k) L.list[k] = c->d_cell_list + k * K;
@@ -113,16 +110,16 @@ int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
                                                                 p.pairs_per_cell, L.list[0], L.list[1], L.list[2],
                                                                 L.ctr, c->d_list_ctr + 8 * (1 - e), p.status);
   {
-    auto kern = k_cells<XB>;
-    const size_t smem = CellTeam<128, XB>::bytes();
-    static_assert(CellTeam<128, XB>::bytes() == 4 * CellTeam<32, XB>::bytes(), "the two team forms share one footprint");
+    auto kern = k_cells;
+    const size_t smem = CellTeam<128>::bytes();
+    static_assert(CellTeam<128>::bytes() == 4 * CellTeam<32>::bytes(), "the two team forms share one footprint");
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return DSMC_ERR_CUDA;
     kern<<<c->num_sms * 8, 128, smem, c->stream>>>(p, L);
   }
   {
-    auto kern = k_cells_big<XB>;
-    const size_t smem = CellTeam<256, XB>::bytes();
+    auto kern = k_cells_big;
+    const size_t smem = CellTeam<256>::bytes();
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return DSMC_ERR_CUDA;
     kern<<<c->num_sms * 2, 256, smem, c->stream>>>(p, L);

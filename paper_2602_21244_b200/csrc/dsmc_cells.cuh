@@ -6,7 +6,6 @@
 
 namespace dsmc {
 
-constexpr int kCellsXB = 0;   // 1: twice as many key buckets (2^(L+1)): fewer shared buckets, longer scan
 constexpr int kRankWin = 4;   // bucket members compared without a loop
 
 struct CellLists {
@@ -73,20 +72,95 @@ __device__ __forceinline__ void cells_rotate(float gx, float gy, float gz, float
   pz = fmaf(gz, cc, -sci * (g * gy * ce + gx * gz * se));
 }
 
-template <int NT, int XB>
+// Philox4x32-10 with the round keys as constant-bank operands (StepParams::rk): per round two 32 x 32 -> 64 bit
+// products and two three-input xors.
+__device__ __forceinline__ uint4 cells_philox(const StepParams &P, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ P.rk[2 * r];
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ P.rk[2 * r + 1];
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
+// In-bucket rank of composite e: the number of smaller composites among the first min(m, 4) members of its bucket
+// (shared address addr), added to rank.  Straight-line predicated code: one predicate per member position, one
+// predicated load, one compare, one predicated add each.
+__device__ __forceinline__ void cells_rank4(uint32_t &rank, uint32_t addr, uint32_t e, uint32_t m) {
+  asm volatile(
+      "{\n\t.reg .pred q1, q2, q3, p;\n\t.reg .u32 v0, v1, v2, v3;\n\t"
+      "setp.gt.u32 q1, %3, 1;\n\t"
+      "setp.gt.u32 q2, %3, 2;\n\t"
+      "setp.gt.u32 q3, %3, 3;\n\t"
+      "mov.u32 v0, %2;\n\t"  // a member that is not there compares as e itself: not smaller
+      "mov.u32 v1, %2;\n\t"
+      "mov.u32 v2, %2;\n\t"
+      "mov.u32 v3, %2;\n\t"
+      "@q1 ld.shared.u32 v0, [%1];\n\t"
+      "@q1 ld.shared.u32 v1, [%1+4];\n\t"
+      "@q2 ld.shared.u32 v2, [%1+8];\n\t"
+      "@q3 ld.shared.u32 v3, [%1+12];\n\t"
+      "setp.lt.u32 p, v0, %2;\n\t"
+      "@p add.u32 %0, %0, 1;\n\t"
+      "setp.lt.u32 p, v1, %2;\n\t"
+      "@p add.u32 %0, %0, 1;\n\t"
+      "setp.lt.u32 p, v2, %2;\n\t"
+      "@p add.u32 %0, %0, 1;\n\t"
+      "setp.lt.u32 p, v3, %2;\n\t"
+      "@p add.u32 %0, %0, 1;\n\t}"
+      : "+r"(rank)
+      : "r"(addr), "r"(e), "r"(m)
+      : "memory");
+}
+
+// Placement of one key (straight-line predicated code).  bo = bucket | arrival index << 16; the bucket's counter
+// holds (start | members << 16).  A key alone in its bucket is ranked: pi[start] = its byte offset.  Otherwise its
+// composite goes to K2[start + arrival index] and the counter word is returned for the ranking (0 = nothing to rank).
+__device__ __forceinline__ uint32_t cells_place(uint32_t bo, int p, int N, uint32_t comp, uint32_t cnt_s, uint32_t k2_s,
+                                                uint32_t pi_s) {
+  uint32_t out;
+  asm volatile(
+      "{\n\t.reg .pred qv, q1, qm;\n\t.reg .u32 w, b0, m, a, t;\n\t.reg .u16 h;\n\t"
+      "setp.lt.s32 qv, %2, %3;\n\t"
+      "and.b32 a, %1, 0xffff;\n\t"
+      "mad.lo.u32 a, a, 4, %5;\n\t"
+      "mov.u32 w, 0;\n\t"
+      "@qv ld.shared.u32 w, [a];\n\t"
+      "shr.u32 m, w, 16;\n\t"
+      "and.b32 b0, w, 0xffff;\n\t"
+      "setp.eq.u32 q1, m, 1;\n\t"
+      "setp.gt.u32 qm, m, 1;\n\t"
+      "mad.lo.u32 t, b0, 2, %7;\n\t"
+      "shl.b32 a, %2, 2;\n\t"
+      "cvt.u16.u32 h, a;\n\t"
+      "@q1 st.shared.u16 [t], h;\n\t"
+      "shr.u32 t, %1, 16;\n\t"
+      "add.u32 t, t, b0;\n\t"
+      "mad.lo.u32 t, t, 4, %6;\n\t"
+      "@qm st.shared.u32 [t], %4;\n\t"
+      "selp.u32 %0, w, 0, qm;\n\t}"
+      : "=r"(out)
+      : "r"(bo), "r"(p), "r"(N), "r"(comp), "r"(cnt_s), "r"(k2_s), "r"(pi_s)
+      : "memory");
+  return out;
+}
+
+template <int NT>
 struct CellTeam {
-  static constexpr int C = 8 * NT;     // slots: a thread holds 8 particles / 8 keys
-  static constexpr int CPT = 8 << XB;  // bucket counters per thread
+  static constexpr int C = 8 * NT;  // slots: a thread holds 8 particles / 8 keys / 8 bucket counters
   static constexpr int NW = NT / 32;
   float *X, *Y, *Z;   // [C] velocities of the cell
-  uint32_t *cnt;      // [C << XB] bucket counters, then (bucket start | members << 16)
+  uint32_t *cnt;      // [C] bucket counters, then (bucket start | members << 16)
   uint32_t *K2;       // [C] composites of the keys that share a bucket, in bucket order
-  uint16_t *pi;       // [C] slots in ascending (key, slot) order
+  uint16_t *pi;       // [C] BYTE OFFSETS (4 slot) of the particles in ascending (key, slot) order
   float4 *part;       // [2][8] per-warp partial sums, before / after the collisions (NT > 32)
   int *misc;          // [0..7] warp totals of the scan, [8..11] next list entry, [12] any pair accepted
   int tid, bar;
 
-  static constexpr size_t bytes() { return (size_t)C * (12 + (4 << XB) + 4 + 2) + 3 * NT; }  // + part, misc (320 B, NT > 32)
+  static constexpr size_t bytes() { return (size_t)C * (12 + 4 + 4 + 2) + 3 * NT; }  // + part, misc (320 B, NT > 32)
 
   __device__ __forceinline__ void init(unsigned char *base, int tid_, int bar_) {
     tid = tid_;
@@ -95,7 +169,7 @@ struct CellTeam {
     Y = X + C;
     Z = Y + C;
     cnt = reinterpret_cast<uint32_t *>(Z + C);
-    K2 = cnt + (C << XB);
+    K2 = cnt + C;
     pi = reinterpret_cast<uint16_t *>(K2 + C);
     part = reinterpret_cast<float4 *>(pi + C);
     misc = reinterpret_cast<int *>(part + 16);
@@ -135,24 +209,46 @@ struct CellTeam {
     while (item.z > 0) item = cell(P, item, list, n_items, work);
   }
 
+  // team sums of (a, b, c, d): per-warp butterfly, then (NT > 32) the warps' partials through shared memory in a
+  // fixed order.  `slot` selects the partial-sum buffer; contains one team barrier when NT > 32.
+  __device__ __forceinline__ void team_sum4(float &a, float &b, float &c, float &d, int slot) const {
+    const int lane = tid & 31, warp = tid >> 5;
+    const float t = warp_sum4(a, b, c, d, lane);
+    if (NT == 32) {
+      a = __shfl_sync(0xffffffffu, t, 0);
+      b = __shfl_sync(0xffffffffu, t, 8);
+      c = __shfl_sync(0xffffffffu, t, 16);
+      d = __shfl_sync(0xffffffffu, t, 24);
+    } else {
+      if ((lane & 7) == 0) reinterpret_cast<float *>(&part[8 * slot + warp])[lane >> 3] = t;
+      sync();
+      a = b = c = d = 0.f;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) {
+        const float4 p = part[8 * slot + w];
+        a += p.x; b += p.y; c += p.z; d += p.w;
+      }
+    }
+  }
+
   // one cell; returns the team's next list entry
   __device__ __forceinline__ int4 cell(const StepParams &P, const int4 item, const int4 *__restrict__ list, int n_items,
                                        int32_t *work) {
     const int lane = tid & 31, warp = tid >> 5;
     const int gs = item.y, N = item.z, M = item.w;
     const uint32_t cell_ctr = (uint32_t)item.x + P.cell_base;
-    const int Lb = 32 - __clz(N - 1) + XB;  // bucket = top Lb bits of the key; 2^(Lb - XB) >= N
+    const int Lb = 32 - __clz(N - 1);  // bucket = top Lb bits of the key; 2^Lb >= N buckets
     const int NB = 1 << Lb;
     const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
+    const float fN = (float)N, invN = 1.0f / fN;
     int next_idx = 0;
     if (tid == 0) {
       next_idx = atomicAdd(work, 1);  // consumed after the loads below have landed
       if (NT > 32) misc[12] = 0;
     }
-    if (CPT * tid < NB) {
-#pragma unroll
-      for (int u = 0; u < CPT / 4; ++u) *reinterpret_cast<uint4 *>(cnt + CPT * tid + 4 * u) = make_uint4(0u, 0u, 0u, 0u);
-    }
+    // bucket counters: thread t owns [4 t, 4 t + 4) and [4 NT + 4 t, 4 NT + 4 t + 4): conflict-free 16-byte accesses
+    if (4 * tid < NB) *reinterpret_cast<uint4 *>(cnt + 4 * tid) = make_uint4(0u, 0u, 0u, 0u);
+    if (4 * (tid + NT) < NB) *reinterpret_cast<uint4 *>(cnt + 4 * (tid + NT)) = make_uint4(0u, 0u, 0u, 0u);
     // ---- load (12 B / particle) + pre-collision sums about the pivot (eq. 10) ----
     float ux, uy, uz, theta;
     {
@@ -198,54 +294,35 @@ struct CellTeam {
           Z[q] = z[r];
         }
       }
-      const float t = warp_sum4(sx, sy, sz, s2, lane);
-      double dsx, dsy, dsz, ds2;
-      if (NT == 32) {
-        dsx = __shfl_sync(0xffffffffu, t, 0);
-        dsy = __shfl_sync(0xffffffffu, t, 8);
-        dsz = __shfl_sync(0xffffffffu, t, 16);
-        ds2 = __shfl_sync(0xffffffffu, t, 24);
-        sync();  // counters zeroed before the first atomic
-      } else {
-        if ((lane & 7) == 0) reinterpret_cast<float *>(&part[warp])[lane >> 3] = t;
-        sync();
-        dsx = dsy = dsz = ds2 = 0.0;
-#pragma unroll
-        for (int w = 0; w < NW; ++w) {
-          const float4 p = part[w];
-          dsx += p.x; dsy += p.y; dsz += p.z; ds2 += p.w;
-        }
-      }
-      const double inv = 1.0 / N;
-      const double dx = dsx * inv, dy = dsy * inv, dz = dsz * inv;
-      ux = (float)((double)pvx + dx);  // pivot + mean(d)
-      uy = (float)((double)pvy + dy);
-      uz = (float)((double)pvz + dz);
-      theta = (float)fmax(ds2 - N * (dx * dx + dy * dy + dz * dz), 0.0);
+      team_sum4(sx, sy, sz, s2, 0);
+      if (NT == 32) sync();  // counters zeroed before the first atomic (NT > 32: the barrier inside team_sum4)
+      // u = pivot + mean(d); Theta = sum d^2 - N |mean d|^2: the pivot lies within a fraction of a thermal speed of
+      // the mean, so the subtraction loses no digits
+      const float mx = sx * invN, my = sy * invN, mz = sz * invN;
+      ux = pvx + mx;
+      uy = pvy + my;
+      uz = pvz + mz;
+      theta = fmaxf(s2 - fN * fmaf(mx, mx, fmaf(my, my, mz * mz)), 0.f);
     }
     int4 next = make_int4(0, 0, 0, 0);
     if (tid == 0) next = entry(list, n_items, next_idx);
     // ---- pairing keys (stream 0: block blk serves slots 4 blk .. 4 blk + 3) and bucket counts ----
+    // per key: comp = key << Lb | slot (the (key, slot) order inside a bucket), bo = bucket | arrival index << 16
     uint32_t comp[8], bo[8];
     {
       const int sh = 32 - Lb;
 #pragma unroll
       for (int r2 = 0; r2 < 2; ++r2) {
         const int blk = tid + NT * r2;
-#pragma unroll
-        for (int w = 0; w < 4; ++w) bo[4 * r2 + w] = 0xFFFFFFFFu;
         if (4 * blk < N) {
-          const uint4 r = philox4x32_10((uint32_t)blk, cell_ctr, P.step, 0u, P.seed_lo, P.seed_hi);
+          const uint4 r = cells_philox(P, (uint32_t)blk, cell_ctr, P.step, 0u);
           const uint32_t k[4] = {r.x, r.y, r.z, r.w};
 #pragma unroll
           for (int w = 0; w < 4; ++w) {
             const int p = 4 * blk + w;
-            if (p < N) {
-              const uint32_t b = k[w] >> sh;
-              const uint32_t old = atomicAdd(&cnt[b], 1u);
-              comp[4 * r2 + w] = (k[w] << Lb) | (uint32_t)p;
-              bo[4 * r2 + w] = b | (old << 16);
-            }
+            comp[4 * r2 + w] = (k[w] << Lb) | (uint32_t)p;
+            bo[4 * r2 + w] = k[w] >> sh;
+            if (p < N) bo[4 * r2 + w] |= atomicAdd(&cnt[k[w] >> sh], 1u) << 16;
           }
         }
       }
@@ -253,73 +330,66 @@ struct CellTeam {
     sync();
     // ---- exclusive scan of the bucket counts: counter -> (start | members << 16) ----
     {
-      uint32_t c[CPT];
-      const bool act = CPT * tid < NB;
-#pragma unroll
-      for (int u = 0; u < CPT / 4; ++u) {
-        uint4 v = make_uint4(0u, 0u, 0u, 0u);
-        if (act) v = *reinterpret_cast<const uint4 *>(cnt + CPT * tid + 4 * u);
-        c[4 * u] = v.x; c[4 * u + 1] = v.y; c[4 * u + 2] = v.z; c[4 * u + 3] = v.w;
-      }
-      uint32_t tot = 0;
-#pragma unroll
-      for (int j = 0; j < CPT; ++j) {
-        const uint32_t t = c[j];
-        c[j] = tot | (t << 16);
-        tot += t;
-      }
-      uint32_t inc = tot;
+      uint4 v[2];
+      v[0] = v[1] = make_uint4(0u, 0u, 0u, 0u);
+      if (4 * tid < NB) v[0] = *reinterpret_cast<const uint4 *>(cnt + 4 * tid);
+      if (4 * (tid + NT) < NB) v[1] = *reinterpret_cast<const uint4 *>(cnt + 4 * (tid + NT));
+      // both blocks of a thread in one packed warp scan (two 16-bit running sums per word)
+      const uint32_t pk = (v[0].x + v[0].y + v[0].z + v[0].w) | ((v[1].x + v[1].y + v[1].z + v[1].w) << 16);
+      uint32_t inc = pk;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += t;
       }
-      uint32_t base = inc - tot;
-      if (NT > 32) {
+      uint32_t exc = inc - pk, all;
+      if (NT == 32) {
+        all = __shfl_sync(0xffffffffu, inc, 31);
+      } else {
         if (lane == 31) misc[warp] = (int)inc;
         sync();
+        all = 0;
 #pragma unroll
-        for (int w = 0; w < NW; ++w) base += (w < warp) ? (uint32_t)misc[w] : 0u;
+        for (int w = 0; w < NW; ++w) {
+          const uint32_t t = (uint32_t)misc[w];
+          exc += (w < warp) ? t : 0u;
+          all += t;
+        }
       }
-      if (act) {
+      // block 0 of every thread precedes block 1 of thread 0
+      const uint32_t base[2] = {exc & 0xFFFFu, (exc >> 16) + (all & 0xFFFFu)};
 #pragma unroll
-        for (int u = 0; u < CPT / 4; ++u)
-          *reinterpret_cast<uint4 *>(cnt + CPT * tid + 4 * u) =
-              make_uint4(c[4 * u] + base, c[4 * u + 1] + base, c[4 * u + 2] + base, c[4 * u + 3] + base);
+      for (int u = 0; u < 2; ++u) {
+        uint4 o;
+        o.x = base[u] | (v[u].x << 16);
+        o.y = (base[u] + v[u].x) | (v[u].y << 16);
+        o.z = (base[u] + v[u].x + v[u].y) | (v[u].z << 16);
+        o.w = (base[u] + v[u].x + v[u].y + v[u].z) | (v[u].w << 16);
+        if (4 * (tid + NT * u) < NB) *reinterpret_cast<uint4 *>(cnt + 4 * (tid + NT * u)) = o;
       }
     }
     sync();
     // ---- placement: a key alone in its bucket is ranked; the others line up in their bucket ----
+    // afterwards bo = (bucket start | members << 16) for the keys that still have to be ranked, 0 otherwise
     const uint32_t slot_mask = (uint32_t)NB - 1u;
+    const uint32_t cnt_s = (uint32_t)__cvta_generic_to_shared(cnt), k2s = (uint32_t)__cvta_generic_to_shared(K2),
+                   pi_s = (uint32_t)__cvta_generic_to_shared(pi);
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      if (bo[j] != 0xFFFFFFFFu) {
-        const uint32_t w = cnt[bo[j] & 0xFFFFu], old = bo[j] >> 16;
-        const uint32_t b0 = w & 0xFFFFu;
-        if ((w >> 16) == 1u) {
-          pi[b0] = (uint16_t)(comp[j] & slot_mask);
-          bo[j] = 0xFFFFFFFFu;
-        } else {
-          K2[b0 + old] = comp[j];
-          bo[j] = w;
-        }
-      }
-    }
+    for (int j = 0; j < 8; ++j)
+      bo[j] = cells_place(bo[j], 4 * (tid + NT * (j >> 2)) + (j & 3), N, comp[j], cnt_s, k2s, pi_s);
     sync();
     // ---- in-bucket ranking by composite = (key, slot) order ----
+    {
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      if (bo[j] != 0xFFFFFFFFu) {
+      for (int j = 0; j < 8; ++j) {
         const uint32_t b0 = bo[j] & 0xFFFFu, m = bo[j] >> 16, e = comp[j];
-        uint32_t rank = 0;
-#pragma unroll
-        for (int t = 0; t < kRankWin; ++t)
-          if ((uint32_t)t < m) rank += (K2[b0 + t] < e) ? 1u : 0u;
+        uint32_t rank = b0;
+        cells_rank4(rank, k2s + 4u * b0, e, m);
         if (m > (uint32_t)kRankWin) {
 #pragma unroll 1
           for (uint32_t t = kRankWin; t < m; ++t) rank += (K2[b0 + t] < e) ? 1u : 0u;
         }
-        pi[b0 + rank] = (uint16_t)(e & slot_mask);
+        if (m > 1u) pi[rank] = (uint16_t)(4u * (e & slot_mask));
       }
     }
     if (NT > 32 && tid == 0) *reinterpret_cast<int4 *>(misc + 8) = next;
@@ -328,6 +398,7 @@ struct CellTeam {
     bool any_acc = false;
     {
       const float nBm1 = (float)(P.table.nB - 1);
+      const char *Xb = reinterpret_cast<const char *>(X);
 #pragma unroll
       for (int r = 0; r < 2; ++r) {
         const int dp = tid + NT * r;
@@ -335,14 +406,14 @@ struct CellTeam {
         if (s0 < M) {
           const uint2 w2 = *reinterpret_cast<const uint2 *>(pi + 4 * dp);
           const bool v1 = s0 + 1 < M;
-          int pi_[2] = {(int)(w2.x & 0xFFFFu), (int)(w2.y & 0xFFFFu)};
-          int pj_[2] = {(int)(w2.x >> 16), (int)(w2.y >> 16)};
-          if (!v1) { pi_[1] = pi_[0]; pj_[1] = pj_[0]; }
-          const uint4 rr = philox4x32_10((uint32_t)dp, cell_ctr, P.step, 1u, P.seed_lo, P.seed_hi);
+          uint32_t oi[2] = {w2.x & 0xFFFFu, w2.y & 0xFFFFu};
+          uint32_t oj[2] = {w2.x >> 16, w2.y >> 16};
+          if (!v1) { oi[1] = oi[0]; oj[1] = oj[0]; }
+          const uint4 rr = cells_philox(P, (uint32_t)dp, cell_ctr, P.step, 1u);
           const float Ub[2] = {u01(rr.x), u01(rr.z)}, Ue[2] = {u01(rr.y), u01(rr.w)};
           float Ua[2] = {0.f, 0.f}, cap = 0.f;
           if (accept) {  // stream 3: U_acc of pair slot s = word s & 3 of block s >> 2
-            const uint4 ra = philox4x32_10((uint32_t)dp >> 1, cell_ctr, P.step, 3u, P.seed_lo, P.seed_hi);
+            const uint4 ra = cells_philox(P, (uint32_t)dp >> 1, cell_ctr, P.step, 3u);
             Ua[0] = u01((dp & 1) ? ra.z : ra.x);
             Ua[1] = u01((dp & 1) ? ra.w : ra.y);
             cap = __ldg(P.cap + item.x);
@@ -350,8 +421,9 @@ struct CellTeam {
           float vix[2], viy[2], viz[2], vjx[2], vjy[2], vjz[2];
 #pragma unroll
           for (int k = 0; k < 2; ++k) {
-            vix[k] = X[pi_[k]]; viy[k] = Y[pi_[k]]; viz[k] = Z[pi_[k]];
-            vjx[k] = X[pj_[k]]; vjy[k] = Y[pj_[k]]; vjz[k] = Z[pj_[k]];
+            const float *pi_ = reinterpret_cast<const float *>(Xb + oi[k]), *pj_ = reinterpret_cast<const float *>(Xb + oj[k]);
+            vix[k] = pi_[0]; viy[k] = pi_[C]; viz[k] = pi_[2 * C];
+            vjx[k] = pj_[0]; vjy[k] = pj_[C]; vjz[k] = pj_[2 * C];
           }
 #pragma unroll
           for (int k = 0; k < 2; ++k) {
@@ -369,14 +441,16 @@ struct CellTeam {
               if (g2 > 0.f) cells_rotate(gx, gy, gz, g2, chi, Ue[k], px, py, pz);
               // eqs. 6-8
               const float cx = 0.5f * (vix[k] + vjx[k]), cy = 0.5f * (viy[k] + vjy[k]), cz = 0.5f * (viz[k] + vjz[k]);
-              X[pi_[k]] = fmaf(0.5f, px, cx); Y[pi_[k]] = fmaf(0.5f, py, cy); Z[pi_[k]] = fmaf(0.5f, pz, cz);
-              X[pj_[k]] = fmaf(-0.5f, px, cx); Y[pj_[k]] = fmaf(-0.5f, py, cy); Z[pj_[k]] = fmaf(-0.5f, pz, cz);
+              float *qi = reinterpret_cast<float *>(const_cast<char *>(Xb) + oi[k]);
+              float *qj = reinterpret_cast<float *>(const_cast<char *>(Xb) + oj[k]);
+              qi[0] = fmaf(0.5f, px, cx); qi[C] = fmaf(0.5f, py, cy); qi[2 * C] = fmaf(0.5f, pz, cz);
+              qj[0] = fmaf(-0.5f, px, cx); qj[C] = fmaf(-0.5f, py, cy); qj[2 * C] = fmaf(-0.5f, pz, cz);
               any_acc = true;
             }
             if (P.dump_any && valid) {
               const int64_t d = (int64_t)gs + s0 + k;
-              if (P.dump.pair_i) P.dump.pair_i[d] = pi_[k];
-              if (P.dump.pair_j) P.dump.pair_j[d] = pj_[k];
+              if (P.dump.pair_i) P.dump.pair_i[d] = (int32_t)(oi[k] >> 2);
+              if (P.dump.pair_j) P.dump.pair_j[d] = (int32_t)(oj[k] >> 2);
               if (P.dump.accepted) P.dump.accepted[d] = acc ? 1 : 0;
               if (P.dump.gprime) { P.dump.gprime[3 * d] = px; P.dump.gprime[3 * d + 1] = py; P.dump.gprime[3 * d + 2] = pz; }
               if (P.dump.aux) P.dump.aux[d] = chi;
@@ -419,42 +493,29 @@ struct CellTeam {
             s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
           }
         }
-        const float t = warp_sum4(sx, sy, sz, s2, lane);
-        double dsx, dsy, dsz, ds2;
-        if (NT == 32) {
-          dsx = __shfl_sync(0xffffffffu, t, 0);
-          dsy = __shfl_sync(0xffffffffu, t, 8);
-          dsz = __shfl_sync(0xffffffffu, t, 16);
-          ds2 = __shfl_sync(0xffffffffu, t, 24);
-        } else {
-          if ((lane & 7) == 0) reinterpret_cast<float *>(&part[8 + warp])[lane >> 3] = t;
-          sync();
-          dsx = dsy = dsz = ds2 = 0.0;
-#pragma unroll
-          for (int w = 0; w < NW; ++w) {
-            const float4 p = part[8 + w];
-            dsx += p.x; dsy += p.y; dsz += p.z; ds2 += p.w;
-          }
-        }
-        const double inv = 1.0 / N;
-        const double dx = dsx * inv, dy = dsy * inv, dz = dsz * inv;  // u_post - u_pre
-        const double th_post = ds2 - N * (dx * dx + dy * dy + dz * dz);
-        double alpha = 1.0, bx = 0.0, by = 0.0, bz = 0.0;
+        team_sum4(sx, sy, sz, s2, 1);
+        const float dx = sx * invN, dy = sy * invN, dz = sz * invN;  // u_post - u_pre
+        const float th_post = s2 - fN * fmaf(dx, dx, fmaf(dy, dy, dz * dz));
         if (P.flags & DSMC_F_MATCH_ENERGY_ONLY) {  // literal eq. 11: v <- v sqrt(E_pre / E_post)
-          const double qx = ux + dx, qy = uy + dy, qz = uz + dz;
-          const double e_pre = (double)theta + N * ((double)ux * ux + (double)uy * uy + (double)uz * uz);
-          const double e_post = th_post + N * (qx * qx + qy * qy + qz * qz);
-          if (e_post > 0.0) alpha = sqrt(e_pre / e_post);
+          const float qx = ux + dx, qy = uy + dy, qz = uz + dz;
+          const float e_pre = theta + fN * fmaf(ux, ux, fmaf(uy, uy, uz * uz));
+          const float e_post = th_post + fN * fmaf(qx, qx, fmaf(qy, qy, qz * qz));
+          if (e_post > 0.f) {
+            const float del = (e_pre - e_post) / e_post;  // alpha - 1 = sqrt(1 + del) - 1 without cancellation
+            am1 = del / (1.0f + sqrtf(1.0f + del));
+          }
         } else {  // v <- u_pre + alpha (v - u_post)
-          if (th_post > 0.0) alpha = sqrt((double)theta / th_post);
-          bx = ux - alpha * (ux + dx);
-          by = uy - alpha * (uy + dy);
-          bz = uz - alpha * (uz + dz);
+          if (th_post > 0.f) {
+            const float del = (theta - th_post) / th_post;
+            am1 = del / (1.0f + sqrtf(1.0f + del));
+          }
+          // B = u_pre - alpha (u_pre + d) = -(alpha - 1) u_pre - alpha d
+          Bx = -fmaf(am1, ux, fmaf(am1, dx, dx));
+          By = -fmaf(am1, uy, fmaf(am1, dy, dy));
+          Bz = -fmaf(am1, uz, fmaf(am1, dz, dz));
         }
-        // alpha is 1 + O(1e-7), which FP32 cannot resolve: the store applies v + (alpha - 1) v + B
-        am1 = (float)(alpha - 1.0);
-        Bx = (float)bx; By = (float)by; Bz = (float)bz;
       }
+      // alpha is 1 + O(1e-7), which FP32 cannot resolve: the store applies v + (alpha - 1) v + B
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
         const int q = tid + NT * r;

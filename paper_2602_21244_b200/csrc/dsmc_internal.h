@@ -51,6 +51,7 @@ struct StepParams {
   float *vx, *vy, *vz;
   const float *cap;  // sigma_cr_max / cr_max or nullptr
   uint32_t seed_lo, seed_hi, step;
+  uint32_t rk[20];     // Philox round keys (seed_lo + r W0, seed_hi + r W1), r = 0..9: constant-bank operands
   uint32_t cell_base;  // RNG cell coordinate of local cell 0
   uint32_t flags;
   int32_t pairs_per_cell;
