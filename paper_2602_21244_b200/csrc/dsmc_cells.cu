@@ -80,13 +80,13 @@ __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const Cell
   extern __shared__ __align__(16) unsigned char smem_raw[];
   {
     CellTeam<128> T;
-    T.init(smem_raw, threadIdx.x, 0);
+    T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
     T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
   }
   __syncthreads();
   {
     CellTeam<32> T;
-    T.init(smem_raw + (threadIdx.x >> 5) * CellTeam<32>::bytes(), threadIdx.x & 31, 0);
+    T.init((uint32_t)__cvta_generic_to_shared(smem_raw) + (threadIdx.x >> 5) * (uint32_t)CellTeam<32>::bytes(), threadIdx.x & 31, 0);
     T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
   }
 }
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const Cell
 __global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   CellTeam<256> T;
-  T.init(smem_raw, threadIdx.x, 0);
+  T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
   T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
 }
 

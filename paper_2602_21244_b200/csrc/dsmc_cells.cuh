@@ -162,9 +162,13 @@ struct CellTeam {
 
   static constexpr size_t bytes() { return (size_t)C * (12 + 4 + 4 + 2) + 3 * NT; }  // + part, misc (320 B, NT > 32)
 
-  __device__ __forceinline__ void init(unsigned char *base, int tid_, int bar_) {
+  // base_s: shared-space address of the team's block.  It is made opaque to the compiler, which otherwise rebuilds
+  // it from the special registers (6-8 instructions) in front of most shared-memory accesses instead of keeping it.
+  __device__ __forceinline__ void init(uint32_t base_s, int tid_, int bar_) {
     tid = tid_;
     bar = bar_;
+    asm volatile("" : "+r"(base_s));
+    unsigned char *base = reinterpret_cast<unsigned char *>(__cvta_shared_to_generic(base_s));
     X = reinterpret_cast<float *>(base);
     Y = X + C;
     Z = Y + C;
@@ -399,8 +403,8 @@ struct CellTeam {
     {
       const float nBm1 = (float)(P.table.nB - 1);
       const char *Xb = reinterpret_cast<const char *>(X);
-#pragma unroll
-      for (int r = 0; r < 2; ++r) {
+#pragma unroll 1
+      for (int r = 0; r < 2; ++r) {  // not unrolled: the body is the largest piece of code of the kernel
         const int dp = tid + NT * r;
         const int s0 = 2 * dp;
         if (s0 < M) {
