@@ -211,6 +211,8 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
   c->table.inv_dlnE = (float)inv;
   c->table.c1 = (float)(0.6931471805599453 * inv);
   c->table.c0 = (float)(-(double)lnE_min * inv);
+  c->table.fE1 = (float)(nE - 1);
+  c->table.fB1 = (float)(nB - 1);
   c->has_table = true;
   return DSMC_OK;
 }
@@ -415,6 +417,8 @@ int dsmc_build_chi_table_lj(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, 
   c->table.inv_dlnE = (float)inv;
   c->table.c1 = (float)(0.6931471805599453 * inv);
   c->table.c0 = (float)(-(double)lnE_min * inv);
+  c->table.fE1 = (float)(nE - 1);
+  c->table.fB1 = (float)(nB - 1);
   c->has_table = true;
   return DSMC_OK;
 }

@@ -28,19 +28,35 @@ __device__ __forceinline__ float warp_sum4(float a, float b, float c, float d, i
   return k;
 }
 
+// packed FP32 pairs (FADD2 / FFMA2 on sm_100a): two rows of a thread's particles per instruction
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ float hsum2(f32x2 v) { float a, b; upk2(v, a, b); return a + b; }
+
+// MUFU wrappers with flush-to-zero (no denormal pre-scaling code around them)
+__device__ __forceinline__ float mufu_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rsqrt(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_sin(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_cos(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 // table coordinate t_E = (ln x - lnE_min) (nE-1)/(lnE_max-lnE_min) from x = E_r/k_B, exponent and mantissa of x
 // handled separately (MUFU.LG2 only sees [1,2), abs. error 2^-22)
 __device__ __forceinline__ float cells_tE(const ChiTableDev &T, float x) {
   const int xi = __float_as_int(x);
   const float e = (float)((xi >> 23) - 127);
   const float m = __int_as_float((xi & 0x007FFFFF) | 0x3F800000);
-  return fmaf(__log2f(m), T.c1, fmaf(e, T.c1, T.c0));
+  return fmaf(mufu_lg2(m), T.c1, fmaf(e, T.c1, T.c0));
 }
 
 // bilinear chi(E~, b~) from the L2-resident quad table, coordinates clamped (Q13)
 __device__ __forceinline__ float cells_chi(const ChiTableDev &T, float tE, float tB) {
-  tE = fminf(fmaxf(tE, 0.f), (float)(T.nE - 1));
-  tB = fminf(fmaxf(tB, 0.f), (float)(T.nB - 1));
+  tE = fminf(fmaxf(tE, 0.f), T.fE1);
+  tB = fminf(fmaxf(tB, 0.f), T.fB1);
   const int iE = min((int)tE, T.nE - 2), iB = min((int)tB, T.nB - 2);
   const float fE = tE - (float)iE, fB = tB - (float)iB;
   const float4 q = __ldg(T.quad + (size_t)iE * (T.nB - 1) + iB);
@@ -48,28 +64,24 @@ __device__ __forceinline__ float cells_chi(const ChiTableDev &T, float tE, float
   return fmaf(fE, hi - lo, lo);
 }
 
-// Rotation of g by deflection chi and azimuth eps = 2 pi U_eps (Q16).  MUFU sin/cos on arguments inside
-// [-pi, pi]: eps is taken as 2 pi (U - 1/2) with both signs flipped.
-__device__ __forceinline__ void cells_rotate(float gx, float gy, float gz, float g2, float chi, float U_eps,
-                                             float &px, float &py, float &pz) {
-  float sc, cc, se, ce;
-  __sincosf(chi, &sc, &cc);
-  __sincosf(6.283185307179586f * (U_eps - 0.5f), &se, &ce);
-  se = -se;
-  ce = -ce;
+// Rotation of g by deflection chi and azimuth eps (Q16); eps in [-pi, pi) (the azimuth is uniform, so
+// 2 pi (U - 1/2) serves as 2 pi U with both signs flipped), MUFU sin / cos.
+__device__ __forceinline__ void cells_rotate(float gx, float gy, float gz, float g2, float chi, float eps, float &px,
+                                             float &py, float &pz) {
+  const float sc = mufu_sin(chi), cc = mufu_cos(chi);
+  const float se = -mufu_sin(eps), ce = -mufu_cos(eps);
   const float gp2 = fmaf(gy, gy, gz * gz);
-  const float g = g2 * rsqrtf(g2);
-  if (gp2 <= 1e-30f * g2 * 1e-30f) {  // g_perp <= 1e-30 g
-    px = gx * cc;
-    py = fabsf(gx) * sc * ce;
-    pz = fabsf(gx) * sc * se;
-    return;
-  }
-  const float inv = rsqrtf(gp2), gperp = gp2 * inv;
+  const float g = g2 * mufu_rsqrt(g2);
+  const float inv = mufu_rsqrt(gp2), gperp = gp2 * inv;
   const float sci = sc * inv;
   px = fmaf(gx, cc, gperp * sc * se);
   py = fmaf(gy, cc, sci * (g * gz * ce - gx * gy * se));
   pz = fmaf(gz, cc, -sci * (g * gy * ce + gx * gz * se));
+  if (__builtin_expect(gp2 <= 1e-30f * g2 * 1e-30f, 0)) {  // g_perp <= 1e-30 g: the other two axes
+    px = gx * cc;
+    py = fabsf(gx) * sc * ce;
+    pz = fabsf(gx) * sc * se;
+  }
 }
 
 // Philox4x32-10 with the round keys as constant-bank operands (StepParams::rk): per round two 32 x 32 -> 64 bit
@@ -285,18 +297,32 @@ struct CellTeam {
         pvy = __shfl_sync(0xffffffffu, t, 8);
         pvz = __shfl_sync(0xffffffffu, t, 16);
       }
-      float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
+      // rows beyond the cell stand at the pivot (d = 0), so the sums need no predicates; two rows per instruction
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
         const int q = tid + NT * r;
         if (q < N) {
-          const float dx = x[r] - pvx, dy = y[r] - pvy, dz = z[r] - pvz;
-          sx += dx; sy += dy; sz += dz;
-          s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
           X[q] = x[r];
           Y[q] = y[r];
           Z[q] = z[r];
+        } else {
+          x[r] = pvx;
+          y[r] = pvy;
+          z[r] = pvz;
         }
+      }
+      float sx, sy, sz, s2;
+      {
+        const f32x2 px2 = pk2(pvx, pvx), py2 = pk2(pvy, pvy), pz2 = pk2(pvz, pvz);
+        f32x2 ax = pk2(0.f, 0.f), ay = ax, az = ax, a2 = ax;
+#pragma unroll
+        for (int r = 0; r < 8; r += 2) {
+          const f32x2 dx = sub2(pk2(x[r], x[r + 1]), px2), dy = sub2(pk2(y[r], y[r + 1]), py2),
+                      dz = sub2(pk2(z[r], z[r + 1]), pz2);
+          ax = add2(ax, dx); ay = add2(ay, dy); az = add2(az, dz);
+          a2 = fma2(dx, dx, a2); a2 = fma2(dy, dy, a2); a2 = fma2(dz, dz, a2);
+        }
+        sx = hsum2(ax); sy = hsum2(ay); sz = hsum2(az); s2 = hsum2(a2);
       }
       team_sum4(sx, sy, sz, s2, 0);
       if (NT == 32) sync();  // counters zeroed before the first atomic (NT > 32: the barrier inside team_sum4)
@@ -401,7 +427,7 @@ struct CellTeam {
     // ---- pairs: thread owns pair slots 2 dp, 2 dp + 1 (one Philox block of stream 1 serves both) ----
     bool any_acc = false;
     {
-      const float nBm1 = (float)(P.table.nB - 1);
+      const float nBm1 = P.table.fB1;
       const char *Xb = reinterpret_cast<const char *>(X);
 #pragma unroll 1
       for (int r = 0; r < 2; ++r) {  // not unrolled: the body is the largest piece of code of the kernel
@@ -414,7 +440,11 @@ struct CellTeam {
           uint32_t oj[2] = {w2.x >> 16, w2.y >> 16};
           if (!v1) { oi[1] = oi[0]; oj[1] = oj[0]; }
           const uint4 rr = cells_philox(P, (uint32_t)dp, cell_ctr, P.step, 1u);
-          const float Ub[2] = {u01(rr.x), u01(rr.z)}, Ue[2] = {u01(rr.y), u01(rr.w)};
+          // U_b = ((x >> 9) + 1/2) 2^-23 built from the float 1.f + (x >> 9) 2^-23; eps = 2 pi (U_eps - 1/2) likewise
+          const float Ub[2] = {__uint_as_float((rr.x >> 9) | 0x3F800000u) - 0.99999994f,
+                               __uint_as_float((rr.z >> 9) | 0x3F800000u) - 0.99999994f};
+          const float eps[2] = {fmaf(__uint_as_float((rr.y >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f),
+                                fmaf(__uint_as_float((rr.w >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f)};
           float Ua[2] = {0.f, 0.f}, cap = 0.f;
           if (accept) {  // stream 3: U_acc of pair slot s = word s & 3 of block s >> 2
             const uint4 ra = cells_philox(P, (uint32_t)dp >> 1, cell_ctr, P.step, 3u);
@@ -439,16 +469,14 @@ struct CellTeam {
             float px = gx, py = gy, pz = gz, chi = 0.f;
             if (acc) {
               // E~ = ln(m g^2 / (4 kB)), b~ = sqrt(U_b)
-              float sb;
-              asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sb) : "f"(Ub[k]));
-              chi = cells_chi(P.table, cells_tE(P.table, P.e_coef * g2), sb * nBm1);
-              if (g2 > 0.f) cells_rotate(gx, gy, gz, g2, chi, Ue[k], px, py, pz);
-              // eqs. 6-8
-              const float cx = 0.5f * (vix[k] + vjx[k]), cy = 0.5f * (viy[k] + vjy[k]), cz = 0.5f * (viz[k] + vjz[k]);
+              chi = cells_chi(P.table, cells_tE(P.table, P.e_coef * g2), mufu_sqrt(Ub[k]) * nBm1);
+              if (g2 > 0.f) cells_rotate(gx, gy, gz, g2, chi, eps[k], px, py, pz);
+              // eqs. 6-8 as v_i + (g' - g) / 2, v_j - (g' - g) / 2
+              const float hx = px - gx, hy = py - gy, hz = pz - gz;
               float *qi = reinterpret_cast<float *>(const_cast<char *>(Xb) + oi[k]);
               float *qj = reinterpret_cast<float *>(const_cast<char *>(Xb) + oj[k]);
-              qi[0] = fmaf(0.5f, px, cx); qi[C] = fmaf(0.5f, py, cy); qi[2 * C] = fmaf(0.5f, pz, cz);
-              qj[0] = fmaf(-0.5f, px, cx); qj[C] = fmaf(-0.5f, py, cy); qj[2 * C] = fmaf(-0.5f, pz, cz);
+              qi[0] = fmaf(0.5f, hx, vix[k]); qi[C] = fmaf(0.5f, hy, viy[k]); qi[2 * C] = fmaf(0.5f, hz, viz[k]);
+              qj[0] = fmaf(-0.5f, hx, vjx[k]); qj[C] = fmaf(-0.5f, hy, vjy[k]); qj[2 * C] = fmaf(-0.5f, hz, vjz[k]);
               any_acc = true;
             }
             if (P.dump_any && valid) {
@@ -476,9 +504,9 @@ struct CellTeam {
       float *__restrict__ ox = P.vx + gs, *__restrict__ oy = P.vy + gs, *__restrict__ oz = P.vz + gs;
       float x[8], y[8], z[8];
 #pragma unroll
-      for (int r = 0; r < 8; ++r) {
+      for (int r = 0; r < 8; ++r) {  // rows beyond the cell stand at u_pre: no contribution to the sums
         const int q = tid + NT * r;
-        x[r] = y[r] = z[r] = 0.f;
+        x[r] = ux; y[r] = uy; z[r] = uz;
         if (q < N) {
           x[r] = X[q];
           y[r] = Y[q];
@@ -487,15 +515,18 @@ struct CellTeam {
       }
       float am1 = 0.f, Bx = 0.f, By = 0.f, Bz = 0.f;
       if (P.flags & DSMC_F_MOMENT_MATCH) {
-        float sx = 0.f, sy = 0.f, sz = 0.f, s2 = 0.f;
+        float sx, sy, sz, s2;
+        {
+          const f32x2 ux2 = pk2(ux, ux), uy2 = pk2(uy, uy), uz2 = pk2(uz, uz);
+          f32x2 ax = pk2(0.f, 0.f), ay = ax, az = ax, a2 = ax;
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-          const int q = tid + NT * r;
-          if (q < N) {
-            const float dx = x[r] - ux, dy = y[r] - uy, dz = z[r] - uz;
-            sx += dx; sy += dy; sz += dz;
-            s2 = fmaf(dx, dx, s2); s2 = fmaf(dy, dy, s2); s2 = fmaf(dz, dz, s2);
+          for (int r = 0; r < 8; r += 2) {
+            const f32x2 dx = sub2(pk2(x[r], x[r + 1]), ux2), dy = sub2(pk2(y[r], y[r + 1]), uy2),
+                        dz = sub2(pk2(z[r], z[r + 1]), uz2);
+            ax = add2(ax, dx); ay = add2(ay, dy); az = add2(az, dz);
+            a2 = fma2(dx, dx, a2); a2 = fma2(dy, dy, a2); a2 = fma2(dz, dz, a2);
           }
+          sx = hsum2(ax); sy = hsum2(ay); sz = hsum2(az); s2 = hsum2(a2);
         }
         team_sum4(sx, sy, sz, s2, 1);
         const float dx = sx * invN, dy = sy * invN, dz = sz * invN;  // u_post - u_pre
@@ -520,13 +551,22 @@ struct CellTeam {
         }
       }
       // alpha is 1 + O(1e-7), which FP32 cannot resolve: the store applies v + (alpha - 1) v + B
+      {
+        const f32x2 a2 = pk2(am1, am1), bx2 = pk2(Bx, Bx), by2 = pk2(By, By), bz2 = pk2(Bz, Bz);
 #pragma unroll
-      for (int r = 0; r < 8; ++r) {
-        const int q = tid + NT * r;
-        if (q < N) {
-          __stcs(ox + q, fmaf(am1, x[r], x[r] + Bx));
-          __stcs(oy + q, fmaf(am1, y[r], y[r] + By));
-          __stcs(oz + q, fmaf(am1, z[r], z[r] + Bz));
+        for (int r = 0; r < 8; r += 2) {
+          float o0, o1;
+          const f32x2 vx2 = pk2(x[r], x[r + 1]), vy2 = pk2(y[r], y[r + 1]), vz2 = pk2(z[r], z[r + 1]);
+          const int q0 = tid + NT * r, q1 = q0 + NT;
+          upk2(fma2(a2, vx2, add2(vx2, bx2)), o0, o1);
+          if (q0 < N) __stcs(ox + q0, o0);
+          if (q1 < N) __stcs(ox + q1, o1);
+          upk2(fma2(a2, vy2, add2(vy2, by2)), o0, o1);
+          if (q0 < N) __stcs(oy + q0, o0);
+          if (q1 < N) __stcs(oy + q1, o1);
+          upk2(fma2(a2, vz2, add2(vz2, bz2)), o0, o1);
+          if (q0 < N) __stcs(oz + q0, o0);
+          if (q1 < N) __stcs(oz + q1, o1);
         }
       }
     }
