@@ -17,6 +17,26 @@ using namespace dsmc;
     if ((x) != cudaSuccess) return DSMC_ERR_CUDA; \
   } while (0)
 
+// the quad table as a linear texture (cell-team kernel: gathers on the TEX pipe); 0 when it cannot be made
+static void make_table_texture(dsmc_ctx *c, size_t n_quads) {
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
+  c->table.tex = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, c->device) != cudaSuccess || n_quads > (size_t)prop.maxTexture1DLinear) return;
+  cudaResourceDesc rd;
+  memset(&rd, 0, sizeof(rd));
+  rd.resType = cudaResourceTypeLinear;
+  rd.res.linear.devPtr = c->d_table;
+  rd.res.linear.desc = cudaCreateChannelDesc<float4>();
+  rd.res.linear.sizeInBytes = n_quads * sizeof(float4);
+  cudaTextureDesc td;
+  memset(&td, 0, sizeof(td));
+  td.readMode = cudaReadModeElementType;
+  cudaTextureObject_t t = 0;
+  if (cudaCreateTextureObject(&t, &rd, &td, nullptr) == cudaSuccess) c->table.tex = t;
+  else cudaGetLastError();
+}
+
 extern "C" {
 
 int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_cells) {
@@ -82,6 +102,7 @@ int dsmc_destroy(dsmc_ctx *c) {
     cudaFree(c->d_weights[s]);
     cudaFree(c->d_tc_blob[s]);
   }
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
   cudaFree(c->d_table);
   cudaFree(c->h_cell);
   for (int a = 0; a < 3; ++a) { cudaFree(c->h_v[a]); cudaFree(c->h_vs[a]); }
@@ -188,6 +209,8 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
     if (!isfinite(chi_host[i])) return DSMC_ERR_INVALID_ARG;  // a non-finite node would poison every pair near it
   CK(cudaSetDevice(c->device));
   CK(cudaStreamSynchronize(c->stream));
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
+  c->table.tex = 0;
   cudaFree(c->d_table);
   c->d_table = nullptr;
   // device layout: the 2x2 nodes of every grid cell side by side, so a lookup is one 16-byte load
@@ -213,6 +236,7 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
   c->table.c0 = (float)(-(double)lnE_min * inv);
   c->table.fE1 = (float)(nE - 1);
   c->table.fB1 = (float)(nB - 1);
+  make_table_texture(c, nq);
   c->has_table = true;
   return DSMC_OK;
 }
@@ -394,6 +418,8 @@ int dsmc_build_chi_table_lj(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, 
     return DSMC_ERR_INVALID_ARG;
   CK(cudaSetDevice(c->device));
   CK(cudaStreamSynchronize(c->stream));
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
+  c->table.tex = 0;
   cudaFree(c->d_table);
   c->d_table = nullptr;
   c->has_table = false;
@@ -419,6 +445,7 @@ int dsmc_build_chi_table_lj(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, 
   c->table.c0 = (float)(-(double)lnE_min * inv);
   c->table.fE1 = (float)(nE - 1);
   c->table.fB1 = (float)(nB - 1);
+  make_table_texture(c, nq);
   c->has_table = true;
   return DSMC_OK;
 }

@@ -59,7 +59,7 @@ __device__ __forceinline__ float cells_chi(const ChiTableDev &T, float tE, float
   tB = fminf(fmaxf(tB, 0.f), T.fB1);
   const int iE = min((int)tE, T.nE - 2), iB = min((int)tB, T.nB - 2);
   const float fE = tE - (float)iE, fB = tB - (float)iB;
-  const float4 q = __ldg(T.quad + (size_t)iE * (T.nB - 1) + iB);
+  const float4 q = T.tex ? tex1Dfetch<float4>(T.tex, iE * (T.nB - 1) + iB) : __ldg(T.quad + (size_t)iE * (T.nB - 1) + iB);
   const float lo = fmaf(fB, q.y - q.x, q.x), hi = fmaf(fB, q.w - q.z, q.z);
   return fmaf(fE, hi - lo, lo);
 }

@@ -42,6 +42,8 @@ struct ChiTableDev {
   float lnE_min, inv_dlnE;  // inv_dlnE = (nE-1)/(lnE_max-lnE_min)
   float c0, c1;             // t_E = c0 + c1 log2(E_r/k_B): c1 = ln2 inv_dlnE, c0 = -lnE_min inv_dlnE
   float fE1, fB1;           // nE - 1, nB - 1 as floats
+  cudaTextureObject_t tex;  // the quad table as a linear float4 texture (0 = none): gathers through the TEX pipe
+                            // leave the LSU pipe to the shared-memory traffic (measured, profiles/r02_probes.md)
 };
 
 struct StepParams {
