@@ -75,8 +75,8 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
   CK(cudaMalloc(&c->d_big2, sizeof(int32_t) * (n_chunks + 1)));
   CK(cudaMalloc(&c->d_work, sizeof(int32_t) * 4));
   CK(cudaMalloc(&c->d_cell_list, sizeof(int4) * 3 * (size_t)(max_cells > 0 ? max_cells : 1)));
-  CK(cudaMalloc(&c->d_list_ctr, sizeof(int32_t) * 16));
-  CK(cudaMemset(c->d_list_ctr, 0, sizeof(int32_t) * 16));
+  CK(cudaMalloc(&c->d_list_ctr, sizeof(int32_t) * 32));
+  CK(cudaMemset(c->d_list_ctr, 0, sizeof(int32_t) * 32));
   *out = c;
   return DSMC_OK;
 }

@@ -99,8 +99,8 @@ __global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const 
   T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
 }
 
-int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
-  CellLists L;
+// cell lists of this step (alternating counter sets: this launch zeroes the set of the next step)
+void launch_cell_lists(dsmc_ctx *c, const StepParams &p, CellLists &L) {
   const size_t K = (size_t)c->max_cells;
   for (int k = 0; k < 3; ++k) L.list[k] = c->d_cell_list + k * K;
   const int e = (int)(c->list_epoch & 1);
@@ -109,6 +109,12 @@ int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
   k_cell_lists<<<(p.n_cells + 255) / 256, 256, 0, c->stream>>>(p.n_cells, p.cell_start, p.pairs_count,
                                                                 p.pairs_per_cell, L.list[0], L.list[1], L.list[2],
                                                                 L.ctr, c->d_list_ctr + 8 * (1 - e), p.status);
+  c->launches += 1;
+}
+
+int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
+  CellLists L;
+  launch_cell_lists(c, p, L);
   {
     auto kern = k_cells;
     const size_t smem = CellTeam<128>::bytes();
@@ -124,7 +130,7 @@ int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
       return DSMC_ERR_CUDA;
     kern<<<c->num_sms * 2, 256, smem, c->stream>>>(p, L);
   }
-  c->launches += 3;
+  c->launches += 2;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
 

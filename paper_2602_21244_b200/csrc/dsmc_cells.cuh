@@ -160,7 +160,16 @@ __device__ __forceinline__ uint32_t cells_place(uint32_t bo, int p, int N, uint3
   return out;
 }
 
-template <int NT>
+// OP 0: chi from the table.  OP 2: chi-MLP through the CTA's tensor-core MLP server (SRV, dsmc_cells_mlp.cu).
+struct NoServer {
+  int buf;
+  __device__ int acquire(int, uint32_t *) { return 0; }
+  __device__ void write_row(int, int, float, float) {}
+  __device__ void publish(int) {}
+  __device__ void wait(int) {}
+};
+
+template <int NT, int OP = 0, class SRV = NoServer>
 struct CellTeam {
   static constexpr int C = 8 * NT;  // slots: a thread holds 8 particles / 8 keys / 8 bucket counters
   static constexpr int NW = NT / 32;
@@ -171,6 +180,7 @@ struct CellTeam {
   float4 *part;       // [2][8] per-warp partial sums, before / after the collisions (NT > 32)
   int *misc;          // [0..7] warp totals of the scan, [8..11] next list entry, [12] any pair accepted
   int tid, bar;
+  SRV *srv;
 
   static constexpr size_t bytes() { return (size_t)C * (12 + 4 + 4 + 2) + 3 * NT; }  // + part, misc (320 B, NT > 32)
 
@@ -225,6 +235,41 @@ struct CellTeam {
     while (item.z > 0) item = cell(P, item, list, n_items, work);
   }
 
+  // OP 2: two cells in flight per team, one in each of its two buffers: while the server works on the tile(s) of one
+  // cell the team loads, sorts and submits the next one
+  __device__ void run2(const StepParams &P, const int4 *__restrict__ list, const int32_t *n_items_ptr, int32_t *work,
+                       uint32_t base0, uint32_t base1) {
+    const int n_items = __ldg(n_items_ptr);
+    const int t = tid, br = bar;
+    init(base0, t, br);
+    int4 item = make_int4(0, 0, 0, 0);
+    if (tid == 0) {
+      item = entry(list, n_items, atomicAdd(work, 1));
+      if (NT > 32) *reinterpret_cast<int4 *>(misc + 8) = item;
+    }
+    if (NT > 32) sync();
+    item = share(item);
+    if (NT > 32) sync();
+    int4 prev = make_int4(0, 0, 0, 0);
+    int b = 0;
+    while (item.z > 0 || prev.z > 0) {
+      int4 nxt = make_int4(0, 0, 0, 0);
+      if (item.z > 0) {
+        init(b ? base1 : base0, t, br);
+        srv->buf = b;
+        nxt = cell<1>(P, item, list, n_items, work);
+      }
+      if (prev.z > 0) {
+        init(b ? base0 : base1, t, br);
+        srv->buf = b ^ 1;
+        cell<2>(P, prev, list, n_items, work);
+      }
+      prev = item;
+      item = nxt;
+      b ^= 1;
+    }
+  }
+
   // team sums of (a, b, c, d): per-warp butterfly, then (NT > 32) the warps' partials through shared memory in a
   // fixed order.  `slot` selects the partial-sum buffer; contains one team barrier when NT > 32.
   __device__ __forceinline__ void team_sum4(float &a, float &b, float &c, float &d, int slot) const {
@@ -247,7 +292,116 @@ struct CellTeam {
     }
   }
 
-  // one cell; returns the team's next list entry
+  // Pairs of the cell: the thread owns pair slots 2 dp, 2 dp + 1, dp = tid + NT r, r = 0, 1 (one Philox block of
+  // stream 1 serves both).  STAGE 0: chi from the table, rotation, commit.  STAGE 1 (chi-MLP): features of every pair
+  // slot -> row ((2 r + k) 32 + lane) of the warp's tile in the MLP server's layer-1 operand; eps (or a sentinel for
+  // a pair that does not collide) parked in cnt[].  STAGE 2: chi = exp(z) from the delivered outputs, rotation, commit.
+  template <int STAGE>
+  __device__ __forceinline__ bool pairs_phase(const StepParams &P, const int4 item, uint32_t cell_ctr, bool accept,
+                                              int slot) {
+    const int lane = tid & 31, warp = tid >> 5;
+    const int gs = item.y, M = item.w;
+    bool any_acc = false;
+    const float nBm1 = P.table.fB1;
+    const char *Xb = reinterpret_cast<const char *>(X);
+    float *park = reinterpret_cast<float *>(cnt) + 128 * warp;  // STAGE 1 -> 2: eps per row (cnt is dead by now)
+    float *stage = reinterpret_cast<float *>(K2) + 256 * warp;  // STAGE 1: features [2][128]; STAGE 2: z [128]
+    const float *zbuf = stage;
+#pragma unroll 1
+    for (int r = 0; r < 2; ++r) {  // not unrolled: the body is the largest piece of code of the kernel
+      const int dp = tid + NT * r;
+      const int s0 = 2 * dp;
+      if (s0 < M) {
+        const uint2 w2 = *reinterpret_cast<const uint2 *>(pi + 4 * dp);
+        const bool v1 = s0 + 1 < M;
+        uint32_t oi[2] = {w2.x & 0xFFFFu, w2.y & 0xFFFFu};
+        uint32_t oj[2] = {w2.x >> 16, w2.y >> 16};
+        if (!v1) { oi[1] = oi[0]; oj[1] = oj[0]; }
+        float Ub[2] = {0.f, 0.f}, eps[2] = {0.f, 0.f}, Ua[2] = {0.f, 0.f}, cap = 0.f;
+        if (STAGE != 2) {
+          const uint4 rr = cells_philox(P, (uint32_t)dp, cell_ctr, P.step, 1u);
+          // U_b = ((x >> 9) + 1/2) 2^-23 built from the float 1.f + (x >> 9) 2^-23; eps = 2 pi (U_eps - 1/2) likewise
+          Ub[0] = __uint_as_float((rr.x >> 9) | 0x3F800000u) - 0.99999994f;
+          Ub[1] = __uint_as_float((rr.z >> 9) | 0x3F800000u) - 0.99999994f;
+          eps[0] = fmaf(__uint_as_float((rr.y >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f);
+          eps[1] = fmaf(__uint_as_float((rr.w >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f);
+          if (accept) {  // stream 3: U_acc of pair slot s = word s & 3 of block s >> 2
+            const uint4 ra = cells_philox(P, (uint32_t)dp >> 1, cell_ctr, P.step, 3u);
+            Ua[0] = u01((dp & 1) ? ra.z : ra.x);
+            Ua[1] = u01((dp & 1) ? ra.w : ra.y);
+            cap = __ldg(P.cap + item.x);
+          }
+        }
+        float vix[2], viy[2], viz[2], vjx[2], vjy[2], vjz[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const float *pi_ = reinterpret_cast<const float *>(Xb + oi[k]), *pj_ = reinterpret_cast<const float *>(Xb + oj[k]);
+          vix[k] = pi_[0]; viy[k] = pi_[C]; viz[k] = pi_[2 * C];
+          vjx[k] = pj_[0]; vjy[k] = pj_[C]; vjz[k] = pj_[2 * C];
+        }
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const bool valid = k == 0 || v1;
+          const int row = (2 * r + k) * 32 + lane;
+          const float gx = vix[k] - vjx[k], gy = viy[k] - vjy[k], gz = viz[k] - vjz[k];  // eq. 1
+          const float g2 = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
+          bool acc = valid;
+          if (STAGE != 2) {
+            if (accept) acc = valid && (Ua[k] * cap < sqrtf(g2));  // constant cross-section: U g_max < g
+          }
+          if (STAGE == 1) {  // chi-MLP inputs (Q15): ((E~ - E~min) / (E~max - E~min) clamped to [0, 1], b~)
+            const float e = (0.6931471806f * mufu_lg2(P.e_coef * g2) - P.lnE_min) * P.inv_lnE_range;
+            stage[row] = !(e > 0.f) ? 0.f : fminf(e, 1.f);
+            stage[128 + row] = mufu_sqrt(Ub[k]);
+            park[row] = acc ? eps[k] : 1e30f;
+            continue;
+          }
+          float px = gx, py = gy, pz = gz, chi = 0.f;
+          if (STAGE == 2) {
+            eps[k] = park[row];
+            acc = valid && eps[k] < 1e29f;
+          }
+          if (acc) {
+            if (STAGE == 2) {
+              chi = __expf(zbuf[row]);  // chi = expm1(softplus(z)) = exp(z)
+            } else {
+              // E~ = ln(m g^2 / (4 kB)) (P:L334, P:L373), b~ = sqrt(U_b)
+              chi = cells_chi(P.table, cells_tE(P.table, P.e_coef * g2), mufu_sqrt(Ub[k]) * nBm1);
+            }
+            if (g2 > 0.f) cells_rotate(gx, gy, gz, g2, chi, eps[k], px, py, pz);
+            // eqs. 6-8 as v_i + (g' - g) / 2, v_j - (g' - g) / 2
+            const float hx = px - gx, hy = py - gy, hz = pz - gz;
+            float *qi = reinterpret_cast<float *>(const_cast<char *>(Xb) + oi[k]);
+            float *qj = reinterpret_cast<float *>(const_cast<char *>(Xb) + oj[k]);
+            qi[0] = fmaf(0.5f, hx, vix[k]); qi[C] = fmaf(0.5f, hy, viy[k]); qi[2 * C] = fmaf(0.5f, hz, viz[k]);
+            qj[0] = fmaf(-0.5f, hx, vjx[k]); qj[C] = fmaf(-0.5f, hy, vjy[k]); qj[2 * C] = fmaf(-0.5f, hz, vjz[k]);
+            any_acc = true;
+          }
+          if (P.dump_any && valid) {
+            const int64_t d = (int64_t)gs + s0 + k;
+            if (P.dump.pair_i) P.dump.pair_i[d] = (int32_t)(oi[k] >> 2);
+            if (P.dump.pair_j) P.dump.pair_j[d] = (int32_t)(oj[k] >> 2);
+            if (P.dump.accepted) P.dump.accepted[d] = acc ? 1 : 0;
+            if (P.dump.gprime) { P.dump.gprime[3 * d] = px; P.dump.gprime[3 * d + 1] = py; P.dump.gprime[3 * d + 2] = pz; }
+            if (P.dump.aux) P.dump.aux[d] = chi;
+          }
+        }
+      } else if (STAGE == 1) {  // rows of pair slots that do not exist: defined inputs, nothing to collide
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          stage[(2 * r + k) * 32 + lane] = 0.f;
+          stage[128 + (2 * r + k) * 32 + lane] = 0.f;
+          park[(2 * r + k) * 32 + lane] = 1e30f;
+        }
+      }
+    }
+    return any_acc;
+  }
+
+  // one cell; returns the team's next list entry.  HALF 0: the whole cell.  OP 2 only: HALF 1 = up to the publication
+  // of the warp's tile (returns the next entry), HALF 2 = from the delivery of z to the store: between the two the
+  // team works on another cell in its other buffer (run2).
+  template <int HALF = 0>
   __device__ __forceinline__ int4 cell(const StepParams &P, const int4 item, const int4 *__restrict__ list, int n_items,
                                        int32_t *work) {
     const int lane = tid & 31, warp = tid >> 5;
@@ -257,6 +411,10 @@ struct CellTeam {
     const int NB = 1 << Lb;
     const bool accept = (P.flags & DSMC_F_ACCEPT) && P.cap != nullptr;
     const float fN = (float)N, invN = 1.0f / fN;
+    float ux = 0.f, uy = 0.f, uz = 0.f, theta = 0.f;
+    int4 next = make_int4(0, 0, 0, 0);
+    float *state = NT == 32 ? reinterpret_cast<float *>(part) : reinterpret_cast<float *>(misc + 16);
+    if (HALF != 2) {
     int next_idx = 0;
     if (tid == 0) {
       next_idx = atomicAdd(work, 1);  // consumed after the loads below have landed
@@ -266,7 +424,6 @@ struct CellTeam {
     if (4 * tid < NB) *reinterpret_cast<uint4 *>(cnt + 4 * tid) = make_uint4(0u, 0u, 0u, 0u);
     if (4 * (tid + NT) < NB) *reinterpret_cast<uint4 *>(cnt + 4 * (tid + NT)) = make_uint4(0u, 0u, 0u, 0u);
     // ---- load (12 B / particle) + pre-collision sums about the pivot (eq. 10) ----
-    float ux, uy, uz, theta;
     {
       const float *__restrict__ gx = P.vx + gs, *__restrict__ gy = P.vy + gs, *__restrict__ gz = P.vz + gs;
       float x[8], y[8], z[8];
@@ -334,7 +491,6 @@ struct CellTeam {
       uz = pvz + mz;
       theta = fmaxf(s2 - fN * fmaf(mx, mx, fmaf(my, my, mz * mz)), 0.f);
     }
-    int4 next = make_int4(0, 0, 0, 0);
     if (tid == 0) next = entry(list, n_items, next_idx);
     // ---- pairing keys (stream 0: block blk serves slots 4 blk .. 4 blk + 3) and bucket counts ----
     // per key: comp = key << Lb | slot (the (key, slot) order inside a bucket), bo = bucket | arrival index << 16
@@ -424,72 +580,41 @@ struct CellTeam {
     }
     if (NT > 32 && tid == 0) *reinterpret_cast<int4 *>(misc + 8) = next;
     sync();
+    }  // HALF != 2
     // ---- pairs: thread owns pair slots 2 dp, 2 dp + 1 (one Philox block of stream 1 serves both) ----
-    bool any_acc = false;
-    {
-      const float nBm1 = P.table.fB1;
-      const char *Xb = reinterpret_cast<const char *>(X);
-#pragma unroll 1
-      for (int r = 0; r < 2; ++r) {  // not unrolled: the body is the largest piece of code of the kernel
-        const int dp = tid + NT * r;
-        const int s0 = 2 * dp;
-        if (s0 < M) {
-          const uint2 w2 = *reinterpret_cast<const uint2 *>(pi + 4 * dp);
-          const bool v1 = s0 + 1 < M;
-          uint32_t oi[2] = {w2.x & 0xFFFFu, w2.y & 0xFFFFu};
-          uint32_t oj[2] = {w2.x >> 16, w2.y >> 16};
-          if (!v1) { oi[1] = oi[0]; oj[1] = oj[0]; }
-          const uint4 rr = cells_philox(P, (uint32_t)dp, cell_ctr, P.step, 1u);
-          // U_b = ((x >> 9) + 1/2) 2^-23 built from the float 1.f + (x >> 9) 2^-23; eps = 2 pi (U_eps - 1/2) likewise
-          const float Ub[2] = {__uint_as_float((rr.x >> 9) | 0x3F800000u) - 0.99999994f,
-                               __uint_as_float((rr.z >> 9) | 0x3F800000u) - 0.99999994f};
-          const float eps[2] = {fmaf(__uint_as_float((rr.y >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f),
-                                fmaf(__uint_as_float((rr.w >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f)};
-          float Ua[2] = {0.f, 0.f}, cap = 0.f;
-          if (accept) {  // stream 3: U_acc of pair slot s = word s & 3 of block s >> 2
-            const uint4 ra = cells_philox(P, (uint32_t)dp >> 1, cell_ctr, P.step, 3u);
-            Ua[0] = u01((dp & 1) ? ra.z : ra.x);
-            Ua[1] = u01((dp & 1) ? ra.w : ra.y);
-            cap = __ldg(P.cap + item.x);
-          }
-          float vix[2], viy[2], viz[2], vjx[2], vjy[2], vjz[2];
+    bool any_acc;
+    if (OP == 2) {
+      // chi-MLP on the tensor cores: every warp sends the features of its (up to) 128 pair slots to the CTA's MLP
+      // server as one tile, waits for z, then rotates and commits
+      if (HALF != 2) {
+        // (the features are staged in the warp's own shared memory first, so that the server never waits for them)
+        pairs_phase<1>(P, item, cell_ctr, accept, 0);
+        __syncwarp();
+        const float *st = reinterpret_cast<const float *>(K2) + 256 * warp;
+        float f0[4], f1[4];
 #pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const float *pi_ = reinterpret_cast<const float *>(Xb + oi[k]), *pj_ = reinterpret_cast<const float *>(Xb + oj[k]);
-            vix[k] = pi_[0]; viy[k] = pi_[C]; viz[k] = pi_[2 * C];
-            vjx[k] = pj_[0]; vjy[k] = pj_[C]; vjz[k] = pj_[2 * C];
-          }
-#pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const bool valid = k == 0 || v1;
-            const float gx = vix[k] - vjx[k], gy = viy[k] - vjy[k], gz = viz[k] - vjz[k];  // eq. 1
-            const float g2 = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
-            bool acc = valid;
-            if (accept) acc = valid && (Ua[k] * cap < sqrtf(g2));  // constant cross-section: U g_max < g
-            float px = gx, py = gy, pz = gz, chi = 0.f;
-            if (acc) {
-              // E~ = ln(m g^2 / (4 kB)) (P:L334, P:L373), b~ = sqrt(U_b)
-              chi = cells_chi(P.table, cells_tE(P.table, P.e_coef * g2), mufu_sqrt(Ub[k]) * nBm1);
-              if (g2 > 0.f) cells_rotate(gx, gy, gz, g2, chi, eps[k], px, py, pz);
-              // eqs. 6-8 as v_i + (g' - g) / 2, v_j - (g' - g) / 2
-              const float hx = px - gx, hy = py - gy, hz = pz - gz;
-              float *qi = reinterpret_cast<float *>(const_cast<char *>(Xb) + oi[k]);
-              float *qj = reinterpret_cast<float *>(const_cast<char *>(Xb) + oj[k]);
-              qi[0] = fmaf(0.5f, hx, vix[k]); qi[C] = fmaf(0.5f, hy, viy[k]); qi[2 * C] = fmaf(0.5f, hz, viz[k]);
-              qj[0] = fmaf(-0.5f, hx, vjx[k]); qj[C] = fmaf(-0.5f, hy, vjy[k]); qj[2 * C] = fmaf(-0.5f, hz, vjz[k]);
-              any_acc = true;
-            }
-            if (P.dump_any && valid) {
-              const int64_t d = (int64_t)gs + s0 + k;
-              if (P.dump.pair_i) P.dump.pair_i[d] = (int32_t)(oi[k] >> 2);
-              if (P.dump.pair_j) P.dump.pair_j[d] = (int32_t)(oj[k] >> 2);
-              if (P.dump.accepted) P.dump.accepted[d] = acc ? 1 : 0;
-              if (P.dump.gprime) { P.dump.gprime[3 * d] = px; P.dump.gprime[3 * d + 1] = py; P.dump.gprime[3 * d + 2] = pz; }
-              if (P.dump.aux) P.dump.aux[d] = chi;
-            }
-          }
+        for (int u = 0; u < 4; ++u) {
+          f0[u] = st[32 * u + lane];
+          f1[u] = st[128 + 32 * u + lane];
         }
+        const int slot = srv->acquire(lane, K2 + 256 * warp);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) srv->write_row(slot, 32 * u + lane, f0[u], f1[u]);
+        srv->publish(slot);
       }
+      if (HALF == 1) {  // the cell's pre-collision state waits in its buffer
+        if (tid == 0) *reinterpret_cast<float4 *>(state) = make_float4(ux, uy, uz, theta);
+        return share(next);
+      }
+      if (HALF == 2) {
+        sync();
+        const float4 st4 = *reinterpret_cast<const float4 *>(state);
+        ux = st4.x; uy = st4.y; uz = st4.z; theta = st4.w;
+      }
+      srv->wait(lane);
+      any_acc = pairs_phase<2>(P, item, cell_ctr, accept, 0);
+    } else {
+      any_acc = pairs_phase<0>(P, item, cell_ctr, accept, 0);
     }
     bool collided = true;
     if (accept) {

@@ -523,7 +523,7 @@ static int launch_tc_pair(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
   if (p_in.op == 0 && !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3)) return DSMC_ERR_UNSUPPORTED_SHAPE;
   if (p_in.op == 2 && !(net->d_in == 2 && net->d_out == 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  if (p_in.op == 2) return launch_collide_pipe(c, p_in, net);  // plain BF16: warp-specialised kernel
+  if (p_in.op == 2) return launch_collide_cells_mlp(c, p_in, net);  // plain BF16: cell teams + MLP server (dsmc_cells_mlp.cu)
   StepParams p = p_in;
   int rc = launch_chunk_map(c, p);
   if (rc != DSMC_OK) return rc;

@@ -140,7 +140,8 @@ int launch_moment_match(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
                         const double *target, uint32_t flags);
 int launch_chunk_map(dsmc_ctx *c, StepParams &p);
 int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
-int launch_collide_cells(dsmc_ctx *c, const StepParams &p);  // cell-team form, chi-table operator (dsmc_cells.cu)
+int launch_collide_cells(dsmc_ctx *c, const StepParams &p);
+int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_collide_pipe(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // warp-specialised, op 2
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
