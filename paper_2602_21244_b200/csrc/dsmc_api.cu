@@ -39,12 +39,7 @@ static void make_table_texture(dsmc_ctx *c, size_t n_quads) {
 
 extern "C" {
 
-int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_cells) {
-  if (!out || max_particles < 0 || max_cells < 0 || max_particles >= (int64_t(1) << 31)) return DSMC_ERR_INVALID_ARG;
-  CK(cudaSetDevice(device));
-  dsmc_ctx *c = new (std::nothrow) dsmc_ctx();
-  if (!c) return DSMC_ERR_CUDA;
-  memset(c, 0, sizeof(*c));
+static int create_impl(dsmc_ctx *c, int device, int64_t max_particles, int32_t max_cells) {
   c->device = device;
   c->stream = 0;
   c->max_particles = max_particles;
@@ -77,6 +72,24 @@ int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_c
   CK(cudaMalloc(&c->d_cell_list, sizeof(int4) * 3 * (size_t)(max_cells > 0 ? max_cells : 1)));
   CK(cudaMalloc(&c->d_list_ctr, sizeof(int32_t) * 32));
   CK(cudaMemset(c->d_list_ctr, 0, sizeof(int32_t) * 32));
+  return DSMC_OK;
+}
+
+int dsmc_destroy(dsmc_ctx *c);
+
+int dsmc_create(dsmc_ctx **out, int device, int64_t max_particles, int32_t max_cells) {
+  if (!out || max_particles < 0 || max_cells < 0 || max_particles >= (int64_t(1) << 31)) return DSMC_ERR_INVALID_ARG;
+  CK(cudaSetDevice(device));
+  dsmc_ctx *c = new (std::nothrow) dsmc_ctx();
+  if (!c) return DSMC_ERR_CUDA;
+  memset(c, 0, sizeof(*c));
+  const int rc = create_impl(c, device, max_particles, max_cells);
+  if (rc != DSMC_OK) {  // frees whatever was allocated before the failure
+    c->device = device;
+    dsmc_destroy(c);
+    cudaGetLastError();
+    return rc;
+  }
   *out = c;
   return DSMC_OK;
 }
@@ -166,40 +179,53 @@ int dsmc_set_mlp(dsmc_ctx *c, int slot, const dsmc_mlp_desc *d) {
   }
   if (slot == 0 && (!(d->dims[0] == 8 || d->dims[0] == 6) || d->dims[d->n_layers] != 3)) return DSMC_ERR_UNSUPPORTED_SHAPE;
   if (slot == 1 && (d->dims[0] != 2 || d->dims[d->n_layers] != 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  // stage transposed fp32 weights: Wt[l][in][out]
+  for (int l = 0; l < d->n_layers; ++l)
+    if (!d->W[l] || !d->b[l]) return DSMC_ERR_INVALID_ARG;
+  // stage transposed fp32 weights: Wt[l][in][out].  The new image is built completely before the old one is released,
+  // so a failure leaves the slot as it was.
   std::vector<float> host((total + 3) & ~size_t(3));
   MlpDev m{};
   m.n_layers = d->n_layers;
   m.act = d->act;
   m.dmax = (dmax + 3) & ~3;
   CK(cudaSetDevice(c->device));
-  CK(cudaStreamSynchronize(c->stream));
-  cudaFree(c->d_weights[slot]);
-  c->d_weights[slot] = nullptr;
-  CK(cudaMalloc(&c->d_weights[slot], sizeof(float) * host.size()));
+  float *wnew = nullptr;
+  CK(cudaMalloc(&wnew, sizeof(float) * host.size()));
   size_t off = 0;
   for (int l = 0; l < d->n_layers; ++l) {
     const int din = d->dims[l], dout = d->dims[l + 1];
     m.dims[l] = din;
     m.dims[l + 1] = dout;
-    if (!d->W[l] || !d->b[l]) return DSMC_ERR_INVALID_ARG;
-    m.Wt[l] = c->d_weights[slot] + off;
+    m.Wt[l] = wnew + off;
     for (int i = 0; i < din; ++i)
       for (int o = 0; o < dout; ++o) host[off + (size_t)i * dout + o] = d->W[l][(size_t)o * din + i];
     off += (size_t)din * dout;
-    m.b[l] = c->d_weights[slot] + off;
+    m.b[l] = wnew + off;
     for (int o = 0; o < dout; ++o) host[off + o] = d->b[l][o];
     off += dout;
   }
-  CK(cudaMemcpy(c->d_weights[slot], host.data(), sizeof(float) * host.size(), cudaMemcpyHostToDevice));
-  c->mlp[slot] = m;
-  c->has_mlp[slot] = true;
+  if (cudaMemcpy(wnew, host.data(), sizeof(float) * host.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaFree(wnew);
+    return DSMC_ERR_CUDA;
+  }
   // tensor-core image when the shape allows it
+  void *blob_new = nullptr;
+  MlpTcDev tc_new;
+  memset(&tc_new, 0, sizeof(tc_new));
+  const int rc = build_tc_blob(d, &blob_new, &tc_new, c->stream);
+  if (rc != DSMC_OK && rc != DSMC_ERR_UNSUPPORTED_SHAPE) {
+    cudaFree(wnew);
+    cudaFree(blob_new);
+    return rc;
+  }
+  CK(cudaStreamSynchronize(c->stream));  // no kernel still reads the old images
+  cudaFree(c->d_weights[slot]);
   cudaFree(c->d_tc_blob[slot]);
-  c->d_tc_blob[slot] = nullptr;
-  memset(&c->mlp_tc[slot], 0, sizeof(MlpTcDev));
-  int rc = build_tc_blob(d, &c->d_tc_blob[slot], &c->mlp_tc[slot], c->stream);
-  if (rc != DSMC_OK && rc != DSMC_ERR_UNSUPPORTED_SHAPE) return rc;
+  c->d_weights[slot] = wnew;
+  c->d_tc_blob[slot] = blob_new;
+  c->mlp[slot] = m;
+  c->mlp_tc[slot] = tc_new;
+  c->has_mlp[slot] = true;
   return DSMC_OK;
 }
 
@@ -208,11 +234,6 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
   for (size_t i = 0; i < (size_t)nE * nB; ++i)
     if (!isfinite(chi_host[i])) return DSMC_ERR_INVALID_ARG;  // a non-finite node would poison every pair near it
   CK(cudaSetDevice(c->device));
-  CK(cudaStreamSynchronize(c->stream));
-  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
-  c->table.tex = 0;
-  cudaFree(c->d_table);
-  c->d_table = nullptr;
   // device layout: the 2x2 nodes of every grid cell side by side, so a lookup is one 16-byte load
   const size_t nq = (size_t)(nE - 1) * (nB - 1);
   std::vector<float> quad(4 * nq);
@@ -224,8 +245,18 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
       q[2] = chi_host[(size_t)(iE + 1) * nB + iB];
       q[3] = chi_host[(size_t)(iE + 1) * nB + iB + 1];
     }
-  CK(cudaMalloc(&c->d_table, sizeof(float) * quad.size()));
-  CK(cudaMemcpy(c->d_table, quad.data(), sizeof(float) * quad.size(), cudaMemcpyHostToDevice));
+  // the new table is on the device before the old one is released: a failure leaves the context as it was
+  float *tnew = nullptr;
+  CK(cudaMalloc(&tnew, sizeof(float) * quad.size()));
+  if (cudaMemcpy(tnew, quad.data(), sizeof(float) * quad.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaFree(tnew);
+    return DSMC_ERR_CUDA;
+  }
+  CK(cudaStreamSynchronize(c->stream));
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
+  c->table.tex = 0;
+  cudaFree(c->d_table);
+  c->d_table = tnew;
   c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
   c->table.nE = nE;
   c->table.nB = nB;
@@ -381,21 +412,26 @@ int dsmc_chi_batch(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b
 
 static int ensure_host_staging(dsmc_ctx *c, int64_t n, int32_t K) {
   if (n <= c->host_cap_n && K <= c->host_cap_cells) return DSMC_OK;
-  cudaFree(c->h_cell);
-  for (int a = 0; a < 3; ++a) { cudaFree(c->h_v[a]); cudaFree(c->h_vs[a]); }
-  cudaFree(c->h_perm);
-  cudaFree(c->h_cell_start);
-  cudaFree(c->h_x[0]);
-  cudaFree(c->h_x[1]);
-  c->h_x[0] = c->h_x[1] = nullptr;
-  cudaFree(c->h_counts);
-  cudaFree(c->h_rem);
-  cudaFree(c->h_cap[0]);
-  cudaFree(c->h_cap[1]);
-  c->h_counts = nullptr;
-  c->h_rem = nullptr;
-  c->h_cap[0] = c->h_cap[1] = nullptr;
+  // every pointer is nulled as it is freed: a failure below leaves nothing dangling for dsmc_destroy or the next call
+  auto drop = [](auto *&p) {
+    cudaFree(p);
+    p = nullptr;
+  };
+  drop(c->h_cell);
+  for (int a = 0; a < 3; ++a) {
+    drop(c->h_v[a]);
+    drop(c->h_vs[a]);
+  }
+  drop(c->h_perm);
+  drop(c->h_cell_start);
+  drop(c->h_x[0]);
+  drop(c->h_x[1]);
+  drop(c->h_counts);
+  drop(c->h_rem);
+  drop(c->h_cap[0]);
+  drop(c->h_cap[1]);
   c->host_cap_n = 0;
+  c->host_cap_cells = 0;
   CK(cudaMalloc(&c->h_cell, sizeof(int32_t) * (size_t)n));
   for (int a = 0; a < 3; ++a) {
     CK(cudaMalloc(&c->h_v[a], sizeof(float) * (size_t)n));
@@ -418,23 +454,28 @@ int dsmc_build_chi_table_lj(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, 
     return DSMC_ERR_INVALID_ARG;
   CK(cudaSetDevice(c->device));
   CK(cudaStreamSynchronize(c->stream));
-  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
-  c->table.tex = 0;
-  cudaFree(c->d_table);
-  c->d_table = nullptr;
-  c->has_table = false;
   const size_t nq = (size_t)(nE - 1) * (nB - 1), nn = (size_t)nE * nB;
-  float *nodes = nullptr;
-  CK(cudaMalloc(&c->d_table, sizeof(float) * 4 * nq));
-  CK(cudaMalloc(&nodes, sizeof(float) * nn));
+  float *nodes = nullptr, *tnew = nullptr;
+  CK(cudaMalloc(&tnew, sizeof(float) * 4 * nq));
+  if (cudaMalloc(&nodes, sizeof(float) * nn) != cudaSuccess) {
+    cudaFree(tnew);
+    return DSMC_ERR_CUDA;
+  }
   int rc = launch_chi_table_lj(c, nE, nB, (double)lnE_min, (double)lnE_max, (double)b_max, (double)eps_over_k,
-                               (double)sigma, nodes, reinterpret_cast<float4 *>(c->d_table));
+                               (double)sigma, nodes, reinterpret_cast<float4 *>(tnew));
   if (rc == DSMC_OK && chi_out &&
       cudaMemcpyAsync(chi_out, nodes, sizeof(float) * nn, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
     rc = DSMC_ERR_CUDA;
   if (cudaStreamSynchronize(c->stream) != cudaSuccess) rc = DSMC_ERR_CUDA;
   cudaFree(nodes);
-  if (rc != DSMC_OK) return rc;
+  if (rc != DSMC_OK) {  // the installed table (if any) stays
+    cudaFree(tnew);
+    return rc;
+  }
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
+  c->table.tex = 0;
+  cudaFree(c->d_table);
+  c->d_table = tnew;
   c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
   c->table.nE = nE;
   c->table.nB = nB;
@@ -498,7 +539,10 @@ int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, con
   else
     rc = dsmc_collide_abinitio(c, n, K, c->h_cell_start, c->h_vs[0], c->h_vs[1], c->h_vs[2], nullptr, abi, seed,
                                step, nullptr);
-  if (rc != DSMC_OK) return rc;
+  if (rc != DSMC_OK) {
+    if (side) cudaStreamSynchronize(c->side_stream);  // the copies into the caller's buffers must not outlive the call
+    return rc;
+  }
   for (int a = 0; a < 3; ++a) CK(cudaMemcpyAsync(dst[a], c->h_vs[a], sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, s));
   if (side) {  // join the side stream before the final synchronisation
     CK(cudaEventRecord(c->ev_side, c->side_stream));

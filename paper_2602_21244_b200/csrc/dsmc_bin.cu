@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(kBinThreads) k_tile_hist(int64_t n, int32_t K,
       const int cc = c[k][r];
       const int64_t i = (int64_t)(t0 + k) * kBinTile + r * kBinThreads + tid;
       if (FIRST && i < n && (cc < 0 || cc >= K)) bad = true;
-      if (cc >= 0 && (!FIRST || cc < K)) atomicAdd(&h[k][bin_digit(cc, ps)], 1);
+      // later passes re-check the range too: when the first pass dropped bad ids, the tail of the ping-pong buffers
+      // behind the kept records is stale, and a stale id must never index outside the digit tables
+      if (cc >= 0 && cc < K) atomicAdd(&h[k][bin_digit(cc, ps)], 1);
     }
   }
   if (FIRST && bad) *status = DSMC_ERR_BAD_CELL_INDEX;
@@ -263,7 +265,7 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
   for (int r = 0; r < kBinItems; ++r) {
     const int j = jbase + r * 32;
     c[r] = j < cnt_tile ? scell[j] : -1;
-    if (FIRST && c[r] >= K) c[r] = -1;  // dropped (status already set by k_tile_hist)
+    if (c[r] >= K) c[r] = -1;  // dropped (status already set by k_tile_hist); later passes: stale tail, see k_tile_hist
   }
 #pragma unroll
   for (int r = 0; r < kBinItems; ++r) {

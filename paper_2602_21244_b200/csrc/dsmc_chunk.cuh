@@ -331,7 +331,7 @@ __device__ void chunk_pre_and_sort(const TM &T, const StepParams &P, CK &S, int 
     ci.ux = (float)((double)ci.ux + dx);  // pivot + mean(d)
     ci.uy = (float)((double)ci.uy + dy);
     ci.uz = (float)((double)ci.uz + dz);
-    ci.theta = (float)(s2 - N * (dx * dx + dy * dy + dz * dz));
+    ci.theta = (float)fmax(s2 - N * (dx * dx + dy * dy + dz * dz), 0.0);  // a cold cell may round below zero
   }
   if (CK::REPLACE) {  // pairs are drawn, not matched: nothing to sort
     T.sync();

@@ -97,6 +97,33 @@ def test_bin_reports_bad_cell_index_and_large_cells(dsmc):
     assert ctx2.sync_status() == dsmc.ERR_CELL_TOO_LARGE
 
 
+def test_bin_bad_cell_index_multi_pass_is_memory_safe(dsmc):
+    """Bad ids with K > 512 (two radix passes): the first pass drops them, so the later pass reads a stale tail of the
+    ping-pong buffers.  Run after another context of the same process has used and freed its workspace (stale, valid-
+    looking data in recycled memory): the call must report the error and leave the CUDA context healthy."""
+    rng = np.random.default_rng(21)
+    warm = wl.mach10_cylinder(nx=80, ny=40, n_total=300_000)
+    ctx0 = dsmc.Context(warm.n, warm.n_cells)
+    binned(dsmc, ctx0, warm)
+    ctx0.close()
+    K = 3000
+    counts = rng.integers(50, 150, K)
+    pop = wl._populate("bad_multi", counts, np.full(K, 300.0), np.zeros(K), np.zeros(K), 21)
+    cell = pop.cell.copy()
+    bad = rng.choice(pop.n, 5000, replace=False)
+    cell[bad[:2500]] = K + rng.integers(0, 1 << 20, 2500)
+    cell[bad[2500:]] = -1 - rng.integers(0, 1000, 2500)
+    ctx = dsmc.Context(pop.n, K)
+    ctx.bin(dev(cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), K)
+    assert ctx.sync_status() == dsmc.ERR_BAD_CELL_INDEX
+    # the context still works: a clean input sorts bit-exactly afterwards
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    rc, perm_o, cs_o = oracle.bin_particles(pop.cell, K)
+    np.testing.assert_array_equal(cs.cpu().numpy(), cs_o)
+    np.testing.assert_array_equal(perm.cpu().numpy(), perm_o)
+    ctx.close()
+
+
 # --------------------------------------------------------------------------------------- a2 / a8
 def test_cell_moments_and_standalone_match(dsmc):
     pop = wl.mach10_cylinder(nx=40, ny=20, n_total=150_000)
