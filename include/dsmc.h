@@ -36,7 +36,10 @@
  * stream 1 = (U_b, U_eps) of pair slot s (words 2(s&1), 2(s&1)+1 of block s>>1), stream 2 = Box-Muller
  * normals of pair slot s, stream 3 = U_acc of pair slot s (word s&3 of block s>>2, drawn only with
  * DSMC_F_ACCEPT); cell = local cell index + cell_base;
- * u = ((x>>9)+0.5) 2^-23.  Results therefore depend only on (seed, step, cell, slot).
+ * u = ((x>>9)+0.5) 2^-23.  Results therefore depend only on (seed, step, cell, slot): runs are bit-reproducible and a
+ * run sharded by cell ranges is bit-identical to the unsharded one.  One exception: with DSMC_F_PAIR_REPLACE the
+ * velocity changes of a particle that sits in several pairs are added with shared-memory floating-point atomics,
+ * whose order is not fixed; those results are reproducible to rounding only (a few ulp of the change).
  */
 #ifndef DSMC_H
 #define DSMC_H

@@ -32,15 +32,20 @@ POT_LJ, POT_HARD_SPHERE, POT_INV_R, POT_INV_R2 = 0, 1, 2, 3
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc -O2 (no fast-math).  Building the checker is not using it."""
-    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < max(
+    """Compile the oracle with gcc -O2 (no fast-math).  Building the checker is not using it.
+    ORACLE_SANITIZE=1 builds (and loads) an AddressSanitizer + UBSan copy instead; run the tests with
+    LD_PRELOAD=$(gcc -print-file-name=libasan.so) (profiles/r02_oracle_asan_ubsan.md)."""
+    san = os.environ.get("ORACLE_SANITIZE") == "1"
+    lib_path = _LIB.replace(".so", "_san.so") if san else _LIB
+    stale = (not os.path.exists(lib_path)) or os.path.getmtime(lib_path) < max(
         os.path.getmtime(_SRC), os.path.getmtime(_HDR))
     if force or stale:
-        tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-Wall", "-o", tmp,
-                               _SRC, "-lm"])
-        os.replace(tmp, _LIB)
-    return _LIB
+        tmp = lib_path + ".tmp.%d" % os.getpid()
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                 "-fno-omit-frame-pointer"] if san else ["-O2"]
+        subprocess.check_call(["gcc", *flags, "-std=c99", "-fPIC", "-shared", "-Wall", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, lib_path)
+    return lib_path
 
 
 class _Mlp(C.Structure):
