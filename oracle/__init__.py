@@ -226,6 +226,16 @@ def pair_uniforms(seed, step, cell, s):
     return np.array(list(u))
 
 
+def pair_uniforms_batch(seed, step, cells, slots):
+    """(U_acc, U_b, U_eps) of many (cell, pair slot): array [n, 3]."""
+    cells = np.ascontiguousarray(cells, np.uint32)
+    slots = np.ascontiguousarray(slots, np.uint32)
+    u = np.empty((cells.shape[0], 3), np.float64)
+    lib().orc_pair_uniforms_batch(C.c_uint64(seed), C.c_uint32(step), C.c_int64(cells.shape[0]),
+                                  _p(cells, C.c_uint32), _p(slots, C.c_uint32), _p(u, C.c_double))
+    return u
+
+
 def pair_draw(seed, step, cell, s, N):
     i, j = C.c_int32(0), C.c_int32(0)
     lib().orc_pair_draw(C.c_uint64(seed), C.c_uint32(step), C.c_uint32(cell), C.c_uint32(s), C.c_int32(N), C.byref(i), C.byref(j))
@@ -272,6 +282,17 @@ def pairing(seed, step, cell, N, M_req=-1):
     M = lib().orc_pairing(C.c_uint64(seed), C.c_uint32(step), C.c_uint32(cell), C.c_int32(N),
                           C.c_int32(M_req), _p(pi, C.c_int32))
     return int(M), pi[:N]
+
+
+def pairing_all(seed, step, cell_start, cell_base=0, M_req=-1):
+    """The matching of every cell (pairing alone, integer work): (pair_i, pair_j) in the layout of the pair dump."""
+    cs = _i32(cell_start)
+    n = int(cs[-1])
+    pi = np.empty(max(n, 1), np.int32)
+    pj = np.empty(max(n, 1), np.int32)
+    lib().orc_pairing_all(C.c_uint64(seed), C.c_uint32(step), C.c_int32(cs.shape[0] - 1), _p(cs, C.c_int32),
+                          C.c_uint32(cell_base), C.c_int32(M_req), _p(pi, C.c_int32), _p(pj, C.c_int32))
+    return pi[:n], pj[:n]
 
 
 def mlp_forward(net: Mlp, x):
@@ -403,6 +424,12 @@ def rmin(pot: Potential, E, b):
 def chi_exact(pot: Potential, E, b, n_panels=16):
     p = pot.c()
     return lib().orc_chi_exact(C.byref(p), C.c_double(E), C.c_double(b), C.c_int32(n_panels))
+
+
+def cap_chi(c):
+    f = lib().orc_cap_chi
+    f.restype = C.c_double
+    return float(f(C.c_double(c)))
 
 
 def build_chi_table(pot: Potential, nE, nB, lnE_min=float(np.log(5.0)),

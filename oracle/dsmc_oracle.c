@@ -65,6 +65,12 @@ void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, 
   u[2] = orc_u01(r[2u * (s & 1u) + 1u]);
 }
 
+/* the same for n (cell, slot) pairs: u[3 i ..] = uniforms of (cell[i], s[i]).  A loop over the function above (test
+ * marshalling only: one call instead of n). */
+void orc_pair_uniforms_batch(uint64_t seed, uint32_t step, int64_t n, const uint32_t *cell, const uint32_t *s, double *u) {
+  for (int64_t i = 0; i < n; ++i) orc_pair_uniforms(seed, step, cell[i], s[i], u + 3 * i);
+}
+
 /* stream 4: with-replacement pair draw ("two particles i, j in C_k are selected uniformly at random") */
 void orc_pair_draw(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, int32_t N, int32_t *i, int32_t *j) {
   uint32_t r[4];
@@ -173,6 +179,24 @@ int32_t orc_pairing(uint64_t seed, uint32_t step, uint32_t cell, int32_t N, int3
   int32_t M = N / 2; /* odd N: last element of pi is a spectator (Q10) */
   if (M_req >= 0 && M_req < M) M = M_req;
   return M;
+}
+
+/* orc_pairing for every cell of a population (a loop over the function above; test marshalling): pair slot s of
+ * cell k at index cell_start[k] + s of pair_i / pair_j (slots relative to the cell's first slot), -1 elsewhere. */
+void orc_pairing_all(uint64_t seed, uint32_t step, int32_t K, const int32_t *cell_start, uint32_t cell_base,
+                     int32_t M_req, int32_t *pair_i, int32_t *pair_j) {
+  for (int32_t k = 0; k < K; ++k) {
+    const int32_t gs = cell_start[k], N = cell_start[k + 1] - gs;
+    for (int32_t q = 0; q < N; ++q) pair_i[gs + q] = pair_j[gs + q] = -1;
+    if (N < 2) continue;
+    int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)N);
+    const int32_t M = orc_pairing(seed, step, (uint32_t)k + cell_base, N, M_req, pi);
+    for (int32_t s = 0; s < M; ++s) {
+      pair_i[gs + s] = pi[2 * s];
+      pair_j[gs + s] = pi[2 * s + 1];
+    }
+    free(pi);
+  }
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -608,6 +632,10 @@ double orc_chi_exact(const orc_potential *pot, double E, double b, int32_t n_pan
   return PI - 4.0 * beta * sum;
 }
 
+/* Q23: a node that falls on the orbiting singularity (chi -> infinity: the pair spirals) is capped at 32 revolutions so
+ * that the fp32 table stays finite; any such angle is as good as another.  Written so that NaN is capped too. */
+double orc_cap_chi(double c) { return (c <= 64.0 * PI) ? c : 64.0 * PI; }
+
 void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, double lnE_min,
                          double lnE_max, double b_max, int32_t n_panels, float *chi) {
   for (int32_t iE = 0; iE < nE; ++iE) {
@@ -615,10 +643,7 @@ void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, doubl
     double E = ORC_KB * exp(lnE);
     for (int32_t iB = 0; iB < nB; ++iB) {
       double b = b_max * (double)iB / (double)(nB - 1);
-      double c = fabs(orc_chi_exact(pot, E, b, n_panels)); /* Q14 */
-      /* Q23: a node that falls on the orbiting singularity (chi -> infinity: the pair spirals) is capped at 32
-       * revolutions so that the fp32 table stays finite; any such angle is as good as another */
-      if (!(c <= 64.0 * PI)) c = 64.0 * PI;
+      double c = orc_cap_chi(fabs(orc_chi_exact(pot, E, b, n_panels))); /* Q14, Q23 */
       chi[(size_t)iE * nB + iB] = (float)c;
     }
   }

@@ -99,6 +99,7 @@ void orc_pair_draw(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, int3
 /* per-pair uniforms: U_acc (stream 3, word s&3 of block s>>2), U_b, U_eps (stream 1, words 2(s&1), 2(s&1)+1
  * of block s>>1) */
 void orc_pair_uniforms(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double u[3]);
+void orc_pair_uniforms_batch(uint64_t seed, uint32_t step, int64_t n, const uint32_t *cell, const uint32_t *s, double *u);
 /* per-pair latent xi ~ N(0, I3) by Box-Muller (stream 2) */
 void orc_pair_normals(uint64_t seed, uint32_t step, uint32_t cell, uint32_t s, double xi[3]);
 
@@ -115,6 +116,8 @@ void orc_cell_state(int64_t N, const double *vx, const double *vy, const double 
 /* ---- a3: disjoint random matching (Q7). pi[N] = slots sorted by (key,slot). returns M ---- */
 int32_t orc_pairing(uint64_t seed, uint32_t step, uint32_t cell, int32_t N, int32_t M_req,
                     int32_t *pi);
+void orc_pairing_all(uint64_t seed, uint32_t step, int32_t K, const int32_t *cell_start, uint32_t cell_base,
+                     int32_t M_req, int32_t *pair_i, int32_t *pair_j);
 
 /* ---- operators ---- */
 void orc_mlp_forward(const orc_mlp *net, const double *x, double *out);
@@ -152,6 +155,7 @@ double orc_rmin(const orc_potential *pot, double E, double b);
 /* signed chi by composite Gauss-Legendre (n_panels x 64 points) after u=r_min/r, u=1-s^2 */
 double orc_chi_exact(const orc_potential *pot, double E, double b, int32_t n_panels);
 /* fills chi[nE*nB] with |chi| rounded to fp32 (Q14) */
+double orc_cap_chi(double c); /* Q23: min(c, 64 pi), NaN -> 64 pi */
 void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, double lnE_min,
                          double lnE_max, double b_max, int32_t n_panels, float *chi);
 

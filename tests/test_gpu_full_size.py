@@ -85,8 +85,15 @@ def test_cfg5_full_size(dsmc, chi):
     flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi == "mlp_tc" else 0)
     cm = 0 if chi == "table" else 1
     prm = dsmc.AbinitioParams(chi_mode=cm, flags=flags)
-    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=4, step=7)
+    dump = dsmc.PairDump(pop.n, "cuda", gprime=False)
+    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=4, step=7, dump=dump)
     ctx.check()
+    # ---- a3 at full size: every one of the 9 993 782 pairs against the oracle's pairing run alone (integer work)
+    want_i, want_j = oracle.pairing_all(4, 7, cs_h)
+    assert int((want_i >= 0).sum()) == 9_993_782
+    np.testing.assert_array_equal(dump.pair_i.cpu().numpy(), want_i)
+    np.testing.assert_array_equal(dump.pair_j.cpu().numpy(), want_j)
+    del dump
     v_out = [t.cpu().numpy() for t in (vx_s, vy_s, vz_s)]
     post = _segment_moments(cs_h, *v_out)
     N = np.diff(cs_h)

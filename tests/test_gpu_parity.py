@@ -284,6 +284,17 @@ def _table_slope(tab, lnE, bt):
     return c.max(axis=0) - c.min(axis=0)
 
 
+def _q25_bound(tab, cs_h, v_in, ref, seed, step):
+    """Q25 on every pair, from the oracle's side alone: |chi_gpu - chi_oracle| <= 1e-5 max(|chi|, 1) + 2e-4 (max - min of
+    the four table nodes around the query) + 1e-6.  Returns (indices of the pair slots, bound, pair speed g)."""
+    idx = np.flatnonzero(ref.pair_i >= 0)
+    k = np.searchsorted(cs_h, idx, side="right") - 1
+    g2 = sum((a[cs_h[k] + ref.pair_i[idx]] - a[cs_h[k] + ref.pair_j[idx]]) ** 2 for a in v_in)
+    bt = np.sqrt(oracle.pair_uniforms_batch(seed, step, k, idx - cs_h[k])[:, 1])
+    sl = _table_slope(tab, np.log(np.maximum(M * g2 / (4 * KB), 1e-300)), bt)
+    return idx, 1e-5 * np.maximum(np.abs(ref.aux[idx]), 1) + 2e-4 * sl + 1e-6, np.sqrt(g2)
+
+
 @pytest.mark.parametrize("mode", ["table", "mlp"])
 def test_collide_abinitio_fp32(dsmc, mode):
     pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
@@ -313,13 +324,12 @@ def test_collide_abinitio_fp32(dsmc, mode):
             dchi = np.abs(chi_g - ref.aux)
             assert (dchi[idx] > 1e-5 * np.maximum(np.abs(ref.aux[idx]), 1)).mean() < 0.01
             assert dchi[idx].max() < 2e-3
-            sub = idx[:: max(1, len(idx) // 1500)]  # slope-aware bound on a sample (python loop)
-            k = np.searchsorted(cs_h, sub, side="right") - 1
-            g2 = sum((a[cs_h[k] + ref.pair_i[sub]] - a[cs_h[k] + ref.pair_j[sub]]) ** 2 for a in v_in)
-            bt = np.sqrt([oracle.pair_uniforms(4, step, int(kk), int(i - cs_h[kk]))[1] for kk, i in zip(k, sub)])
-            sl = _table_slope(tab, np.log(M * g2 / (4 * KB)), bt)
-            assert np.all(dchi[sub] <= 1e-5 * np.maximum(np.abs(ref.aux[sub]), 1) + 2e-4 * sl + 1e-6)
-            slope = 1.01 * dchi  # a lookup difference rotates g' by exactly that angle
+            # the slope-aware bound of Q25 on EVERY pair, from the oracle's inputs alone (table nodes around the
+            # query, pair uniforms): it bounds chi, and with it the angle by which g' may differ
+            idx, bound, _ = _q25_bound(tab, cs_h, v_in, ref, 4, step)
+            assert np.all(dchi[idx] <= bound), "chi outside the Q25 bound: %d pairs" % (dchi[idx] > bound).sum()
+            slope = np.zeros_like(dchi)
+            slope[idx] = bound  # a lookup difference rotates g' by exactly that angle
         else:
             assert np.abs(chi_g[sel] - ref.aux[sel]).max() <= 2e-5 * np.maximum(np.abs(ref.aux[sel]), 1).max()
         _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5 if mode == "table" else 3e-5, 1e-6, slope=slope)
@@ -642,16 +652,26 @@ def test_collide_abinitio_with_replacement(dsmc, mode, match):
     np.testing.assert_array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
     sel = ref.pair_i >= 0
     dchi = np.abs(dump.aux.cpu().numpy().astype(np.float64) - ref.aux)
-    slope = 1.01 * dchi if mode == "table" else None
-    _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5 if mode == "table" else 3e-5, 1e-6, slope=slope)
+    slope = None
     N = np.diff(cs_h)
     pre = oracle.cell_moments(cs_h, *v_in)
     got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
     ok = N >= 2
     scale = np.repeat(np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1)), N)
-    tol_v = 1e-5 + (2.1 * dchi[sel].max() if mode == "table" else 1e-4)
+    allow_v = np.full(pop.n, 1e-5 if mode == "table" else 1e-4)
+    if mode == "table":  # Q25 on every pair (oracle-side bound), carried to g' and to the particles of the pair
+        idx, bound, gn = _q25_bound(tab, cs_h, v_in, ref, 6, 1)
+        assert np.all(dchi[idx] <= bound), "chi outside the Q25 bound: %d pairs" % (dchi[idx] > bound).sum()
+        slope = np.zeros_like(dchi)
+        slope[idx] = bound
+        # a particle moves by (g' - g) / 2 for every pair it sits in: its allowance adds up over those pairs
+        kk = np.searchsorted(cs_h, idx, side="right") - 1
+        dv = 0.5 * gn * (1e-5 + bound)
+        for side in (ref.pair_i, ref.pair_j):
+            np.add.at(allow_v, cs_h[kk] + side[idx], 1.05 * dv / scale[cs_h[kk] + side[idx]])
+    _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5 if mode == "table" else 3e-5, 1e-6, slope=slope)
     for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
-        assert (np.abs(a.cpu().numpy().astype(np.float64) - want) / scale).max() < tol_v
+        assert np.all(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale < allow_v)
     assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
     if match:
         assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6

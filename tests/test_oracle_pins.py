@@ -741,3 +741,20 @@ def test_with_replacement_vhs_nn_batch_semantics():
     post2 = oracle.cell_moments(cs, r2.vx, r2.vy, r2.vz)
     np.testing.assert_allclose(post2[:, 3], pre[:, 3], rtol=1e-12)
     np.testing.assert_allclose(post2[:, :3], pre[:, :3], atol=1e-8)
+
+
+def test_table_builder_caps_non_finite_nodes_at_64_pi():
+    """Q23: a node on the orbiting singularity has no finite deflection angle; the table builder stores 64 pi (32
+    revolutions) there and leaves every smaller angle alone.  The quadrature itself never returns a non-finite value on
+    the grids used here, so the cap is pinned at its own seam (the function orc_build_chi_table applies to every node):
+    +inf, NaN and anything above 64 pi give 64 pi exactly, everything else passes unchanged; and a real LJ table stays
+    far below the cap."""
+    cap = 64.0 * np.pi
+    assert oracle.cap_chi(float("inf")) == cap
+    assert oracle.cap_chi(float("nan")) == cap  # a comparison written as c > cap would let NaN through
+    assert oracle.cap_chi(cap * 1.0000001) == cap and oracle.cap_chi(1e300) == cap
+    for c in (0.0, 1e-12, np.pi, 17.25, cap):
+        assert oracle.cap_chi(c) == c
+    assert np.isfinite(np.float32(cap))
+    good = oracle.build_chi_table(oracle.lj_argon(), 8, 9, n_panels=1)
+    assert np.all(np.isfinite(good.chi)) and good.chi.max() < 4 * np.pi and np.all(good.chi >= 0)
