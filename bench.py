@@ -54,13 +54,19 @@ def peaks():
     return 6650.0, 1590.0, 1400.0, "fallback"
 
 
+TRAFFIC_FILE = "profiles/r02_kernel_traffic.json"
+
+
 def measured_traffic(chi):
     """dram__bytes_read.sum + dram__bytes_write.sum of the fused collide kernel, per launch, from the committed
-    `ncu --set full` capture (profiles/r01_kernel_traffic.json); None if that file has no entry."""
-    p = os.path.join(ROOT, "profiles", "r01_kernel_traffic.json")
+    `ncu --set full` capture named in TRAFFIC_FILE (not measured in this run: ncu cannot run inside a timed bench);
+    returns (bytes or None, where the number comes from)."""
+    p = os.path.join(ROOT, TRAFFIC_FILE)
     if os.path.exists(p):
-        return json.load(open(p)).get(chi, {}).get("dram_bytes_per_launch")
-    return None
+        e = json.load(open(p)).get(chi, {})
+        if e.get("dram_bytes_per_launch") is not None:
+            return e["dram_bytes_per_launch"], "%s: %s" % (TRAFFIC_FILE, e.get("capture", "ncu --set full capture"))
+    return None, "no capture for this variant"
 
 
 def population(args, rank=0):
@@ -75,7 +81,7 @@ def config_dict(args, pop, pairs):
                         "by %s + rotation + moment matching; step = dsmc_bin + fused collide" % (
                             NX if args.scale == 1.0 else -1, NY if args.scale == 1.0 else -1, pop.n, pairs, args.chi),
             "chi_mode": args.chi, "n_particles": pop.n, "n_cells": pop.n_cells, "pairs_per_step": pairs,
-            "table": "%dx%d fp32 LJ 12-6 (oracle quadrature)" % (TABLE_N, TABLE_N),
+            "table": "%dx%d fp32 LJ 12-6 (quadrature; device-built in the product arm, oracle-built in the reference arm)" % (TABLE_N, TABLE_N),
             "l2_policy": "inputs larger than L2 (%.0f MB touched per step)" % (pop.n * 48 / 1e6),
             "scale": args.scale}
 
@@ -119,6 +125,64 @@ def time_oracle(pop, chi, table, mlp_w, steps, warmup, target_pairs=150_000):
     t = float(np.mean(times))
     return pairs / t, t, pairs, "cells [%d,%d) of the cfg5 population: %d particles, %d pairs, bin + fused ab initio " \
                                "(%s) step, fp64 single thread" % (k0, k1, int(keep.sum()), pairs, chi)
+
+
+_MP = {}
+
+
+def _oracle_worker(args):
+    """One process of the all-cores oracle run: bin + fused step on its own contiguous cell range.  cell_base keeps
+    the Philox counters global, so the union of the workers' results is the single-thread result (cells are
+    independent)."""
+    import oracle
+    k0, k1, it = args
+    pop, chi, table, mlp_w = _MP["pop"], _MP["chi"], _MP["table"], _MP["mlp_w"]
+    lo, hi = int(_MP["cum"][k0]), int(_MP["cum"][k1])
+    idx = _MP["order"][lo:hi]
+    cell = (pop.cell[idx] - k0).astype(np.int32)
+    otab = oracle.ChiTable(table.chi, table.lnE_min, table.lnE_max)
+    net = oracle.Mlp(mlp_w[0], mlp_w[1], oracle.ACT_SILU)
+    prm = oracle.AbinitioParams(chi_mode=0 if chi == "table" else 1, cell_base=k0)
+    rc, perm, cs = oracle.bin_particles(cell, k1 - k0)
+    v = [a[idx][perm].astype(np.float64) for a in (pop.vx, pop.vy, pop.vz)]
+    oracle.collide_abinitio(cs, *v, prm, 4, it, net=net, table=otab)
+    return hi - lo
+
+
+def time_oracle_all_cores(pop, chi, table, mlp_w, target_pairs_per_core):
+    """The same oracle on every host core: N processes over contiguous cell ranges of one sample.
+    Returns pairs/s, seconds, pairs, cores, description."""
+    import multiprocessing as mp
+    cores = len(os.sched_getaffinity(0))
+    k0, k1, keep = oracle_sample(pop, chi, target_pairs_per_core * cores)
+    order = np.argsort(pop.cell, kind="stable")
+    cum = np.concatenate([[0], np.cumsum(pop.counts)])
+    half = np.cumsum(pop.counts[k0:k1] // 2)
+    cuts = [k0] + [k0 + int(np.searchsorted(half, half[-1] * (w + 1) / cores)) for w in range(cores - 1)] + [k1]
+    cuts = sorted(set(min(max(c, k0), k1) for c in cuts))
+    _MP.update(pop=pop, chi=chi, table=table, mlp_w=mlp_w, order=order, cum=cum)
+    pairs = int((pop.counts[k0:k1] // 2).sum())
+    ctx = mp.get_context("fork")
+    with ctx.Pool(len(cuts) - 1) as pool:
+        pool.map(_oracle_worker, [(a, b, 0) for a, b in zip(cuts[:-1], cuts[1:])])  # warm-up: pages, library
+        t0 = time.perf_counter()
+        pool.map(_oracle_worker, [(a, b, 1) for a, b in zip(cuts[:-1], cuts[1:])])
+        t = time.perf_counter() - t0
+    return pairs / t, t, pairs, len(cuts) - 1, "cells [%d,%d) of the cfg5 population split into %d contiguous ranges, one " \
+        "process each: %d pairs, bin + fused ab initio (%s) step, fp64" % (k0, k1, len(cuts) - 1, pairs, chi)
+
+
+def host_info():
+    model = "unknown"
+    try:
+        for l in open("/proc/cpuinfo"):
+            if l.startswith("model name"):
+                model = l.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count(), "usable_cores": len(os.sched_getaffinity(0)), "cpu_model": model,
+            "oracle_build": "gcc -O2 -std=c99 (no fast-math), oracle/dsmc_oracle.c"}
 
 
 def build_operators(chi_needed=True):
@@ -232,10 +296,16 @@ def run_b200(args):
     hbm_peak, tc_burst, tc_sust, peak_src = peaks()
 
     pop = population(args, rank)       # weak scaling: every rank owns one full cfg-5 population
-    table, mlp_w, t_table = build_operators()
+    # the product arm builds its chi table with the product (dsmc_build_chi_table_lj: the LJ quadrature on the
+    # device); oracle/ is touched only by the cpu_baseline leg at the end
+    from paper_2602_21244_b200 import workloads as wl
+    mlp_w = wl.random_mlp(3, [2, 128, 128, 1])
     pairs = pop.pairs_per_step(-1)
     ctx = dsmc.Context(pop.n, pop.n_cells, device=local)
-    ctx.set_chi_table(table.chi, table.lnE_min, table.lnE_max)
+    t0 = time.perf_counter()
+    ctx.build_chi_table_lj(TABLE_N, TABLE_N, b_max=B_MAX)
+    torch.cuda.synchronize()
+    t_table = time.perf_counter() - t0
     ctx.set_mlp(1, mlp_w[0], mlp_w[1], dsmc.ACT_SILU)
     dev = torch.device("cuda", local)
     cell = torch.from_numpy(pop.cell).to(dev)
@@ -483,8 +553,9 @@ def run_b200(args):
         clk = (sampler.summary().get("sm_mhz") or 1965.0) * 1e6
         t_xu = pairs * 256 / (16.0 * 148 * clk)
         roof["xu_bound"] = {"ms": t_xu * 1e3, "frac": t_xu / (coll_ms * 1e-3)}
-    roof["traffic"] = measured_traffic("table" if args.chi == "table" else args.chi)
-    roof["kernel"] = "fused collide (k_collide_*)"
+    roof["traffic"], roof["traffic_source"] = measured_traffic("table" if args.chi == "table" else args.chi)
+    roof["kernel"] = {"table": "fused collide: dsmc::k_cells (+ k_cell_lists, k_cells_big)",
+                      "mlp_tc": "fused collide: dsmc::k_cells_mlp (+ k_cell_lists)"}.get(args.chi, "fused collide: dsmc::k_collide<fp32 MLP>")
     roof["kernel_ms"] = coll_ms
     roof["peak_source"] = peak_src
     roof["algorithmic"] = {"bytes_per_launch": bytes_alg, "flops_per_launch": flops_alg}
@@ -501,9 +572,16 @@ def run_b200(args):
             "table_build_s": t_table}
     if not args.no_cpu_baseline and world >= 1:
         chi = "table" if args.chi == "table" else "mlp"
+        table, _, _ = build_operators()
         v, t, sp, sample = time_oracle(pop, chi, table, mlp_w, steps=3, warmup=1,
                                        target_pairs=4_000_000 if chi == "table" else 300_000)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                                "host": host_info()}
+        try:  # the same oracle on every host core (it is a baseline, not the target)
+            va, ta, pa, ca, sa = time_oracle_all_cores(pop, chi, table, mlp_w, 400_000 if chi == "table" else 30_000)
+            line["cpu_baseline"]["all_cores"] = {"value": va, "unit": UNIT, "cores": ca, "seconds": ta, "sample": sa}
+        except Exception as e:  # a host without fork / affinity: the single-thread figure stands
+            line["cpu_baseline"]["all_cores"] = {"unavailable": repr(e)[:200]}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
