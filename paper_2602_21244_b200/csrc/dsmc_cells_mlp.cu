@@ -204,14 +204,51 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
     // Fixed order, blocking waits (as in k_chi_batch_tc): round r = tiles 2 r (slot 0) and 2 r + 1 (slot 1).
     const int aw = warp - NTW;
     uint32_t phe[2] = {0u, 0u}, pho[2] = {0u, 0u};
+    bool pend1 = false;  // slot 1 of the previous round is still to be delivered
+    // rows 32 aw .. 32 aw + 31 of the layer-3 output of tile (slot s2, round rr) -> the feeding warp (aw < 4)
+    auto deliver = [&](int s2, int rr) {
+      tc::mbar_wait(pipe.full_o + s2, pho[s2]);
+      pho[s2] ^= 1u;
+      tc::fence_after();
+      uint32_t v[4];
+      tc::tmem_ld4(pipe.tmem + (((uint32_t)(aw * 32)) << 16) + s2 * SH::SLOT_COLS + SH::COL_OUT, v);
+      tc::wait_ld();
+      tc::fence_before();
+      float *dest = *reinterpret_cast<float *volatile *>(&ctl->dest[s2][rr & 3]);
+      const int f = cm_ld_volatile(&ctl->feeder[s2][rr & 3]);
+      dest[aw * 32 + lane] = __uint_as_float(v[0]);
+      __syncwarp();
+      if (lane == 0) {
+        __threadfence_block();
+        cm_arrive(&ctl->out_bar[s2]);  // the output columns may be overwritten (layer 3 of the next round)
+        cm_arrive(&ctl->done_bar[f]);  // z is in the feeding warp's shared memory
+      }
+    };
+    // Order of a round: act(0, L1), [deliver slot 1 of the previous round], act(1, L1), act(0, L2), act(1, L2),
+    // deliver slot 0.  Slot 1's layer 3 is issued only when act(1, L2) ends, so its delivery waits until the next
+    // activation is done rather than hold up four of the activation warps.
     for (int r = 0;; ++r) {
 #pragma unroll
       for (int layer = 0; layer < 2; ++layer) {
 #pragma unroll
         for (int s2 = 0; s2 < 2; ++s2) {
-          tc::mbar_wait(pipe.full_e + s2, phe[s2]);
+          if (layer == 0 && s2 == 0 && aw < 4 && r >= 1) {
+            // the next round normally stands ready (its layer 1 was issued early); if it does not, slot 1 of the last
+            // round is delivered while waiting: a submitted tile never depends on further tiles being fed
+            while (!cm_test(pipe.full_e + 0, phe[0])) {
+              if (pend1 && cm_test(pipe.full_o + 1, pho[1])) {
+                deliver(1, r - 1);
+                pend1 = false;
+              }
+            }
+          } else {
+            tc::mbar_wait(pipe.full_e + s2, phe[s2]);
+          }
           phe[s2] ^= 1u;
-          if (layer == 0 && s2 == 0 && r == cm_ld_volatile(&ctl->poison)) goto server_done;
+          if (layer == 0 && s2 == 0 && r == cm_ld_volatile(&ctl->poison)) {
+            if (aw < 4 && pend1) deliver(1, r - 1);
+            goto server_done;
+          }
           if (layer == 0 && aw == 0 && lane == 0) {  // the slot's layer-1 operand buffer may be rewritten
             *reinterpret_cast<volatile int *>(&ctl->op_done[s2]) = r + 1;
             __threadfence_block();
@@ -219,28 +256,15 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
           }
           __syncwarp();
           pipe.template act_body<NA / 4>(net.act, s2, aw);
-        }
-      }
-      if (aw < 4) {  // rows 32 aw .. 32 aw + 31 of both tiles' layer-3 outputs -> the feeding warps
-#pragma unroll
-        for (int s2 = 0; s2 < 2; ++s2) {
-          tc::mbar_wait(pipe.full_o + s2, pho[s2]);
-          pho[s2] ^= 1u;
-          tc::fence_after();
-          uint32_t v[4];
-          tc::tmem_ld4(pipe.tmem + (((uint32_t)(aw * 32)) << 16) + s2 * SH::SLOT_COLS + SH::COL_OUT, v);
-          tc::wait_ld();
-          tc::fence_before();
-          float *dest = *reinterpret_cast<float *volatile *>(&ctl->dest[s2][r & 3]);
-          const int f = cm_ld_volatile(&ctl->feeder[s2][r & 3]);
-          dest[aw * 32 + lane] = __uint_as_float(v[0]);
-          __syncwarp();
-          if (lane == 0) {
-            __threadfence_block();
-            cm_arrive(&ctl->out_bar[s2]);  // the output columns may be overwritten (layer 3 of the next round)
-            cm_arrive(&ctl->done_bar[f]);  // z is in the feeding warp's shared memory
+          if (layer == 0 && s2 == 0 && aw < 4 && pend1) {
+            deliver(1, r - 1);
+            pend1 = false;
           }
         }
+      }
+      if (aw < 4) {
+        deliver(0, r);
+        pend1 = true;
       }
     }
   } else {
@@ -296,19 +320,25 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
           pa[s2] ^= 1u;
           pipe.issue_layer2(s2);
         }
+        bool stop = false;
 #pragma unroll
         for (int s2 = 0; s2 < 2; ++s2) {
           tc::mbar_wait(pipe.a_ready + s2, pa[s2]);
           pa[s2] ^= 1u;
           if (r >= 1) tc::mbar_wait(&ctl->out_bar[s2], (uint32_t)(r - 1) & 1u);  // previous round delivered
           pipe.issue_layer3(s2);
+          // slot 0's next layer 1 goes out ahead of slot 1's layer 3 when its rows are there (the usual case): the
+          // activation warps then find work the moment they finish act(1, L2).  Otherwise it waits until both layer 3s
+          // are out, so that every submitted tile is delivered whatever the team warps do next.
+          if (s2 == (early0 ? 0 : 1)) {
+            stop = !early0 && rows(0, r + 1) == 2;
+            if (stop) {
+              *reinterpret_cast<volatile int *>(&ctl->poison) = r + 1;
+              __threadfence_block();
+            }
+            pipe.issue_layer1(0, (r + 1) & 1, false);
+          }
         }
-        const bool stop = !early0 && rows(0, r + 1) == 2;
-        if (stop) {
-          *reinterpret_cast<volatile int *>(&ctl->poison) = r + 1;
-          __threadfence_block();
-        }
-        pipe.issue_layer1(0, (r + 1) & 1, false);
         if (stop) break;
         if (!early1) rows(1, r + 1);
         pipe.issue_layer1(1, (r + 1) & 1, false);
