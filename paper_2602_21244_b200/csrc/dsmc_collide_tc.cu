@@ -6,7 +6,7 @@
 //   k_collide_tc     a2-a9 with the VHS-NN operator (split-BF16 operands): persistent fused step; one CTA pulls
 //                    chunks (dsmc_chunk.cuh) from a work counter, keeps the packed weights resident, and feeds
 //                    the chunk's pairs through the tile engine 128 at a time
-//   (the ab initio chi-MLP fused step is the warp-specialised k_collide_pipe, dsmc_collide_pipe.cu)
+//   (the ab initio chi-MLP fused step is k_cells_mlp: cell teams + a tcgen05 MLP server, dsmc_cells_mlp.cu)
 #include <algorithm>
 #include <vector>
 

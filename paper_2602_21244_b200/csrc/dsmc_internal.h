@@ -143,7 +143,6 @@ int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
 int launch_collide_cells(dsmc_ctx *c, const StepParams &p);
 int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
-int launch_collide_pipe(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // warp-specialised, op 2
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
                      float lnE_min, float lnE_max, const MlpDev *net);
 int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
