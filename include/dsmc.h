@@ -224,6 +224,18 @@ int dsmc_step_host(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cel
                    const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi, uint64_t seed,
                    uint32_t step);
 
+/* The same step, enqueued only: returns as soon as the copies and kernels are on the context's stream (argument
+ * errors are still returned at once).  The caller's host buffers (inputs and outputs) must stay valid and untouched
+ * until dsmc_sync_status(ctx) has returned, which also delivers the device-detected data errors.  One submitted step
+ * per context at a time.  Two contexts on two streams, fed alternately, overlap the host->device copy of one batch
+ * with the device->host copy of the previous one (the PCIe link is full duplex): that is how bench.py measures the
+ * end-to-end throughput of independent batches. */
+int dsmc_step_host_submit(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell_h,
+                          const float *vx_h, const float *vy_h, const float *vz_h, float *vx_out_h,
+                          float *vy_out_h, float *vz_out_h, int32_t *perm_h, int32_t *cell_start_h,
+                          const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi, uint64_t seed,
+                          uint32_t step);
+
 /* ---- f1: NTC candidate count with a carried remainder (Q31) ---------------------------
  * "a number of candidate pairs is drawn proportional to N_k (N_k - 1) and a cell-wise upper bound (sigma v_r)max,k":
  * m = 1/2 N_k (N_k - 1) coef sigma_cr_max[k] + remainder[k]; counts[k] = floor(m); remainder[k] = m - counts[k],

@@ -500,10 +500,10 @@ int dsmc_chi_exact_batch(dsmc_ctx *c, int64_t n, const float *E_over_k, const fl
   return launch_chi_exact(c, n, E_over_k, b, chi, (double)eps_over_k, (double)sigma, (flags & DSMC_F_CHI_ABS) ? 1 : 0);
 }
 
-int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, const float *vx_h, const float *vy_h,
-                   const float *vz_h, float *vx_out_h, float *vy_out_h, float *vz_out_h, int32_t *perm_h,
-                   int32_t *cell_start_h, const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi,
-                   uint64_t seed, uint32_t step) {
+int dsmc_step_host_submit(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, const float *vx_h,
+                          const float *vy_h, const float *vz_h, float *vx_out_h, float *vy_out_h, float *vz_out_h,
+                          int32_t *perm_h, int32_t *cell_start_h, const dsmc_vhs_params *vhs,
+                          const dsmc_abinitio_params *abi, uint64_t seed, uint32_t step) {
   if (!c || n <= 0 || K <= 0 || K > c->max_cells || (!vhs && !abi) || (vhs && abi)) return DSMC_ERR_INVALID_ARG;
   if (!cell_h || !vx_h || !vy_h || !vz_h || !vx_out_h || !vy_out_h || !vz_out_h) return DSMC_ERR_INVALID_ARG;
   CK(cudaSetDevice(c->device));
@@ -547,6 +547,19 @@ int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, con
   if (side) {  // join the side stream before the final synchronisation
     CK(cudaEventRecord(c->ev_side, c->side_stream));
     CK(cudaStreamWaitEvent(s, c->ev_side, 0));
+  }
+  return DSMC_OK;
+}
+
+int dsmc_step_host(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell_h, const float *vx_h, const float *vy_h,
+                   const float *vz_h, float *vx_out_h, float *vy_out_h, float *vz_out_h, int32_t *perm_h,
+                   int32_t *cell_start_h, const dsmc_vhs_params *vhs, const dsmc_abinitio_params *abi,
+                   uint64_t seed, uint32_t step) {
+  const int rc = dsmc_step_host_submit(c, n, K, cell_h, vx_h, vy_h, vz_h, vx_out_h, vy_out_h, vz_out_h, perm_h,
+                                       cell_start_h, vhs, abi, seed, step);
+  if (rc != DSMC_OK) {
+    if (c) cudaStreamSynchronize(c->stream);  // copies into the caller's buffers must not outlive a failed call
+    return rc;
   }
   return dsmc_sync_status(c);
 }

@@ -28,7 +28,7 @@ ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
-           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host", "dsmc_move_couette",
+           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host", "dsmc_step_host_submit", "dsmc_move_couette",
            "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run", "dsmc_ntc_counts"]
 
 
@@ -377,13 +377,15 @@ class Context:
 
     # ---- end to end on host buffers (pinned CPU tensors)
     def step_host(self, cell_h, vx_h, vy_h, vz_h, n_cells, out_h, vhs: VhsParams = None,
-                  abi: AbinitioParams = None, seed=0, step=0):
-        """out_h = (vx_out, vy_out, vz_out, perm, cell_start) CPU tensors.  Synchronous."""
+                  abi: AbinitioParams = None, seed=0, step=0, submit_only=False):
+        """out_h = (vx_out, vy_out, vz_out, perm, cell_start) CPU tensors.  Synchronous, unless submit_only: then the
+        step is only enqueued (dsmc_step_host_submit) and the buffers belong to the library until sync_status()."""
         pv = vhs.c() if vhs is not None else None
         pa = abi.c() if abi is not None else None
         hp = lambda t: C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
         self._stream()
-        _chk(_lib.dsmc_step_host(
+        fn = _lib.dsmc_step_host_submit if submit_only else _lib.dsmc_step_host
+        _chk(fn(
             self._h, C.c_int64(cell_h.shape[0]), C.c_int32(n_cells), hp(cell_h), hp(vx_h), hp(vy_h), hp(vz_h),
             hp(out_h[0]), hp(out_h[1]), hp(out_h[2]), hp(out_h[3]), hp(out_h[4]),
             C.byref(pv) if pv is not None else None, C.byref(pa) if pa is not None else None,

@@ -835,3 +835,49 @@ def test_step_host_equals_the_device_path(dsmc):
         for got, want in zip(hout, (vx_s, vy_s, vz_s, perm, cs)):
             assert torch.equal(got, want.cpu())
     ctx.close()
+
+
+def test_step_host_submit_two_contexts_alternating(dsmc):
+    """dsmc_step_host_submit (enqueue only) on two contexts, each on its own stream, fed alternately as bench.py's e2e
+    loop does: every batch gives, bit for bit, what the synchronous dsmc_step_host gives for the same (input, step)."""
+    pops = [wl.mach10_cylinder(seed=s, nx=60, ny=30, n_total=300_000) for s in (4, 5)]
+    tab = _lj_table()
+    prm = dsmc.AbinitioParams(chi_mode=0, flags=dsmc.F_MOMENT_MATCH)
+    ctxs, streams = [], []
+    for _ in range(2):
+        c = dsmc.Context(pops[0].n, pops[0].n_cells)
+        c.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+        ctxs.append(c)
+        streams.append(torch.cuda.Stream())
+    ref = dsmc.Context(pops[0].n, pops[0].n_cells)
+    ref.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+
+    def host_in(pop):
+        return [torch.from_numpy(a).pin_memory() for a in (pop.cell, pop.vx, pop.vy, pop.vz)]
+
+    def host_out(pop):
+        return [torch.empty(pop.n, dtype=torch.float32).pin_memory() for _ in range(3)] + \
+               [torch.empty(pop.n, dtype=torch.int32).pin_memory(), torch.empty(pop.n_cells + 1, dtype=torch.int32).pin_memory()]
+
+    hin = [host_in(p) for p in pops]
+    houts = [host_out(pops[0]) for _ in range(2)]
+    want = host_out(pops[0])
+    torch.cuda.synchronize()
+    results = []
+    for t in range(6):
+        k = t & 1
+        if t >= 2:  # the lane's previous batch must be complete before its buffers are reused
+            ctxs[k].check()
+            results.append((t - 2, [x.clone() for x in houts[k]]))
+        with torch.cuda.stream(streams[k]):
+            ctxs[k].step_host(*hin[(t // 2) & 1], pops[0].n_cells, houts[k], abi=prm, seed=9, step=t, submit_only=True)
+    for k in (0, 1):
+        ctxs[k].check()
+        results.append((4 + k, [x.clone() for x in houts[k]]))
+    assert sorted(t for t, _ in results) == list(range(6))
+    for t, got in results:
+        ref.step_host(*hin[(t // 2) & 1], pops[0].n_cells, want, abi=prm, seed=9, step=t)
+        for g, w in zip(got, want):
+            assert torch.equal(g, w), "batch %d differs" % t
+    for c in ctxs + [ref]:
+        c.close()
