@@ -3,15 +3,17 @@
 The oracle cannot run 2e7 particles in seconds, so (prompt section 3):
   * binning is checked exactly through properties that pin the unique stable sort (cell_start = cumulative
     counts, perm a permutation, cells constant and ids ascending inside every segment);
-  * the fused step is checked (a) on SAMPLED cells that the oracle recomputes one by one -- cell_base makes
-    the oracle draw exactly the randoms of the full run -- with bit-exact pairing and the per-pair tolerances of
-    DESIGN.md, and (b) on ALL cells through the conserved moments (1e-6);
+  * the fused step is checked (a) on ALL pairs: the pair indices against the oracle's pairing run alone (integer
+    work), (b) on SAMPLED cells that the oracle recomputes one by one -- cell_base makes the oracle draw exactly the
+    randoms of the full run -- particle by particle against allowances derived from the per-pair tolerances of
+    DESIGN.md, and (c) on ALL cells through the conserved moments (1e-6);
   * the chi batch (cfg 4, 1e7 pairs) on a sample of outputs.
 """
 import numpy as np
 import pytest
 
 import oracle
+from conftest import _OBSERVED
 from paper_2602_21244_b200 import workloads as wl
 
 torch = pytest.importorskip("torch")
@@ -39,9 +41,27 @@ def _segment_moments(cs, vx, vy, vz):
     return np.stack(out, axis=1)
 
 
-def _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, seed, step, tol_pair, net=None, table=None,
-                         chi_tol_rel=None):
-    worst = 0.0
+KB = 1.380649e-23
+
+
+def _table_slope(tab, lnE, bt):
+    """max - min of the four table nodes around each query (Q25)."""
+    nE, nB = tab.chi.shape
+    tE = np.clip((lnE - tab.lnE_min) / (tab.lnE_max - tab.lnE_min) * (nE - 1), 0, nE - 1)
+    tB = np.clip(bt * (nB - 1), 0, nB - 1)
+    iE = np.minimum(tE.astype(int), nE - 2)
+    iB = np.minimum(tB.astype(int), nB - 2)
+    c = np.stack([tab.chi[iE, iB], tab.chi[iE, iB + 1], tab.chi[iE + 1, iB], tab.chi[iE + 1, iB + 1]])
+    return c.max(axis=0) - c.min(axis=0)
+
+
+def _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, seed, step, chi_kind, net=None, table=None, tab=None):
+    """Final velocities of sampled cells against the oracle, particle by particle, each against ITS OWN allowance
+    (DESIGN "Tolerances"): a pair whose deflection angle may differ by dchi moves its two particles by g dchi / 2, the
+    fp32 rotation adds 1e-5 g / 2, matching and storage 2e-6 s (s = thermal scale of the cell).  dchi comes from the
+    oracle's side alone: table -> the Q25 slope-aware bound of that pair's query, fp32 MLP -> 1e-5 max(chi, 1),
+    bf16 MLP -> Q26, 2e-2 (1 + chi).  Returns the worst deviation / allowance and the worst deviation / s."""
+    worst, worst_abs = 0.0, 0.0
     for k in cells:
         q0, q1 = int(cs_h[k]), int(cs_h[k + 1])
         if q1 - q0 < 2:
@@ -50,13 +70,26 @@ def _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, seed, step, tol_
         lcs = np.array([0, q1 - q0], np.int32)
         prm_o.cell_base = int(k)
         ref = oracle.collide_abinitio(lcs, *loc, prm_o, seed, step, net=net, table=table)
-        # after moment matching every particle of the cell moved by the same affine map, so comparing final
-        # velocities tests pairing, operator, rotation and matching together
         scale = np.sqrt((loc[0] ** 2 + loc[1] ** 2 + loc[2] ** 2).mean())
-        for a, want in zip(v_out, (ref.vx, ref.vy, ref.vz)):
-            d = np.abs(a[q0:q1].astype(np.float64) - want).max() / scale
-            worst = max(worst, d)
-    return worst
+        idx = np.flatnonzero(ref.pair_i >= 0)
+        g2 = sum((a[ref.pair_i[idx]] - a[ref.pair_j[idx]]) ** 2 for a in loc)
+        chi = np.abs(ref.aux[idx])
+        if chi_kind == "table":
+            bt = np.sqrt(oracle.pair_uniforms_batch(seed, step, np.full(len(idx), k), idx)[:, 1])
+            sl = _table_slope(tab, np.log(np.maximum(wl.MASS_AR * g2 / (4 * KB), 1e-300)), bt)
+            dchi = 1e-5 * np.maximum(chi, 1) + 2e-4 * sl + 1e-6
+        elif chi_kind == "mlp":
+            dchi = 1e-5 * np.maximum(chi, 1)
+        else:
+            dchi = 2e-2 * (1 + chi)
+        allow = np.full(q1 - q0, 2e-6)
+        pair_allow = 0.5 * np.sqrt(g2) * (dchi + 1e-5) / scale
+        allow[ref.pair_i[idx]] += pair_allow
+        allow[ref.pair_j[idx]] += pair_allow
+        d = np.sqrt(sum((a[q0:q1].astype(np.float64) - want) ** 2 for a, want in zip(v_out, (ref.vx, ref.vy, ref.vz)))) / scale
+        worst = max(worst, float((d / allow).max()))
+        worst_abs = max(worst_abs, float(d.max()))
+    return worst, worst_abs
 
 
 @pytest.mark.parametrize("chi", ["table", "mlp_tc"])
@@ -115,11 +148,51 @@ def test_cfg5_full_size(dsmc, chi):
     lo, hi = float(np.float32(prm.lnE_min)), float(np.float32(prm.lnE_max))
     prm_o = oracle.AbinitioParams(chi_mode=cm, lnE_min=lo, lnE_max=hi)
     otab = oracle.ChiTable(tab.chi, float(np.float32(tab.lnE_min)), float(np.float32(tab.lnE_max)))
-    worst = _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, 4, 7, None,
-                                 net=oracle.Mlp(Ws, bs, oracle.ACT_SILU), table=otab)
-    print("cfg5 %s: worst sampled-cell velocity deviation / thermal scale = %.3e over %d cells" % (chi, worst, len(cells)))
-    # table: fp32 table coordinates move chi by up to ~2e-3 near the orbiting band (Q25); MLP: Q26 (2e-2 (1 + chi))
-    assert worst < (3e-3 if chi == "table" else 3e-2)
+    worst, worst_abs = _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, 4, 7, "table" if chi == "table" else "bf16",
+                                            net=oracle.Mlp(Ws, bs, oracle.ACT_SILU), table=otab, tab=tab)
+    print("cfg5 %s: worst particle deviation = %.3f of its allowance (%.3e of the thermal scale) over %d cells" % (chi, worst, worst_abs, len(cells)))
+    _OBSERVED("test_cfg5_full_size[%s] particle deviation over its allowance" % chi, worst, 1.0)
+    _OBSERVED("test_cfg5_full_size[%s] particle deviation / thermal scale" % chi, worst_abs, float("inf"))
+    assert worst <= 1.0
+    ctx.close()
+
+
+def test_cfg5_sixteenth_fp32_chi_mlp(dsmc):
+    """The FP32 chi-MLP operator (85 ms per full cfg-5 step: the reference variant) on 1/16 of the cfg-5 population
+    (100 x 50 cells, 1.25e6 particles, same per-cell populations): every pair index against the oracle's pairing,
+    every cell's moments, sampled cells particle by particle at the FP32 tolerances."""
+    pop = wl.mach10_cylinder(nx=100, ny=50, n_total=1_250_000)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = ctx.bin(dev(pop.cell), dev(pop.vx), dev(pop.vy), dev(pop.vz), pop.n_cells)
+    ctx.check()
+    cs_h = cs.cpu().numpy()
+    np.testing.assert_array_equal(cs_h, np.concatenate([[0], np.cumsum(pop.counts)]).astype(np.int32))
+    v_in = [t.cpu().numpy() for t in (vx_s, vy_s, vz_s)]
+    pre = _segment_moments(cs_h, *v_in)
+    prm = dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_MOMENT_MATCH)
+    dump = dsmc.PairDump(pop.n, "cuda", gprime=False)
+    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=4, step=7, dump=dump)
+    ctx.check()
+    want_i, want_j = oracle.pairing_all(4, 7, cs_h)
+    np.testing.assert_array_equal(dump.pair_i.cpu().numpy(), want_i)
+    np.testing.assert_array_equal(dump.pair_j.cpu().numpy(), want_j)
+    v_out = [t.cpu().numpy() for t in (vx_s, vy_s, vz_s)]
+    post = _segment_moments(cs_h, *v_out)
+    N = np.diff(cs_h)
+    ok = N >= 2
+    assert np.abs(post[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+    assert (np.linalg.norm(post[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    rng = np.random.default_rng(0)
+    sizes = np.unique(N[N >= 2])
+    cells = np.concatenate([rng.choice(np.flatnonzero(N == s), size=min(2, int((N == s).sum())), replace=False)
+                            for s in sizes[:: max(1, len(sizes) // 8)]] + [rng.choice(np.flatnonzero(ok), 24)])
+    prm_o = oracle.AbinitioParams(chi_mode=1, lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
+    worst, worst_abs = _check_sampled_cells(dsmc, cs_h, v_in, v_out, cells, prm_o, 4, 7, "mlp", net=oracle.Mlp(Ws, bs, oracle.ACT_SILU))
+    print("cfg5/16 fp32 chi-MLP: worst particle deviation = %.3f of its allowance (%.3e of the thermal scale) over %d cells" % (worst, worst_abs, len(cells)))
+    _OBSERVED("test_cfg5_sixteenth_fp32_chi_mlp particle deviation over its allowance", worst, 1.0)
+    assert worst <= 1.0
     ctx.close()
 
 

@@ -199,7 +199,11 @@ def _compare_step(dsmc, ctx, cs, v_in, v_out, dump, ref, tol_pair, tol_moment, g
     return err
 
 
-def _velocity_and_moment_checks(ctx, cs, v_in, out, ref, tol_v, tol_moment):
+def _velocity_and_moment_checks(ctx, cs, v_in, out, ref, tol_pair, tol_moment):
+    """Final velocities against the oracle's, in units of the cell's thermal scale s = sqrt(E/N).  The tolerance follows
+    from the per-pair one (DESIGN "Tolerances"): v' = cm +- g'/2, so a pair whose g' is off by tol_pair * g moves its two
+    particles by tol_pair * g / 2; the matching then rescales by alpha = 1 + O(tol_moment) and shifts by O(tol_moment) s,
+    and fp32 storage adds 6e-8 |v|.  Hence tol_v = tol_pair * max(g / s) / 2 + 2e-6, g / s from the oracle's pairs."""
     cs_h = cs.cpu().numpy()
     N = np.diff(cs_h)
     pre = oracle.cell_moments(cs_h, *v_in)
@@ -209,11 +213,17 @@ def _velocity_and_moment_checks(ctx, cs, v_in, out, ref, tol_v, tol_moment):
     _note("cell momentum", (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max(), tol_moment)
     assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < tol_moment
     assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < tol_moment
-    scale = np.repeat(np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1)), N)
+    cell_scale = np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1))
+    scale = np.repeat(cell_scale, N)
+    idx = np.flatnonzero(ref.pair_i >= 0)
+    k = np.searchsorted(cs_h, idx, side="right") - 1
+    g = np.sqrt(sum((a[cs_h[k] + ref.pair_i[idx]] - a[cs_h[k] + ref.pair_j[idx]]) ** 2 for a in v_in))
+    tol_v = 0.5 * tol_pair * (g / cell_scale[k]).max() + 2e-6
+    assert tol_v < 5e-5  # never looser than the fixed figure this replaced
     for a, want in zip(out, (ref.vx, ref.vy, ref.vz)):
         d = np.abs(a.cpu().numpy().astype(np.float64) - want) / scale
         _note("velocity / thermal scale", d.max(), tol_v)
-        assert d.max() < tol_v, "velocity mismatch %.3e" % d.max()
+        assert d.max() < tol_v, "velocity mismatch %.3e (allowed %.3e)" % (d.max(), tol_v)
 
 
 @pytest.mark.parametrize("case", ["cfg1_tiny", "cfg2_couette_small", "cfg3_cavity_small", "ragged"])
@@ -244,7 +254,7 @@ def test_collide_vhs_nn_fp32(dsmc, case):
         hn = ref.aux
         med = np.median(hn[ref.pair_i >= 0])
         err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, gate=hn >= 0.25 * med)
-        _velocity_and_moment_checks(ctx, cs, v_in, (vx_s, vy_s, vz_s), ref, 5e-5, 1e-6)
+        _velocity_and_moment_checks(ctx, cs, v_in, (vx_s, vy_s, vz_s), ref, 1e-5, 1e-6)
     ctx.close()
 
 
@@ -279,7 +289,7 @@ def test_collide_vhs_nn_variants(dsmc):
         gate = (hn >= 0.25 * np.median(hn[sel & (ref.accepted == 1)])) | (ref.accepted == 0)
         if not flags & dsmc.F_ENERGY_SHELL:
             gate = np.ones_like(gate)
-        _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 2e-5, 1e-6, gate=gate)
+        _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, gate=gate)
         for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
             assert np.abs(a.cpu().numpy() - want).max() < 2e-4 * 400
         ctx.close()
@@ -347,10 +357,10 @@ def test_collide_abinitio_fp32(dsmc, mode):
             slope = np.zeros_like(dchi)
             slope[idx] = bound  # a lookup difference rotates g' by exactly that angle
         else:
-            _note("chi / max(|chi|,1)", np.abs(chi_g[sel] - ref.aux[sel]).max() / np.maximum(np.abs(ref.aux[sel]), 1).max(), 2e-5)
-            _note("chi range max", np.abs(ref.aux[sel]).max(), np.inf)
-            assert np.abs(chi_g[sel] - ref.aux[sel]).max() <= 2e-5 * np.maximum(np.abs(ref.aux[sel]), 1).max()
-        _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5 if mode == "table" else 3e-5, 1e-6, slope=slope)
+            rel = np.abs(chi_g[sel] - ref.aux[sel]) / np.maximum(np.abs(ref.aux[sel]), 1)
+            _note("chi / max(|chi|,1), per pair", rel.max(), 1e-5)
+            assert rel.max() <= 1e-5
+        _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=slope)
         N = np.diff(cs_h)
         pre = oracle.cell_moments(cs_h, *v_in)
         got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
@@ -404,7 +414,8 @@ def test_chi_batch(dsmc, mode):
         assert np.all(np.abs(got - want) <= 1e-5 * np.maximum(np.abs(want), 1) + 2e-4 * sl + 1e-6)
     else:
         want = oracle.chi_batch(E, b, 1, 1e-9, net=oracle.Mlp(Ws, bs, oracle.ACT_SILU), lnE_min=lo, lnE_max=hi)
-        assert np.all(np.abs(got - want) <= 2e-5 * np.maximum(np.abs(want), 1))
+        _note("chi / max(|chi|,1), per pair", (np.abs(got - want) / np.maximum(np.abs(want), 1)).max(), 1e-5)
+        assert np.all(np.abs(got - want) <= 1e-5 * np.maximum(np.abs(want), 1))
 
 
 def test_empty_inputs_and_unconfigured_operators(dsmc):
@@ -474,8 +485,9 @@ def test_collide_abinitio_bf16_tc(dsmc):
         print("abinitio bf16 chi: %s" % _quantiles(rel))
         assert rel.max() <= 2e-2  # Q26
         # a chi difference rotates g' by exactly that angle: allow it on top of the fp32 rotation error
-        err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 3e-5, 1e-6, slope=1.01 * np.abs(chi_g - ref.aux))
-        assert err.max() <= 2e-2 * (1 + np.abs(ref.aux[sel]).max())
+        # (the chi error of EVERY pair has just passed the Q26 bound, which is computed from the oracle's chi alone)
+        err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=1.01 * np.abs(chi_g - ref.aux))
+        assert np.all(err <= 2e-2 * (1 + np.abs(ref.aux[sel])) + 1e-5)  # per pair, from the oracle's side alone
         N = np.diff(cs_h)
         pre = oracle.cell_moments(cs_h, *v_in)
         got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
@@ -687,7 +699,7 @@ def test_collide_abinitio_with_replacement(dsmc, mode, match):
         dv = 0.5 * gn * (1e-5 + bound)
         for side in (ref.pair_i, ref.pair_j):
             np.add.at(allow_v, cs_h[kk] + side[idx], 1.05 * dv / scale[cs_h[kk] + side[idx]])
-    _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5 if mode == "table" else 3e-5, 1e-6, slope=slope)
+    _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=slope)
     for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
         assert np.all(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale < allow_v)
     assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
@@ -733,7 +745,8 @@ def test_collide_vhs_nn_with_replacement(dsmc):
         k = np.searchsorted(cs_h, idx, side="right") - 1
         g = np.stack([a[cs_h[k] + ref.pair_i[idx]] - a[cs_h[k] + ref.pair_j[idx]] for a in v_in], axis=1)
         err = np.linalg.norm(dump.gprime.cpu().numpy()[idx].astype(np.float64) - ref.gprime[idx], axis=1) / np.linalg.norm(g, axis=1)
-        assert err.max() < 2e-5
+        _note("pair |dg'|/g", err.max(), 1e-5)
+        assert err.max() < 1e-5
         scale = np.repeat(np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1)), N)
         for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
             assert np.median(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale) < 1e-5
