@@ -18,10 +18,11 @@
 //   rank      ... and count the smaller composites of their bucket: pi = the unique ascending order of
 //             (key << 32 | slot) (Q7); pairs are (pi[2s], pi[2s+1])
 //   pairs     two pair slots per thread (they share one Philox block of stream 1): gather, table lookup
-//             (one 16 B load from the L2-resident quad table), rotation by (chi, eps) (Q16),
+//             (one 16 B fetch from the L2-resident quad table through the TEX pipe), rotation by (chi, eps) (Q16),
 //             centre-of-mass update (eqs. 6-8) written back to shared memory
 //   finish    post-collision sums from shared memory into registers, matching coefficients (eqs. 10-11, P:L46,
-//             Q5) in FP64, v <- v + (alpha - 1) v + B applied to the registers, 12 B / particle stored
+//             Q5) in FP32 (alpha - 1 = del / (1 + sqrt(1 + del)): no cancellation), v <- v + (alpha - 1) v + B
+//             applied to the registers, 12 B / particle stored
 //
 // Work distribution: k_cell_lists sorts the cells that have pairs to collide into three lists by size; the
 // CTAs of k_cells are persistent and draw list entries from a counter (the next entry is fetched while the
