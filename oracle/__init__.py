@@ -442,6 +442,15 @@ def build_chi_table(pot: Potential, nE, nB, lnE_min=float(np.log(5.0)),
     return ChiTable(chi, lnE_min, lnE_max)
 
 
+def build_chi_table_mlp(net: Mlp, nE, nB, lnE_min=float(np.log(5.0)), lnE_max=float(np.log(6.0e4))) -> ChiTable:
+    """f2: the chi-MLP evaluated on the table nodes."""
+    chi = np.empty((nE, nB), np.float32)
+    m = net.c()
+    lib().orc_build_chi_table_mlp(C.byref(m), C.c_int32(nE), C.c_int32(nB), C.c_double(lnE_min), C.c_double(lnE_max),
+                                  _p(chi, C.c_float))
+    return ChiTable(chi, lnE_min, lnE_max)
+
+
 # ------------------------------------------------------------- f4: move + walls + sampling (Q30)
 class _Couette(C.Structure):
     _fields_ = [("L", C.c_double), ("dt", C.c_double), ("u_wall", C.c_double), ("rt_wall", C.c_double),

@@ -650,6 +650,20 @@ void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, doubl
 }
 
 
+/* f2, the paper's neural table generation ("the neural network can generate a complete 512 x 512 table in less
+ * than 1.0 s"): the chi-MLP of P:L277-283 evaluated on the table nodes of Q13 (lnE uniform in [lnE_min, lnE_max],
+ * b~ = j / (nB - 1)), abs value (Q14), capped (Q23), rounded to fp32 like the quadrature table. */
+void orc_build_chi_table_mlp(const orc_mlp *net, int32_t nE, int32_t nB, double lnE_min, double lnE_max, float *chi) {
+  for (int32_t iE = 0; iE < nE; ++iE) {
+    double lnE = lnE_min + (lnE_max - lnE_min) * (double)iE / (double)(nE - 1);
+    for (int32_t iB = 0; iB < nB; ++iB) {
+      double bt = (double)iB / (double)(nB - 1);
+      chi[(size_t)iE * nB + iB] = (float)orc_cap_chi(fabs(orc_chi_mlp(net, lnE_min, lnE_max, lnE, bt)));
+    }
+  }
+}
+
+
 /* ------------------------------------------------------------------------------------------
  * f4.  Free flight + Maxwell walls for the 1-D Couette layout (Q30), and the
  * per-cell sampling sums.

@@ -158,6 +158,8 @@ double orc_chi_exact(const orc_potential *pot, double E, double b, int32_t n_pan
 double orc_cap_chi(double c); /* Q23: min(c, 64 pi), NaN -> 64 pi */
 void orc_build_chi_table(const orc_potential *pot, int32_t nE, int32_t nB, double lnE_min,
                          double lnE_max, double b_max, int32_t n_panels, float *chi);
+/* f2: the chi-MLP evaluated on the table nodes (Q13), abs (Q14), capped (Q23), fp32 */
+void orc_build_chi_table_mlp(const orc_mlp *net, int32_t nE, int32_t nB, double lnE_min, double lnE_max, float *chi);
 
 /* ---- f1: NTC candidate count with a carried remainder (Bird 1994 eq. 11.3; Q31) ----
  * "a number of candidate pairs is drawn proportional to N_k (N_k - 1) and a cell-wise upper bound (sigma v_r)max,k":

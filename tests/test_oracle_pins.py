@@ -758,3 +758,34 @@ def test_table_builder_caps_non_finite_nodes_at_64_pi():
     assert np.isfinite(np.float32(cap))
     good = oracle.build_chi_table(oracle.lj_argon(), 8, 9, n_panels=1)
     assert np.all(np.isfinite(good.chi)) and good.chi.max() < 4 * np.pi and np.all(good.chi >= 0)
+
+
+def test_neural_table_builder_nodes_closed_form_and_lookup():
+    """f2, orc_build_chi_table_mlp: with a linear probe network the head makes chi = exp(z) (expm1 o softplus),
+    so node (i, j) must hold exp(a i/(nE-1) + c j/(nB-1) + d) to fp32 rounding: pins the node coordinates of Q13
+    (row = energy, column = impact parameter, both ends included) and the abs / cap seam; a lookup through the table
+    at the nodes returns the node; a real SiLU network's table equals orc_chi_mlp at the node coordinates."""
+    a, c, d = 1.75, -2.5, 0.25  # exact in fp32
+    net = oracle.Mlp([np.array([[a, c]], np.float32)], [np.array([d], np.float32)], oracle.ACT_SILU)
+    lo, hi = math.log(5.0), math.log(6e4)
+    nE, nB = 7, 5
+    tab = oracle.build_chi_table_mlp(net, nE, nB, lo, hi)
+    assert tab.chi.shape == (nE, nB) and tab.chi.dtype == np.float32
+    i, j = np.meshgrid(np.arange(nE), np.arange(nB), indexing="ij")
+    want = np.exp(a * i / (nE - 1) + c * j / (nB - 1) + d)
+    np.testing.assert_allclose(tab.chi, want, rtol=6e-8)  # half an fp32 ulp: the rounding of the stored node
+    assert tab.chi[nE - 1, 0] == pytest.approx(math.exp(a + d), rel=6e-8) and tab.chi[0, nB - 1] == pytest.approx(math.exp(c + d), rel=6e-8)
+    for ii, jj in ((0, 0), (3, 2), (nE - 1, nB - 1), (5, 1)):
+        got = oracle.chi_bilinear(tab, lo + (hi - lo) * ii / (nE - 1), jj / (nB - 1))
+        assert got == pytest.approx(float(tab.chi[ii, jj]), rel=1e-12)
+    # a network whose output would exceed the cap: exp(6) = 403 > 64 pi = 201 -> capped (Q23)
+    big = oracle.Mlp([np.array([[0.0, 0.0]], np.float32)], [np.array([6.0], np.float32)], oracle.ACT_SILU)
+    assert np.all(oracle.build_chi_table_mlp(big, 3, 3, lo, hi).chi == np.float32(64 * np.pi))
+    # hidden layers: the table is orc_chi_mlp at the node coordinates
+    rng = np.random.default_rng(5)
+    Ws = [rng.uniform(-1, 1, (16, 2)).astype(np.float32), rng.uniform(-0.3, 0.3, (1, 16)).astype(np.float32)]
+    bs = [rng.uniform(-1, 1, 16).astype(np.float32), np.array([0.1], np.float32)]
+    deep = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
+    t2 = oracle.build_chi_table_mlp(deep, 4, 6, lo, hi)
+    for ii, jj in ((0, 0), (1, 4), (3, 5), (2, 2)):
+        assert t2.chi[ii, jj] == np.float32(oracle.chi_mlp(deep, lo, hi, lo + (hi - lo) * ii / 3, jj / 5))
