@@ -475,6 +475,16 @@ def run_b200(args):
         ctx_t.build_chi_table_lj(TABLE_N, TABLE_N, b_max=B_MAX)
         torch.cuda.synchronize()
         cfg4["table_build_on_device_ms"] = (time.perf_counter() - tb0) * 1e3
+        # (f2 as the paper states it) the table generated by the chi-MLP on its nodes; paper: "< 1.0 s" for 512 x 512
+        ctx_t.set_mlp(1, mlp_w[0], mlp_w[1], dsmc.ACT_SILU)
+        for key, nn_, fl in (("table_build_from_mlp_512_tc_ms", 512, dsmc.F_BF16_TC), ("table_build_from_mlp_512_fp32_ms", 512, 0),
+                             ("table_build_from_mlp_1024_tc_ms", TABLE_N, dsmc.F_BF16_TC)):
+            ctx_t.build_chi_table_mlp(nn_, nn_, flags=fl)
+            torch.cuda.synchronize()
+            tb0 = time.perf_counter()
+            ctx_t.build_chi_table_mlp(nn_, nn_, flags=fl)
+            torch.cuda.synchronize()
+            cfg4[key] = (time.perf_counter() - tb0) * 1e3
         ctx_t.close()
         fl4 = n4 * 2 * (2 * 128 + 128 * 128 + 128)
         cfg4["mlp_tc"]["tensor_frac"] = fl4 / (cfg4["mlp_tc"]["ms"] * 1e-3) / 1e12 / tc_sust

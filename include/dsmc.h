@@ -14,6 +14,7 @@
  *   dsmc_chi_batch         chi for independent (E_r, b) pairs
  *   dsmc_chi_exact_batch   chi by the deflection-integral quadrature itself (eq. 16), LJ 12-6
  *   dsmc_build_chi_table_lj  the chi table generated on the device by that quadrature
+ *   dsmc_build_chi_table_mlp the chi table generated on the device by the chi-MLP
  *   dsmc_step_host         bin + fused step on HOST buffers (copies inside), for end-to-end timing
  *   dsmc_ntc_counts        NTC candidate counts with carried remainder
  *   dsmc_move_couette, dsmc_gather_f32, dsmc_sample_cells, dsmc_couette_run
@@ -213,6 +214,16 @@ int dsmc_chi_exact_batch(dsmc_ctx *ctx, int64_t n, const float *E_over_k, const 
  * receives the node values.  Synchronises the stream. */
 int dsmc_build_chi_table_lj(dsmc_ctx *ctx, int32_t nE, int32_t nB, float lnE_min, float lnE_max, float b_max,
                             float eps_over_k, float sigma, float *chi_out);
+
+/* f2 as the paper states it ("the neural network can generate a complete 512 x 512 table in less than 1.0 s"):
+ * evaluates the chi-MLP of operator slot 1 (dsmc_set_mlp, readings Q13-Q15) on the nE x nB table nodes
+ * ON THE DEVICE and installs the result as the context's table exactly as dsmc_set_chi_table would: node (i, j) =
+ * chi(lnE_min + i (lnE_max - lnE_min) / (nE - 1), b~ = j / (nB - 1)), abs value (Q14), capped at 64 pi (Q23), fp32.
+ * flags: 0 (FP32 CUDA-core MLP) or DSMC_F_BF16_TC (tensor cores; DSMC_ERR_UNSUPPORTED_SHAPE if slot 1 has no
+ * tensor-core image).  chi_out: optional DEVICE array [nE][nB] that receives the node values.  Synchronises the
+ * stream.  DSMC_ERR_NOT_CONFIGURED without a slot-1 network; on any error the installed table (if any) stays. */
+int dsmc_build_chi_table_mlp(dsmc_ctx *ctx, int32_t nE, int32_t nB, float lnE_min, float lnE_max, uint32_t flags,
+                             float *chi_out);
 
 /* ---- end-to-end helper on HOST buffers ----------------------------------------------------
  * Copies cell/vx/vy/vz (HOST, ideally pinned) to context-owned device buffers, runs dsmc_bin and

@@ -229,6 +229,26 @@ int dsmc_set_mlp(dsmc_ctx *c, int slot, const dsmc_mlp_desc *d) {
   return DSMC_OK;
 }
 
+// makes `tnew` (device, 4 (nE-1)(nB-1) floats in quad layout, ownership passes to the context) the context's table
+static void install_quad_table(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, float lnE_max, float *tnew) {
+  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
+  c->table.tex = 0;
+  cudaFree(c->d_table);
+  c->d_table = tnew;
+  c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
+  c->table.nE = nE;
+  c->table.nB = nB;
+  c->table.lnE_min = lnE_min;
+  const double inv = (double)(nE - 1) / ((double)lnE_max - (double)lnE_min);
+  c->table.inv_dlnE = (float)inv;
+  c->table.c1 = (float)(0.6931471805599453 * inv);
+  c->table.c0 = (float)(-(double)lnE_min * inv);
+  c->table.fE1 = (float)(nE - 1);
+  c->table.fB1 = (float)(nB - 1);
+  make_table_texture(c, (size_t)(nE - 1) * (nB - 1));
+  c->has_table = true;
+}
+
 int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t nB, float lnE_min, float lnE_max) {
   if (!c || !chi_host || nE < 2 || nB < 2 || !(lnE_max > lnE_min)) return DSMC_ERR_INVALID_ARG;
   for (size_t i = 0; i < (size_t)nE * nB; ++i)
@@ -253,22 +273,7 @@ int dsmc_set_chi_table(dsmc_ctx *c, const float *chi_host, int32_t nE, int32_t n
     return DSMC_ERR_CUDA;
   }
   CK(cudaStreamSynchronize(c->stream));
-  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
-  c->table.tex = 0;
-  cudaFree(c->d_table);
-  c->d_table = tnew;
-  c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
-  c->table.nE = nE;
-  c->table.nB = nB;
-  c->table.lnE_min = lnE_min;
-  const double inv = (double)(nE - 1) / ((double)lnE_max - (double)lnE_min);
-  c->table.inv_dlnE = (float)inv;
-  c->table.c1 = (float)(0.6931471805599453 * inv);
-  c->table.c0 = (float)(-(double)lnE_min * inv);
-  c->table.fE1 = (float)(nE - 1);
-  c->table.fB1 = (float)(nB - 1);
-  make_table_texture(c, nq);
-  c->has_table = true;
+  install_quad_table(c, nE, nB, lnE_min, lnE_max, tnew);
   return DSMC_OK;
 }
 
@@ -472,22 +477,44 @@ int dsmc_build_chi_table_lj(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, 
     cudaFree(tnew);
     return rc;
   }
-  if (c->table.tex) cudaDestroyTextureObject(c->table.tex);
-  c->table.tex = 0;
-  cudaFree(c->d_table);
-  c->d_table = tnew;
-  c->table.quad = reinterpret_cast<const float4 *>(c->d_table);
-  c->table.nE = nE;
-  c->table.nB = nB;
-  c->table.lnE_min = lnE_min;
-  const double inv = (double)(nE - 1) / ((double)lnE_max - (double)lnE_min);
-  c->table.inv_dlnE = (float)inv;
-  c->table.c1 = (float)(0.6931471805599453 * inv);
-  c->table.c0 = (float)(-(double)lnE_min * inv);
-  c->table.fE1 = (float)(nE - 1);
-  c->table.fB1 = (float)(nB - 1);
-  make_table_texture(c, nq);
-  c->has_table = true;
+  install_quad_table(c, nE, nB, lnE_min, lnE_max, tnew);
+  return DSMC_OK;
+}
+
+int dsmc_build_chi_table_mlp(dsmc_ctx *c, int32_t nE, int32_t nB, float lnE_min, float lnE_max, uint32_t flags,
+                             float *chi_out) {
+  if (!c || nE < 2 || nB < 2 || !(lnE_max > lnE_min) || (flags & ~(uint32_t)DSMC_F_BF16_TC)) return DSMC_ERR_INVALID_ARG;
+  if (!c->has_mlp[1]) return DSMC_ERR_NOT_CONFIGURED;
+  if ((flags & DSMC_F_BF16_TC) && c->mlp_tc[1].H == 0) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  CK(cudaSetDevice(c->device));
+  CK(cudaStreamSynchronize(c->stream));
+  const size_t nq = (size_t)(nE - 1) * (nB - 1), nn = (size_t)nE * nB;
+  float *nodes = nullptr, *tnew = nullptr, *coord = nullptr;
+  CK(cudaMalloc(&tnew, sizeof(float) * 4 * nq));
+  if (cudaMalloc(&nodes, sizeof(float) * nn) != cudaSuccess || cudaMalloc(&coord, sizeof(float) * 2 * nn) != cudaSuccess) {
+    cudaFree(tnew);
+    cudaFree(nodes);
+    return DSMC_ERR_CUDA;
+  }
+  // node coordinates as a pair batch (E_r / k_B = exp(lnE_i), b = j / (nB - 1) with b_max = 1), the chi-MLP on them
+  // through the same kernels dsmc_chi_batch uses, then the cap (Q23) and the quad layout
+  int rc = launch_table_node_coords(c, nE, nB, (double)lnE_min, (double)lnE_max, coord, coord + nn);
+  if (rc == DSMC_OK)
+    rc = (flags & DSMC_F_BF16_TC)
+             ? launch_chi_batch_tc(c, (int64_t)nn, coord, coord + nn, nodes, 1.f, lnE_min, lnE_max, &c->mlp_tc[1])
+             : launch_chi_batch(c, (int64_t)nn, coord, coord + nn, nodes, 1, 1.f, lnE_min, lnE_max, &c->mlp[1]);
+  if (rc == DSMC_OK) rc = launch_cap_and_quad(c, nE, nB, nodes, reinterpret_cast<float4 *>(tnew));
+  if (rc == DSMC_OK && chi_out &&
+      cudaMemcpyAsync(chi_out, nodes, sizeof(float) * nn, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+    rc = DSMC_ERR_CUDA;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) rc = DSMC_ERR_CUDA;
+  cudaFree(nodes);
+  cudaFree(coord);
+  if (rc != DSMC_OK) {  // the installed table (if any) stays
+    cudaFree(tnew);
+    return rc;
+  }
+  install_quad_table(c, nE, nB, lnE_min, lnE_max, tnew);
   return DSMC_OK;
 }
 

@@ -116,6 +116,43 @@ __global__ void k_quad_from_table(int nE, int nB, const float *__restrict__ tabl
   }
 }
 
+// f2, neural table generation: the node coordinates of the table as a pair batch (E_r / k_B, b / b_max) ...
+__global__ void k_table_node_coords(int nE, int nB, double lnE_min, double dlnE, float *__restrict__ E,
+                                    float *__restrict__ b) {
+  const int64_t total = (int64_t)nE * nB;
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < total; p += (int64_t)gridDim.x * blockDim.x) {
+    const int iE = (int)(p / nB), iB = (int)(p % nB);
+    E[p] = (float)exp(lnE_min + dlnE * iE);
+    b[p] = (float)((double)iB / (double)(nB - 1));
+  }
+}
+
+// ... and, after the network: abs (Q14), cap at 64 pi (Q23, written so that NaN is capped too), quad layout
+__global__ void k_cap_nodes(int64_t total, float *__restrict__ table) {
+  for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < total; p += (int64_t)gridDim.x * blockDim.x) {
+    const float cap = (float)(64.0 * 3.141592653589793);
+    const float c = fabsf(table[p]);
+    table[p] = (c <= cap) ? c : cap;
+  }
+}
+
+int launch_table_node_coords(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_max, float *E, float *b) {
+  const int64_t total = (int64_t)nE * nB;
+  const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->num_sms * 8);
+  k_table_node_coords<<<grid, 256, 0, c->stream>>>(nE, nB, lnE_min, (lnE_max - lnE_min) / (nE - 1), E, b);
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+int launch_cap_and_quad(dsmc_ctx *c, int nE, int nB, float *table_dev, float4 *quad_dev) {
+  const int64_t total = (int64_t)nE * nB;
+  const int grid = (int)std::min<int64_t>((total + 255) / 256, (int64_t)c->num_sms * 8);
+  k_cap_nodes<<<grid, 256, 0, c->stream>>>(total, table_dev);
+  k_quad_from_table<<<grid, 256, 0, c->stream>>>(nE, nB, table_dev, quad_dev);
+  c->launches += 2;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
 // Gauss-Legendre nodes / weights on [0, 1] by Newton iteration on the Legendre polynomial P_n (host, once)
 static void gauss_legendre_01(int n, double *x, double *w) {
   for (int i = 0; i < n; ++i) {

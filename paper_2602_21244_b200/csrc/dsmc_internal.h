@@ -149,6 +149,8 @@ int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, 
                         float lnE_min, float lnE_max, const MlpTcDev *net);
 int launch_chi_exact(dsmc_ctx *c, int64_t n, const float *E_over_k, const float *b, float *chi, double eps_over_k,
                      double sigma, int take_abs);
+int launch_table_node_coords(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_max, float *E, float *b);
+int launch_cap_and_quad(dsmc_ctx *c, int nE, int nB, float *table_dev, float4 *quad_dev);
 int launch_chi_table_lj(dsmc_ctx *c, int nE, int nB, double lnE_min, double lnE_max, double b_max, double eps_over_k,
                         double sigma, float *table_dev, float4 *quad_dev);
 int launch_move_couette(dsmc_ctx *c, int64_t n, float *x, float *vx, float *vy, float *vz, int32_t *cell,

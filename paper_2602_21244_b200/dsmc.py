@@ -28,7 +28,7 @@ ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
-           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_step_host", "dsmc_step_host_submit", "dsmc_move_couette",
+           "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_build_chi_table_mlp", "dsmc_step_host", "dsmc_step_host_submit", "dsmc_move_couette",
            "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run", "dsmc_ntc_counts"]
 
 
@@ -306,6 +306,17 @@ class Context:
                                           C.c_float(b_max), C.c_float(eps_over_k), C.c_float(sigma),
                                           _ptr(out, torch.float32) if out is not None else C.c_void_p(0)),
              "dsmc_build_chi_table_lj")
+        return out
+
+    def build_chi_table_mlp(self, nE: int, nB: int, lnE_min=float(np.log(5.0)), lnE_max=float(np.log(6.0e4)),
+                            flags: int = 0, want_nodes: bool = False):
+        """Generate the chi table on the device from the slot-1 chi-MLP and install it; flags 0 or F_BF16_TC."""
+        out = torch.empty((nE, nB), dtype=torch.float32, device=self.device) if want_nodes else None
+        self._stream()
+        _chk(_lib.dsmc_build_chi_table_mlp(self._h, C.c_int32(nE), C.c_int32(nB), C.c_float(lnE_min), C.c_float(lnE_max),
+                                           C.c_uint32(flags),
+                                           _ptr(out, torch.float32) if out is not None else C.c_void_p(0)),
+             "dsmc_build_chi_table_mlp")
         return out
 
     def chi_exact_batch(self, E_over_k, b, eps_over_k: float = 119.8, sigma: float = 3.405e-10, flags: int = 0,

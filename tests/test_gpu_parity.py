@@ -630,6 +630,42 @@ def test_build_chi_table_on_device(dsmc):
     ctx.close()
 
 
+@pytest.mark.parametrize("tc", [False, True])
+def test_build_chi_table_from_the_chi_mlp(dsmc, tc):
+    """(f2 as the paper states it) the chi table generated on the device by the slot-1 chi-MLP against the
+    oracle's orc_build_chi_table_mlp on EVERY node (FP32: 1e-5 max(chi, 1); tensor cores: Q26), lookups through the
+    installed table, the cap (Q23) on a network that exceeds it, and the error paths."""
+    nE, nB = 96, 80
+    lo, hi = float(np.float32(np.log(5.0))), float(np.float32(np.log(6.0e4)))
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx = dsmc.Context(1 << 16, 1)
+    with pytest.raises(RuntimeError):
+        ctx.build_chi_table_mlp(nE, nB, lo, hi)  # no slot-1 network yet
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    got = ctx.build_chi_table_mlp(nE, nB, lo, hi, flags=dsmc.F_BF16_TC if tc else 0, want_nodes=True).cpu().numpy()
+    ctx.check()
+    want = oracle.build_chi_table_mlp(oracle.Mlp(Ws, bs, oracle.ACT_SILU), nE, nB, lo, hi).chi.astype(np.float64)
+    rel = np.abs(got.astype(np.float64) - want) / (np.maximum(want, 1) if not tc else 1 + want)
+    _note("node error", rel.max(), 2e-2 if tc else 1e-5)
+    assert rel.max() <= (2e-2 if tc else 1e-5)
+    # the installed table serves lookups: bilinear interpolation of the nodes the device produced
+    E, b = wl.abinitio_pair_batch(seed=9, n=50_000)
+    chi = ctx.chi_batch(dev(E), dev(b), 0, 1e-9).cpu().numpy().astype(np.float64)
+    tab_g = oracle.ChiTable(got, lo, hi)
+    ref = oracle.chi_batch(E, b, 0, 1e-9, table=tab_g)
+    sl = _table_slope(tab_g, np.log(E.astype(np.float64)), b.astype(np.float64) / 1e-9)
+    assert np.all(np.abs(chi - ref) <= 1e-5 * np.maximum(np.abs(ref), 1) + 2e-4 * sl + 1e-6)
+    if not tc:
+        # Q23: a network whose output exceeds 64 pi everywhere is capped, node by node
+        big = [np.zeros((16, 2), np.float32), np.zeros((1, 16), np.float32)], [np.zeros(16, np.float32), np.array([6.0], np.float32)]
+        ctx.set_mlp(1, big[0], big[1], dsmc.ACT_SILU)
+        capped = ctx.build_chi_table_mlp(8, 8, lo, hi, want_nodes=True).cpu().numpy()
+        assert np.all(capped == np.float32(64 * np.pi))
+        with pytest.raises(RuntimeError):
+            ctx.build_chi_table_mlp(8, 8, lo, hi, flags=dsmc.F_BF16_TC)  # this shape has no tensor-core image
+    ctx.close()
+
+
 def test_chapman_enskog_from_the_gpu_quadrature(dsmc):
     """(f2) physics check that does not involve the oracle: Omega^(2,2)*(T*) of the LJ gas from the GPU's own
     deflection angles (eqs. 18-19, standard Chapman-Enskog form) against the textbook table."""
