@@ -597,6 +597,10 @@ struct CellTeam {
           f0[u] = st[32 * u + lane];
           f1[u] = st[128 + 32 * u + lane];
         }
+        // (the same words then receive z: the server ADDS the partial sums of its column groups into them)
+        __syncwarp();
+#pragma unroll
+        for (int u = 0; u < 4; ++u) reinterpret_cast<float *>(K2 + 256 * warp)[32 * u + lane] = 0.f;
         const int slot = srv->acquire(lane, K2 + 256 * warp);
 #pragma unroll
         for (int u = 0; u < 4; ++u) srv->write_row(slot, 32 * u + lane, f0[u], f1[u]);

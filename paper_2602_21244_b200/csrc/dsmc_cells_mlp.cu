@@ -9,16 +9,23 @@
 //                      into that tile's layer-1 operand and publishes it; then it starts on its next cell in the
 //                      other buffer and only afterwards sleeps until z of the first tile has been delivered into its
 //                      shared memory, rotates, commits, matches and stores as in the table kernel.
-//   MLP server         NA activation warps + one MMA warp around the two-slot tcgen05 pipeline of dsmc_tc_pipe.cuh:
-//                      layer 1 from shared memory (SS), layers 2 and 3 with the activations kept in tensor memory (TS).
-//                      Tile t runs in slot t & 1; a ROUND is the two tiles 2 r, 2 r + 1 and both kinds of server warps
-//                      walk the rounds in a fixed order on blocking mbarrier waits (a wake-up costs ~60 cycles, a poll
-//                      ~150: measured, profiles/r02_*).  The first four activation warps deliver the layer-3 outputs.
-//                      The MMA warp fills slot 1 with an empty tile when nobody feeds it (so that a tile in slot 0 is
-//                      never held back), and stops the server when every team warp has finished.
+//   MLP server         two independent pipelines, one per tensor-memory slot (tile t runs in slot t & 1): an MMA
+//                      issue warp and NA / 2 activation warps each, around the operands of dsmc_tc_pipe.cuh.  Layer 1
+//                      from shared memory (SS), layer 2 with the activations kept in tensor memory (TS); the output
+//                      layer (d_out = 1) is NOT a third tensor-core layer: the warps that apply the second activation
+//                      form z = b3 + sum_j w3[j] act(D[row][j]) on the CUDA cores (FP32 weights as constant-bank
+//                      operands) and add their partial sums into the feeding warp's shared memory -- one hand-off
+//                      (tensor core -> activation warps -> delivery warps) and its ~1300 cycles per tile are gone.
+//                      Every wait is a blocking mbarrier wait on the data it needs; a slot never looks at the other
+//                      one, so nothing has to be injected when one of them runs dry, and each MMA warp stops when
+//                      every team warp has finished and its next tile number was never taken.
 //
-// The server is bound by the XU pipe (one MUFU per hidden activation); the team warps exist to keep its two slots
-// full, so their own latencies (HBM loads, waiting for z) cost nothing as long as enough tiles are in flight.
+// Measured on cfg 5: with the activations switched off the kernel still takes 0.98 ms -- twelve
+// team warps per SM (shared memory: two cell buffers each beside 82 KB of weights and operands) are latency-bound at
+// ~35 000 cycles per cell -- and the server's chain per tile (activation 1, layer 2, activation 2, layer 1 of the next
+// tile) is ~8 000 cycles per slot.  Both sides run at about the same pace, which is why variants of either one alone
+// (lock-step rounds, an XU-pipe lock between the slots, 20 single-buffered team warps with 8 activation warps) all
+// land within 4 % of one another.
 #include <algorithm>
 
 #include "dsmc_cells.cuh"
@@ -26,7 +33,15 @@
 
 namespace dsmc {
 
+#ifdef CM_TRACE
+// per-warp trace region, plain stores (no atomics: a stamp must not stall the warp)
+#define CM_STAMP(tag) do { if (blockIdx.x == 0 && lane == 0 && P.cap && cm_n < 900) { long long *tb = (long long *)P.cap; tb[1 + cm_region * 900 + cm_n++] = ((long long)(tag) << 40) | (clock64() & 0xFFFFFFFFFFll); } } while (0)
+#else
+#define CM_STAMP(tag) do { } while (0)
+#endif
+
 constexpr int kMlpMaxFeeders = 32;
+
 
 // Hand-offs between the team warps and the server.  Tiles are numbered by a ticket t: tile t runs in tensor-memory
 // slot s = t & 1 and is the k-th tile of that slot, k = t >> 1; its layer-1 operand lives in buffer par = k & 1 of the
@@ -35,16 +50,14 @@ constexpr int kMlpMaxFeeders = 32;
 struct CellsMlpCtl {
   uint64_t in_bar[2][2];               // rows of the tile in (slot, par) are written            (1 arrival)
   uint64_t op_bar[2];                  // one phase per finished layer 1 of the slot            (1 arrival)
-  uint64_t out_bar[2];                 // one phase per delivered tile of the slot              (4 arrivals)
-  uint64_t done_bar[2 * kMlpMaxFeeders];  // [feeding warp][its buffer]: one phase per delivered tile (4 arrivals);
+  uint64_t done_bar[2 * kMlpMaxFeeders];  // [feeding warp][its buffer]: one phase per delivered tile (NA / 2 arrivals);
                                           // one tile in flight per barrier, so a phase parity identifies it
   float *dest[2][4];                   // where the outputs of tile k of the slot go (ring: entry k & 3 is rewritten
   int feeder[2][4];                    // for tile k + 4, after tile k has been delivered), and who waits for them
   int op_done[2];                      // finished layer 1s of the slot
   int ticket;
   int done;                            // team warps that ran out of work
-  int poison;                          // the round after the last one with real tiles (set by the last team warp)
-  float scratch[128];                  // outputs of empty tiles
+  int stop_k[2];                       // per slot: the tile index at which its server warps stop (set by its MMA warp)
 };
 
 // warp-uniform test of an mbarrier phase (lanes may observe the completion at different times)
@@ -74,6 +87,13 @@ __device__ __forceinline__ bool cm_try_wait(uint64_t *bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
+
+// output layer (d_out = 1) of the chi-MLP in FP32, passed by value: the weights are then constant-bank operands of the
+// FMAs that form z (no load, no latency)
+struct CellsMlpW3 {
+  float w[128];
+  float b;
+};
 
 // what a team warp sees of the server
 template <int H>
@@ -125,14 +145,40 @@ struct CellsMlpFeeder {
   }
 };
 
-template <int H, int NA, int NTW>
-__global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const StepParams P, const CellLists Lst,
-                                                                      const MlpTcDev net) {
+// this thread's share of z for its row: sum over the columns of column group HALF of w3[j] act(D[row][j]) (+ b3 in
+// group 0); the column indices are compile-time, so the weights are constant-bank operands
+template <int H, int NQ, int HALF, int ACT>
+__device__ __forceinline__ float out_partial(uint32_t d0, const CellsMlpW3 &W3) {
+  constexpr int NC = H / (16 * NQ), C0 = HALF * (H / NQ);
+  uint32_t v[2][16];
+  float acc0 = HALF == 0 ? W3.b : 0.f, acc1 = 0.f;
+  tc::tmem_ld16(d0, v[0]);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    tc::wait_ld();
+    if (c + 1 < NC) tc::tmem_ld16(d0 + (c + 1) * 16, v[(c + 1) & 1]);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const float z = __uint_as_float(v[c & 1][j]);
+      float h;
+      if (ACT == DSMC_ACT_TANH) h = tc::tanh_approx(z);
+      else if (ACT == DSMC_ACT_RELU) h = fmaxf(z, 0.f);
+      else h = fmaf(z, tc::tanh_approx(z), z);  // SiLU(2 y) = y + y tanh(y), y = z (the weights carry the 1/2)
+      if (j & 1) acc1 = fmaf(h, W3.w[C0 + 16 * c + j], acc1);
+      else acc0 = fmaf(h, W3.w[C0 + 16 * c + j], acc0);
+    }
+  }
+  return acc0 + acc1;
+}
+
+template <int H, int NA, int NTW, int NBUF>
+__global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const StepParams P, const CellLists Lst,
+                                                                      const MlpTcDev net, const CellsMlpW3 W3) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   using SH = PipeShape<H>;
   using Feeder = CellsMlpFeeder<H>;
   constexpr size_t SLICE = CellTeam<32>::bytes();
-  constexpr size_t TEAMS = (2 * NTW * SLICE + 127) & ~(size_t)127;  // two buffers per team
+  constexpr size_t TEAMS = (NBUF * NTW * SLICE + 127) & ~(size_t)127;  // NBUF cells in flight per team
   unsigned char *pipe_base = smem_raw + TEAMS;
   CellsMlpCtl *ctl = reinterpret_cast<CellsMlpCtl *>(pipe_base + SH::SMEM_BYTES);
   TcPipe<H> pipe;
@@ -141,18 +187,17 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
       tc::mbar_init(&ctl->in_bar[s2][0], 1);
       tc::mbar_init(&ctl->in_bar[s2][1], 1);
       tc::mbar_init(&ctl->op_bar[s2], 1);
-      tc::mbar_init(&ctl->out_bar[s2], 4);
       ctl->op_done[s2] = 0;
     }
-    for (int f = 0; f < 2 * kMlpMaxFeeders; ++f) tc::mbar_init(&ctl->done_bar[f], 4);
+    for (int f = 0; f < 2 * kMlpMaxFeeders; ++f) tc::mbar_init(&ctl->done_bar[f], NA / 2);
     ctl->ticket = 0;
-    ctl->poison = 0x7FFFFFFF;
+    ctl->stop_k[0] = ctl->stop_k[1] = 0x7FFFFFFF;
     ctl->done = 0;
     tc::mbar_fence_init();
   }
-  pipe.init(pipe_base, net.w_blob, NA, 1);  // one feeding warp per tile; ends with CTA-wide barriers
+  pipe.init(pipe_base, net.w_blob, NA / 2, 1);  // eight activation warps per slot; ends with CTA-wide barriers
   // constant part of the layer-1 operands (zeros and the bias column block), both slots
-  for (int i = threadIdx.x; i < 4 * 128; i += (NTW + NA + 1) * 32) {
+  for (int i = threadIdx.x; i < 4 * 128; i += (NTW + NA + 2) * 32) {
     unsigned char *a = pipe.a1 + (i >> 7) * SH::A1_BYTES + (i & 127) * 16;
 #pragma unroll
     for (int j = 0; j < 3; ++j) *reinterpret_cast<uint4 *>(a + j * 128 * 16) = make_uint4(0u, 0u, 0u, 0u);
@@ -160,6 +205,10 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
   }
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#ifdef CM_TRACE
+  int cm_n = 0;
+  const int cm_region = warp >= NTW + NA ? 2 + (warp - NTW - NA) : ((warp - NTW) >> 2) & 1;  // ACT leaders 0/1, MMA 2/3
+#endif
   // the team warps come first (NTW is a multiple of 4): activation warp aw reads the tensor-memory lanes
   // 32 (aw & 3) .., which the hardware ties to (warp index & 3); and the scheduler prefers the higher warp indices,
   // which keeps the server ahead of the teams that feed it
@@ -175,24 +224,30 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
     if (tw < 8 * G8) {  // cells of 1025..2048 particles: groups of eight warps
       const int g = tw >> 3;
       CellTeam<256, 2, Feeder> T;
-      T.init(base_s + (uint32_t)(16 * g * SLICE), ttid - 256 * g, 1 + g);
+      const uint32_t b0 = base_s + (uint32_t)(8 * NBUF * g * SLICE);
+      T.init(b0, ttid - 256 * g, 1 + g);
       T.srv = &srv;
-      T.run2(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2, base_s + (uint32_t)(16 * g * SLICE), base_s + (uint32_t)((16 * g + 8) * SLICE));
+      if (NBUF == 2) T.run2(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2, b0, b0 + (uint32_t)(8 * SLICE));
+      else T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
       asm volatile("bar.sync %0, 256;" ::"r"(1 + g) : "memory");
     }
     if (tw < 4 * G4) {  // cells of 257..1024 particles: groups of four warps
       const int g = tw >> 2;
       CellTeam<128, 2, Feeder> T;
-      T.init(base_s + (uint32_t)(8 * g * SLICE), ttid - 128 * g, 1 + G8 + g);
+      const uint32_t b0 = base_s + (uint32_t)(4 * NBUF * g * SLICE);
+      T.init(b0, ttid - 128 * g, 1 + G8 + g);
       T.srv = &srv;
-      T.run2(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1, base_s + (uint32_t)(8 * g * SLICE), base_s + (uint32_t)((8 * g + 4) * SLICE));
+      if (NBUF == 2) T.run2(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1, b0, b0 + (uint32_t)(4 * SLICE));
+      else T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
       asm volatile("bar.sync %0, 128;" ::"r"(1 + G8 + g) : "memory");
     }
     {
       CellTeam<32, 2, Feeder> T;
-      T.init(base_s + (uint32_t)(2 * tw * SLICE), lane, 0);
+      const uint32_t b0 = base_s + (uint32_t)(NBUF * tw * SLICE);
+      T.init(b0, lane, 0);
       T.srv = &srv;
-      T.run2(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0, base_s + (uint32_t)(2 * tw * SLICE), base_s + (uint32_t)((2 * tw + 1) * SLICE));
+      if (NBUF == 2) T.run2(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0, b0, b0 + (uint32_t)SLICE);
+      else T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
     }
     }
     if (lane == 0) {
@@ -201,148 +256,100 @@ __global__ void __launch_bounds__((NTW + NA + 1) * 32, 1) k_cells_mlp(const Step
     }
   } else if (warp < NTW + NA) {
     // ---------------- MLP server: activation + delivery warps ----------------
-    // Fixed order, blocking waits (as in k_chi_batch_tc): round r = tiles 2 r (slot 0) and 2 r + 1 (slot 1).
+    // Two independent pipelines, one per slot: activation warp aw serves slot (aw >> 2) & 1 (eight warps per slot: the
+    // four lane quadrants x two column halves), walks that slot's tiles k = 0, 1, ... on blocking waits and never
+    // looks at the other slot.  While one group waits for its tensor-core layer or delivers, the other has the XU
+    // pipe to itself, so the latencies of one slot's hand-offs hide behind the other slot's activations.
     const int aw = warp - NTW;
-    uint32_t phe[2] = {0u, 0u}, pho[2] = {0u, 0u};
-    bool pend1 = false;  // slot 1 of the previous round is still to be delivered
-    // rows 32 aw .. 32 aw + 31 of the layer-3 output of tile (slot s2, round rr) -> the feeding warp (aw < 4)
-    auto deliver = [&](int s2, int rr) {
-      tc::mbar_wait(pipe.full_o + s2, pho[s2]);
-      pho[s2] ^= 1u;
-      tc::fence_after();
-      uint32_t v[4];
-      tc::tmem_ld4(pipe.tmem + (((uint32_t)(aw * 32)) << 16) + s2 * SH::SLOT_COLS + SH::COL_OUT, v);
-      tc::wait_ld();
-      tc::fence_before();
-      float *dest = *reinterpret_cast<float *volatile *>(&ctl->dest[s2][rr & 3]);
-      const int f = cm_ld_volatile(&ctl->feeder[s2][rr & 3]);
-      dest[aw * 32 + lane] = __uint_as_float(v[0]);
+    const int s2 = (aw >> 2) & 1, q = aw & 3, half = aw >> 3;
+    const int aw_slot = q | (half << 2);  // act_body: lane quadrant = aw_slot & 3, column group = aw_slot >> 2
+    constexpr int NQ = NA / 8;  // column groups per slot
+    uint32_t phe = 0u;
+    for (int k = 0;; ++k) {
+      // ---- hidden layer 1: D -> activation -> bf16 A operand of layer 2 (tensor memory) ----
+      tc::mbar_wait(pipe.full_e + s2, phe);
+      phe ^= 1u;
+      if (aw_slot == 0) CM_STAMP(10 + 10 * s2);
+      if (k == cm_ld_volatile(&ctl->stop_k[s2])) goto server_done;
+      if (aw_slot == 0 && lane == 0) {  // the slot's layer-1 operand buffer may be rewritten
+        *reinterpret_cast<volatile int *>(&ctl->op_done[s2]) = k + 1;
+        __threadfence_block();
+        cm_arrive(&ctl->op_bar[s2]);
+      }
+      __syncwarp();
+      pipe.template act_body<NQ>(net.act, s2, aw_slot);
+      if (aw_slot == 0) CM_STAMP(11 + 10 * s2);
+      // ---- hidden layer 2 and the output layer (d_out = 1) in one pass: z = b3 + sum_j w3[j] act(D[row][j]) on the
+      // CUDA cores, so no third tensor-core layer and no hand-off for it; the two column groups of a row add their
+      // partial sums into the feeding warp's (zeroed) buffer: x + y = y + x, the result does not depend on the order
+      tc::mbar_wait(pipe.full_e + s2, phe);
+      phe ^= 1u;
+      if (aw_slot == 0) CM_STAMP(12 + 10 * s2);
+      float *dest = *reinterpret_cast<float *volatile *>(&ctl->dest[s2][k & 3]);
+      const int f = cm_ld_volatile(&ctl->feeder[s2][k & 3]);
+      {
+        tc::fence_after();
+        const uint32_t d0 = pipe.tmem + (((uint32_t)(q * 32)) << 16) + s2 * SH::SLOT_COLS + SH::COL_D + half * (H / NQ);
+        float part;
+        if (net.act == DSMC_ACT_SILU)
+          part = half == 0 ? out_partial<H, NQ, 0, DSMC_ACT_SILU>(d0, W3) : out_partial<H, NQ, 1, DSMC_ACT_SILU>(d0, W3);
+        else if (net.act == DSMC_ACT_TANH)
+          part = half == 0 ? out_partial<H, NQ, 0, DSMC_ACT_TANH>(d0, W3) : out_partial<H, NQ, 1, DSMC_ACT_TANH>(d0, W3);
+        else
+          part = half == 0 ? out_partial<H, NQ, 0, DSMC_ACT_RELU>(d0, W3) : out_partial<H, NQ, 1, DSMC_ACT_RELU>(d0, W3);
+        tc::fence_before();
+        asm volatile("red.shared.add.f32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(dest + q * 32 + lane)), "f"(part)
+                     : "memory");
+      }
+      if (aw_slot == 0) CM_STAMP(13 + 10 * s2);
       __syncwarp();
       if (lane == 0) {
         __threadfence_block();
-        cm_arrive(&ctl->out_bar[s2]);  // the output columns may be overwritten (layer 3 of the next round)
-        cm_arrive(&ctl->done_bar[f]);  // z is in the feeding warp's shared memory
-      }
-    };
-    // Order of a round: act(0, L1), [deliver slot 1 of the previous round], act(1, L1), act(0, L2), act(1, L2),
-    // deliver slot 0.  Slot 1's layer 3 is issued only when act(1, L2) ends, so its delivery waits until the next
-    // activation is done rather than hold up four of the activation warps.
-    for (int r = 0;; ++r) {
-#pragma unroll
-      for (int layer = 0; layer < 2; ++layer) {
-#pragma unroll
-        for (int s2 = 0; s2 < 2; ++s2) {
-          if (layer == 0 && s2 == 0 && aw < 4 && r >= 1) {
-            // the next round normally stands ready (its layer 1 was issued early); if it does not, slot 1 of the last
-            // round is delivered while waiting: a submitted tile never depends on further tiles being fed
-            while (!cm_test(pipe.full_e + 0, phe[0])) {
-              if (pend1 && cm_test(pipe.full_o + 1, pho[1])) {
-                deliver(1, r - 1);
-                pend1 = false;
-              }
-            }
-          } else {
-            tc::mbar_wait(pipe.full_e + s2, phe[s2]);
-          }
-          phe[s2] ^= 1u;
-          if (layer == 0 && s2 == 0 && r == cm_ld_volatile(&ctl->poison)) {
-            if (aw < 4 && pend1) deliver(1, r - 1);
-            goto server_done;
-          }
-          if (layer == 0 && aw == 0 && lane == 0) {  // the slot's layer-1 operand buffer may be rewritten
-            *reinterpret_cast<volatile int *>(&ctl->op_done[s2]) = r + 1;
-            __threadfence_block();
-            cm_arrive(&ctl->op_bar[s2]);
-          }
-          __syncwarp();
-          pipe.template act_body<NA / 4>(net.act, s2, aw);
-          if (layer == 0 && s2 == 0 && aw < 4 && pend1) {
-            deliver(1, r - 1);
-            pend1 = false;
-          }
-        }
-      }
-      if (aw < 4) {
-        deliver(0, r);
-        pend1 = true;
+        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(pipe.a_ready + s2)) : "memory");  // D may be overwritten
+        cm_arrive(&ctl->done_bar[f]);  // this warp's share of z is in the feeding warp's shared memory
       }
     }
   } else {
-    // ---------------- MLP server: MMA issue warp ----------------
-    // layer 3 of both slots goes out before the warp waits for the rows of the next round, so every submitted tile
-    // is delivered whatever the team warps do next
-    uint32_t pa[2] = {0u, 0u};
-    // Rows of tile 2 r + s2.  0: they are there.  1: nobody has taken that tile number and either every team warp has
-    // finished or slot 1 has waited long enough while slot 0 holds a real tile: the warp takes the number itself and the
-    // round runs with an empty tile in slot 1 (stale operand, outputs to nobody).  2 (slot 0 only): no tile will ever
-    // come: stop.
-    auto rows = [&](int s2, int r) -> int {
-      const int t = 2 * r + s2;
-      uint64_t *bar = &ctl->in_bar[s2][r & 1];
-      const uint32_t par = (uint32_t)(r >> 1) & 1u;
-      for (int it = 0;; ++it) {
-        if (__any_sync(0xffffffffu, tc::mbar_test(bar, par))) return 0;
-        int act = 0;
-        if (lane == 0 && cm_ld_volatile(&ctl->ticket) == t) {
-          const bool all_done = cm_ld_volatile(&ctl->done) == NTW;  // then no number is taken any more
-          if (s2 == 0) {
-            if (all_done && cm_ld_volatile(&ctl->ticket) == t) act = 2;
-          } else if ((all_done || it > 8) && atomicCAS(&ctl->ticket, t, t + 1) == t) {
-            *reinterpret_cast<float *volatile *>(&ctl->dest[s2][r & 3]) = ctl->scratch;
-            *reinterpret_cast<volatile int *>(&ctl->feeder[s2][r & 3]) = 2 * kMlpMaxFeeders - 1;
-            __threadfence_block();
-            cm_arrive(bar);
-            act = 1;
-          }
+    // ---------------- MLP server: one MMA issue warp per slot ----------------
+    const int s2 = warp - NTW - NA;
+    uint32_t pa = 0u;
+    for (int k = 0;; ++k) {
+      // rows of tile t = 2 k + s2: wait for them; stop when nobody has taken that number and nobody will
+      const int t = 2 * k + s2;
+      uint64_t *bar = &ctl->in_bar[s2][k & 1];
+      const uint32_t par = (uint32_t)(k >> 1) & 1u;
+      bool stop = false;
+      CM_STAMP(33 + 10 * s2);
+      for (;;) {
+        if (cm_try_wait_ns(bar, par, 2000u)) break;
+        int st = 0;
+        if (lane == 0) {
+          const int d = cm_ld_volatile(&ctl->done);      // read first: once every team warp has finished ...
+          const int tk = cm_ld_volatile(&ctl->ticket);   // ... no tile number is taken any more
+          st = (d == NTW && tk <= t) ? 1 : 0;
         }
-        act = __shfl_sync(0xffffffffu, act, 0);
-        if (act) return act;
+        if (__shfl_sync(0xffffffffu, st, 0)) {
+          stop = true;
+          break;
+        }
       }
-    };
-    bool first = true;
-    if (rows(0, 0) == 2) {
-      *reinterpret_cast<volatile int *>(&ctl->poison) = 0;
-      __threadfence_block();
-    }
-    pipe.issue_layer1(0, 0, first);  // (an empty one when stopping: it wakes the activation warps)
-    first = false;
-    if (cm_ld_volatile(&ctl->poison) != 0) {
-      rows(1, 0);
-      pipe.issue_layer1(1, 0, false);
-      for (int r = 0;; ++r) {
-        // are the rows of the next round there already?  (asked now, while the activation warps work, because the
-        // answer takes ~150 cycles; normally they are, and the round ends without looking again)
-        const bool early0 = __any_sync(0xffffffffu, tc::mbar_test(&ctl->in_bar[0][(r + 1) & 1], (uint32_t)((r + 1) >> 1) & 1u));
-        const bool early1 = __any_sync(0xffffffffu, tc::mbar_test(&ctl->in_bar[1][(r + 1) & 1], (uint32_t)((r + 1) >> 1) & 1u));
-#pragma unroll
-        for (int s2 = 0; s2 < 2; ++s2) {
-          tc::mbar_wait(pipe.a_ready + s2, pa[s2]);
-          pa[s2] ^= 1u;
-          pipe.issue_layer2(s2);
+      if (stop) {
+        if (lane == 0) {
+          *reinterpret_cast<volatile int *>(&ctl->stop_k[s2]) = k;
+          __threadfence_block();
         }
-        bool stop = false;
-#pragma unroll
-        for (int s2 = 0; s2 < 2; ++s2) {
-          tc::mbar_wait(pipe.a_ready + s2, pa[s2]);
-          pa[s2] ^= 1u;
-          if (r >= 1) tc::mbar_wait(&ctl->out_bar[s2], (uint32_t)(r - 1) & 1u);  // previous round delivered
-          pipe.issue_layer3(s2);
-          // slot 0's next layer 1 goes out ahead of slot 1's layer 3 when its rows are there (the usual case): the
-          // activation warps then find work the moment they finish act(1, L2).  Otherwise it waits until both layer 3s
-          // are out, so that every submitted tile is delivered whatever the team warps do next.
-          if (s2 == (early0 ? 0 : 1)) {
-            stop = !early0 && rows(0, r + 1) == 2;
-            if (stop) {
-              *reinterpret_cast<volatile int *>(&ctl->poison) = r + 1;
-              __threadfence_block();
-            }
-            pipe.issue_layer1(0, (r + 1) & 1, false);
-          }
-        }
-        if (stop) break;
-        if (!early1) rows(1, r + 1);
-        pipe.issue_layer1(1, (r + 1) & 1, false);
+        __syncwarp();
+        pipe.issue_layer1(s2, k & 1, k == 0);  // an empty one: it wakes the slot's activation warps, which then stop
+        break;
       }
+      CM_STAMP(30 + 10 * s2);
+      pipe.issue_layer1(s2, k & 1, k == 0);
+      tc::mbar_wait(pipe.a_ready + s2, pa);
+      pa ^= 1u;
+      CM_STAMP(31 + 10 * s2);
+      pipe.issue_layer2(s2);
+      tc::mbar_wait(pipe.a_ready + s2, pa);  // the second activation has read D: the next tile's layer 1 may go
+      pa ^= 1u;
     }
   }
 server_done:
@@ -351,14 +358,15 @@ server_done:
 
 void launch_cell_lists(dsmc_ctx *c, const StepParams &p, CellLists &L);  // dsmc_cells.cu
 
-template <int H, int NA, int NTW>
-static int launch_cells_mlp_one(dsmc_ctx *c, const StepParams &p, const CellLists &L, const MlpTcDev &net) {
-  auto kern = k_cells_mlp<H, NA, NTW>;
-  const size_t smem = ((2 * NTW * CellTeam<32>::bytes() + 127) & ~(size_t)127) + PipeShape<H>::SMEM_BYTES +
+template <int H, int NA, int NTW, int NBUF>
+static int launch_cells_mlp_one(dsmc_ctx *c, const StepParams &p, const CellLists &L, const MlpTcDev &net,
+                               const CellsMlpW3 &w3) {
+  auto kern = k_cells_mlp<H, NA, NTW, NBUF>;
+  const size_t smem = ((NBUF * NTW * CellTeam<32>::bytes() + 127) & ~(size_t)127) + PipeShape<H>::SMEM_BYTES +
                       sizeof(CellsMlpCtl) + 128;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
-  kern<<<c->num_sms, (NTW + NA + 1) * 32, smem, c->stream>>>(p, L, net);
+  kern<<<c->num_sms, (NTW + NA + 2) * 32, smem, c->stream>>>(p, L, net, w3);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
@@ -369,8 +377,11 @@ int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *n
     return DSMC_ERR_UNSUPPORTED_SHAPE;
   CellLists L;
   launch_cell_lists(c, p, L);
-  if (net->H == 128) return launch_cells_mlp_one<128, 16, 12>(c, p, L, *net);
-  return launch_cells_mlp_one<64, 16, 12>(c, p, L, *net);
+  CellsMlpW3 w3;
+  for (int i = 0; i < 128; ++i) w3.w[i] = i < net->H ? net->w3_host[i] : 0.f;
+  w3.b = net->w3_host[128];
+  if (net->H == 128) return launch_cells_mlp_one<128, 16, 12, 2>(c, p, L, *net, w3);
+  return launch_cells_mlp_one<64, 16, 12, 2>(c, p, L, *net, w3);
 }
 
 }  // namespace dsmc

@@ -80,6 +80,11 @@ int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStre
   out->act = d->act;
   out->w_blob = *d_blob;
   out->blob_bytes = (uint32_t)bytes;
+  for (int k = 0; k < 129; ++k) out->w3_host[k] = 0.f;
+  if (d_out == 1) {
+    for (int k = 0; k < H; ++k) out->w3_host[k] = d->W[2][k];
+    out->w3_host[128] = d->b[2][0];
+  }
   return DSMC_OK;
 }
 

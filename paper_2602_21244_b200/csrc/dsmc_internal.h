@@ -34,6 +34,7 @@ struct MlpTcDev {
   int d_in, d_out, act;
   const void *w_blob;         // bf16 weights and biases (hi + lo parts) in UMMA K-major core-matrix layout
   uint32_t blob_bytes;
+  float w3_host[129];         // HOST copy of the FP32 output layer when d_out = 1: w[0..H), bias at [128]
 };
 
 struct ChiTableDev {
