@@ -88,13 +88,6 @@ __device__ __forceinline__ bool cm_try_wait(uint64_t *bar, uint32_t parity) {
   return ok != 0;
 }
 
-// output layer (d_out = 1) of the chi-MLP in FP32, passed by value: the weights are then constant-bank operands of the
-// FMAs that form z (no load, no latency)
-struct CellsMlpW3 {
-  float w[128];
-  float b;
-};
-
 // what a team warp sees of the server
 template <int H>
 struct CellsMlpFeeder {
@@ -145,35 +138,9 @@ struct CellsMlpFeeder {
   }
 };
 
-// this thread's share of z for its row: sum over the columns of column group HALF of w3[j] act(D[row][j]) (+ b3 in
-// group 0); the column indices are compile-time, so the weights are constant-bank operands
-template <int H, int NQ, int HALF, int ACT>
-__device__ __forceinline__ float out_partial(uint32_t d0, const CellsMlpW3 &W3) {
-  constexpr int NC = H / (16 * NQ), C0 = HALF * (H / NQ);
-  uint32_t v[2][16];
-  float acc0 = HALF == 0 ? W3.b : 0.f, acc1 = 0.f;
-  tc::tmem_ld16(d0, v[0]);
-#pragma unroll
-  for (int c = 0; c < NC; ++c) {
-    tc::wait_ld();
-    if (c + 1 < NC) tc::tmem_ld16(d0 + (c + 1) * 16, v[(c + 1) & 1]);
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-      const float z = __uint_as_float(v[c & 1][j]);
-      float h;
-      if (ACT == DSMC_ACT_TANH) h = tc::tanh_approx(z);
-      else if (ACT == DSMC_ACT_RELU) h = fmaxf(z, 0.f);
-      else h = fmaf(z, tc::tanh_approx(z), z);  // SiLU(2 y) = y + y tanh(y), y = z (the weights carry the 1/2)
-      if (j & 1) acc1 = fmaf(h, W3.w[C0 + 16 * c + j], acc1);
-      else acc0 = fmaf(h, W3.w[C0 + 16 * c + j], acc0);
-    }
-  }
-  return acc0 + acc1;
-}
-
 template <int H, int NA, int NTW, int NBUF>
 __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const StepParams P, const CellLists Lst,
-                                                                      const MlpTcDev net, const CellsMlpW3 W3) {
+                                                                      const MlpTcDev net, const TcOutLayer W3) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   using SH = PipeShape<H>;
   using Feeder = CellsMlpFeeder<H>;
@@ -292,11 +259,11 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
         const uint32_t d0 = pipe.tmem + (((uint32_t)(q * 32)) << 16) + s2 * SH::SLOT_COLS + SH::COL_D + half * (H / NQ);
         float part;
         if (net.act == DSMC_ACT_SILU)
-          part = half == 0 ? out_partial<H, NQ, 0, DSMC_ACT_SILU>(d0, W3) : out_partial<H, NQ, 1, DSMC_ACT_SILU>(d0, W3);
+          part = half == 0 ? tc_out_partial<H, NQ, 0, DSMC_ACT_SILU>(d0, W3) : tc_out_partial<H, NQ, 1, DSMC_ACT_SILU>(d0, W3);
         else if (net.act == DSMC_ACT_TANH)
-          part = half == 0 ? out_partial<H, NQ, 0, DSMC_ACT_TANH>(d0, W3) : out_partial<H, NQ, 1, DSMC_ACT_TANH>(d0, W3);
+          part = half == 0 ? tc_out_partial<H, NQ, 0, DSMC_ACT_TANH>(d0, W3) : tc_out_partial<H, NQ, 1, DSMC_ACT_TANH>(d0, W3);
         else
-          part = half == 0 ? out_partial<H, NQ, 0, DSMC_ACT_RELU>(d0, W3) : out_partial<H, NQ, 1, DSMC_ACT_RELU>(d0, W3);
+          part = half == 0 ? tc_out_partial<H, NQ, 0, DSMC_ACT_RELU>(d0, W3) : tc_out_partial<H, NQ, 1, DSMC_ACT_RELU>(d0, W3);
         tc::fence_before();
         asm volatile("red.shared.add.f32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(dest + q * 32 + lane)), "f"(part)
                      : "memory");
@@ -360,7 +327,7 @@ void launch_cell_lists(dsmc_ctx *c, const StepParams &p, CellLists &L);  // dsmc
 
 template <int H, int NA, int NTW, int NBUF>
 static int launch_cells_mlp_one(dsmc_ctx *c, const StepParams &p, const CellLists &L, const MlpTcDev &net,
-                               const CellsMlpW3 &w3) {
+                               const TcOutLayer &w3) {
   auto kern = k_cells_mlp<H, NA, NTW, NBUF>;
   const size_t smem = ((NBUF * NTW * CellTeam<32>::bytes() + 127) & ~(size_t)127) + PipeShape<H>::SMEM_BYTES +
                       sizeof(CellsMlpCtl) + 128;
@@ -377,9 +344,7 @@ int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *n
     return DSMC_ERR_UNSUPPORTED_SHAPE;
   CellLists L;
   launch_cell_lists(c, p, L);
-  CellsMlpW3 w3;
-  for (int i = 0; i < 128; ++i) w3.w[i] = i < net->H ? net->w3_host[i] : 0.f;
-  w3.b = net->w3_host[128];
+  const TcOutLayer w3 = tc_out_layer(*net);
   if (net->H == 128) return launch_cells_mlp_one<128, 16, 12, 2>(c, p, L, *net, w3);
   return launch_cells_mlp_one<64, 16, 12, 2>(c, p, L, *net, w3);
 }

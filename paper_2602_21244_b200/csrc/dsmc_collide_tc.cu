@@ -302,23 +302,61 @@ __device__ __forceinline__ unsigned char *align128(unsigned char *p) {
 // a10: chi for independent pairs, chi = expm1(softplus(z)) = exp(z) (Q15), z = MLP(E~_n, b~).
 // Persistent, warp-specialised (dsmc_tc_pipe.cuh): the k-th tile of a CTA goes through slot k & 1.
 // ---------------------------------------------------------------------------------------------
+// The output layer (d_out = 1) is folded into the second activation (tc_out_partial, dsmc_tc_pipe.cuh): every
+// activation warp leaves the partial sum of its 32 columns in shared memory, the IO warps add the four of a row in a
+// fixed order.  zs[slot][round & 1][column group][row]: double-buffered by round, so a buffer is rewritten only after
+// the IO warps have published the features of the round after its last reader's (a barrier chain, not a timing guess).
+template <int H, int ACT>
+__device__ __forceinline__ void chi_out_tile(TcPipe<H> &pipe, int s, int act_warp, const TcOutLayer &W3, float *zrow,
+                                             uint64_t *z_bar) {
+  using SH = PipeShape<H>;
+  constexpr int NQ = kPipeActWarps / 4;
+  tc::mbar_wait(pipe.full_e + s, pipe.ph_e[s]);
+  pipe.ph_e[s] ^= 1u;
+  tc::fence_after();
+  const int grp = act_warp >> 2, lane = threadIdx.x & 31;
+  const uint32_t d0 = pipe.tmem + (((uint32_t)((act_warp & 3) * 32)) << 16) + s * SH::SLOT_COLS + SH::COL_D + grp * (H / NQ);
+  float part;
+  if (grp == 0) part = tc_out_partial<H, NQ, 0, ACT>(d0, W3);
+  else if (grp == 1) part = tc_out_partial<H, NQ, 1, ACT>(d0, W3);
+  else if (grp == 2) part = tc_out_partial<H, NQ, 2, ACT>(d0, W3);
+  else part = tc_out_partial<H, NQ, 3, ACT>(d0, W3);
+  zrow[grp * 128 + (act_warp & 3) * 32 + lane] = part;
+  tc::fence_before();
+  __syncwarp();
+  if (lane == 0) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(pipe.a_ready + s)) : "memory");  // D is free
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(z_bar)) : "memory");
+  }
+}
+
 template <int H>
 __global__ void __launch_bounds__(kPipeThreads, 1)
     k_chi_batch_tc(int64_t n, const float *__restrict__ E, const float *__restrict__ b, float *__restrict__ chi,
-                   const MlpTcDev net, float inv_bmax, float lnE_min, float inv_range) {
+                   const MlpTcDev net, const TcOutLayer W3, float inv_bmax, float lnE_min, float inv_range) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TcPipe<H> pipe;
-  pipe.init(smem_raw, net.w_blob, kPipeActWarps, kPipeIoWarps);
+  float *zs = reinterpret_cast<float *>(smem_raw + PipeShape<H>::SMEM_BYTES);  // [2][2][4][128]
+  uint64_t *z_bar = reinterpret_cast<uint64_t *>(zs + 2 * 2 * 4 * 128);         // [2]
+  if (threadIdx.x == 0) {
+    tc::mbar_init(z_bar + 0, kPipeActWarps);
+    tc::mbar_init(z_bar + 1, kPipeActWarps);
+  }
+  pipe.init(smem_raw, net.w_blob, kPipeActWarps, kPipeIoWarps);  // (fences the barrier inits, ends with CTA barriers)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n_tiles = (n + 127) / 128;
   const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
   const int64_t n_rounds = (mine + 1) / 2;  // two slots per round; a missing second tile runs as zeros
   if (warp < kPipeActWarps) {
     for (int64_t r = 0; r < n_rounds; ++r) {
+      pipe.act_tile(net.act, 0, warp);
+      pipe.act_tile(net.act, 1, warp);
 #pragma unroll 1
-      for (int layer = 0; layer < 2; ++layer) {
-        pipe.act_tile(net.act, 0, warp);
-        pipe.act_tile(net.act, 1, warp);
+      for (int s = 0; s < 2; ++s) {
+        float *zrow = zs + (size_t)((s * 2 + (int)(r & 1)) * 4) * 128;
+        if (net.act == DSMC_ACT_SILU) chi_out_tile<H, DSMC_ACT_SILU>(pipe, s, warp, W3, zrow, z_bar + s);
+        else if (net.act == DSMC_ACT_TANH) chi_out_tile<H, DSMC_ACT_TANH>(pipe, s, warp, W3, zrow, z_bar + s);
+        else chi_out_tile<H, DSMC_ACT_RELU>(pipe, s, warp, W3, zrow, z_bar + s);
       }
     }
   } else if (warp < kPipeActWarps + kPipeIoWarps) {
@@ -341,20 +379,23 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
       features(0, 0);
       features(1, 1);
     }
+    uint32_t phz[2] = {0u, 0u};
     for (int64_t r = 0; r < n_rounds; ++r) {
 #pragma unroll 1
       for (int s = 0; s < 2; ++s) {
         const int64_t k = 2 * r + s;
         if (r + 1 < n_rounds) features(s, k + 2);  // a round ahead: off the critical path
-        float y[4];
-        pipe.io_read_out(s, io_warp, y);
+        tc::mbar_wait(z_bar + s, phz[s]);
+        phz[s] ^= 1u;
+        const float *zrow = zs + (size_t)((s * 2 + (int)(r & 1)) * 4) * 128 + row;
+        const float z = ((zrow[0] + zrow[128]) + zrow[256]) + zrow[384];
         const int64_t p = (blockIdx.x + k * gridDim.x) * 128 + row;
-        if (k < mine && p < n) chi[p] = __expf(y[0]);
+        if (k < mine && p < n) chi[p] = __expf(z);
       }
     }
   } else {
-    // issue order keeps one layer of the other slot between a slot's consecutive layers, and the next
-    // tile's layer 1 ahead of the other slot's layer 3
+    // per round: layer 2 of both slots as their first activations end, then -- as the second activations end and free
+    // the accumulators -- layer 1 of the next round's tiles
     if (n_rounds > 0) {
       pipe.mma_layer1(0, 0, true);
       pipe.mma_layer1(1, 0, false);
@@ -364,10 +405,12 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
       const int par = (int)((r + 1) & 1);
       pipe.mma_layer2(0);
       pipe.mma_layer2(1);
-      pipe.mma_layer3(0, r == 0);
-      if (more) pipe.mma_layer1(0, par, false);
-      pipe.mma_layer3(1, r == 0);
-      if (more) pipe.mma_layer1(1, par, false);
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {
+        tc::mbar_wait(pipe.a_ready + s, pipe.ph_a[s]);
+        pipe.ph_a[s] ^= 1u;
+        if (more) pipe.mma_layer1(s, par, false);
+      }
     }
   }
   pipe.teardown();
@@ -378,10 +421,10 @@ static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const f
                                  float lnE_min, float lnE_max, const MlpTcDev *net) {
   const float inv_range = 1.0f / (lnE_max - lnE_min);
   const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms);
-  const int smem = PipeShape<H>::SMEM_BYTES + 128;
+  const int smem = PipeShape<H>::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 16 + 128;
   if (cudaFuncSetAttribute(k_chi_batch_tc<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
     return DSMC_ERR_CUDA;
-  k_chi_batch_tc<H><<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, 1.0f / b_max, lnE_min, inv_range);
+  k_chi_batch_tc<H><<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }

@@ -39,6 +39,48 @@ struct PipeShape {
   static constexpr int TMEM_COLS = 2 * SLOT_COLS;
 };
 
+// Output layer (d_out = 1) of a 3-layer MLP in FP32, passed to the kernel by value: its weights are then constant-bank
+// operands of the FMAs that form z, no load and no latency.  With a single output the third layer is a dot product per
+// row, which the activation warps take in the same pass as the second activation (instead of a third tensor-core
+// layer with its own commit, wake-up and read-back).
+struct TcOutLayer {
+  float w[128];
+  float b;
+};
+inline TcOutLayer tc_out_layer(const MlpTcDev &net) {
+  TcOutLayer o;
+  for (int i = 0; i < 128; ++i) o.w[i] = i < net.H ? net.w3_host[i] : 0.f;
+  o.b = net.w3_host[128];
+  return o;
+}
+
+// this thread's share of z for its row: sum over the columns of column group GRP (of NQ) of w3[j] act(D[row][j]), + b3
+// in group 0; d0 = tensor-memory address of the group's first D column in the thread's lane; the column indices are
+// compile-time.  The caller has done tcgen05.fence::after_thread_sync.
+template <int H, int NQ, int GRP, int ACT>
+__device__ __forceinline__ float tc_out_partial(uint32_t d0, const TcOutLayer &W3) {
+  constexpr int NC = H / (16 * NQ), C0 = GRP * (H / NQ);
+  uint32_t v[2][16];
+  float acc0 = GRP == 0 ? W3.b : 0.f, acc1 = 0.f;
+  tc::tmem_ld16(d0, v[0]);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    tc::wait_ld();
+    if (c + 1 < NC) tc::tmem_ld16(d0 + (c + 1) * 16, v[(c + 1) & 1]);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const float z = __uint_as_float(v[c & 1][j]);
+      float h;
+      if (ACT == DSMC_ACT_TANH) h = tc::tanh_approx(z);
+      else if (ACT == DSMC_ACT_RELU) h = fmaxf(z, 0.f);
+      else h = fmaf(z, tc::tanh_approx(z), z);  // SiLU(2 y) = y + y tanh(y), y = z (the weights carry the 1/2)
+      if (j & 1) acc1 = fmaf(h, W3.w[C0 + 16 * c + j], acc1);
+      else acc0 = fmaf(h, W3.w[C0 + 16 * c + j], acc0);
+    }
+  }
+  return acc0 + acc1;
+}
+
 template <int H>
 struct TcPipe {
   using SH = PipeShape<H>;
