@@ -315,7 +315,8 @@ def run_b200(args):
            torch.empty(pop.n_cells + 1, dtype=torch.int32, device=dev))
 
     def params(chi):
-        flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi == "mlp_tc" else 0) | \
+        flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi.startswith("mlp_tc") else 0) | \
+            (dsmc.F_TC_ONE_KERNEL if chi == "mlp_tc_one_kernel" else 0) | \
             (dsmc.F_PAIR_REPLACE if chi == "table_replace" else 0)
         return dsmc.AbinitioParams(chi_mode=0 if chi.startswith("table") else 1, flags=flags, b_max=B_MAX)
 
@@ -422,7 +423,7 @@ def run_b200(args):
     variants = {}
     if not args.no_variants and rank == 0 or (not args.no_variants and world > 1):
         # table_replace: the same step with pairs drawn WITH replacement (DSMC_F_PAIR_REPLACE)
-        for chi in ("table", "mlp", "mlp_tc", "table_replace"):
+        for chi in ("table", "mlp", "mlp_tc", "mlp_tc_one_kernel", "table_replace"):
             if chi == args.chi:
                 variants[chi] = {"pairs_per_s": pairs / (ms_step * 1e-3), "collide_ms": coll_ms, "step_ms": ms_step}
                 continue
@@ -598,7 +599,7 @@ def run_b200(args):
         roof["xu_bound"] = {"ms": t_xu * 1e3, "frac": t_xu / (coll_ms * 1e-3)}
     roof["traffic"], roof["traffic_source"] = measured_traffic("table" if args.chi == "table" else args.chi)
     roof["kernel"] = {"table": "fused collide: dsmc::k_cells (+ k_cell_lists, k_cells_big)",
-                      "mlp_tc": "fused collide: dsmc::k_cells_mlp (+ k_cell_lists)"}.get(args.chi, "fused collide: dsmc::k_collide<fp32 MLP>")
+                      "mlp_tc": "fused collide, three passes: dsmc::k_cells<3> | k_chi_batch_tc | k_cells<4> (+ k_cell_lists x2, k_cells_big x2)"}.get(args.chi, "fused collide: dsmc::k_collide<fp32 MLP>")
     roof["kernel_ms"] = coll_ms
     roof["peak_source"] = peak_src
     roof["algorithmic"] = {"bytes_per_launch": bytes_alg, "flops_per_launch": flops_alg}

@@ -121,12 +121,17 @@ enum {
   DSMC_F_ACCEPT = 8,            /* NTC acceptance test; needs the *_max array          */
   DSMC_F_BF16_TC = 16,          /* MLP layers as tcgen05 BF16 GEMMs over 128-pair tiles        */
   DSMC_F_MATCH_ENERGY_ONLY = 32, /* literal eq. 11: scale raw velocities by sqrt(E_pre/E_post)  */
-  DSMC_F_PAIR_REPLACE = 128     /* pairs drawn WITH replacement, i = mulhi(R0, N), j = mulhi(R1, N-1)
+  DSMC_F_PAIR_REPLACE = 128,    /* pairs drawn WITH replacement, i = mulhi(R0, N), j = mulhi(R1, N-1)
                                    + (j >= i) from Philox stream 4; every pair of a cell is evaluated on the
                                    pre-collision velocities (one batch) and the velocity changes of a
                                    particle that appears in several pairs add up.  Momentum is conserved exactly,
                                    energy is restored by DSMC_F_MOMENT_MATCH.  Both operators, FP32 / table paths
                                    (not with DSMC_F_BF16_TC).  No key sort: the cheapest selection. */
+  DSMC_F_TC_ONE_KERNEL = 256    /* dsmc_collide_abinitio, chi-MLP with DSMC_F_BF16_TC: run the step as ONE kernel (cell
+                                   teams + a tcgen05 MLP server sharing every SM) instead of the default three passes
+                                   (pairing + network inputs | chi batch on the tensor cores | rotation + matching).
+                                   Same pairs, same randoms; chi differs within the BF16 tolerance (the two forms add
+                                   the output layer's partial sums in a different order).  Slower on large steps. */
 };
 
 typedef struct {

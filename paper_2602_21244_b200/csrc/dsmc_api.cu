@@ -60,7 +60,8 @@ static int create_impl(dsmc_ctx *c, int device, int64_t max_particles, int32_t m
     CK(cudaMalloc(&c->d_cell_tile_sums, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) / 4096 + 2)));
     for (int i = 0; i < 2; ++i) {
       CK(cudaMalloc(&c->d_bin_cell[i], sizeof(int32_t) * np));
-      if (i < passes - 1) CK(cudaMalloc(&c->d_bin_rec[i], sizeof(float4) * np));
+      // (buffer 0 always exists: the split chi-MLP step keeps its pair arrays there, 8 B / particle + 48 B)
+      if (i == 0 || i < passes - 1) CK(cudaMalloc(&c->d_bin_rec[i], sizeof(float4) * (np + 4)));
     }
   }
   const size_t n_chunks = (size_t)(max_particles / kChunk + 2);

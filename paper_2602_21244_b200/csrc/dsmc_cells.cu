@@ -77,25 +77,28 @@ __global__ void __launch_bounds__(256) k_cell_lists(int32_t K, const int32_t *__
 // ---------------------------------------------------------------------------------------------
 // main kernel: 128-thread CTAs.  First the cells of 257..1024 particles, one per CTA at a time; then the cells of
 // up to 256 particles, one per warp at a time.  Both forms use the same shared-memory footprint.
+// OP 0: the whole step with the chi table.  OP 3 / 4: first / second pass of the split chi-MLP step (below).
+template <int OP>
 __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   {
-    CellTeam<128> T;
+    CellTeam<128, OP> T;
     T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
     T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
   }
   __syncthreads();
   {
-    CellTeam<32> T;
+    CellTeam<32, OP> T;
     T.init((uint32_t)__cvta_generic_to_shared(smem_raw) + (threadIdx.x >> 5) * (uint32_t)CellTeam<32>::bytes(), threadIdx.x & 31, 0);
     T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
   }
 }
 
 // cells of 1025..2048 particles: one 256-thread CTA per cell at a time
+template <int OP>
 __global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  CellTeam<256> T;
+  CellTeam<256, OP> T;
   T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
   T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
 }
@@ -113,11 +116,12 @@ void launch_cell_lists(dsmc_ctx *c, const StepParams &p, CellLists &L) {
   c->launches += 1;
 }
 
-int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
+template <int OP>
+static int launch_cells_pass(dsmc_ctx *c, const StepParams &p) {
   CellLists L;
   launch_cell_lists(c, p, L);
   {
-    auto kern = k_cells;
+    auto kern = k_cells<OP>;
     const size_t smem = CellTeam<128>::bytes();
     static_assert(CellTeam<128>::bytes() == 4 * CellTeam<32>::bytes(), "the two team forms share one footprint");
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
@@ -125,7 +129,7 @@ int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
     kern<<<c->num_sms * 8, 128, smem, c->stream>>>(p, L);
   }
   {
-    auto kern = k_cells_big;
+    auto kern = k_cells_big<OP>;
     const size_t smem = CellTeam<256>::bytes();
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return DSMC_ERR_CUDA;
@@ -133,6 +137,36 @@ int launch_collide_cells(dsmc_ctx *c, const StepParams &p) {
   }
   c->launches += 2;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+int launch_collide_cells(dsmc_ctx *c, const StepParams &p) { return launch_cells_pass<0>(c, p); }
+
+// chi-MLP step on the tensor cores, SPLIT form: three passes at full occupancy instead of one kernel in which twelve
+// team warps and the MLP server share an SM (dsmc_cells_mlp.cu; measured: that kernel's team side alone needs 0.98 ms
+// on cfg 5).
+//   pass 1 (OP 3)  load, key sort -> pairing (stored, 2 B / particle), pair gather -> the two network inputs of every
+//                  pair (8 B / pair)
+//   pass 2         k_chi_batch_tc on the pair arrays (rows = pair slots): chi, 4 B / pair
+//   pass 3 (OP 4)  load, pre-collision sums, stored pairing, gather, acceptance, rotation by (chi, eps), commit,
+//                  matching, store
+// Everything random is regenerated from (seed, step, cell, slot) in both passes; results do not depend on the launch
+// geometry.  The pair arrays and the stored pairing live in the radix sort's first ping-pong buffer (16 B / particle,
+// idle while a collision step runs; 8 B / particle needed).
+int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
+  if (p_in.op != 2 || net->d_in != 2 || net->d_out != 1 || (net->H != 64 && net->H != 128))
+    return DSMC_ERR_UNSUPPORTED_SHAPE;
+  StepParams p = p_in;
+  const int64_t np = (p.n / 2 + 4) & ~(int64_t)3;  // pair index = first slot of the cell / 2 + pair slot < n / 2 + 1
+  float *base = reinterpret_cast<float *>(c->d_bin_rec[0]);
+  p.feat0 = base;
+  p.feat1 = base + np;
+  p.chi_pair = base + 2 * np;
+  p.pi_g = reinterpret_cast<uint16_t *>(base + 3 * np);
+  int rc = launch_cells_pass<3>(c, p);
+  if (rc != DSMC_OK) return rc;
+  rc = launch_chi_rows_tc(c, p.n / 2 + 1, p.feat0, p.feat1, p.chi_pair, net);
+  if (rc != DSMC_OK) return rc;
+  return launch_cells_pass<4>(c, p);
 }
 
 }  // namespace dsmc

@@ -349,11 +349,18 @@ struct CellTeam {
           if (STAGE != 2) {
             if (accept) acc = valid && (Ua[k] * cap < sqrtf(g2));  // constant cross-section: U g_max < g
           }
-          if (STAGE == 1) {  // chi-MLP inputs (Q15): ((E~ - E~min) / (E~max - E~min) clamped to [0, 1], b~)
+          if (STAGE == 1 || STAGE == 3) {  // chi-MLP inputs (Q15): ((E~ - E~min) / (E~max - E~min) clamped to [0, 1], b~)
             const float e = (0.6931471806f * mufu_lg2(P.e_coef * g2) - P.lnE_min) * P.inv_lnE_range;
-            stage[row] = !(e > 0.f) ? 0.f : fminf(e, 1.f);
-            stage[128 + row] = mufu_sqrt(Ub[k]);
-            park[row] = acc ? eps[k] : 1e30f;
+            const float x0 = !(e > 0.f) ? 0.f : fminf(e, 1.f), x1 = mufu_sqrt(Ub[k]);
+            if (STAGE == 1) {
+              stage[row] = x0;
+              stage[128 + row] = x1;
+              park[row] = acc ? eps[k] : 1e30f;
+            } else if (valid) {  // split form: the inputs go to the pair arrays, the rest is redone by the second pass
+              const int64_t pp = (int64_t)(gs >> 1) + s0 + k;
+              P.feat0[pp] = x0;
+              P.feat1[pp] = x1;
+            }
             continue;
           }
           float px = gx, py = gy, pz = gz, chi = 0.f;
@@ -364,6 +371,8 @@ struct CellTeam {
           if (acc) {
             if (STAGE == 2) {
               chi = __expf(zbuf[row]);  // chi = expm1(softplus(z)) = exp(z)
+            } else if (STAGE == 4) {
+              chi = __ldg(P.chi_pair + (int64_t)(gs >> 1) + s0 + k);  // split form: chi of the batch kernel
             } else {
               // E~ = ln(m g^2 / (4 kB)), b~ = sqrt(U_b)
               chi = cells_chi(P.table, cells_tE(P.table, P.e_coef * g2), mufu_sqrt(Ub[k]) * nBm1);
@@ -492,6 +501,14 @@ struct CellTeam {
       theta = fmaxf(s2 - fN * fmaf(mx, mx, fmaf(my, my, mz * mz)), 0.f);
     }
     if (tid == 0) next = entry(list, n_items, next_idx);
+    if (OP == 4) {  // split form, second pass: the pairing was made (and stored) by the first pass
+      const uint16_t *__restrict__ gp = P.pi_g + gs;
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int q = tid + NT * r;
+        if (q < N) pi[q] = __ldg(gp + q);
+      }
+    } else {
     // ---- pairing keys (stream 0: block blk serves slots 4 blk .. 4 blk + 3) and bucket counts ----
     // per key: comp = key << Lb | slot (the (key, slot) order inside a bucket), bo = bucket | arrival index << 16
     uint32_t comp[8], bo[8];
@@ -578,8 +595,17 @@ struct CellTeam {
         if (m > 1u) pi[rank] = (uint16_t)(4u * (e & slot_mask));
       }
     }
+    }  // OP != 4
     if (NT > 32 && tid == 0) *reinterpret_cast<int4 *>(misc + 8) = next;
     sync();
+    if (OP == 3) {  // split form, first pass: the pairing goes to HBM for the second pass
+      uint16_t *__restrict__ gp = P.pi_g + gs;
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int q = tid + NT * r;
+        if (q < N) gp[q] = pi[q];
+      }
+    }
     }  // HALF != 2
     // ---- pairs: thread owns pair slots 2 dp, 2 dp + 1 (one Philox block of stream 1 serves both) ----
     bool any_acc;
@@ -617,10 +643,14 @@ struct CellTeam {
       }
       srv->wait(lane);
       any_acc = pairs_phase<2>(P, item, cell_ctr, accept, 0);
+    } else if (OP == 3) {
+      any_acc = pairs_phase<3>(P, item, cell_ctr, accept, 0);
+    } else if (OP == 4) {
+      any_acc = pairs_phase<4>(P, item, cell_ctr, accept, 0);
     } else {
       any_acc = pairs_phase<0>(P, item, cell_ctr, accept, 0);
     }
-    bool collided = true;
+    bool collided = OP != 3;  // (first pass of the split form: nothing is committed, nothing to store)
     if (accept) {
       collided = __any_sync(0xffffffffu, any_acc);
       if (NT > 32 && collided && lane == 0) misc[12] = 1;

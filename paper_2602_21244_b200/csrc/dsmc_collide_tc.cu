@@ -330,7 +330,8 @@ __device__ __forceinline__ void chi_out_tile(TcPipe<H> &pipe, int s, int act_war
   }
 }
 
-template <int H>
+// RAW: E, b already hold the network inputs (x0, x1) of every row (the split fused step, dsmc_cells.cu)
+template <int H, bool RAW>
 __global__ void __launch_bounds__(kPipeThreads, 1)
     k_chi_batch_tc(int64_t n, const float *__restrict__ E, const float *__restrict__ b, float *__restrict__ chi,
                    const MlpTcDev net, const TcOutLayer W3, float inv_bmax, float lnE_min, float inv_range) {
@@ -366,7 +367,12 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
       float x[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) x[j] = 0.f;
-      if (k < mine && p < n) {
+      if (RAW) {
+        if (k < mine && p < n) {
+          x[0] = __ldg(E + p);
+          x[1] = __ldg(b + p);
+        }
+      } else if (k < mine && p < n) {
         const float e = (__logf(__ldg(E + p)) - lnE_min) * inv_range;
         x[0] = !(e > 0.f) ? 0.f : fminf(e, 1.f);
         const float bt = __ldg(b + p) * inv_bmax;
@@ -416,15 +422,15 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
   pipe.teardown();
 }
 
-template <int H>
+template <int H, bool RAW>
 static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
                                  float lnE_min, float lnE_max, const MlpTcDev *net) {
   const float inv_range = 1.0f / (lnE_max - lnE_min);
   const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms);
   const int smem = PipeShape<H>::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 16 + 128;
-  if (cudaFuncSetAttribute(k_chi_batch_tc<H>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-    return DSMC_ERR_CUDA;
-  k_chi_batch_tc<H><<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
+  auto kern = k_chi_batch_tc<H, RAW>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return DSMC_ERR_CUDA;
+  kern<<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
@@ -432,8 +438,15 @@ static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const f
 int launch_chi_batch_tc(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, float b_max,
                         float lnE_min, float lnE_max, const MlpTcDev *net) {
   if (net->d_in != 2 || net->d_out != 1) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  return net->H == 128 ? launch_chi_batch_tc_h<128>(c, n, E, b, chi, b_max, lnE_min, lnE_max, net)
-                       : launch_chi_batch_tc_h<64>(c, n, E, b, chi, b_max, lnE_min, lnE_max, net);
+  return net->H == 128 ? launch_chi_batch_tc_h<128, false>(c, n, E, b, chi, b_max, lnE_min, lnE_max, net)
+                       : launch_chi_batch_tc_h<64, false>(c, n, E, b, chi, b_max, lnE_min, lnE_max, net);
+}
+
+// chi = exp(MLP(x0, x1)) for rows whose network inputs are given as they are (no normalisation, no clamping)
+int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1, float *chi, const MlpTcDev *net) {
+  if (net->d_in != 2 || net->d_out != 1) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  return net->H == 128 ? launch_chi_batch_tc_h<128, true>(c, n, x0, x1, chi, 1.f, 0.f, 1.f, net)
+                       : launch_chi_batch_tc_h<64, true>(c, n, x0, x1, chi, 1.f, 0.f, 1.f, net);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -571,7 +584,10 @@ static int launch_tc_pair(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
   if (p_in.op == 0 && !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3)) return DSMC_ERR_UNSUPPORTED_SHAPE;
   if (p_in.op == 2 && !(net->d_in == 2 && net->d_out == 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  if (p_in.op == 2) return launch_collide_cells_mlp(c, p_in, net);  // plain BF16: cell teams + MLP server (dsmc_cells_mlp.cu)
+  // plain BF16 chi-MLP: three passes at full occupancy (dsmc_cells.cu), or, with DSMC_F_TC_ONE_KERNEL, the single kernel
+  // of cell teams + MLP server (dsmc_cells_mlp.cu)
+  if (p_in.op == 2)
+    return (p_in.flags & DSMC_F_TC_ONE_KERNEL) ? launch_collide_cells_mlp(c, p_in, net) : launch_collide_cells_split(c, p_in, net);
   StepParams p = p_in;
   int rc = launch_chunk_map(c, p);
   if (rc != DSMC_OK) return rc;

@@ -73,6 +73,10 @@ struct StepParams {
   dsmc_pair_dump dump;
   int32_t dump_any;
   int32_t *status;
+  // split form of the chi-MLP step (dsmc_cells.cu): per pair (index = first slot of the cell / 2 + pair slot) the two
+  // network inputs and chi; per particle the pairing permutation as 16-bit byte offsets
+  float *feat0, *feat1, *chi_pair;
+  uint16_t *pi_g;
   // chunk decomposition (filled by launch_chunk_map)
   int32_t n_chunks;
   const int32_t *chunk_first;  // [n_chunks + 1]
@@ -142,7 +146,9 @@ int launch_moment_match(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
 int launch_chunk_map(dsmc_ctx *c, StepParams &p);
 int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
 int launch_collide_cells(dsmc_ctx *c, const StepParams &p);
-int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
+int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
+int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
+int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1, float *chi, const MlpTcDev *net);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
                      float lnE_min, float lnE_max, const MlpDev *net);

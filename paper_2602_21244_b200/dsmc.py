@@ -23,6 +23,7 @@ MAX_CELL_PARTICLES = 2048
 
 F_NOISE, F_ENERGY_SHELL, F_MOMENT_MATCH, F_ACCEPT, F_BF16_TC, F_MATCH_ENERGY_ONLY, F_CHI_ABS = 1, 2, 4, 8, 16, 32, 64
 F_PAIR_REPLACE = 128
+F_TC_ONE_KERNEL = 256
 ACT_TANH, ACT_RELU, ACT_SILU = 0, 1, 2
 
 EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status", "dsmc_strerror",

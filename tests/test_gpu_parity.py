@@ -463,7 +463,10 @@ def test_chi_batch_bf16_tc(dsmc, H, act):
     ctx.close()
 
 
-def test_collide_abinitio_bf16_tc(dsmc):
+@pytest.mark.parametrize("one_kernel", [False, True])
+def test_collide_abinitio_bf16_tc(dsmc, one_kernel):
+    """chi-MLP on the tensor cores, both forms: the default three passes (pairing + inputs | chi batch | rotation +
+    matching) and, with F_TC_ONE_KERNEL, the single kernel of cell teams + MLP server."""
     pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
     ctx = dsmc.Context(pop.n, pop.n_cells)
     Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
@@ -471,7 +474,7 @@ def test_collide_abinitio_bf16_tc(dsmc):
     net = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
     vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
     cs_h = cs.cpu().numpy()
-    prm = dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC)
+    prm = dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC | (dsmc.F_TC_ONE_KERNEL if one_kernel else 0))
     oprm = oracle.AbinitioParams(chi_mode=1, lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
     for step in range(2):
         v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
@@ -494,6 +497,40 @@ def test_collide_abinitio_bf16_tc(dsmc):
         ok = N >= 2
         assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
         assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    ctx.close()
+
+
+@pytest.mark.parametrize("one_kernel", [False, True])
+def test_collide_abinitio_bf16_tc_few_cells_and_ragged(dsmc, one_kernel):
+    """Both tensor-core forms on contexts whose radix sort needs a single pass (<= 512 cells: the split form's pair
+    arrays must exist all the same) and on ragged cells (empty, 1, 2, 3, odd, 2048 particles)."""
+    rng = np.random.default_rng(3)
+    counts = rng.integers(0, 30, 200)
+    counts[5], counts[6], counts[7], counts[8], counts[50], counts[120] = 0, 1, 2, 3, 2048, 777
+    pop = wl._populate("ragged", counts, np.full(200, 273.0), np.zeros(200), np.zeros(200), 3)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    net = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    prm = dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC | (dsmc.F_TC_ONE_KERNEL if one_kernel else 0))
+    oprm = oracle.AbinitioParams(chi_mode=1, lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
+    v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+    dump = dsmc.PairDump(pop.n, "cuda")
+    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=6, step=1, dump=dump)
+    ctx.check()
+    ref = oracle.collide_abinitio(cs_h, *v_in, oprm, 6, 1, net=net)
+    sel = ref.pair_i >= 0
+    chi_g = dump.aux.cpu().numpy().astype(np.float64)
+    assert (np.abs(chi_g[sel] - ref.aux[sel]) / (1 + np.abs(ref.aux[sel]))).max() <= 2e-2  # Q26
+    _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=1.01 * np.abs(chi_g - ref.aux))
+    N = np.diff(cs_h)
+    pre = oracle.cell_moments(cs_h, *v_in)
+    got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+    ok = N >= 2
+    assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+    assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
     ctx.close()
 
 
@@ -537,7 +574,7 @@ def test_collide_vhs_nn_bf16_tc(dsmc, case):
 
 
 # --------------------------------------------------------------------------------------- (e) sharding
-@pytest.mark.parametrize("tc", [False, True])
+@pytest.mark.parametrize("tc", [False, True, "one_kernel"])
 def test_sharded_step_matches_unsharded(dsmc, tc):
     """Two cell-range shards run one after the other on this GPU (independent launches, no rank waits on
     another) give bit-identical velocities to the unsharded step: RNG is keyed by the GLOBAL cell id."""
@@ -550,7 +587,7 @@ def test_sharded_step_matches_unsharded(dsmc, tc):
     ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
     vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
     cs_h = cs.cpu().numpy()
-    flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if tc else 0)
+    flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if tc else 0) | (dsmc.F_TC_ONE_KERNEL if tc == "one_kernel" else 0)
     full = [t.clone() for t in (vx_s, vy_s, vz_s)]
     ctx.collide_abinitio(cs, *full, dsmc.AbinitioParams(chi_mode=1 if tc else 0, flags=flags), seed=9, step=2)
     ctx.check()
