@@ -57,6 +57,7 @@ extern "C" {
 #define DSMC_ERR_NOT_CONFIGURED (-4)
 #define DSMC_ERR_CUDA (-5)
 #define DSMC_ERR_UNSUPPORTED_SHAPE (-6)
+#define DSMC_ERR_NOALLOC_LIMIT (-7) /* dsmc_bin_noalloc: n or n_cells beyond the fixed scratch array */
 
 /* largest cell the SMEM-resident fused step accepts */
 #define DSMC_MAX_CELL_PARTICLES 2048
@@ -112,6 +113,28 @@ int dsmc_set_chi_table(dsmc_ctx *ctx, const float *chi_host, int32_t nE, int32_t
 int dsmc_bin(dsmc_ctx *ctx, int64_t n, int32_t n_cells, const int32_t *cell, const float *vx,
              const float *vy, const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm,
              int32_t *cell_start);
+
+/* ---- a1 without any allocation --------------------------------------------------------------------------
+ * The same sort as dsmc_bin (same kernels, bit-identical outputs) for callers that cannot call cudaMalloc: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it.  No context: the workspace is one file-scope
+ * device array of fixed size (22.5 MB; every GPU that loads the library holds it until the process exits), so the call
+ * allocates and frees NOTHING (no cudaMalloc / cudaFree / allocating library routine; it enqueues memsets, kernels and
+ * one 4-byte device-to-device copy on `stream`, a cudaStream_t passed as void *, and returns without synchronising).
+ * Runs on the CURRENT device.  Limits: n <= DSMC_NOALLOC_MAX_PARTICLES and n_cells <= DSMC_NOALLOC_MAX_CELLS,
+ * otherwise DSMC_ERR_NOALLOC_LIMIT (nothing is enqueued).  All arrays are caller-owned DEVICE pointers as in dsmc_bin.
+ * status_dev: optional DEVICE int32 that receives DSMC_OK or DSMC_ERR_BAD_CELL_INDEX when the call's work completes
+ * (there is no context to hold a sticky status).
+ * SHARED STATE: every call on a device uses the same array, which keeps the previous call's contents (what must start
+ * at zero is cleared by the call itself).  Calls that overlap on the GPU -- two streams, two host threads, a captured
+ * graph replayed concurrently with itself -- RACE; order them on one stream or with events.
+ * dsmc_noalloc_setup(): the once-per-device set-up (the array's device address, SM count) for the current device;
+ * dsmc_bin_noalloc does it on first use, call it beforehand where even that is unwelcome (before a graph capture). */
+#define DSMC_NOALLOC_MAX_PARTICLES 1048576
+#define DSMC_NOALLOC_MAX_CELLS 131072
+int dsmc_noalloc_setup(void);
+int dsmc_bin_noalloc(void *stream, int64_t n, int32_t n_cells, const int32_t *cell, const float *vx,
+                     const float *vy, const float *vz, float *vx_s, float *vy_s, float *vz_s, int32_t *perm,
+                     int32_t *cell_start, int32_t *status_dev);
 
 /* ---- fused collision steps -------------------------------------------------------------- */
 enum {

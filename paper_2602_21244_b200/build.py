@@ -11,7 +11,7 @@ import sys
 _DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_DIR, "csrc")
 LIB = os.path.join(_DIR, "libdsmc_b200.so")
-SOURCES = ["dsmc_api.cu", "dsmc_bin.cu", "dsmc_moments.cu", "dsmc_collide.cu", "dsmc_cells.cu", "dsmc_cells_mlp.cu", "dsmc_collide_tc.cu", "dsmc_chi_exact.cu", "dsmc_move.cu"]
+SOURCES = ["dsmc_api.cu", "dsmc_bin.cu", "dsmc_moments.cu", "dsmc_collide.cu", "dsmc_cells.cu", "dsmc_cells_mlp.cu", "dsmc_collide_tc.cu", "dsmc_chi_exact.cu", "dsmc_move.cu", "dsmc_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

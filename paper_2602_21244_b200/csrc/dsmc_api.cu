@@ -161,6 +161,7 @@ const char *dsmc_strerror(int s) {
     case DSMC_ERR_NOT_CONFIGURED: return "operator (MLP or chi table) not set";
     case DSMC_ERR_CUDA: return "CUDA runtime error";
     case DSMC_ERR_UNSUPPORTED_SHAPE: return "MLP shape not supported by the requested path";
+    case DSMC_ERR_NOALLOC_LIMIT: return "size beyond the fixed scratch array of the no-allocation entry point (DSMC_NOALLOC_MAX_*)";
     default: return "unknown status";
   }
 }

@@ -30,7 +30,7 @@ EXPORTS = ["dsmc_create", "dsmc_destroy", "dsmc_set_stream", "dsmc_sync_status",
            "dsmc_launch_count", "dsmc_set_mlp", "dsmc_set_chi_table", "dsmc_bin", "dsmc_collide_vhs_nn",
            "dsmc_collide_abinitio", "dsmc_cell_moments", "dsmc_moment_match", "dsmc_chi_batch",
            "dsmc_chi_exact_batch", "dsmc_build_chi_table_lj", "dsmc_build_chi_table_mlp", "dsmc_step_host", "dsmc_step_host_submit", "dsmc_move_couette",
-           "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run", "dsmc_ntc_counts"]
+           "dsmc_gather_f32", "dsmc_sample_cells", "dsmc_couette_run", "dsmc_ntc_counts", "dsmc_noalloc_setup", "dsmc_bin_noalloc"]
 
 
 class DsmcError(RuntimeError):
@@ -170,6 +170,27 @@ class PairDump:
     def c(self):
         return _PairDump(_ptr(self.pair_i), _ptr(self.pair_j), _ptr(self.accepted), _ptr(self.gprime),
                          _ptr(self.aux))
+
+
+NOALLOC_MAX_PARTICLES, NOALLOC_MAX_CELLS = 1 << 20, 1 << 17
+
+
+def noalloc_setup():
+    """once-per-device set-up of the no-allocation entry point, for the CURRENT device (torch.cuda.current_device())"""
+    _chk(_lib.dsmc_noalloc_setup(), "dsmc_noalloc_setup")
+
+
+def bin_noalloc(cell, vx, vy, vz, n_cells: int, out, status=None):
+    """dsmc_bin_noalloc: the cell sort with a fixed file-scope scratch array instead of a context; allocates nothing
+    (so `out` = (vx_s, vy_s, vz_s, perm, cell_start) must be given).  status: optional int32 device tensor [1].
+    Enqueued on torch's current stream of the current device; calls that overlap on the GPU race on the scratch."""
+    vx_s, vy_s, vz_s, perm, cell_start = out
+    _chk(_lib.dsmc_bin_noalloc(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.c_int64(cell.shape[0]),
+                               C.c_int32(n_cells), _ptr(cell, torch.int32), _ptr(vx, torch.float32),
+                               _ptr(vy, torch.float32), _ptr(vz, torch.float32), _ptr(vx_s), _ptr(vy_s), _ptr(vz_s),
+                               _ptr(perm), _ptr(cell_start), _ptr(status, torch.int32) if status is not None else C.c_void_p(0)),
+         "dsmc_bin_noalloc")
+    return out
 
 
 class Context:
