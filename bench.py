@@ -317,7 +317,7 @@ def run_b200(args):
     def params(chi):
         flags = dsmc.F_MOMENT_MATCH | (dsmc.F_BF16_TC if chi.startswith("mlp_tc") else 0) | \
             (dsmc.F_TC_ONE_KERNEL if chi == "mlp_tc_one_kernel" else 0) | \
-            (dsmc.F_PAIR_REPLACE if chi == "table_replace" else 0)
+            (dsmc.F_PAIR_REPLACE if chi.endswith("_replace") else 0)
         return dsmc.AbinitioParams(chi_mode=0 if chi.startswith("table") else 1, flags=flags, b_max=B_MAX)
 
     def one_step(chi, t, ev=None):
@@ -423,7 +423,7 @@ def run_b200(args):
     variants = {}
     if not args.no_variants and rank == 0 or (not args.no_variants and world > 1):
         # table_replace: the same step with pairs drawn WITH replacement (DSMC_F_PAIR_REPLACE)
-        for chi in ("table", "mlp", "mlp_tc", "mlp_tc_one_kernel", "table_replace"):
+        for chi in ("table", "mlp", "mlp_tc", "mlp_tc_one_kernel", "table_replace", "mlp_tc_replace"):
             if chi == args.chi:
                 variants[chi] = {"pairs_per_s": pairs / (ms_step * 1e-3), "collide_ms": coll_ms, "step_ms": ms_step}
                 continue

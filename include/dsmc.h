@@ -148,8 +148,9 @@ enum {
                                    + (j >= i) from Philox stream 4; every pair of a cell is evaluated on the
                                    pre-collision velocities (one batch) and the velocity changes of a
                                    particle that appears in several pairs add up.  Momentum is conserved exactly,
-                                   energy is restored by DSMC_F_MOMENT_MATCH.  Both operators, FP32 / table paths
-                                   (not with DSMC_F_BF16_TC).  No key sort: the cheapest selection. */
+                                   energy is restored by DSMC_F_MOMENT_MATCH.  Both operators on the FP32 / table
+                                   paths; with DSMC_F_BF16_TC for the ab initio chi-MLP (dsmc_collide_abinitio), not
+                                   for the VHS-NN operator.  No key sort: the cheapest selection. */
   DSMC_F_TC_ONE_KERNEL = 256    /* dsmc_collide_abinitio, chi-MLP with DSMC_F_BF16_TC: run the step as ONE kernel (cell
                                    teams + a tcgen05 MLP server sharing every SM) instead of the default three passes
                                    (pairing + network inputs | chi batch on the tensor cores | rotation + matching).

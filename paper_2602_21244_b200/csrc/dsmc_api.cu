@@ -395,7 +395,7 @@ int dsmc_collide_abinitio(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, 
   p.table = c->table;
   CK(cudaSetDevice(c->device));
   if (prm->chi_mode == 1 && (prm->flags & DSMC_F_BF16_TC)) {
-    if (c->mlp_tc[1].H == 0 || (prm->flags & DSMC_F_PAIR_REPLACE)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    if (c->mlp_tc[1].H == 0) return DSMC_ERR_UNSUPPORTED_SHAPE;
     return launch_collide_tc(c, p, &c->mlp_tc[1]);
   }
   return launch_collide(c, p, prm->chi_mode == 1 ? &c->mlp[1] : nullptr);

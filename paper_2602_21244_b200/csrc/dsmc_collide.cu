@@ -101,14 +101,23 @@ template <class TM, class CK>
 __device__ __forceinline__ void pairs_table(const TM &T, const StepParams &P, CK &S, int q0) {
   const int n_pairs = S.misc[MI_NPAIRS];
   const float nBm1 = (float)(P.table.nB - 1);
+  const int stage = P.split_stage;
   for (int t = T.tid; t < n_pairs; t += TM::kN) {
     PairCtx c = pair_setup(P, S, t, true);
     float px = c.gx, py = c.gy, pz = c.gz, chi = 0.f;
+    float sb;  // b~ = sqrt(U_b)
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sb) : "f"(c.U_b));
+    // split form of the chi-MLP step (launch_collide_replace_split): pair index = first slot of the cell / 2 + pair slot
+    const int64_t pidx = ((int64_t)(q0 + c.start) >> 1) + c.s;
+    if (stage == 3) {  // network inputs only (Q15): ((E~ - E~min) / (E~max - E~min) clamped to [0, 1], b~)
+      const float e = (0.6931471806f * __log2f(P.e_coef * c.g2) - P.lnE_min) * P.inv_lnE_range;
+      P.feat0[pidx] = !(e > 0.f) ? 0.f : fminf(e, 1.f);
+      P.feat1[pidx] = sb;
+      continue;
+    }
     if (c.acc) {
-      // E~ = ln(m g^2 / (4 kB)), b~ = sqrt(U_b)
-      float sb;
-      asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sb) : "f"(c.U_b));
-      chi = chi_table_t(P.table, table_tE(P.table, P.e_coef * c.g2), sb * nBm1);
+      // E~ = ln(m g^2 / (4 kB))
+      chi = stage == 4 ? __ldg(P.chi_pair + pidx) : chi_table_t(P.table, table_tE(P.table, P.e_coef * c.g2), sb * nBm1);
       if (c.g2 > 0.f) rotate_fast(c, chi, c.U_eps, px, py, pz);
     }
     pair_commit(P, S, c, px, py, pz, chi, q0);
@@ -210,6 +219,7 @@ __device__ __forceinline__ void process_chunk(const StepParams &P, const MlpDev 
   chunk_pre_and_sort(T, P, S, n_loc);
   if (OP_TABLE) {
     pairs_table(T, P, S, q0);
+    if (P.split_stage == 3) return;  // (uniform) first pass of the split form: nothing committed, nothing to store
   } else {
     pairs_mlp_fp32<TP>(P, net, S, mlp, q0);
   }
@@ -258,6 +268,41 @@ int launch_chunk_map(dsmc_ctx *c, StepParams &p) {
                                                              c->d_chunk_meta);
   c->launches += 2;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+// chi-MLP on the tensor cores with pairs drawn WITH replacement (DSMC_F_PAIR_REPLACE | DSMC_F_BF16_TC): the split form
+// of dsmc_cells.cu on the with-replacement chunk kernels.  Pass 1 draws the pairs and writes the two network inputs of
+// every pair, pass 2 is k_chi_batch_tc on those arrays, pass 3 draws the same pairs again (counter-based randoms),
+// rotates by the chi of pass 2, adds up the changes and matches.
+static int launch_replace_table_kernels(dsmc_ctx *c, const StepParams &p) {
+  MlpDev nd{};
+  int rc = launch_one<704, 32, true, 64, 0, 1, 9, 128, true>(c, p, nd, p.n_chunks, 0);
+  if (rc != DSMC_OK) return rc;
+  rc = launch_one<1024, 8, true, 64, 1, 2, 7, 128, true>(c, p, nd, c->num_sms * 7, 0);
+  if (rc != DSMC_OK) return rc;
+  return launch_one<kLmaxBig, kAmaxBig, true, 64, 2, 0, 1, kThreads, true>(c, p, nd, c->num_sms, 0);
+}
+
+int launch_collide_replace_split(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
+  if (p_in.op != 2 || net->d_in != 2 || net->d_out != 1 || (net->H != 64 && net->H != 128))
+    return DSMC_ERR_UNSUPPORTED_SHAPE;
+  StepParams p = p_in;
+  const int64_t np = (p.n / 2 + 4) & ~(int64_t)3;
+  float *base = reinterpret_cast<float *>(c->d_bin_rec[0]);
+  p.feat0 = base;
+  p.feat1 = base + np;
+  p.chi_pair = base + 2 * np;
+  int rc = launch_chunk_map(c, p);
+  if (rc != DSMC_OK) return rc;
+  p.split_stage = 3;
+  rc = launch_replace_table_kernels(c, p);
+  if (rc != DSMC_OK) return rc;
+  rc = launch_chi_rows_tc(c, p.n / 2 + 1, p.feat0, p.feat1, p.chi_pair, net);
+  if (rc != DSMC_OK) return rc;
+  rc = launch_chunk_map(c, p);  // (resets the deferred-chunk lists and work counters)
+  if (rc != DSMC_OK) return rc;
+  p.split_stage = 4;
+  return launch_replace_table_kernels(c, p);
 }
 
 int launch_collide(dsmc_ctx *c, const StepParams &p_in, const MlpDev *net) {

@@ -586,6 +586,7 @@ int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) 
   if (p_in.op == 2 && !(net->d_in == 2 && net->d_out == 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
   // plain BF16 chi-MLP: three passes at full occupancy (dsmc_cells.cu), or, with DSMC_F_TC_ONE_KERNEL, the single kernel
   // of cell teams + MLP server (dsmc_cells_mlp.cu)
+  if (p_in.op == 2 && (p_in.flags & DSMC_F_PAIR_REPLACE)) return launch_collide_replace_split(c, p_in, net);
   if (p_in.op == 2)
     return (p_in.flags & DSMC_F_TC_ONE_KERNEL) ? launch_collide_cells_mlp(c, p_in, net) : launch_collide_cells_split(c, p_in, net);
   StepParams p = p_in;

@@ -77,6 +77,7 @@ struct StepParams {
   // network inputs and chi; per particle the pairing permutation as 16-bit byte offsets
   float *feat0, *feat1, *chi_pair;
   uint16_t *pi_g;
+  int32_t split_stage;  // chunk kernels (with-replacement selection): 0 = whole step, 3 = network inputs only, 4 = chi from chi_pair
   // chunk decomposition (filled by launch_chunk_map)
   int32_t n_chunks;
   const int32_t *chunk_first;  // [n_chunks + 1]
@@ -148,6 +149,7 @@ int launch_collide(dsmc_ctx *c, const StepParams &p, const MlpDev *net);
 int launch_collide_cells(dsmc_ctx *c, const StepParams &p);
 int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
+int launch_collide_replace_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // dsmc_collide.cu
 int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1, float *chi, const MlpTcDev *net);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,

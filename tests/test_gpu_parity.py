@@ -726,11 +726,13 @@ def test_chapman_enskog_from_the_gpu_quadrature(dsmc):
 
 
 # --------------------------------------------------------------------------------------- (f1) with replacement
-@pytest.mark.parametrize("mode,match", [("table", True), ("table", False), ("mlp", True)])
+@pytest.mark.parametrize("mode,match", [("table", True), ("table", False), ("mlp", True), ("mlp_tc", True), ("mlp_tc", False)])
 def test_collide_abinitio_with_replacement(dsmc, mode, match):
     """pairs drawn with replacement, batch semantics.  Pair indices bit-exact, per-pair g' to the FP32
     tolerance, final velocities to 1e-5 of the thermal scale (the changes of a particle are summed by shared-memory
-    atomics in no fixed order), conserved moments to 1e-6 with matching; momentum exact without."""
+    atomics in no fixed order), conserved moments to 1e-6 with matching; momentum exact without.  mlp_tc: the chi-MLP
+    on the tensor cores (split form on the with-replacement kernels), chi within Q26 of the oracle for every pair and
+    every particle within the sum of the allowances of the pairs it sits in."""
     pop = wl.mach10_cylinder(nx=60, ny=30, n_total=300_000)
     ctx = dsmc.Context(pop.n, pop.n_cells)
     tab = _lj_table()
@@ -741,7 +743,7 @@ def test_collide_abinitio_with_replacement(dsmc, mode, match):
     vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
     cs_h = cs.cpu().numpy()
     cm = 0 if mode == "table" else 1
-    flags = dsmc.F_PAIR_REPLACE | (dsmc.F_MOMENT_MATCH if match else 0)
+    flags = dsmc.F_PAIR_REPLACE | (dsmc.F_MOMENT_MATCH if match else 0) | (dsmc.F_BF16_TC if mode == "mlp_tc" else 0)
     oflags = oracle.F_PAIR_REPLACE | (oracle.F_MOMENT_MATCH if match else 0)
     prm = dsmc.AbinitioParams(chi_mode=cm, flags=flags)
     oprm = oracle.AbinitioParams(chi_mode=cm, flags=oflags, lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
@@ -772,6 +774,25 @@ def test_collide_abinitio_with_replacement(dsmc, mode, match):
         dv = 0.5 * gn * (1e-5 + bound)
         for side in (ref.pair_i, ref.pair_j):
             np.add.at(allow_v, cs_h[kk] + side[idx], 1.05 * dv / scale[cs_h[kk] + side[idx]])
+    if mode == "mlp_tc":  # Q26 on every pair from the oracle's chi alone, carried to g' and to the particles
+        idx = np.flatnonzero(sel)
+        bound = 2e-2 * (1 + np.abs(ref.aux[idx]))
+        assert np.all(dchi[idx] <= bound)
+        slope = np.zeros_like(dchi)
+        slope[idx] = bound
+        kk = np.searchsorted(cs_h, idx, side="right") - 1
+        gn = np.sqrt(sum((a[cs_h[kk] + ref.pair_i[idx]] - a[cs_h[kk] + ref.pair_j[idx]]) ** 2 for a in v_in))
+        dv = 0.5 * gn * (1e-5 + bound)
+        for side in (ref.pair_i, ref.pair_j):
+            np.add.at(allow_v, cs_h[kk] + side[idx], 1.05 * dv / scale[cs_h[kk] + side[idx]])
+        if match:
+            # the matching factor alpha = sqrt(Theta_pre / Theta_post) sees the chi differences of ALL pairs of the cell:
+            # d(alpha) <= sum_p |c_p| dv_p / Theta with |c_p| <= 4 s and Theta ~ N s^2, and it moves every particle of
+            # the cell by d(alpha) |c| <= 16 s mean_p(dv_p / s)  (momentum is exact pair by pair: no shift term)
+            pair_part = allow_v - 1e-4
+            cell_of = np.repeat(np.arange(len(N)), N)
+            mean_part = np.bincount(cell_of, weights=pair_part, minlength=len(N)) / np.maximum(N, 1)
+            allow_v = allow_v + 16 * mean_part[cell_of]
     _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=slope)
     for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
         assert np.all(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale < allow_v)
