@@ -374,24 +374,71 @@ def test_collide_abinitio_fp32(dsmc, mode):
     ctx.close()
 
 
-def test_abinitio_acceptance_and_partial_pairs(dsmc):
+@pytest.mark.parametrize("mode", ["table", "mlp_tc", "mlp_tc_one_kernel"])
+def test_abinitio_acceptance_and_partial_pairs(dsmc, mode):
+    """NTC acceptance and a pair count below N / 2 (uniform request, then a per-cell array with zeros): pairs and
+    decisions against the oracle, per-pair g' (table: FP32; tensor cores: chi within Q26), moments of every cell, and
+    cells in which nothing was accepted stay bit-identical.  The tensor-core forms see gaps in their pair arrays here."""
     pop = wl.tiny_box(seed=12, n_cells=30, per_cell=501, T=500.0)
     ctx = dsmc.Context(pop.n, pop.n_cells)
     tab = _lj_table(64, 64)
     ctx.set_chi_table(tab.chi, tab.lnE_min, tab.lnE_max)
+    Ws, bs = wl.random_mlp(3, [2, 128, 128, 1])
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    net = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
     vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
     cs_h = cs.cpu().numpy()
-    v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
     gmax = np.full(pop.n_cells, 6 * math.sqrt(2 * KB * 500.0 / M), np.float32)
+    cm = 0 if mode == "table" else 1
     flags = dsmc.F_MOMENT_MATCH | dsmc.F_ACCEPT
-    dump = dsmc.PairDump(pop.n, "cuda")
-    ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, dsmc.AbinitioParams(flags=flags, pairs_per_cell=100), 8, 1, cr_max=dev(gmax), dump=dump)
-    ctx.check()
+    gflags = flags | (dsmc.F_BF16_TC if cm else 0) | (dsmc.F_TC_ONE_KERNEL if mode == "mlp_tc_one_kernel" else 0)
     otab = oracle.ChiTable(tab.chi, float(np.float32(tab.lnE_min)), float(np.float32(tab.lnE_max)))
-    ref = oracle.collide_abinitio(cs_h, *v_in, oracle.AbinitioParams(flags=flags, pairs_per_cell=100), 8, 1, table=otab, cr_max=gmax)
-    np.testing.assert_array_equal(dump.pair_i.cpu().numpy(), ref.pair_i)
-    assert (ref.pair_i >= 0).sum() == 3000
-    assert (dump.accepted.cpu().numpy() != ref.accepted).sum() <= 1
+    counts = np.full(pop.n_cells, 100, np.int32)
+    counts[[2, 3, 17]] = 0
+    counts[5] = 1
+    counts[9] = 250
+    for step, (ppc, pc) in enumerate(((100, None), (-1, counts))):
+        v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+        before = [t.clone() for t in (vx_s, vy_s, vz_s)]
+        dump = dsmc.PairDump(pop.n, "cuda")
+        prm = dsmc.AbinitioParams(chi_mode=cm, flags=gflags, pairs_per_cell=ppc)
+        oprm = oracle.AbinitioParams(chi_mode=cm, flags=flags, pairs_per_cell=ppc, lnE_min=float(np.float32(prm.lnE_min)),
+                                     lnE_max=float(np.float32(prm.lnE_max)))
+        if pc is not None:
+            prm.pairs_count = dev(pc)
+            oprm.pairs_count = pc
+        ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, 8, step, cr_max=dev(gmax), dump=dump)
+        ctx.check()
+        ref = oracle.collide_abinitio(cs_h, *v_in, oprm, 8, step, table=otab, net=net, cr_max=gmax)
+        np.testing.assert_array_equal(dump.pair_i.cpu().numpy(), ref.pair_i)
+        np.testing.assert_array_equal(dump.pair_j.cpu().numpy(), ref.pair_j)
+        assert (ref.pair_i >= 0).sum() == (3000 if pc is None else int(counts.sum()))
+        diff = dump.accepted.cpu().numpy() != ref.accepted
+        assert diff.sum() <= 1  # Q22
+        if diff.any():
+            continue
+        chi_g = dump.aux.cpu().numpy().astype(np.float64)
+        sel = (ref.pair_i >= 0) & (ref.accepted == 1)
+        if cm:
+            assert (np.abs(chi_g[sel] - ref.aux[sel]) / (1 + np.abs(ref.aux[sel]))).max() <= 2e-2
+            slope = 1.01 * np.abs(chi_g - ref.aux)
+        else:
+            idx, bound, _ = _q25_bound(tab, cs_h, v_in, ref, 8, step)
+            acc_idx = ref.accepted[idx] == 1
+            assert np.all(np.abs(chi_g - ref.aux)[idx][acc_idx] <= bound[acc_idx])
+            slope = np.zeros_like(chi_g)
+            slope[idx] = bound
+        _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=slope)
+        N = np.diff(cs_h)
+        pre = oracle.cell_moments(cs_h, *v_in)
+        got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+        assert np.abs(got[:, 3] / pre[:, 3] - 1).max() < 1e-6
+        assert (np.linalg.norm(got[:, :3] - pre[:, :3], axis=1) / (N * np.sqrt(pre[:, 3] / N))).max() < 1e-6
+        if pc is not None:  # cells that were asked for no pairs are untouched
+            for k in (2, 3, 17):
+                for a, b in zip((vx_s, vy_s, vz_s), before):
+                    assert torch.equal(a[cs_h[k]:cs_h[k + 1]], b[cs_h[k]:cs_h[k + 1]])
+    ctx.close()
 
 
 # --------------------------------------------------------------------------------------- a10
