@@ -189,14 +189,14 @@ struct TcEngine {
         const float z0 = __uint_as_float(v[2 * j]), z1 = __uint_as_float(v[2 * j + 1]);
         float h0, h1;
         if (ACT == DSMC_ACT_TANH) {
-          h0 = SPLIT ? tanhf(z0) : tc::tanh_approx(z0);
-          h1 = SPLIT ? tanhf(z1) : tc::tanh_approx(z1);
+          h0 = SPLIT ? tc::tanh_abs(z0) : tc::tanh_approx(z0);
+          h1 = SPLIT ? tc::tanh_abs(z1) : tc::tanh_approx(z1);
         } else if (ACT == DSMC_ACT_RELU) {
           h0 = fmaxf(z0, 0.f);
           h1 = fmaxf(z1, 0.f);
         } else {  // SiLU(2 y) = y + y tanh(y); the packed weights already carry the factor 1/2
-          h0 = fmaf(z0, SPLIT ? tanhf(z0) : tc::tanh_approx(z0), z0);
-          h1 = fmaf(z1, SPLIT ? tanhf(z1) : tc::tanh_approx(z1), z1);
+          h0 = fmaf(z0, SPLIT ? tc::tanh_abs(z0) : tc::tanh_approx(z0), z0);
+          h1 = fmaf(z1, SPLIT ? tc::tanh_abs(z1) : tc::tanh_approx(z1), z1);
         }
         o[j] = tc::pack_bf16(h0, h1);
         if (SPLIT) {  // keep the residuals for the lo pass

@@ -151,6 +151,15 @@ __device__ __forceinline__ float tanh_approx(float x) {
   asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// tanh to ~3e-7 ABSOLUTE error with two MUFU (ex2, rcp) and three FMA-pipe instructions: 1 - 2 / (e^{2x} + 1).  For the
+// split-precision (VHS-NN) path, whose operands resolve 2^-17: tanh.approx (5e-4) is too coarse there, libm's tanhf
+// (relative 1e-7, ~25 instructions with a branch) more than it needs.  Saturates correctly (e -> inf or 0).
+__device__ __forceinline__ float tanh_abs(float x) {
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 2.8853900817779268f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
+  return fmaf(-2.0f, r, 1.0f);
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
