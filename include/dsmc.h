@@ -151,9 +151,10 @@ enum {
                                    energy is restored by DSMC_F_MOMENT_MATCH.  Both operators on the FP32 / table
                                    paths; with DSMC_F_BF16_TC for the ab initio chi-MLP (dsmc_collide_abinitio), not
                                    for the VHS-NN operator.  No key sort: the cheapest selection. */
-  DSMC_F_TC_ONE_KERNEL = 256    /* dsmc_collide_abinitio, chi-MLP with DSMC_F_BF16_TC: run the step as ONE kernel (cell
-                                   teams + a tcgen05 MLP server sharing every SM) instead of the default three passes
-                                   (pairing + network inputs | chi batch on the tensor cores | rotation + matching).
+  DSMC_F_TC_ONE_KERNEL = 256    /* with DSMC_F_BF16_TC: run the fused step as ONE kernel (chi-MLP: cell teams + a tcgen05
+                                   MLP server sharing every SM; VHS-NN: chunks with a per-CTA engine) instead of the
+                                   default three passes (pairing + network inputs | MLP batch on the tensor cores |
+                                   rotation or eq. 5 + matching).
                                    Same pairs, same randoms; chi differs within the BF16 tolerance (the two forms add
                                    the output layer's partial sums in a different order).  Slower on large steps. */
 };

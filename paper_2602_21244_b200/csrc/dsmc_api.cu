@@ -59,9 +59,9 @@ static int create_impl(dsmc_ctx *c, int device, int64_t max_particles, int32_t m
     CK(cudaMalloc(&c->d_cell_count, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) + 1)));
     CK(cudaMalloc(&c->d_cell_tile_sums, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) / 4096 + 2)));
     for (int i = 0; i < 2; ++i) {
-      CK(cudaMalloc(&c->d_bin_cell[i], sizeof(int32_t) * np));
-      // (buffer 0 always exists: the split chi-MLP step keeps its pair arrays there, 8 B / particle + 48 B)
-      if (i == 0 || i < passes - 1) CK(cudaMalloc(&c->d_bin_rec[i], sizeof(float4) * (np + 4)));
+      CK(cudaMalloc(&c->d_bin_cell[i], sizeof(int32_t) * (np + 16)));  // (+ slack: the VHS-NN split form keeps its outputs here)
+      // (buffer 0 always exists: the split tensor-core steps keep their pair arrays there, up to 16 B / particle + 128 B)
+      if (i == 0 || i < passes - 1) CK(cudaMalloc(&c->d_bin_rec[i], sizeof(float4) * (np + 16)));
     }
   }
   const size_t n_chunks = (size_t)(max_particles / kChunk + 2);
@@ -227,6 +227,18 @@ int dsmc_set_mlp(dsmc_ctx *c, int slot, const dsmc_mlp_desc *d) {
   c->d_tc_blob[slot] = blob_new;
   c->mlp[slot] = m;
   c->mlp_tc[slot] = tc_new;
+  memset(&c->tc_tail[slot], 0, sizeof(c->tc_tail[slot]));
+  if (tc_new.H != 0 && d->n_layers == 3 && d->dims[3] <= 3) {
+    dsmc::TcTailF32 &t = c->tc_tail[slot];
+    const int H = d->dims[1];
+    const float hs = d->act == DSMC_ACT_SILU ? 0.5f : 1.0f;
+    t.d_out = d->dims[3];
+    for (int k = 0; k < H; ++k) t.b2[k] = hs * d->b[1][k];
+    for (int o = 0; o < t.d_out; ++o) {
+      for (int k = 0; k < H; ++k) t.w3[o][k] = d->W[2][(size_t)o * H + k];
+      t.b3[o] = d->b[2][o];
+    }
+  }
   c->has_mlp[slot] = true;
   return DSMC_OK;
 }

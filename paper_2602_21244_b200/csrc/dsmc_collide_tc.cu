@@ -450,6 +450,242 @@ int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1,
 }
 
 // ---------------------------------------------------------------------------------------------
+// Rows -> MLP outputs in SPLIT precision on the two-slot pipeline (the VHS-NN operator of the split fused step,
+// dsmc_collide.cu): d_in <= 8 inputs per row, up to three outputs.  Layer 1 as everywhere (split operand, bias column);
+// the hidden activations are carried as bf16 hi + bf16 lo in tensor memory (A_hi where the plain pipe keeps A, A_lo in
+// the columns the plain pipe uses for its bias and output blocks) and layer 2 is three UMMA passes
+// (hi.hi + lo.hi + hi.lo, FP32 accumulate); its bias and the whole output layer are FP32 on the CUDA cores, folded
+// into the second activation (constant-bank operands): more exact than a split third tensor-core layer and no third
+// hand-off.  Eq. 5 divides by |h|, so the activation is tanh_abs (3e-7), not tanh.approx.
+// ---------------------------------------------------------------------------------------------
+template <int ACT>
+__device__ __forceinline__ float act_split(float z) {
+  if (ACT == DSMC_ACT_TANH) return tc::tanh_abs(z);
+  if (ACT == DSMC_ACT_RELU) return fmaxf(z, 0.f);
+  return fmaf(z, tc::tanh_abs(z), z);  // SiLU(2 y) = y + y tanh(y), y = z (weights and biases carry the 1/2)
+}
+
+// first activation: D -> act -> (hi, lo) bf16 -> A_hi, A_lo of the slot
+template <int H, int ACT>
+__device__ __forceinline__ void act1_split(TcPipe<H> &pipe, int s, int act_warp) {
+  using SH = PipeShape<H>;
+  constexpr int NQ = kPipeActWarps / 4, NC = H / (16 * NQ);
+  tc::mbar_wait(pipe.full_e + s, pipe.ph_e[s]);
+  pipe.ph_e[s] ^= 1u;
+  tc::fence_after();
+  const uint32_t base = pipe.tmem + (((uint32_t)((act_warp & 3) * 32)) << 16) + s * SH::SLOT_COLS;
+  const int grp = act_warp >> 2;
+  const uint32_t d0 = base + SH::COL_D + grp * (H / NQ), ah = base + SH::COL_A + grp * (H / (2 * NQ)),
+                 al = base + SH::COL_BIAS + grp * (H / (2 * NQ));
+  uint32_t v[2][16];
+  tc::tmem_ld16(d0, v[0]);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    tc::wait_ld();
+    if (c + 1 < NC) tc::tmem_ld16(d0 + (c + 1) * 16, v[(c + 1) & 1]);
+    uint32_t hi[8], lo[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const float h0 = act_split<ACT>(__uint_as_float(v[c & 1][2 * j])), h1 = act_split<ACT>(__uint_as_float(v[c & 1][2 * j + 1]));
+      hi[j] = tc::pack_bf16(h0, h1);
+      lo[j] = tc::pack_bf16(h0 - __uint_as_float(hi[j] << 16), h1 - __uint_as_float(hi[j] & 0xFFFF0000u));
+    }
+    tc::tmem_st8(ah + c * 8, hi);
+    tc::tmem_st8(al + c * 8, lo);
+  }
+  tc::wait_st();
+  tc::fence_before();
+  pipe.warp_arrive(pipe.a_ready + s);
+}
+
+// second activation and the output layer: this thread's partial sums (its row, column group GRP) of the d_out outputs
+template <int H, int GRP, int ACT>
+__device__ __forceinline__ void out_split(uint32_t d0, const TcTailF32 &T, float (&y)[3]) {
+  constexpr int NQ = kPipeActWarps / 4, NC = H / (16 * NQ), C0 = GRP * (H / NQ);
+  uint32_t v[2][16];
+  y[0] = GRP == 0 ? T.b3[0] : 0.f;
+  y[1] = GRP == 0 ? T.b3[1] : 0.f;
+  y[2] = GRP == 0 ? T.b3[2] : 0.f;
+  tc::tmem_ld16(d0, v[0]);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    tc::wait_ld();
+    if (c + 1 < NC) tc::tmem_ld16(d0 + (c + 1) * 16, v[(c + 1) & 1]);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const float h = act_split<ACT>(__uint_as_float(v[c & 1][j]) + T.b2[C0 + 16 * c + j]);
+      y[0] = fmaf(h, T.w3[0][C0 + 16 * c + j], y[0]);
+      y[1] = fmaf(h, T.w3[1][C0 + 16 * c + j], y[1]);
+      y[2] = fmaf(h, T.w3[2][C0 + 16 * c + j], y[2]);
+    }
+  }
+}
+
+template <int H, int ACT>
+__device__ __forceinline__ void act2_split(TcPipe<H> &pipe, int s, int act_warp, const TcTailF32 &T, float *zrow,
+                                           uint64_t *z_bar) {
+  using SH = PipeShape<H>;
+  constexpr int NQ = kPipeActWarps / 4;
+  tc::mbar_wait(pipe.full_e + s, pipe.ph_e[s]);
+  pipe.ph_e[s] ^= 1u;
+  tc::fence_after();
+  const int grp = act_warp >> 2, lane = threadIdx.x & 31;
+  const uint32_t d0 = pipe.tmem + (((uint32_t)((act_warp & 3) * 32)) << 16) + s * SH::SLOT_COLS + SH::COL_D + grp * (H / NQ);
+  float y[3];
+  if (grp == 0) out_split<H, 0, ACT>(d0, T, y);
+  else if (grp == 1) out_split<H, 1, ACT>(d0, T, y);
+  else if (grp == 2) out_split<H, 2, ACT>(d0, T, y);
+  else out_split<H, 3, ACT>(d0, T, y);
+  float *zr = zrow + (grp * 128 + (act_warp & 3) * 32 + lane) * 4;  // [group][row][4]
+  *reinterpret_cast<float4 *>(zr) = make_float4(y[0], y[1], y[2], 0.f);
+  tc::fence_before();
+  __syncwarp();
+  if (lane == 0) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(pipe.a_ready + s)) : "memory");  // D is free
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc::smem_u32(z_bar)) : "memory");
+  }
+}
+
+template <int H>
+__global__ void __launch_bounds__(kPipeThreads, 1)
+    k_mlp_rows_tc_split(int64_t n, const float *__restrict__ x, int64_t x_stride, int d_in, float *__restrict__ y0,
+                        float *__restrict__ y1, float *__restrict__ y2, const MlpTcDev net, const TcTailF32 T) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  using SH = PipeShape<H>;
+  TcPipe<H> pipe;
+  unsigned char *w2lo = smem_raw + ((SH::SMEM_BYTES + 127) & ~127);
+  float *zs = reinterpret_cast<float *>(w2lo + H * H * 2);               // [2][2][4][128][4]
+  uint64_t *z_bar = reinterpret_cast<uint64_t *>(zs + 2 * 2 * 4 * 128 * 4);  // [2], then the W2lo barrier
+  uint64_t *w_bar = z_bar + 2;
+  if (threadIdx.x == 0) {
+    tc::mbar_init(z_bar + 0, kPipeActWarps);
+    tc::mbar_init(z_bar + 1, kPipeActWarps);
+    tc::mbar_init(w_bar, 1);
+  }
+  pipe.init(smem_raw, net.w_blob, kPipeActWarps, kPipeIoWarps);  // (fences the barrier inits, ends with CTA barriers)
+  if (threadIdx.x == 0) {
+    tc::mbar_expect_tx(w_bar, (uint32_t)(H * H * 2));
+    tc::bulk_g2s(w2lo, reinterpret_cast<const unsigned char *>(net.w_blob) + SH::BLOB_BYTES, (uint32_t)(H * H * 2), w_bar);
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t n_tiles = (n + 127) / 128;
+  const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const int64_t n_rounds = (mine + 1) / 2;
+  if (warp < kPipeActWarps) {
+    for (int64_t r = 0; r < n_rounds; ++r) {
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {
+        if (net.act == DSMC_ACT_TANH) act1_split<H, DSMC_ACT_TANH>(pipe, s, warp);
+        else if (net.act == DSMC_ACT_RELU) act1_split<H, DSMC_ACT_RELU>(pipe, s, warp);
+        else act1_split<H, DSMC_ACT_SILU>(pipe, s, warp);
+      }
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {
+        float *zrow = zs + (size_t)((s * 2 + (int)(r & 1)) * 4) * 128 * 4;
+        if (net.act == DSMC_ACT_TANH) act2_split<H, DSMC_ACT_TANH>(pipe, s, warp, T, zrow, z_bar + s);
+        else if (net.act == DSMC_ACT_RELU) act2_split<H, DSMC_ACT_RELU>(pipe, s, warp, T, zrow, z_bar + s);
+        else act2_split<H, DSMC_ACT_SILU>(pipe, s, warp, T, zrow, z_bar + s);
+      }
+    }
+  } else if (warp < kPipeActWarps + kPipeIoWarps) {
+    const int io_warp = warp - kPipeActWarps, row = io_warp * 32 + lane;
+    auto features = [&](int s, int64_t k) {
+      const int64_t p = (blockIdx.x + k * gridDim.x) * 128 + row;
+      float f[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) f[j] = (k < mine && p < n && j < d_in) ? __ldg(x + j * x_stride + p) : 0.f;
+      pipe.write_a1_row(s, (int)((k >> 1) & 1), row, f);
+      pipe.io_publish(s);
+    };
+    if (n_rounds > 0) {
+      features(0, 0);
+      features(1, 1);
+    }
+    uint32_t phz[2] = {0u, 0u};
+    for (int64_t r = 0; r < n_rounds; ++r) {
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {
+        const int64_t k = 2 * r + s;
+        if (r + 1 < n_rounds) features(s, k + 2);
+        tc::mbar_wait(z_bar + s, phz[s]);
+        phz[s] ^= 1u;
+        const float4 *zr = reinterpret_cast<const float4 *>(zs + (size_t)((s * 2 + (int)(r & 1)) * 4) * 128 * 4) + row;
+        const float4 a = zr[0], b = zr[128], c = zr[256], d = zr[384];
+        const int64_t p = (blockIdx.x + k * gridDim.x) * 128 + row;
+        if (k < mine && p < n) {
+          y0[p] = ((a.x + b.x) + c.x) + d.x;
+          y1[p] = ((a.y + b.y) + c.y) + d.y;
+          y2[p] = ((a.z + b.z) + c.z) + d.z;
+        }
+      }
+    }
+  } else {
+    // layer 2 in three passes: hi.hi + lo.hi + hi.lo
+    auto layer2 = [&](int s) {
+      tc::mbar_wait(pipe.a_ready + s, pipe.ph_a[s]);
+      pipe.ph_a[s] ^= 1u;
+      if (lane == 0) {
+        tc::fence_after();
+        constexpr uint32_t idesc = tc::instr_desc(128, H);
+        const uint32_t tD = pipe.tmem + s * SH::SLOT_COLS + SH::COL_D, tAh = pipe.tmem + s * SH::SLOT_COLS + SH::COL_A,
+                       tAl = pipe.tmem + s * SH::SLOT_COLS + SH::COL_BIAS;
+        const uint32_t wh = tc::smem_u32(pipe.w) + SH::OFF_W2, wl = tc::smem_u32(w2lo);
+#pragma unroll
+        for (int ks = 0; ks < H / 16; ++ks)
+          tc::mma_ts(tD, tAh + ks * 8, tc::smem_desc(wh + ks * 2 * H * 16, H * 16, 128), idesc, ks > 0 ? 1u : 0u);
+#pragma unroll
+        for (int ks = 0; ks < H / 16; ++ks)
+          tc::mma_ts(tD, tAl + ks * 8, tc::smem_desc(wh + ks * 2 * H * 16, H * 16, 128), idesc, 1u);
+#pragma unroll
+        for (int ks = 0; ks < H / 16; ++ks)
+          tc::mma_ts(tD, tAh + ks * 8, tc::smem_desc(wl + ks * 2 * H * 16, H * 16, 128), idesc, 1u);
+        tc::mma_commit(pipe.full_e + s);
+      }
+      __syncwarp();
+    };
+    if (n_rounds > 0) {
+      pipe.mma_layer1(0, 0, true);
+      pipe.mma_layer1(1, 0, false);
+      if (lane == 0) tc::mbar_wait(w_bar, 0);  // W2lo has landed
+      __syncwarp();
+    }
+    for (int64_t r = 0; r < n_rounds; ++r) {
+      const bool more = r + 1 < n_rounds;
+      const int par = (int)((r + 1) & 1);
+      layer2(0);
+      layer2(1);
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {
+        tc::mbar_wait(pipe.a_ready + s, pipe.ph_a[s]);  // the second activation has read D
+        pipe.ph_a[s] ^= 1u;
+        if (more) pipe.mma_layer1(s, par, false);
+      }
+    }
+  }
+  pipe.teardown();
+}
+
+template <int H>
+static int launch_mlp_rows_tc_split_h(dsmc_ctx *c, int64_t n, const float *x, int64_t x_stride, float *y0, float *y1,
+                                      float *y2, const MlpTcDev *net, const TcTailF32 *tail) {
+  const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms);
+  const int smem = ((PipeShape<H>::SMEM_BYTES + 127) & ~127) + H * H * 2 + 2 * 2 * 4 * 128 * 16 + 64 + 128;
+  auto kern = k_mlp_rows_tc_split<H>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return DSMC_ERR_CUDA;
+  kern<<<grid, kPipeThreads, smem, c->stream>>>(n, x, x_stride, net->d_in, y0, y1, y2, *net, *tail);
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+// y[o][p] = MLP(x[0..d_in)[p])[o], o < 3, rows p < n; x: d_in arrays x + j x_stride; split-precision tensor-core path
+int launch_mlp_rows_tc_split(dsmc_ctx *c, int64_t n, const float *x, int64_t x_stride, float *y0, float *y1, float *y2,
+                             const MlpTcDev *net, const TcTailF32 *tail) {
+  if (net->d_in < 1 || net->d_in > 8 || tail->d_out < 1 || tail->d_out > 3) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  return net->H == 128 ? launch_mlp_rows_tc_split_h<128>(c, n, x, x_stride, y0, y1, y2, net, tail)
+                       : launch_mlp_rows_tc_split_h<64>(c, n, x, x_stride, y0, y1, y2, net, tail);
+}
+
+// ---------------------------------------------------------------------------------------------
 // a2-a9 fused step, tensor-core operator.  P.op = 0: VHS-NN (eqs. 1-5), P.op = 2: chi-MLP + rotation.
 // ---------------------------------------------------------------------------------------------
 template <int H, bool SPLIT, class CK>
@@ -589,6 +825,8 @@ int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) 
   if (p_in.op == 2 && (p_in.flags & DSMC_F_PAIR_REPLACE)) return launch_collide_replace_split(c, p_in, net);
   if (p_in.op == 2)
     return (p_in.flags & DSMC_F_TC_ONE_KERNEL) ? launch_collide_cells_mlp(c, p_in, net) : launch_collide_cells_split(c, p_in, net);
+  // VHS-NN: the split form (dsmc_collide.cu) unless the one-kernel form is asked for
+  if (p_in.op == 0 && !(p_in.flags & (DSMC_F_TC_ONE_KERNEL | DSMC_F_PAIR_REPLACE))) return launch_collide_vhs_split(c, p_in, net);
   StepParams p = p_in;
   int rc = launch_chunk_map(c, p);
   if (rc != DSMC_OK) return rc;

@@ -37,6 +37,16 @@ struct MlpTcDev {
   float w3_host[129];         // HOST copy of the FP32 output layer when d_out = 1: w[0..H), bias at [128]
 };
 
+// FP32 tail of a 3-layer MLP with up to three outputs (the VHS-NN operator on the split tensor-core path): bias of
+// the second hidden layer (already scaled by 1/2 for SiLU, like the packed weights) and the whole output layer.
+// Passed to the batch kernel by value: constant-bank operands.
+struct TcTailF32 {
+  float b2[128];
+  float w3[3][128];
+  float b3[3];
+  int d_out;
+};
+
 struct ChiTableDev {
   const float4 *quad;  // [(nE-1)(nB-1)] the four nodes around each grid cell (one 16 B load per lookup)
   int nE, nB;
@@ -77,6 +87,9 @@ struct StepParams {
   // network inputs and chi; per particle the pairing permutation as 16-bit byte offsets
   float *feat0, *feat1, *chi_pair;
   uint16_t *pi_g;
+  float *out3[3];       // VHS-NN split form: the three network outputs per pair
+  int64_t split_np;     // VHS-NN split form: stride between the input arrays feat0 + k split_np, k < split_din
+  int32_t split_din;
   int32_t split_stage;  // chunk kernels (with-replacement selection): 0 = whole step, 3 = network inputs only, 4 = chi from chi_pair
   // chunk decomposition (filled by launch_chunk_map)
   int32_t n_chunks;
@@ -119,6 +132,7 @@ struct dsmc_ctx {
   dsmc::MlpDev mlp[2];
   dsmc::MlpTcDev mlp_tc[2];
   float *d_weights[2];
+  dsmc::TcTailF32 tc_tail[2];  // HOST copies, filled by dsmc_set_mlp when the tensor-core image exists
   void *d_tc_blob[2];
   bool has_table;
   dsmc::ChiTableDev table;
@@ -150,7 +164,10 @@ int launch_collide_cells(dsmc_ctx *c, const StepParams &p);
 int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_collide_replace_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // dsmc_collide.cu
-int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1, float *chi, const MlpTcDev *net);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
+int launch_collide_vhs_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);      // dsmc_collide.cu
+int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1, float *chi, const MlpTcDev *net);
+int launch_mlp_rows_tc_split(dsmc_ctx *c, int64_t n, const float *x, int64_t x_stride, float *y0, float *y1, float *y2,
+                             const MlpTcDev *net, const TcTailF32 *tail);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_chi_batch(dsmc_ctx *c, int64_t n, const float *E, const float *b, float *chi, int mode, float b_max,
                      float lnE_min, float lnE_max, const MlpDev *net);

@@ -581,9 +581,12 @@ def test_collide_abinitio_bf16_tc_few_cells_and_ragged(dsmc, one_kernel):
     ctx.close()
 
 
+@pytest.mark.parametrize("one_kernel", [False, True])
 @pytest.mark.parametrize("case", ["cfg1_tiny", "cfg3_cavity_small", "ragged6"])
-def test_collide_vhs_nn_bf16_tc(dsmc, case):
-    """BF16 tensor-core VHS-NN: bit-exact pairing, 2e-2 per pair on the gated set (Q21), 1e-6 on moments."""
+def test_collide_vhs_nn_bf16_tc(dsmc, case, one_kernel):
+    """BF16 tensor-core VHS-NN, both forms (default: three passes around a persistent split-precision batch kernel;
+    F_TC_ONE_KERNEL: the chunk kernel with its own engine): bit-exact pairing, 2e-2 per pair on the gated set (Q21),
+    1e-6 on moments; with NTC acceptance in the last step."""
     n_in = 8
     if case == "cfg1_tiny":
         pop, H, ppc, sw = wl.tiny_box(), 64, 50, 0
@@ -598,19 +601,32 @@ def test_collide_vhs_nn_bf16_tc(dsmc, case):
     ctx, net = _setup_vhs(dsmc, pop, H, sw, n_in=n_in)
     vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
     cs_h = cs.cpu().numpy()
-    flags = dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC
+    flags = dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC | (dsmc.F_TC_ONE_KERNEL if one_kernel else 0)
     prm = dsmc.VhsParams(sigma_v=wl.SIGMA_V, pairs_per_cell=ppc, flags=flags)
     oprm = oracle.VhsParams(sigma_v=float(np.float32(wl.SIGMA_V)), pairs_per_cell=ppc)
-    for step in range(2):
+    for step in range(3):
         v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
         dump = dsmc.PairDump(pop.n, "cuda")
-        ctx.collide_vhs_nn(cs, vx_s, vy_s, vz_s, prm, seed=sw, step=step, dump=dump)
+        cap = None
+        if step == 2:  # NTC acceptance on top
+            prm = dsmc.VhsParams(sigma_v=wl.SIGMA_V, pairs_per_cell=ppc, flags=flags | dsmc.F_ACCEPT)
+            oprm = oracle.VhsParams(sigma_v=float(np.float32(wl.SIGMA_V)), pairs_per_cell=ppc,
+                                    flags=oracle.F_NOISE | oracle.F_ENERGY_SHELL | oracle.F_MOMENT_MATCH | oracle.F_ACCEPT)
+            cap = np.full(pop.n_cells, oracle.vhs_sigma_g(6 * wl.SIGMA_V, oprm), np.float32)
+        ctx.collide_vhs_nn(cs, vx_s, vy_s, vz_s, prm, seed=sw, step=step, sigma_cr_max=dev(cap) if cap is not None else None, dump=dump)
         ctx.check()
-        ref = oracle.collide_vhs_nn(cs_h, *v_in, net, oprm, sw, step)
+        ref = oracle.collide_vhs_nn(cs_h, *v_in, net, oprm, sw, step, sigma_cr_max=cap)
+        if cap is not None:
+            diff = dump.accepted.cpu().numpy() != ref.accepted
+            assert diff.sum() <= 2  # Q22
+            assert 0.2 < ref.accepted[ref.pair_i >= 0].mean() < 0.95
+            if diff.any():
+                continue
         hn = ref.aux
         med = np.median(hn[ref.pair_i >= 0])
-        err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 2e-2, 1e-6, gate=hn >= 0.25 * med)
-        print("vhs bf16 %s: all pairs %s; excluded %.2f%%" % (case, _quantiles(err), 100 * (1 - (hn[ref.pair_i >= 0] >= 0.25 * med).mean())))
+        gate = (hn >= 0.25 * med) | (ref.accepted == 0)
+        err = _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 2e-2, 1e-6, gate=gate)
+        print("vhs bf16 %s one_kernel=%s: all pairs %s; excluded %.2f%%" % (case, one_kernel, _quantiles(err), 100 * (1 - gate[ref.pair_i >= 0].mean())))
         N = np.diff(cs_h)
         pre = oracle.cell_moments(cs_h, *v_in)
         got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
