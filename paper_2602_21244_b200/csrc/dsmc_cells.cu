@@ -169,4 +169,29 @@ int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p_in, const MlpTcD
   return launch_cells_pass<4>(c, p);
 }
 
+// VHS-NN operator on the tensor cores, split form on the cell-team kernels (default for DSMC_F_BF16_TC;
+// DSMC_F_TC_ONE_KERNEL keeps the chunk kernel with its own engine, k_collide_tc): OP 5 (pairing + the 8 or 6 network inputs of
+// every pair, eqs. 1-3), k_mlp_rows_tc_split (split-precision batch, dsmc_collide_tc.cu), OP 6 (stored pairing, outputs
+// -> eq. 5 -> eqs. 6-8, matching, store).  Pair arrays: inputs in the radix sort's record buffer (16 B / particle),
+// outputs and the stored pairing in its two cell-id buffers.
+int launch_collide_cells_vhs_split(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
+  const TcTailF32 *tail = &c->tc_tail[0];
+  if (p_in.op != 0 || !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3) || tail->d_out != 3)
+    return DSMC_ERR_UNSUPPORTED_SHAPE;
+  StepParams p = p_in;
+  const int64_t np = (p.n / 2 + 4) & ~(int64_t)3;
+  p.feat0 = reinterpret_cast<float *>(c->d_bin_rec[0]);
+  p.split_np = np;
+  p.split_din = net->d_in;
+  p.out3[0] = reinterpret_cast<float *>(c->d_bin_cell[0]);
+  p.out3[1] = p.out3[0] + np;
+  p.out3[2] = reinterpret_cast<float *>(c->d_bin_cell[1]);
+  p.pi_g = reinterpret_cast<uint16_t *>(p.out3[2] + np);
+  int rc = launch_cells_pass<5>(c, p);
+  if (rc != DSMC_OK) return rc;
+  rc = launch_mlp_rows_tc_split(c, p.n / 2 + 1, p.feat0, np, p.out3[0], p.out3[1], p.out3[2], net, tail);
+  if (rc != DSMC_OK) return rc;
+  return launch_cells_pass<6>(c, p);
+}
+
 }  // namespace dsmc

@@ -298,7 +298,7 @@ struct CellTeam {
   // a pair that does not collide) parked in cnt[].  STAGE 2: chi = exp(z) from the delivered outputs, rotation, commit.
   template <int STAGE>
   __device__ __forceinline__ bool pairs_phase(const StepParams &P, const int4 item, uint32_t cell_ctr, bool accept,
-                                              int slot) {
+                                              int slot, float tfeat = 0.f) {
     const int lane = tid & 31, warp = tid >> 5;
     const int gs = item.y, M = item.w;
     bool any_acc = false;
@@ -319,12 +319,14 @@ struct CellTeam {
         if (!v1) { oi[1] = oi[0]; oj[1] = oj[0]; }
         float Ub[2] = {0.f, 0.f}, eps[2] = {0.f, 0.f}, Ua[2] = {0.f, 0.f}, cap = 0.f;
         if (STAGE != 2) {
-          const uint4 rr = cells_philox(P, (uint32_t)dp, cell_ctr, P.step, 1u);
-          // U_b = ((x >> 9) + 1/2) 2^-23 built from the float 1.f + (x >> 9) 2^-23; eps = 2 pi (U_eps - 1/2) likewise
-          Ub[0] = __uint_as_float((rr.x >> 9) | 0x3F800000u) - 0.99999994f;
-          Ub[1] = __uint_as_float((rr.z >> 9) | 0x3F800000u) - 0.99999994f;
-          eps[0] = fmaf(__uint_as_float((rr.y >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f);
-          eps[1] = fmaf(__uint_as_float((rr.w >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f);
+          if (STAGE < 5) {  // (the VHS-NN stages 5, 6 draw no impact parameter and no azimuth)
+            const uint4 rr = cells_philox(P, (uint32_t)dp, cell_ctr, P.step, 1u);
+            // U_b = ((x >> 9) + 1/2) 2^-23 built from the float 1.f + (x >> 9) 2^-23; eps = 2 pi (U_eps - 1/2) likewise
+            Ub[0] = __uint_as_float((rr.x >> 9) | 0x3F800000u) - 0.99999994f;
+            Ub[1] = __uint_as_float((rr.z >> 9) | 0x3F800000u) - 0.99999994f;
+            eps[0] = fmaf(__uint_as_float((rr.y >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f);
+            eps[1] = fmaf(__uint_as_float((rr.w >> 9) | 0x3F800000u) - 1.5f, 6.2831855f, 3.7450704e-7f);
+          }
           if (accept) {  // stream 3: U_acc of pair slot s = word s & 3 of block s >> 2
             const uint4 ra = cells_philox(P, (uint32_t)dp >> 1, cell_ctr, P.step, 3u);
             Ua[0] = u01((dp & 1) ? ra.z : ra.x);
@@ -347,7 +349,29 @@ struct CellTeam {
           const float g2 = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
           bool acc = valid;
           if (STAGE != 2) {
-            if (accept) acc = valid && (Ua[k] * cap < sqrtf(g2));  // constant cross-section: U g_max < g
+            // ab initio: constant cross-section, U g_max < g; VHS-NN: U (sigma g)_max < sigma_T(g) g
+            if (accept) acc = valid && (Ua[k] * cap < (STAGE >= 5 ? P.vhs_c * powf(sqrtf(g2), P.vhs_e) : sqrtf(g2)));
+          }
+          if (STAGE == 5) {  // VHS-NN inputs (eqs. 1-3, Q1-Q3) -> pair arrays feat0 + k split_np
+            if (valid) {
+              float n0 = 0.f, n1 = 0.f, n2 = 0.f;
+              if (P.flags & DSMC_F_NOISE) {
+                const uint4 rn = cells_philox(P, (uint32_t)(s0 + k), cell_ctr, P.step, 2u);
+                box_muller3(rn, n0, n1, n2);
+                n0 *= P.noise_sigma; n1 *= P.noise_sigma; n2 *= P.noise_sigma;
+              }
+              float *f = P.feat0 + (int64_t)(gs >> 1) + s0 + k;
+              const int64_t np = P.split_np;
+              f[0] = gx * P.inv_sigma_v; f[np] = gy * P.inv_sigma_v; f[2 * np] = gz * P.inv_sigma_v;
+              if (P.split_din == 8) {
+                f[3 * np] = sqrtf(g2) * P.inv_sigma_v;
+                f[4 * np] = tfeat;
+                f[5 * np] = n0; f[6 * np] = n1; f[7 * np] = n2;
+              } else {
+                f[3 * np] = n0; f[4 * np] = n1; f[5 * np] = n2;
+              }
+            }
+            continue;
           }
           if (STAGE == 1 || STAGE == 3) {  // chi-MLP inputs (Q15): ((E~ - E~min) / (E~max - E~min) clamped to [0, 1], b~)
             const float e = (0.6931471806f * mufu_lg2(P.e_coef * g2) - P.lnE_min) * P.inv_lnE_range;
@@ -368,7 +392,26 @@ struct CellTeam {
             eps[k] = park[row];
             acc = valid && eps[k] < 1e29f;
           }
-          if (acc) {
+          if (acc && STAGE == 6) {  // VHS-NN: outputs of the batch kernel -> eq. 5 (guard Q4) -> eqs. 6-8
+            const int64_t pp = (int64_t)(gs >> 1) + s0 + k;
+            const float h0 = __ldg(P.out3[0] + pp), h1 = __ldg(P.out3[1] + pp), h2 = __ldg(P.out3[2] + pp);
+            const float hn = sqrtf(h0 * h0 + h1 * h1 + h2 * h2);
+            chi = hn;  // (dumped as aux)
+            if (P.flags & DSMC_F_ENERGY_SHELL) {
+              if (hn >= P.shell_eps) {
+                const float sc = sqrtf(g2) / hn;
+                px = sc * h0; py = sc * h1; pz = sc * h2;
+              }
+            } else {
+              px = P.sigma_v * h0; py = P.sigma_v * h1; pz = P.sigma_v * h2;
+            }
+            const float hx = px - gx, hy = py - gy, hz = pz - gz;
+            float *qi = reinterpret_cast<float *>(const_cast<char *>(Xb) + oi[k]);
+            float *qj = reinterpret_cast<float *>(const_cast<char *>(Xb) + oj[k]);
+            qi[0] = fmaf(0.5f, hx, vix[k]); qi[C] = fmaf(0.5f, hy, viy[k]); qi[2 * C] = fmaf(0.5f, hz, viz[k]);
+            qj[0] = fmaf(-0.5f, hx, vjx[k]); qj[C] = fmaf(-0.5f, hy, vjy[k]); qj[2 * C] = fmaf(-0.5f, hz, vjz[k]);
+            any_acc = true;
+          } else if (acc) {
             if (STAGE == 2) {
               chi = __expf(zbuf[row]);  // chi = expm1(softplus(z)) = exp(z)
             } else if (STAGE == 4) {
@@ -501,7 +544,7 @@ struct CellTeam {
       theta = fmaxf(s2 - fN * fmaf(mx, mx, fmaf(my, my, mz * mz)), 0.f);
     }
     if (tid == 0) next = entry(list, n_items, next_idx);
-    if (OP == 4) {  // split form, second pass: the pairing was made (and stored) by the first pass
+    if (OP == 4 || OP == 6) {  // split form, second pass: the pairing was made (and stored) by the first pass
       const uint16_t *__restrict__ gp = P.pi_g + gs;
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
@@ -595,10 +638,10 @@ struct CellTeam {
         if (m > 1u) pi[rank] = (uint16_t)(4u * (e & slot_mask));
       }
     }
-    }  // OP != 4
+    }  // OP != 4, 6
     if (NT > 32 && tid == 0) *reinterpret_cast<int4 *>(misc + 8) = next;
     sync();
-    if (OP == 3) {  // split form, first pass: the pairing goes to HBM for the second pass
+    if (OP == 3 || OP == 5) {  // split form, first pass: the pairing goes to HBM for the second pass
       uint16_t *__restrict__ gp = P.pi_g + gs;
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
@@ -647,10 +690,14 @@ struct CellTeam {
       any_acc = pairs_phase<3>(P, item, cell_ctr, accept, 0);
     } else if (OP == 4) {
       any_acc = pairs_phase<4>(P, item, cell_ctr, accept, 0);
+    } else if (OP == 5) {  // VHS-NN split form: T_cell = m Theta / (3 kB N) is one of the network inputs
+      any_acc = pairs_phase<5>(P, item, cell_ctr, accept, 0, theta * P.T_coef * invN * P.inv_T_scale);
+    } else if (OP == 6) {
+      any_acc = pairs_phase<6>(P, item, cell_ctr, accept, 0);
     } else {
       any_acc = pairs_phase<0>(P, item, cell_ctr, accept, 0);
     }
-    bool collided = OP != 3;  // (first pass of the split form: nothing is committed, nothing to store)
+    bool collided = OP != 3 && OP != 5;  // (first pass of the split forms: nothing is committed, nothing to store)
     if (accept) {
       collided = __any_sync(0xffffffffu, any_acc);
       if (NT > 32 && collided && lane == 0) misc[12] = 1;
