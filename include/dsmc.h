@@ -94,8 +94,10 @@ typedef struct {
  *         the paper's eq. 3 as read in Q1); dims[n_layers] = 3.
  * slot 1: chi-MLP: dims[0] = 2 ((E~-E~min)/(E~max-E~min), b~), output 1,
  *         chi = expm1(softplus(z)) (Q15).
- * The BF16 tensor-core path (DSMC_F_BF16_TC) needs n_layers = 3 and equal hidden widths in
- * {64, 128}; other shapes run only on the FP32 path (DSMC_ERR_UNSUPPORTED_SHAPE otherwise). */
+ * The BF16 tensor-core paths (DSMC_F_BF16_TC) take at most 8 inputs and hidden widths <= 128 (any widths: narrower
+ * layers are zero-padded on the device to 64 or 128).  chi-MLP (slot 1): 2 to 5 hidden layers (n_layers 3..6), e.g. the
+ * paper's five hidden layers of decreasing width; VHS-NN (slot 0) and every DSMC_F_TC_ONE_KERNEL form: exactly 2 hidden
+ * layers.  Other shapes run only on the FP32 path (DSMC_ERR_UNSUPPORTED_SHAPE otherwise). */
 int dsmc_set_mlp(dsmc_ctx *ctx, int slot, const dsmc_mlp_desc *desc);
 
 /* chi table: chi_host HOST fp32 [nE][nB] row-major, node (iE,iB) at

@@ -230,7 +230,7 @@ int dsmc_set_mlp(dsmc_ctx *c, int slot, const dsmc_mlp_desc *d) {
   memset(&c->tc_tail[slot], 0, sizeof(c->tc_tail[slot]));
   if (tc_new.H != 0 && d->n_layers == 3 && d->dims[3] <= 3) {
     dsmc::TcTailF32 &t = c->tc_tail[slot];
-    const int H = d->dims[1];
+    const int H = d->dims[2];  // width of the second hidden layer (units beyond it are zero padding)
     const float hs = d->act == DSMC_ACT_SILU ? 0.5f : 1.0f;
     t.d_out = d->dims[3];
     for (int k = 0; k < H; ++k) t.b2[k] = hs * d->b[1][k];

@@ -36,23 +36,33 @@ static inline size_t panel_off(int r, int k, int R) { return (size_t)(k / 8) * R
 
 int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStream_t s) {
   out->H = 0;
-  if (d->n_layers != 3) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  const int d_in = d->dims[0], H = d->dims[1], d_out = d->dims[3];
-  if (d->dims[2] != H || (H != 64 && H != 128) || d_in < 1 || d_in > 8 || d_out < 1 || d_out > 16)
-    return DSMC_ERR_UNSUPPORTED_SHAPE;
+  // 2..5 hidden layers (n_layers 3..6), hidden widths <= 128 (zero-padded to H = 64 or 128: a padded unit has zero
+  // weights and bias, act(0) = 0 for tanh / ReLU / SiLU, and zero weights into the next layer)
+  if (d->n_layers < 3 || d->n_layers > 6) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  const int nh = d->n_layers - 1, d_in = d->dims[0], d_out = d->dims[d->n_layers];
+  int wmax = 0;
+  for (int l = 1; l <= nh; ++l) {
+    if (d->dims[l] < 1 || d->dims[l] > 128) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    wmax = std::max(wmax, d->dims[l]);
+  }
+  const int H = wmax <= 64 ? 64 : 128;
+  if (d_in < 1 || d_in > 8 || d_out < 1 || d_out > 16) return DSMC_ERR_UNSUPPORTED_SHAPE;
   // SiLU(z) = y + y tanh(y) with y = z / 2: the hidden layers produce y directly (exact scaling by 1/2)
   const float hs = (d->act == DSMC_ACT_SILU) ? 0.5f : 1.0f;
-  // image: [W1 H x 32 | W2hi H x H | B2 H x 16 | W3hi 16 x H | B3 16 x 16 | W2lo H x H | W3lo 16 x H]; every weight
-  // w is carried as bf16 hi + bf16 lo = w - hi; the plain BF16 engine stages only the part before W2lo.
+  // image: [W1 H x 32 | W2hi H x H | B2 H x 16 | Wout_hi 16 x H | Bout 16 x 16 | W2lo H x H | Wout_lo 16 x H |
+  //         (W_l hi H x H | B_l H x 16) for the hidden layers l = 3 .. nh]; every weight w of the first part is carried
+  // as bf16 hi + bf16 lo = w - hi; the plain BF16 engines stage only the part before W2lo (and the extra layers).
   const size_t n1 = (size_t)H * 32, n2 = (size_t)H * H, nb2 = (size_t)H * 16, n3 = (size_t)16 * H, nb3 = 256;
-  std::vector<uint16_t> blob(n1 + n2 + nb2 + n3 + nb3 + n2 + n3, 0);
+  const size_t n_main = n1 + n2 + nb2 + n3 + nb3 + n2 + n3;
+  std::vector<uint16_t> blob(n_main + (size_t)(nh - 2) * (n2 + nb2), 0);
   uint16_t *w1 = blob.data(), *w2h = w1 + n1, *b2 = w2h + n2, *w3h = b2 + nb2, *b3 = w3h + n3, *w2l = b3 + nb3,
            *w3l = w2l + n2;
   auto split = [](float w, uint16_t &hi, uint16_t &lo) {
     hi = bf16_rne(w);
     lo = bf16_rne(w - bf16_to_float(hi));
   };
-  for (int n = 0; n < H; ++n) {
+  const int h1 = d->dims[1], h2 = d->dims[2];
+  for (int n = 0; n < h1; ++n) {
     // layer 1 always in split precision: z = W_hi x_hi + W_hi x_lo + W_lo x_hi + (b_hi + b_lo);
     // operand columns [x_hi | x_lo | x_hi | 1 1 0 ...]
     for (int k = 0; k < d_in; ++k) {
@@ -63,12 +73,23 @@ int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStre
       w1[panel_off(n, 16 + k, H)] = lo;
     }
     split(hs * d->b[0][n], w1[panel_off(n, 24, H)], w1[panel_off(n, 25, H)]);
-    for (int k = 0; k < H; ++k) split(hs * d->W[1][(size_t)n * H + k], w2h[panel_off(n, k, H)], w2l[panel_off(n, k, H)]);
+  }
+  for (int n = 0; n < h2; ++n) {
+    for (int k = 0; k < h1; ++k) split(hs * d->W[1][(size_t)n * h1 + k], w2h[panel_off(n, k, H)], w2l[panel_off(n, k, H)]);
     split(hs * d->b[1][n], b2[panel_off(n, 0, H)], b2[panel_off(n, 1, H)]);
   }
+  for (int l = 3; l <= nh; ++l) {  // hidden layers beyond the second: plain BF16 weights, split bias
+    uint16_t *wl = blob.data() + n_main + (size_t)(l - 3) * (n2 + nb2), *bl = wl + n2;
+    const int win = d->dims[l - 1], wout = d->dims[l];
+    for (int n = 0; n < wout; ++n) {
+      for (int k = 0; k < win; ++k) wl[panel_off(n, k, H)] = bf16_rne(hs * d->W[l - 1][(size_t)n * win + k]);
+      split(hs * d->b[l - 1][n], bl[panel_off(n, 0, H)], bl[panel_off(n, 1, H)]);
+    }
+  }
+  const int hl = d->dims[nh];  // width of the last hidden layer
   for (int n = 0; n < d_out; ++n) {
-    for (int k = 0; k < H; ++k) split(d->W[2][(size_t)n * H + k], w3h[panel_off(n, k, 16)], w3l[panel_off(n, k, 16)]);
-    split(d->b[2][n], b3[panel_off(n, 0, 16)], b3[panel_off(n, 1, 16)]);
+    for (int k = 0; k < hl; ++k) split(d->W[nh][(size_t)n * hl + k], w3h[panel_off(n, k, 16)], w3l[panel_off(n, k, 16)]);
+    split(d->b[nh][n], b3[panel_off(n, 0, 16)], b3[panel_off(n, 1, 16)]);
   }
   const size_t bytes = blob.size() * sizeof(uint16_t);
   if (cudaMalloc(d_blob, bytes) != cudaSuccess) return DSMC_ERR_CUDA;
@@ -80,10 +101,12 @@ int build_tc_blob(const dsmc_mlp_desc *d, void **d_blob, MlpTcDev *out, cudaStre
   out->act = d->act;
   out->w_blob = *d_blob;
   out->blob_bytes = (uint32_t)bytes;
+  out->n_hidden = nh;
+  out->extra_off = (uint32_t)(n_main * sizeof(uint16_t));
   for (int k = 0; k < 129; ++k) out->w3_host[k] = 0.f;
   if (d_out == 1) {
-    for (int k = 0; k < H; ++k) out->w3_host[k] = d->W[2][k];
-    out->w3_host[128] = d->b[2][0];
+    for (int k = 0; k < hl; ++k) out->w3_host[k] = d->W[nh][k];
+    out->w3_host[128] = d->b[nh][0];
   }
   return DSMC_OK;
 }
@@ -337,23 +360,37 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
                    const MlpTcDev net, const TcOutLayer W3, float inv_bmax, float lnE_min, float inv_range) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   TcPipe<H> pipe;
-  float *zs = reinterpret_cast<float *>(smem_raw + PipeShape<H>::SMEM_BYTES);  // [2][2][4][128]
-  uint64_t *z_bar = reinterpret_cast<uint64_t *>(zs + 2 * 2 * 4 * 128);         // [2]
+  using SH = PipeShape<H>;
+  float *zs = reinterpret_cast<float *>(smem_raw + SH::SMEM_BYTES);      // [2][2][4][128]
+  uint64_t *z_bar = reinterpret_cast<uint64_t *>(zs + 2 * 2 * 4 * 128);  // [2], then the barrier of the extra layers
+  uint64_t *x_bar = z_bar + 2;
+  // hidden layers 3 .. n_hidden (W [H x H] | B [H x 16] each), behind everything else
+  unsigned char *extra = smem_raw + ((SH::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 32 + 127) & ~127);
+  const int n_extra = net.n_hidden - 2;
+  constexpr uint32_t kLayerBytes = SH::W2_BYTES + SH::B2_BYTES;
   if (threadIdx.x == 0) {
     tc::mbar_init(z_bar + 0, kPipeActWarps);
     tc::mbar_init(z_bar + 1, kPipeActWarps);
+    tc::mbar_init(x_bar, 1);
   }
   pipe.init(smem_raw, net.w_blob, kPipeActWarps, kPipeIoWarps);  // (fences the barrier inits, ends with CTA barriers)
+  if (threadIdx.x == 0 && n_extra > 0) {
+    tc::mbar_expect_tx(x_bar, (uint32_t)n_extra * kLayerBytes);
+    tc::bulk_g2s(extra, reinterpret_cast<const unsigned char *>(net.w_blob) + net.extra_off, (uint32_t)n_extra * kLayerBytes, x_bar);
+  }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n_tiles = (n + 127) / 128;
   const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
   const int64_t n_rounds = (mine + 1) / 2;  // two slots per round; a missing second tile runs as zeros
   if (warp < kPipeActWarps) {
     for (int64_t r = 0; r < n_rounds; ++r) {
-      pipe.act_tile(net.act, 0, warp);
-      pipe.act_tile(net.act, 1, warp);
 #pragma unroll 1
-      for (int s = 0; s < 2; ++s) {
+      for (int l = 1; l < net.n_hidden; ++l) {  // every hidden activation but the last: D -> act -> bf16 A operand
+        pipe.act_tile(net.act, 0, warp);
+        pipe.act_tile(net.act, 1, warp);
+      }
+#pragma unroll 1
+      for (int s = 0; s < 2; ++s) {  // the last one, with the output layer folded in
         float *zrow = zs + (size_t)((s * 2 + (int)(r & 1)) * 4) * 128;
         if (net.act == DSMC_ACT_SILU) chi_out_tile<H, DSMC_ACT_SILU>(pipe, s, warp, W3, zrow, z_bar + s);
         else if (net.act == DSMC_ACT_TANH) chi_out_tile<H, DSMC_ACT_TANH>(pipe, s, warp, W3, zrow, z_bar + s);
@@ -406,11 +443,21 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
       pipe.mma_layer1(0, 0, true);
       pipe.mma_layer1(1, 0, false);
     }
+    if (n_rounds > 0 && n_extra > 0) {
+      if (lane == 0) tc::mbar_wait(x_bar, 0);  // the extra layers have landed
+      __syncwarp();
+    }
     for (int64_t r = 0; r < n_rounds; ++r) {
       const bool more = r + 1 < n_rounds;
       const int par = (int)((r + 1) & 1);
       pipe.mma_layer2(0);
       pipe.mma_layer2(1);
+#pragma unroll 1
+      for (int l = 0; l < n_extra; ++l) {
+        const uint32_t wa = tc::smem_u32(extra) + (uint32_t)l * kLayerBytes;
+        pipe.mma_hidden_at(0, wa, wa + SH::W2_BYTES);
+        pipe.mma_hidden_at(1, wa, wa + SH::W2_BYTES);
+      }
 #pragma unroll 1
       for (int s = 0; s < 2; ++s) {
         tc::mbar_wait(pipe.a_ready + s, pipe.ph_a[s]);
@@ -427,7 +474,9 @@ static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const f
                                  float lnE_min, float lnE_max, const MlpTcDev *net) {
   const float inv_range = 1.0f / (lnE_max - lnE_min);
   const int grid = (int)std::min<int64_t>((n + 127) / 128, (int64_t)c->num_sms);
-  const int smem = PipeShape<H>::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 16 + 128;
+  const int smem = ((PipeShape<H>::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 32 + 127) & ~127) +
+                   (net->n_hidden - 2) * (PipeShape<H>::W2_BYTES + PipeShape<H>::B2_BYTES) + 128;
+  if (smem > 227 * 1024) return DSMC_ERR_UNSUPPORTED_SHAPE;
   auto kern = k_chi_batch_tc<H, RAW>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return DSMC_ERR_CUDA;
   kern<<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
@@ -680,7 +729,7 @@ static int launch_mlp_rows_tc_split_h(dsmc_ctx *c, int64_t n, const float *x, in
 // y[o][p] = MLP(x[0..d_in)[p])[o], o < 3, rows p < n; x: d_in arrays x + j x_stride; split-precision tensor-core path
 int launch_mlp_rows_tc_split(dsmc_ctx *c, int64_t n, const float *x, int64_t x_stride, float *y0, float *y1, float *y2,
                              const MlpTcDev *net, const TcTailF32 *tail) {
-  if (net->d_in < 1 || net->d_in > 8 || tail->d_out < 1 || tail->d_out > 3) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  if (net->d_in < 1 || net->d_in > 8 || tail->d_out < 1 || tail->d_out > 3 || net->n_hidden != 2) return DSMC_ERR_UNSUPPORTED_SHAPE;
   return net->H == 128 ? launch_mlp_rows_tc_split_h<128>(c, n, x, x_stride, y0, y1, y2, net, tail)
                        : launch_mlp_rows_tc_split_h<64>(c, n, x, x_stride, y0, y1, y2, net, tail);
 }
@@ -818,7 +867,8 @@ static int launch_tc_pair(dsmc_ctx *c, const StepParams &p, const MlpTcDev &net)
 }
 
 int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
-  if (p_in.op == 0 && !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  if (p_in.op == 0 && !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3 && net->n_hidden == 2)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+  if (p_in.op == 2 && (p_in.flags & DSMC_F_TC_ONE_KERNEL) && net->n_hidden != 2) return DSMC_ERR_UNSUPPORTED_SHAPE;
   if (p_in.op == 2 && !(net->d_in == 2 && net->d_out == 1)) return DSMC_ERR_UNSUPPORTED_SHAPE;
   // plain BF16 chi-MLP: three passes at full occupancy (dsmc_cells.cu), or, with DSMC_F_TC_ONE_KERNEL, the single kernel
   // of cell teams + MLP server (dsmc_cells_mlp.cu)

@@ -28,12 +28,15 @@ struct MlpDev {
   const float *b[7];
 };
 
-// BF16 tensor-core image of a 3-layer MLP (in<=16 -> H -> H -> out<=16), see dsmc_collide_tc.cu
+// BF16 tensor-core image of an MLP with 2..5 hidden layers of width <= H (in <= 8 -> H -> ... -> H -> out <= 16), see
+// dsmc_collide_tc.cu; more than two hidden layers: plain-BF16 batch path only (chi-MLP)
 struct MlpTcDev {
   int H;                      // 64 or 128, 0 = not available
   int d_in, d_out, act;
   const void *w_blob;         // bf16 weights and biases (hi + lo parts) in UMMA K-major core-matrix layout
   uint32_t blob_bytes;
+  int n_hidden;               // hidden layers (2..5); widths below H are zero-padded to H
+  uint32_t extra_off;         // byte offset in w_blob of the hidden layers 3..n_hidden: (W [H x H] | B [H x 16]) each, plain BF16
   float w3_host[129];         // HOST copy of the FP32 output layer when d_out = 1: w[0..H), bias at [128]
 };
 

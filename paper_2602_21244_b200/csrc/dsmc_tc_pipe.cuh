@@ -221,6 +221,22 @@ struct TcPipe {
     }
     __syncwarp();
   }
+  // a hidden layer whose weights [H x H] and bias block [H x 16] sit at the given shared-memory addresses
+  __device__ __forceinline__ void mma_hidden_at(int s, uint32_t w_addr, uint32_t b_addr) {
+    tc::mbar_wait(a_ready + s, ph_a[s]);
+    ph_a[s] ^= 1u;
+    if ((threadIdx.x & 31) == 0) {
+      tc::fence_after();
+      constexpr uint32_t idesc = tc::instr_desc(128, H);
+      const uint32_t tD = tmem + s * SH::SLOT_COLS + SH::COL_D, tA = tmem + s * SH::SLOT_COLS + SH::COL_A;
+#pragma unroll
+      for (int ks = 0; ks < H / 16; ++ks)
+        tc::mma_ts(tD, tA + ks * 8, tc::smem_desc(w_addr + ks * 2 * H * 16, H * 16, 128), idesc, ks > 0 ? 1u : 0u);
+      tc::mma_ts(tD, tmem + s * SH::SLOT_COLS + SH::COL_BIAS, tc::smem_desc(b_addr, H * 16, 128), idesc, 1u);
+      tc::mma_commit(full_e + s);
+    }
+    __syncwarp();
+  }
   __device__ __forceinline__ void mma_layer2(int s) {
     mma_hidden<H>(s, SH::OFF_W2, SH::OFF_B2, full_e + s, SH::COL_D, false);
   }

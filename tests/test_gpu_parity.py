@@ -167,7 +167,7 @@ def test_cell_moments_and_standalone_match(dsmc):
 # --------------------------------------------------------------------------------------- fused steps
 def _setup_vhs(dsmc, pop, H, seed_w, n_in=8, act=None):
     ctx = dsmc.Context(pop.n, pop.n_cells)
-    Ws, bs = wl.random_mlp(seed_w, [n_in, H, H, 3])
+    Ws, bs = wl.random_mlp(seed_w, [n_in, H, H, 3] if isinstance(H, int) else [n_in, H[0], H[1], 3])
     act = dsmc.ACT_TANH if act is None else act
     ctx.set_mlp(0, Ws, bs, act)
     return ctx, oracle.Mlp(Ws, bs, act)
@@ -477,9 +477,9 @@ def test_empty_inputs_and_unconfigured_operators(dsmc):
     assert e.value.status == dsmc.ERR_NOT_CONFIGURED
     with pytest.raises(dsmc.DsmcError):
         ctx.collide_vhs_nn(cs, v, v.clone(), v.clone(), dsmc.VhsParams(), 0, 0)
-    Ws, bs = wl.random_mlp(0, [8, 48, 48, 3])
+    Ws, bs = wl.random_mlp(0, [8, 200, 200, 3])
     ctx.set_mlp(0, Ws, bs, dsmc.ACT_TANH)
-    with pytest.raises(dsmc.DsmcError) as e:  # BF16 TC path supports H in {64,128} only
+    with pytest.raises(dsmc.DsmcError) as e:  # the BF16 TC paths take hidden widths up to 128 only
         ctx.collide_vhs_nn(cs, v, v.clone(), v.clone(), dsmc.VhsParams(flags=dsmc.F_BF16_TC), 0, 0)
     assert e.value.status == dsmc.ERR_UNSUPPORTED_SHAPE
 
@@ -489,23 +489,30 @@ def _quantiles(x):
     return "median %.2e, 99%% %.2e, 99.9%% %.2e, max %.2e" % tuple(np.quantile(x, [0.5, 0.99, 0.999, 1.0]))
 
 
-@pytest.mark.parametrize("H,act", [(128, "silu"), (64, "silu"), (128, "tanh"), (64, "relu")])
+_DEEP = {"paper5": [2, 128, 96, 64, 48, 32, 1],   # five hidden layers, decreasing width, SiLU
+         "deep4": [2, 64, 64, 48, 16, 1], "three": [2, 128, 128, 100, 1], "narrow": [2, 40, 24, 1]}
+
+
+@pytest.mark.parametrize("H,act", [(128, "silu"), (64, "silu"), (128, "tanh"), (64, "relu"), ("paper5", "silu"),
+                                   ("deep4", "tanh"), ("three", "relu"), ("narrow", "silu")])
 def test_chi_batch_bf16_tc(dsmc, H, act):
-    """a10 on the tensor cores; tolerance Q26: abs(dchi) <= 2e-2 (1 + abs(chi))."""
+    """a10 on the tensor cores; tolerance Q26: abs(dchi) <= 2e-2 (1 + abs(chi)).  Shapes: the BASELINE 2-H-H-1 and
+    networks with up to five hidden layers of unequal widths <= 128 (zero-padded on the device), among them the
+    paper's chi-MLP shape."""
     n = 300_017  # 2343 full tiles + a ragged tail of 113 pairs
     E, b = wl.abinitio_pair_batch(seed=3, n=n)
     E[:4] = [1.0, 1e6, 5.0, 6e4]
     a_g = {"silu": dsmc.ACT_SILU, "tanh": dsmc.ACT_TANH, "relu": dsmc.ACT_RELU}[act]
     a_o = {"silu": oracle.ACT_SILU, "tanh": oracle.ACT_TANH, "relu": oracle.ACT_RELU}[act]
     ctx = dsmc.Context(n, 1)
-    Ws, bs = wl.random_mlp(3, [2, H, H, 1])
+    Ws, bs = wl.random_mlp(3, _DEEP[H] if isinstance(H, str) else [2, H, H, 1])
     ctx.set_mlp(1, Ws, bs, a_g)
     got = ctx.chi_batch(dev(E), dev(b), 1, 1e-9, flags=dsmc.F_BF16_TC).cpu().numpy().astype(np.float64)
     ctx.check()
     lo, hi = float(np.float32(np.log(5.0))), float(np.float32(np.log(6.0e4)))
     want = oracle.chi_batch(E, b, 1, 1e-9, net=oracle.Mlp(Ws, bs, a_o), lnE_min=lo, lnE_max=hi)
     rel = np.abs(got - want) / (1 + np.abs(want))
-    print("chi bf16 H=%d %s: %s" % (H, act, _quantiles(rel)))
+    print("chi bf16 H=%s %s: %s" % (H, act, _quantiles(rel)))
     assert rel.max() <= 2e-2
     ctx.close()
 
@@ -547,6 +554,44 @@ def test_collide_abinitio_bf16_tc(dsmc, one_kernel):
     ctx.close()
 
 
+def test_collide_abinitio_bf16_tc_paper_shape(dsmc):
+    """The fused chi-MLP step on the tensor cores with the paper's chi-MLP shape (five hidden layers of decreasing width,
+    SiLU): pairs bit-exact, chi within Q26 on every pair, moments; with-replacement selection too; the
+    one-kernel form has no image for this shape and says so."""
+    pop = wl.mach10_cylinder(nx=40, ny=20, n_total=120_000)
+    ctx = dsmc.Context(pop.n, pop.n_cells)
+    Ws, bs = wl.random_mlp(7, _DEEP["paper5"])
+    Ws = [w * np.float32(2.5) for w in Ws]  # (a random-init deep network is nearly constant: raise the gain of every layer)
+    ctx.set_mlp(1, Ws, bs, dsmc.ACT_SILU)
+    net = oracle.Mlp(Ws, bs, oracle.ACT_SILU)
+    vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
+    cs_h = cs.cpu().numpy()
+    for step, extra in enumerate((0, dsmc.F_PAIR_REPLACE)):
+        prm = dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_MOMENT_MATCH | dsmc.F_BF16_TC | extra)
+        oprm = oracle.AbinitioParams(chi_mode=1, flags=oracle.F_MOMENT_MATCH | (oracle.F_PAIR_REPLACE if extra else 0),
+                                     lnE_min=float(np.float32(prm.lnE_min)), lnE_max=float(np.float32(prm.lnE_max)))
+        v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
+        dump = dsmc.PairDump(pop.n, "cuda")
+        ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, prm, seed=5, step=step, dump=dump)
+        ctx.check()
+        ref = oracle.collide_abinitio(cs_h, *v_in, oprm, 5, step, net=net)
+        sel = ref.pair_i >= 0
+        chi_g = dump.aux.cpu().numpy().astype(np.float64)
+        assert (np.abs(chi_g[sel] - ref.aux[sel]) / (1 + np.abs(ref.aux[sel]))).max() <= 2e-2  # Q26
+        assert np.ptp(ref.aux[sel]) > 0.05
+        _compare_step(dsmc, ctx, cs, v_in, (vx_s, vy_s, vz_s), dump, ref, 1e-5, 1e-6, slope=1.01 * np.abs(chi_g - ref.aux))
+        N = np.diff(cs_h)
+        pre = oracle.cell_moments(cs_h, *v_in)
+        got = ctx.cell_moments(cs, vx_s, vy_s, vz_s).cpu().numpy()
+        ok = N >= 2
+        assert np.abs(got[ok, 3] / pre[ok, 3] - 1).max() < 1e-6
+        assert (np.linalg.norm(got[ok, :3] - pre[ok, :3], axis=1) / (N[ok] * np.sqrt(pre[ok, 3] / N[ok]))).max() < 1e-6
+    with pytest.raises(dsmc.DsmcError) as e:
+        ctx.collide_abinitio(cs, vx_s, vy_s, vz_s, dsmc.AbinitioParams(chi_mode=1, flags=dsmc.F_BF16_TC | dsmc.F_TC_ONE_KERNEL), seed=5, step=9)
+    assert e.value.status == dsmc.ERR_UNSUPPORTED_SHAPE
+    ctx.close()
+
+
 @pytest.mark.parametrize("one_kernel", [False, True])
 def test_collide_abinitio_bf16_tc_few_cells_and_ragged(dsmc, one_kernel):
     """Both tensor-core forms on contexts whose radix sort needs a single pass (<= 512 cells: the split form's pair
@@ -582,7 +627,7 @@ def test_collide_abinitio_bf16_tc_few_cells_and_ragged(dsmc, one_kernel):
 
 
 @pytest.mark.parametrize("one_kernel", [False, True])
-@pytest.mark.parametrize("case", ["cfg1_tiny", "cfg3_cavity_small", "ragged6"])
+@pytest.mark.parametrize("case", ["cfg1_tiny", "cfg3_cavity_small", "ragged6", "narrow"])
 def test_collide_vhs_nn_bf16_tc(dsmc, case, one_kernel):
     """BF16 tensor-core VHS-NN, both forms (default: three passes around a persistent split-precision batch kernel;
     F_TC_ONE_KERNEL: the chunk kernel with its own engine): bit-exact pairing, 2e-2 per pair on the gated set (Q21),
@@ -592,6 +637,8 @@ def test_collide_vhs_nn_bf16_tc(dsmc, case, one_kernel):
         pop, H, ppc, sw = wl.tiny_box(), 64, 50, 0
     elif case == "cfg3_cavity_small":
         pop, H, ppc, sw = wl.cavity(nx=20, ny=20), 128, 50, 2
+    elif case == "narrow":  # unequal hidden widths below 64 / 128: zero-padded on the device
+        pop, H, ppc, sw = wl.cavity(nx=12, ny=12), (100, 72), 50, 4
     else:
         rng = np.random.default_rng(3)
         counts = rng.integers(0, 30, 400)
