@@ -354,7 +354,8 @@ __device__ __forceinline__ void chi_out_tile(TcPipe<H> &pipe, int s, int act_war
 }
 
 // RAW: E, b already hold the network inputs (x0, x1) of every row (the split fused step, dsmc_cells.cu)
-template <int H, bool RAW>
+// DEEP: more than two hidden layers (run-time count); otherwise the layer loops fold away
+template <int H, bool RAW, bool DEEP>
 __global__ void __launch_bounds__(kPipeThreads, 1)
     k_chi_batch_tc(int64_t n, const float *__restrict__ E, const float *__restrict__ b, float *__restrict__ chi,
                    const MlpTcDev net, const TcOutLayer W3, float inv_bmax, float lnE_min, float inv_range) {
@@ -366,7 +367,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
   uint64_t *x_bar = z_bar + 2;
   // hidden layers 3 .. n_hidden (W [H x H] | B [H x 16] each), behind everything else
   unsigned char *extra = smem_raw + ((SH::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 32 + 127) & ~127);
-  const int n_extra = net.n_hidden - 2;
+  const int n_hidden = DEEP ? net.n_hidden : 2, n_extra = n_hidden - 2;
   constexpr uint32_t kLayerBytes = SH::W2_BYTES + SH::B2_BYTES;
   if (threadIdx.x == 0) {
     tc::mbar_init(z_bar + 0, kPipeActWarps);
@@ -385,7 +386,7 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
   if (warp < kPipeActWarps) {
     for (int64_t r = 0; r < n_rounds; ++r) {
 #pragma unroll 1
-      for (int l = 1; l < net.n_hidden; ++l) {  // every hidden activation but the last: D -> act -> bf16 A operand
+      for (int l = 1; l < n_hidden; ++l) {  // every hidden activation but the last: D -> act -> bf16 A operand
         pipe.act_tile(net.act, 0, warp);
         pipe.act_tile(net.act, 1, warp);
       }
@@ -477,7 +478,7 @@ static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const f
   const int smem = ((PipeShape<H>::SMEM_BYTES + 2 * 2 * 4 * 128 * 4 + 32 + 127) & ~127) +
                    (net->n_hidden - 2) * (PipeShape<H>::W2_BYTES + PipeShape<H>::B2_BYTES) + 128;
   if (smem > 227 * 1024) return DSMC_ERR_UNSUPPORTED_SHAPE;
-  auto kern = k_chi_batch_tc<H, RAW>;
+  auto kern = net->n_hidden > 2 ? k_chi_batch_tc<H, RAW, true> : k_chi_batch_tc<H, RAW, false>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return DSMC_ERR_CUDA;
   kern<<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
   c->launches += 1;
