@@ -150,9 +150,8 @@ enum {
                                    + (j >= i) from Philox stream 4; every pair of a cell is evaluated on the
                                    pre-collision velocities (one batch) and the velocity changes of a
                                    particle that appears in several pairs add up.  Momentum is conserved exactly,
-                                   energy is restored by DSMC_F_MOMENT_MATCH.  Both operators on the FP32 / table
-                                   paths; with DSMC_F_BF16_TC for the ab initio chi-MLP (dsmc_collide_abinitio), not
-                                   for the VHS-NN operator.  No key sort: the cheapest selection. */
+                                   energy is restored by DSMC_F_MOMENT_MATCH.  Both operators, on the FP32 / table
+                                   paths and with DSMC_F_BF16_TC.  No key sort: the cheapest selection. */
   DSMC_F_TC_ONE_KERNEL = 256    /* with DSMC_F_BF16_TC: run the fused step as ONE kernel (chi-MLP: cell teams + a tcgen05
                                    MLP server sharing every SM; VHS-NN: chunks with a per-CTA engine) instead of the
                                    default three passes (pairing + network inputs | MLP batch on the tensor cores |

@@ -376,7 +376,7 @@ int dsmc_collide_vhs_nn(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cs, fl
   }
   CK(cudaSetDevice(c->device));
   if (prm->flags & DSMC_F_BF16_TC) {
-    if (c->mlp_tc[0].H == 0 || (prm->flags & DSMC_F_PAIR_REPLACE)) return DSMC_ERR_UNSUPPORTED_SHAPE;
+    if (c->mlp_tc[0].H == 0) return DSMC_ERR_UNSUPPORTED_SHAPE;
     return launch_collide_tc(c, p, &c->mlp_tc[0]);
   }
   return launch_collide(c, p, &c->mlp[0]);

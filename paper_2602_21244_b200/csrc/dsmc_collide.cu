@@ -270,6 +270,138 @@ int launch_chunk_map(dsmc_ctx *c, StepParams &p) {
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
 
+// ---------------------------------------------------------------------------------------------
+// VHS-NN operator on the tensor cores with pairs drawn WITH replacement (DSMC_F_PAIR_REPLACE | DSMC_F_BF16_TC): the
+// split form on the with-replacement chunk machinery.  Pass 1: draw the pairs, network inputs of every pair (eqs. 1-3)
+// -> pair arrays.  Pass 2: k_mlp_rows_tc_split (dsmc_collide_tc.cu).  Pass 3: draw the same pairs again, outputs ->
+// eq. 5 -> changes added up per particle (batch semantics, Q29), moment matching, store.  (Without replacement the
+// split form runs on the cell-team kernels, dsmc_cells.cu.)
+// ---------------------------------------------------------------------------------------------
+template <class TM, class CK>
+__device__ __forceinline__ void pairs_vhs_split(const TM &T, const StepParams &P, CK &S, int q0) {
+  const int n_pairs = S.misc[MI_NPAIRS];
+  const int stage = P.split_stage, d_in = P.split_din;
+  const int64_t np = P.split_np;
+  for (int t = T.tid; t < n_pairs; t += TM::kN) {
+    PairCtx c = pair_setup(P, S, t, false);
+    const int64_t pidx = ((int64_t)(q0 + c.start) >> 1) + c.s;
+    if (stage == 3) {  // VHS-NN features (eqs. 1-3, Q1-Q3)
+      float x[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      float n0 = 0.f, n1 = 0.f, n2 = 0.f;
+      if (P.flags & DSMC_F_NOISE) {
+        const uint4 r = philox4x32_10((uint32_t)c.s, c.cell + P.cell_base, P.step, 2u, P.seed_lo, P.seed_hi);
+        box_muller3(r, n0, n1, n2);
+        n0 *= P.noise_sigma; n1 *= P.noise_sigma; n2 *= P.noise_sigma;
+      }
+      x[0] = c.gx * P.inv_sigma_v; x[1] = c.gy * P.inv_sigma_v; x[2] = c.gz * P.inv_sigma_v;
+      if (d_in == 8) {
+        const CellInfo &ci = S.cells[c.a];
+        x[3] = sqrtf(c.g2) * P.inv_sigma_v;
+        x[4] = ci.theta * P.T_coef / (float)ci.N * P.inv_T_scale;  // T = m Theta / (3 kB N)
+        x[5] = n0; x[6] = n1; x[7] = n2;
+      } else {
+        x[3] = n0; x[4] = n1; x[5] = n2;
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        if (k < d_in) P.feat0[k * np + pidx] = x[k];
+      continue;
+    }
+    float px = c.gx, py = c.gy, pz = c.gz, aux = 0.f;
+    if (c.acc) {
+      const float hx = __ldg(P.out3[0] + pidx), hy = __ldg(P.out3[1] + pidx), hz = __ldg(P.out3[2] + pidx);
+      const float hn = sqrtf(hx * hx + hy * hy + hz * hz);
+      aux = hn;
+      if (P.flags & DSMC_F_ENERGY_SHELL) {
+        if (hn >= P.shell_eps) {  // eq. 5 with the guard of Q4
+          const float sc = sqrtf(c.g2) / hn;
+          px = sc * hx; py = sc * hy; pz = sc * hz;
+        }
+      } else {
+        px = P.sigma_v * hx; py = P.sigma_v * hy; pz = P.sigma_v * hz;
+      }
+    }
+    pair_commit(P, S, c, px, py, pz, aux, q0);
+  }
+}
+
+template <int LMAX, int AMAX, int SRC, int DST, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) k_vhs_replace_split(const StepParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  using CK = Chunk<LMAX, AMAX, true, false>;
+  CK S;
+  S.carve(smem_raw);
+  const TeamT<kThreads> T{(int)threadIdx.x, 0};
+  auto one = [&](int chunk) {
+    int q0 = 0;
+    const int n_loc = chunk_begin(T, P, S, chunk, q0);
+    if (n_loc == 0) return;
+    if (n_loc < 0) {
+      if (threadIdx.x == 0) {
+        if (DST == 0) {
+          *P.status = DSMC_ERR_CELL_TOO_LARGE;
+        } else {
+          const int i = atomicAdd(P.big, 1);
+          P.big[1 + i] = chunk;
+        }
+      }
+      return;
+    }
+    chunk_pre_and_sort(T, P, S, n_loc);
+    pairs_vhs_split(T, P, S, q0);
+    if (P.split_stage == 3) return;
+    T.sync();
+    chunk_finish(T, P, S, n_loc, q0);
+  };
+  if (SRC == 0) {
+    one(blockIdx.x);
+  } else {
+    const int n_list = *reinterpret_cast<volatile const int32_t *>(P.big);
+    for (int i = blockIdx.x; i < n_list; i += gridDim.x) {
+      one(P.big[1 + i]);
+      __syncthreads();
+    }
+  }
+}
+
+template <int LMAX, int AMAX, int SRC, int DST, int MINB>
+static int launch_vhs_replace_split_one(dsmc_ctx *c, const StepParams &p, int grid) {
+  auto kern = k_vhs_replace_split<LMAX, AMAX, SRC, DST, MINB>;
+  const size_t smem = Chunk<LMAX, AMAX>::bytes();
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return DSMC_ERR_CUDA;
+  kern<<<grid, kThreads, smem, c->stream>>>(p);
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
+}
+
+int launch_collide_vhs_replace_split(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) {
+  const TcTailF32 *tail = &c->tc_tail[0];
+  if (p_in.op != 0 || !((net->d_in == 8 || net->d_in == 6) && net->d_out == 3) || tail->d_out != 3)
+    return DSMC_ERR_UNSUPPORTED_SHAPE;
+  StepParams p = p_in;
+  const int64_t np = (p.n / 2 + 4) & ~(int64_t)3;
+  p.feat0 = reinterpret_cast<float *>(c->d_bin_rec[0]);  // 8 arrays of np floats: 16 B / particle + 128 B
+  p.split_np = np;
+  p.split_din = net->d_in;
+  p.out3[0] = reinterpret_cast<float *>(c->d_bin_cell[0]);
+  p.out3[1] = p.out3[0] + np;
+  p.out3[2] = reinterpret_cast<float *>(c->d_bin_cell[1]);
+  for (int stage = 3; stage <= 4; ++stage) {
+    int rc = launch_chunk_map(c, p);  // (also resets the deferred-chunk list)
+    if (rc != DSMC_OK) return rc;
+    p.split_stage = stage;
+    rc = launch_vhs_replace_split_one<kLmaxSmall, kAmaxSmall, 0, 1, 3>(c, p, p.n_chunks);
+    if (rc != DSMC_OK) return rc;
+    rc = launch_vhs_replace_split_one<kLmaxBig, kAmaxBig, 1, 0, 1>(c, p, c->num_sms);
+    if (rc != DSMC_OK) return rc;
+    if (stage == 3) {
+      rc = launch_mlp_rows_tc_split(c, p.n / 2 + 1, p.feat0, np, p.out3[0], p.out3[1], p.out3[2], net, tail);
+      if (rc != DSMC_OK) return rc;
+    }
+  }
+  return DSMC_OK;
+}
+
 // chi-MLP on the tensor cores with pairs drawn WITH replacement (DSMC_F_PAIR_REPLACE | DSMC_F_BF16_TC): the split form
 // of dsmc_cells.cu on the with-replacement chunk kernels.  Pass 1 draws the pairs and writes the two network inputs of
 // every pair, pass 2 is k_chi_batch_tc on those arrays, pass 3 draws the same pairs again (counter-based randoms),

@@ -877,7 +877,8 @@ int launch_collide_tc(dsmc_ctx *c, const StepParams &p_in, const MlpTcDev *net) 
   if (p_in.op == 2)
     return (p_in.flags & DSMC_F_TC_ONE_KERNEL) ? launch_collide_cells_mlp(c, p_in, net) : launch_collide_cells_split(c, p_in, net);
   // VHS-NN: the split form (dsmc_collide.cu) unless the one-kernel form is asked for
-  if (p_in.op == 0 && !(p_in.flags & (DSMC_F_TC_ONE_KERNEL | DSMC_F_PAIR_REPLACE))) return launch_collide_cells_vhs_split(c, p_in, net);
+  if (p_in.op == 0 && (p_in.flags & DSMC_F_PAIR_REPLACE)) return launch_collide_vhs_replace_split(c, p_in, net);
+  if (p_in.op == 0 && !(p_in.flags & DSMC_F_TC_ONE_KERNEL)) return launch_collide_cells_vhs_split(c, p_in, net);
   StepParams p = p_in;
   int rc = launch_chunk_map(c, p);
   if (rc != DSMC_OK) return rc;

@@ -168,6 +168,7 @@ int launch_collide_cells_mlp(dsmc_ctx *c, const StepParams &p, const MlpTcDev *n
 int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);
 int launch_collide_replace_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // dsmc_collide.cu
 int launch_collide_cells_vhs_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // dsmc_cells.cu
+int launch_collide_vhs_replace_split(dsmc_ctx *c, const StepParams &p, const MlpTcDev *net);  // dsmc_collide.cu
 int launch_chi_rows_tc(dsmc_ctx *c, int64_t n, const float *x0, const float *x1, float *chi, const MlpTcDev *net);
 int launch_mlp_rows_tc_split(dsmc_ctx *c, int64_t n, const float *x, int64_t x_stride, float *y0, float *y1, float *y2,
                              const MlpTcDev *net, const TcTailF32 *tail);  // chi-MLP on tcgen05 (dsmc_cells_mlp.cu)  // cell-team form, chi-table operator (dsmc_cells.cu)

@@ -914,16 +914,17 @@ def test_collide_abinitio_with_replacement(dsmc, mode, match):
     ctx.close()
 
 
-def test_collide_vhs_nn_with_replacement(dsmc):
+@pytest.mark.parametrize("tc", [False, True])
+def test_collide_vhs_nn_with_replacement(dsmc, tc):
     """SURVEY 8(f1) for the VHS-surrogate operator with NTC acceptance: pairs drawn with replacement, batch
-    semantics.  Pair indices and acceptance bit-exact, g' to the FP32 tolerance on the gated set (Q21), velocities
-    to 1e-4 of the thermal scale, conserved moments to 1e-6."""
+    semantics.  Pair indices and acceptance bit-exact, g' to the FP32 tolerance on the gated set (Q21; tensor cores:
+    2e-2), velocities to 1e-4 of the thermal scale, conserved moments to 1e-6."""
     pop = wl.cavity(nx=16, ny=16)
     ctx, net = _setup_vhs(dsmc, pop, 64, 5)
     vx_s, vy_s, vz_s, perm, cs = binned(dsmc, ctx, pop)
     cs_h = cs.cpu().numpy()
     flags = dsmc.F_NOISE | dsmc.F_ENERGY_SHELL | dsmc.F_MOMENT_MATCH | dsmc.F_ACCEPT | dsmc.F_PAIR_REPLACE
-    prm = dsmc.VhsParams(sigma_v=wl.SIGMA_V, flags=flags)
+    prm = dsmc.VhsParams(sigma_v=wl.SIGMA_V, flags=flags | (dsmc.F_BF16_TC if tc else 0))
     oprm = oracle.VhsParams(sigma_v=float(np.float32(wl.SIGMA_V)), flags=flags)
     cap = np.full(pop.n_cells, oracle.vhs_sigma_g(6 * wl.SIGMA_V, oprm), np.float32)
     v_in = [t.cpu().numpy().astype(np.float64) for t in (vx_s, vy_s, vz_s)]
@@ -949,11 +950,11 @@ def test_collide_vhs_nn_with_replacement(dsmc):
         k = np.searchsorted(cs_h, idx, side="right") - 1
         g = np.stack([a[cs_h[k] + ref.pair_i[idx]] - a[cs_h[k] + ref.pair_j[idx]] for a in v_in], axis=1)
         err = np.linalg.norm(dump.gprime.cpu().numpy()[idx].astype(np.float64) - ref.gprime[idx], axis=1) / np.linalg.norm(g, axis=1)
-        _note("pair |dg'|/g", err.max(), 1e-5)
-        assert err.max() < 1e-5
+        _note("pair |dg'|/g", err.max(), 2e-2 if tc else 1e-5)
+        assert err.max() < (2e-2 if tc else 1e-5)
         scale = np.repeat(np.sqrt(np.maximum(pre[:, 3], 1e-30) / np.maximum(N, 1)), N)
         for a, want in zip((vx_s, vy_s, vz_s), (ref.vx, ref.vy, ref.vz)):
-            assert np.median(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale) < 1e-5
+            assert np.median(np.abs(a.cpu().numpy().astype(np.float64) - want) / scale) < (1e-3 if tc else 1e-5)
     multi = np.bincount(np.r_[ref.pair_i[sel] + cs_h[k_all(cs_h, sel)], ref.pair_j[sel] + cs_h[k_all(cs_h, sel)]], minlength=pop.n)
     assert (multi >= 2).mean() > 0.15                         # particles drawn into several pairs of one batch
     ctx.close()
