@@ -33,12 +33,6 @@
 
 namespace dsmc {
 
-#ifdef CM_TRACE
-// per-warp trace region, plain stores (no atomics: a stamp must not stall the warp)
-#define CM_STAMP(tag) do { if (blockIdx.x == 0 && lane == 0 && P.cap && cm_n < 900) { long long *tb = (long long *)P.cap; tb[1 + cm_region * 900 + cm_n++] = ((long long)(tag) << 40) | (clock64() & 0xFFFFFFFFFFll); } } while (0)
-#else
-#define CM_STAMP(tag) do { } while (0)
-#endif
 
 constexpr int kMlpMaxFeeders = 32;
 
@@ -172,10 +166,6 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
   }
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#ifdef CM_TRACE
-  int cm_n = 0;
-  const int cm_region = warp >= NTW + NA ? 2 + (warp - NTW - NA) : ((warp - NTW) >> 2) & 1;  // ACT leaders 0/1, MMA 2/3
-#endif
   // the team warps come first (NTW is a multiple of 4): activation warp aw reads the tensor-memory lanes
   // 32 (aw & 3) .., which the hardware ties to (warp index & 3); and the scheduler prefers the higher warp indices,
   // which keeps the server ahead of the teams that feed it
@@ -236,7 +226,6 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
       // ---- hidden layer 1: D -> activation -> bf16 A operand of layer 2 (tensor memory) ----
       tc::mbar_wait(pipe.full_e + s2, phe);
       phe ^= 1u;
-      if (aw_slot == 0) CM_STAMP(10 + 10 * s2);
       if (k == cm_ld_volatile(&ctl->stop_k[s2])) goto server_done;
       if (aw_slot == 0 && lane == 0) {  // the slot's layer-1 operand buffer may be rewritten
         *reinterpret_cast<volatile int *>(&ctl->op_done[s2]) = k + 1;
@@ -245,13 +234,11 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
       }
       __syncwarp();
       pipe.template act_body<NQ>(net.act, s2, aw_slot);
-      if (aw_slot == 0) CM_STAMP(11 + 10 * s2);
       // ---- hidden layer 2 and the output layer (d_out = 1) in one pass: z = b3 + sum_j w3[j] act(D[row][j]) on the
       // CUDA cores, so no third tensor-core layer and no hand-off for it; the two column groups of a row add their
       // partial sums into the feeding warp's (zeroed) buffer: x + y = y + x, the result does not depend on the order
       tc::mbar_wait(pipe.full_e + s2, phe);
       phe ^= 1u;
-      if (aw_slot == 0) CM_STAMP(12 + 10 * s2);
       float *dest = *reinterpret_cast<float *volatile *>(&ctl->dest[s2][k & 3]);
       const int f = cm_ld_volatile(&ctl->feeder[s2][k & 3]);
       {
@@ -268,7 +255,6 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
         asm volatile("red.shared.add.f32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(dest + q * 32 + lane)), "f"(part)
                      : "memory");
       }
-      if (aw_slot == 0) CM_STAMP(13 + 10 * s2);
       __syncwarp();
       if (lane == 0) {
         __threadfence_block();
@@ -286,7 +272,6 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
       uint64_t *bar = &ctl->in_bar[s2][k & 1];
       const uint32_t par = (uint32_t)(k >> 1) & 1u;
       bool stop = false;
-      CM_STAMP(33 + 10 * s2);
       for (;;) {
         if (cm_try_wait_ns(bar, par, 2000u)) break;
         int st = 0;
@@ -309,11 +294,9 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
         pipe.issue_layer1(s2, k & 1, k == 0);  // an empty one: it wakes the slot's activation warps, which then stop
         break;
       }
-      CM_STAMP(30 + 10 * s2);
       pipe.issue_layer1(s2, k & 1, k == 0);
       tc::mbar_wait(pipe.a_ready + s2, pa);
       pa ^= 1u;
-      CM_STAMP(31 + 10 * s2);
       pipe.issue_layer2(s2);
       tc::mbar_wait(pipe.a_ready + s2, pa);  // the second activation has read D: the next tile's layer 1 may go
       pa ^= 1u;
