@@ -369,7 +369,7 @@ def run_b200(args):
     hv = [torch.from_numpy(a).pin_memory() for a in (pop.vx, pop.vy, pop.vz)]
     hout = [torch.empty(pop.n, dtype=torch.float32).pin_memory() for _ in range(3)] + \
            [torch.empty(pop.n, dtype=torch.int32).pin_memory(), torch.empty(pop.n_cells + 1, dtype=torch.int32).pin_memory()]
-    e2e_steps = max(4, min(args.steps, 10))
+    e2e_steps = max(6, min(args.steps, 12))
     for t in range(2):
         ctx.step_host(hcell, *hv, pop.n_cells, hout, abi=params(args.chi), seed=4, step=t)
     if world > 1:
@@ -380,31 +380,37 @@ def run_b200(args):
         ctx.step_host(hcell, *hv, pop.n_cells, hout, abi=params(args.chi), seed=4, step=10 + t)
     torch.cuda.synchronize()
     e2e_sync_s = (time.perf_counter() - t0) / e2e_steps
-    # the same through two contexts on two streams fed alternately (dsmc_step_host_submit / dsmc_sync_status): every
-    # step still copies its inputs in and its results out, but the H2D of one batch runs under the D2H of the previous
-    ctx2 = dsmc.Context(pop.n, pop.n_cells, device=local)
-    ctx2.build_chi_table_lj(TABLE_N, TABLE_N, b_max=B_MAX)
-    ctx2.set_mlp(1, mlp_w[0], mlp_w[1], dsmc.ACT_SILU)
-    hout2 = [torch.empty_like(t).pin_memory() for t in hout]
-    lanes = [(ctx, torch.cuda.Stream(device=dev), hout), (ctx2, torch.cuda.Stream(device=dev), hout2)]
+    # the same through three contexts on three streams fed in turn (dsmc_step_host_submit / dsmc_sync_status): every
+    # step still copies its inputs in and its results out, but the H2D of one batch runs under the D2H of an earlier one
+    # and under the kernels of another (two lanes leave the link idle while a lane computes)
+    N_LANES = 3
+    extra_ctx = []
+    lanes = [(ctx, torch.cuda.Stream(device=dev), hout)]
+    for _ in range(N_LANES - 1):
+        cx = dsmc.Context(pop.n, pop.n_cells, device=local)
+        cx.build_chi_table_lj(TABLE_N, TABLE_N, b_max=B_MAX)
+        cx.set_mlp(1, mlp_w[0], mlp_w[1], dsmc.ACT_SILU)
+        extra_ctx.append(cx)
+        lanes.append((cx, torch.cuda.Stream(device=dev), [torch.empty_like(t).pin_memory() for t in hout]))
     torch.cuda.synchronize()
 
     def pipelined(first, count):
-        busy = [False, False]
+        busy = [False] * N_LANES
         for t in range(count):
-            c, st, ho = lanes[t & 1]
-            if busy[t & 1]:
+            k = t % N_LANES
+            c, st, ho = lanes[k]
+            if busy[k]:
                 with torch.cuda.stream(st):
                     c.check()
             with torch.cuda.stream(st):
                 c.step_host(hcell, *hv, pop.n_cells, ho, abi=params(args.chi), seed=4, step=first + t, submit_only=True)
-            busy[t & 1] = True
-        for k in (0, 1):
+            busy[k] = True
+        for k in range(N_LANES):
             if busy[k]:
                 with torch.cuda.stream(lanes[k][1]):
                     lanes[k][0].check()
 
-    pipelined(100, 2)
+    pipelined(100, N_LANES)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -412,7 +418,8 @@ def run_b200(args):
     pipelined(110, e2e_steps)
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    ctx2.close()
+    for cx in extra_ctx:
+        cx.close()
     if world > 1:
         tt = torch.tensor([e2e_s, e2e_sync_s], device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -612,7 +619,7 @@ def run_b200(args):
             "config": config_dict(args, pop, pairs), "clocks": sampler.summary(),
             "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3,
-                    "api": "dsmc_step_host_submit + dsmc_sync_status, two contexts on two streams fed alternately "
+                    "api": "dsmc_step_host_submit + dsmc_sync_status, three contexts on three streams fed in turn "
                            "(pinned host buffers; every step copies its inputs in and its results out)",
                     "single_context_sync": {"value": world * pairs / e2e_sync_s, "ms_per_step": e2e_sync_s * 1e3,
                                             "api": "dsmc_step_host"}},
