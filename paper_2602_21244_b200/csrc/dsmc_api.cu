@@ -57,6 +57,9 @@ static int create_impl(dsmc_ctx *c, int device, int64_t max_particles, int32_t m
     CK(cudaMalloc(&c->d_bin_hist, sizeof(int32_t) * tiles * kBinMaxRadix));
     CK(cudaMalloc(&c->d_bin_group, sizeof(int32_t) * (size_t)c->num_sms * kBinMaxRadix));
     CK(cudaMalloc(&c->d_cell_count, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) + 1)));
+    // both are kept zero between calls by the kernels that consume them (no memsets inside dsmc_bin)
+    CK(cudaMemset(c->d_bin_group, 0, sizeof(int32_t) * (size_t)c->num_sms * kBinMaxRadix));
+    CK(cudaMemset(c->d_cell_count, 0, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) + 1)));
     CK(cudaMalloc(&c->d_cell_tile_sums, sizeof(int32_t) * ((size_t)(max_cells > 0 ? max_cells : 1) / 4096 + 2)));
     for (int i = 0; i < 2; ++i) {
       CK(cudaMalloc(&c->d_bin_cell[i], sizeof(int32_t) * (np + 16)));  // (+ slack: the VHS-NN split form keeps its outputs here)

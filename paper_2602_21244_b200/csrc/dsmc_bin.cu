@@ -199,7 +199,8 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 template <bool FIRST, bool LAST>
 __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t K, BinPass ps, BinIo io,
-                                                              const int32_t *__restrict__ hist) {
+                                                              const int32_t *__restrict__ hist,
+                                                              int32_t *__restrict__ group, int group_rows) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   // staging (unsorted, tile order): cell ids, then (FIRST) vx | vy | vz, else records
   int32_t *scell = reinterpret_cast<int32_t *>(smem_raw);                 // [tile]
@@ -245,6 +246,9 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
       bulk_g2s(srec, io.rec_in + tbase, (uint32_t)cnt_tile * 16u, &bar[1]);
     }
   }
+  // the group sums of this pass have been consumed by k_prefix: leave them zero for the next pass / the next call (no
+  // memset between the kernels: every boundary in this chain of short kernels costs microseconds)
+  if (t < group_rows) group[(size_t)t * kBinMaxRadix + tid] = 0;
   for (int i = tid; i < kBinWarps * kBinMaxRadix / 2; i += kBinThreads) reinterpret_cast<uint32_t *>(wc)[i] = 0u;
   // items the bulk copies do not cover (ragged tail, or unaligned caller arrays)
   for (int j = n_bulk + tid; j < cnt_tile; j += kBinThreads) {
@@ -375,7 +379,7 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_tile_sums(int32_t n, cons
   }
 }
 
-__global__ void __launch_bounds__(kScanThreads) k_cell_scan(int32_t n, const int32_t *__restrict__ count,
+__global__ void __launch_bounds__(kScanThreads) k_cell_scan(int32_t n, int32_t *__restrict__ count,
                                                            const int32_t *__restrict__ tile_sums,
                                                            int32_t *__restrict__ cell_start) {
   __shared__ int ws[kScanThreads / 32];
@@ -392,7 +396,12 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(int32_t n, const int
 #pragma unroll
   for (int r = 0; r < kScanItems; ++r) {
     const int i = base + r * kScanThreads + tid;
-    sc[r * kScanThreads + tid] = i < n ? __ldg(count + i) : 0;
+    int cnt_i = 0;
+    if (i < n) {
+      cnt_i = count[i];
+      count[i] = 0;  // left zero for the next call (k_cell_tile_sums has read it already)
+    }
+    sc[r * kScanThreads + tid] = cnt_i;
   }
   __syncthreads();
   before = 0;
@@ -429,12 +438,12 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(int32_t n, const int
 
 template <bool FIRST, bool LAST>
 static void launch_downsweep(int n_tiles, cudaStream_t s, int64_t n, int32_t K, const BinPass &ps, const BinIo &io,
-                             const int32_t *hist) {
+                             const int32_t *hist, int32_t *group, int group_rows) {
   auto kern = k_downsweep<FIRST, LAST>;
   const size_t smem = (size_t)kBinTile * (FIRST ? 16 : 20) + 2 * 4 * kBinMaxRadix + 2 * kBinWarps * kBinMaxRadix +
                       2 * kBinTile + 128;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  kern<<<n_tiles, kBinThreads, smem, s>>>(n, K, ps, io, hist);
+  kern<<<n_tiles, kBinThreads, smem, s>>>(n, K, ps, io, hist, group, group_rows);
 }
 
 int bin_num_passes(int32_t K) {
@@ -450,7 +459,8 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     return cudaMemsetAsync(cell_start, 0, sizeof(int32_t) * (size_t)(K + 1), s) == cudaSuccess ? DSMC_OK
                                                                                                 : DSMC_ERR_CUDA;
   }
-  if (cudaMemsetAsync(c->d_cell_count, 0, sizeof(int32_t) * (size_t)(K + 1), s) != cudaSuccess) return DSMC_ERR_CUDA;
+  // (d_cell_count and d_bin_group are zero on entry: zeroed once when the workspace is made, and every call leaves them
+  // zero -- k_cell_scan clears the counts it has read, the down-sweeps clear the group sums)
   int bits = 1;
   while ((int64_t(1) << bits) < (int64_t)K) ++bits;
   const int passes = (bits + 8) / 9;
@@ -477,8 +487,6 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     io.cell_count = c->d_cell_count;
     io.bulk_ok = ((reinterpret_cast<uintptr_t>(cell) | reinterpret_cast<uintptr_t>(vx) |
                    reinterpret_cast<uintptr_t>(vy) | reinterpret_cast<uintptr_t>(vz)) & 15) == 0;
-    if (cudaMemsetAsync(c->d_bin_group, 0, sizeof(int32_t) * (size_t)groups * kBinMaxRadix, s) != cudaSuccess)
-      return DSMC_ERR_CUDA;
     if (first)
       k_tile_hist<true><<<hist_grid, kBinThreads, 0, s>>>(n, K, n_tiles, cell, ps, tpg, c->d_bin_hist,
                                                           c->d_bin_group, c->d_status);
@@ -486,10 +494,10 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
       k_tile_hist<false><<<hist_grid, kBinThreads, 0, s>>>(n, K, n_tiles, io.cell_in, ps, tpg, c->d_bin_hist,
                                                            c->d_bin_group, c->d_status);
     k_prefix<<<groups, kBinThreads, 0, s>>>(n_tiles, groups, tpg, ps, c->d_bin_hist, c->d_bin_group);
-    if (first && last) launch_downsweep<true, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
-    else if (first) launch_downsweep<true, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
-    else if (last) launch_downsweep<false, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
-    else launch_downsweep<false, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist);
+    if (first && last) launch_downsweep<true, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
+    else if (first) launch_downsweep<true, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
+    else if (last) launch_downsweep<false, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
+    else launch_downsweep<false, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
     c->launches += 3;
     if (last) {
       const int n_scan = K + 1, scan_tiles = (n_scan + kScanTile - 1) / kScanTile;

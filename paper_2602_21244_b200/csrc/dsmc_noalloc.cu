@@ -10,8 +10,9 @@
 // HOST code the array's name is a host-side stand-in, not a device address, so its address is taken once per device
 // with cudaGetSymbolAddress (device current) and only that pointer ever reaches a kernel.
 //
-// Every call shares the array and the array keeps the last call's contents: what must start at zero (status word,
-// per-cell counts, group sums) is cleared on the caller's stream at the start of the call.  Calls that overlap on the
+// Every call shares the array and the array keeps the last call's contents: the status word is cleared on the caller's
+// stream at the start of the call; the per-cell counts and the group sums start at zero because the array is
+// zero-initialised when the module loads and the kernels that consume them leave them zero (as in dsmc_bin).  Calls that overlap on the
 // GPU (two streams, two threads, or a dsmc_bin_noalloc graph replayed concurrently with itself) RACE on the array.
 #include <mutex>
 
