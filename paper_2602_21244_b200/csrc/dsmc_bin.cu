@@ -50,6 +50,8 @@ __global__ void __launch_bounds__(kBinThreads) k_tile_hist(int64_t n, int32_t K,
   __shared__ int h[kHistTiles][kBinMaxRadix];
   const int tid = threadIdx.x;
   const int t0 = blockIdx.x * kHistTiles;
+  if (!FIRST) pdl_wait();  // (the first kernel of the chain is launched the ordinary way)
+  pdl_launch_dependents();
 #pragma unroll
   for (int k = 0; k < kHistTiles; ++k) h[k][tid] = 0;
   int c[kHistTiles][kBinItems];
@@ -102,6 +104,8 @@ __global__ void __launch_bounds__(kBinThreads) k_prefix(int n_tiles, int n_group
   __shared__ int scratch[kBinWarps + 1];
   const int d = threadIdx.x, lane = d & 31, warp = d >> 5;
   const int g = blockIdx.x;
+  pdl_wait();
+  pdl_launch_dependents();
   int before = 0, total = 0;
   if (d < ps.R) {
     for (int gg = 0; gg < n_groups; ++gg) {
@@ -216,6 +220,8 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int t = blockIdx.x;
+  pdl_wait();
+  pdl_launch_dependents();
   const int64_t tbase = (int64_t)t * kBinTile;
   const int cnt_tile = (int)min((int64_t)kBinTile, n - tbase);
   const int32_t *cin = FIRST ? io.cell : io.cell_in;
@@ -361,6 +367,8 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_tile_sums(int32_t n, cons
                                                                 int32_t *__restrict__ tile_sums) {
   __shared__ int ws[kScanThreads / 32];
   const int base = blockIdx.x * kScanTile;
+  pdl_wait();
+  pdl_launch_dependents();
   int sum = 0;
 #pragma unroll
   for (int r = 0; r < kScanItems; ++r) {
@@ -386,6 +394,8 @@ __global__ void __launch_bounds__(kScanThreads) k_cell_scan(int32_t n, int32_t *
   __shared__ int sc[kScanTile];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int base = blockIdx.x * kScanTile;
+  pdl_wait();
+  pdl_launch_dependents();
   // tiles before this one
   int before = 0;
   for (int t = tid; t < (int)blockIdx.x; t += kScanThreads) before += __ldg(tile_sums + t);
@@ -443,7 +453,7 @@ static void launch_downsweep(int n_tiles, cudaStream_t s, int64_t n, int32_t K, 
   const size_t smem = (size_t)kBinTile * (FIRST ? 16 : 20) + 2 * 4 * kBinMaxRadix + 2 * kBinWarps * kBinMaxRadix +
                       2 * kBinTile + 128;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  kern<<<n_tiles, kBinThreads, smem, s>>>(n, K, ps, io, hist, group, group_rows);
+  launch_pdl(kern, n_tiles, kBinThreads, smem, s, n, K, ps, io, hist, group, group_rows);
 }
 
 int bin_num_passes(int32_t K) {
@@ -491,9 +501,9 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
       k_tile_hist<true><<<hist_grid, kBinThreads, 0, s>>>(n, K, n_tiles, cell, ps, tpg, c->d_bin_hist,
                                                           c->d_bin_group, c->d_status);
     else
-      k_tile_hist<false><<<hist_grid, kBinThreads, 0, s>>>(n, K, n_tiles, io.cell_in, ps, tpg, c->d_bin_hist,
-                                                           c->d_bin_group, c->d_status);
-    k_prefix<<<groups, kBinThreads, 0, s>>>(n_tiles, groups, tpg, ps, c->d_bin_hist, c->d_bin_group);
+      launch_pdl(k_tile_hist<false>, hist_grid, kBinThreads, 0, s, n, K, n_tiles, io.cell_in, ps, tpg, c->d_bin_hist,
+                 c->d_bin_group, c->d_status);
+    launch_pdl(k_prefix, groups, kBinThreads, 0, s, n_tiles, groups, tpg, ps, c->d_bin_hist, c->d_bin_group);
     if (first && last) launch_downsweep<true, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
     else if (first) launch_downsweep<true, false>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
     else if (last) launch_downsweep<false, true>(n_tiles, s, n, K, ps, io, c->d_bin_hist, c->d_bin_group, groups);
@@ -501,8 +511,8 @@ int launch_bin(dsmc_ctx *c, int64_t n, int32_t K, const int32_t *cell, const flo
     c->launches += 3;
     if (last) {
       const int n_scan = K + 1, scan_tiles = (n_scan + kScanTile - 1) / kScanTile;
-      k_cell_tile_sums<<<scan_tiles, kScanThreads, 0, s>>>(n_scan, c->d_cell_count, c->d_cell_tile_sums);
-      k_cell_scan<<<scan_tiles, kScanThreads, 0, s>>>(n_scan, c->d_cell_count, c->d_cell_tile_sums, cell_start);
+      launch_pdl(k_cell_tile_sums, scan_tiles, kScanThreads, 0, s, n_scan, c->d_cell_count, c->d_cell_tile_sums);
+      launch_pdl(k_cell_scan, scan_tiles, kScanThreads, 0, s, n_scan, c->d_cell_count, c->d_cell_tile_sums, cell_start);
       c->launches += 2;
     }
   }

@@ -42,6 +42,8 @@ __global__ void __launch_bounds__(256) k_cell_lists(int32_t K, const int32_t *__
                                                     int4 *__restrict__ list2, int32_t *__restrict__ ctr,
                                                     int32_t *__restrict__ ctr_other, int32_t *__restrict__ status) {
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  pdl_wait();  // (cell_start may come from the kernel before this one: dsmc_bin's last)
+  pdl_launch_dependents();
   if (c < 8) ctr_other[c] = 0;  // the counters of the next step (this step's were zeroed by the previous one)
   int cls = -1;
   int4 item = make_int4(0, 0, 0, 0);
@@ -81,6 +83,8 @@ __global__ void __launch_bounds__(256) k_cell_lists(int32_t K, const int32_t *__
 template <int OP>
 __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  pdl_wait();
+  pdl_launch_dependents();
   {
     CellTeam<128, OP> T;
     T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
@@ -98,6 +102,8 @@ __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const Cell
 template <int OP>
 __global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const CellLists Lst) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  pdl_wait();
+  pdl_launch_dependents();
   CellTeam<256, OP> T;
   T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
   T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
@@ -110,9 +116,8 @@ void launch_cell_lists(dsmc_ctx *c, const StepParams &p, CellLists &L) {
   const int e = (int)(c->list_epoch & 1);
   c->list_epoch += 1;
   L.ctr = c->d_list_ctr + 8 * e;
-  k_cell_lists<<<(p.n_cells + 255) / 256, 256, 0, c->stream>>>(p.n_cells, p.cell_start, p.pairs_count,
-                                                                p.pairs_per_cell, L.list[0], L.list[1], L.list[2],
-                                                                L.ctr, c->d_list_ctr + 8 * (1 - e), p.status);
+  launch_pdl(k_cell_lists, (p.n_cells + 255) / 256, 256, 0, c->stream, p.n_cells, p.cell_start, p.pairs_count,
+             p.pairs_per_cell, L.list[0], L.list[1], L.list[2], L.ctr, c->d_list_ctr + 8 * (1 - e), p.status);
   c->launches += 1;
 }
 
@@ -126,14 +131,14 @@ static int launch_cells_pass(dsmc_ctx *c, const StepParams &p) {
     static_assert(CellTeam<128>::bytes() == 4 * CellTeam<32>::bytes(), "the two team forms share one footprint");
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return DSMC_ERR_CUDA;
-    kern<<<c->num_sms * 8, 128, smem, c->stream>>>(p, L);
+    launch_pdl(kern, c->num_sms * 8, 128, smem, c->stream, p, L);
   }
   {
     auto kern = k_cells_big<OP>;
     const size_t smem = CellTeam<256>::bytes();
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return DSMC_ERR_CUDA;
-    kern<<<c->num_sms * 2, 256, smem, c->stream>>>(p, L);
+    launch_pdl(kern, c->num_sms * 2, 256, smem, c->stream, p, L);
   }
   c->launches += 2;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;

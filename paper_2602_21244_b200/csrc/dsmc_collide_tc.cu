@@ -379,6 +379,8 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
     tc::mbar_expect_tx(x_bar, (uint32_t)n_extra * kLayerBytes);
     tc::bulk_g2s(extra, reinterpret_cast<const unsigned char *>(net.w_blob) + net.extra_off, (uint32_t)n_extra * kLayerBytes, x_bar);
   }
+  pdl_wait();  // the set-up above (weights, tensor memory) ran under the tail of the kernel before this one
+  pdl_launch_dependents();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n_tiles = (n + 127) / 128;
   const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -480,7 +482,7 @@ static int launch_chi_batch_tc_h(dsmc_ctx *c, int64_t n, const float *E, const f
   if (smem > 227 * 1024) return DSMC_ERR_UNSUPPORTED_SHAPE;
   auto kern = net->n_hidden > 2 ? k_chi_batch_tc<H, RAW, true> : k_chi_batch_tc<H, RAW, false>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return DSMC_ERR_CUDA;
-  kern<<<grid, kPipeThreads, smem, c->stream>>>(n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
+  launch_pdl(kern, grid, kPipeThreads, (size_t)smem, c->stream, n, E, b, chi, *net, tc_out_layer(*net), 1.0f / b_max, lnE_min, inv_range);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }
@@ -617,6 +619,8 @@ __global__ void __launch_bounds__(kPipeThreads, 1)
     tc::mbar_expect_tx(w_bar, (uint32_t)(H * H * 2));
     tc::bulk_g2s(w2lo, reinterpret_cast<const unsigned char *>(net.w_blob) + SH::BLOB_BYTES, (uint32_t)(H * H * 2), w_bar);
   }
+  pdl_wait();  // the set-up above ran under the tail of the kernel before this one
+  pdl_launch_dependents();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n_tiles = (n + 127) / 128;
   const int64_t mine = n_tiles > blockIdx.x ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
@@ -722,7 +726,7 @@ static int launch_mlp_rows_tc_split_h(dsmc_ctx *c, int64_t n, const float *x, in
   const int smem = ((PipeShape<H>::SMEM_BYTES + 127) & ~127) + H * H * 2 + 2 * 2 * 4 * 128 * 16 + 64 + 128;
   auto kern = k_mlp_rows_tc_split<H>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return DSMC_ERR_CUDA;
-  kern<<<grid, kPipeThreads, smem, c->stream>>>(n, x, x_stride, net->d_in, y0, y1, y2, *net, *tail);
+  launch_pdl(kern, grid, kPipeThreads, (size_t)smem, c->stream, n, x, x_stride, net->d_in, y0, y1, y2, *net, *tail);
   c->launches += 1;
   return cudaGetLastError() == cudaSuccess ? DSMC_OK : DSMC_ERR_CUDA;
 }

@@ -6,6 +6,13 @@
 
 namespace dsmc {
 
+// Programmatic dependent launch (a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
+// while its predecessor in the stream drains): pdl_wait() returns when the predecessor grid has completed and its
+// writes are visible -- it must come before the first access to anything the predecessor touches; after
+// pdl_launch_dependents() in every CTA the next kernel's CTAs may be scheduled as this grid's last wave frees SMs.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // Philox4x32-10 (Salmon et al. SC'11): counter (c0..c3), key (k0,k1).
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
                                                uint32_t k1) {
