@@ -44,7 +44,8 @@ __global__ void __launch_bounds__(256) k_cell_lists(int32_t K, const int32_t *__
   const int c = blockIdx.x * blockDim.x + threadIdx.x;
   pdl_wait();  // (cell_start may come from the kernel before this one: dsmc_bin's last)
   pdl_launch_dependents();
-  if (c < 8) ctr_other[c] = 0;  // the counters of the next step (this step's were zeroed by the previous one)
+  if (c < 8) ctr_other[c] = 0;  // the counters of the next launch (this launch's list lengths were zeroed by the previous one)
+  if (c < 4) ctr[4 + c] = 0;    // this launch's work counters (nobody reads them before this kernel has completed)
   int cls = -1;
   int4 item = make_int4(0, 0, 0, 0);
   if (c < K) {
@@ -88,13 +89,13 @@ __global__ void __launch_bounds__(128, 8) k_cells(const StepParams P, const Cell
   {
     CellTeam<128, OP> T;
     T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
-    T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
+    T.run(P, Lst.list[1], Lst.ctr + 1, Lst.work + 1);
   }
   __syncthreads();
   {
     CellTeam<32, OP> T;
     T.init((uint32_t)__cvta_generic_to_shared(smem_raw) + (threadIdx.x >> 5) * (uint32_t)CellTeam<32>::bytes(), threadIdx.x & 31, 0);
-    T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
+    T.run(P, Lst.list[0], Lst.ctr + 0, Lst.work + 0);
   }
 }
 
@@ -106,7 +107,7 @@ __global__ void __launch_bounds__(256, 2) k_cells_big(const StepParams P, const 
   pdl_launch_dependents();
   CellTeam<256, OP> T;
   T.init((uint32_t)__cvta_generic_to_shared(smem_raw), threadIdx.x, 0);
-  T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
+  T.run(P, Lst.list[2], Lst.ctr + 2, Lst.work + 2);
 }
 
 // cell lists of this step (alternating counter sets: this launch zeroes the set of the next step)
@@ -116,15 +117,26 @@ void launch_cell_lists(dsmc_ctx *c, const StepParams &p, CellLists &L) {
   const int e = (int)(c->list_epoch & 1);
   c->list_epoch += 1;
   L.ctr = c->d_list_ctr + 8 * e;
+  L.work = L.ctr + 4;
   launch_pdl(k_cell_lists, (p.n_cells + 255) / 256, 256, 0, c->stream, p.n_cells, p.cell_start, p.pairs_count,
              p.pairs_per_cell, L.list[0], L.list[1], L.list[2], L.ctr, c->d_list_ctr + 8 * (1 - e), p.status);
   c->launches += 1;
 }
 
-template <int OP>
+// REUSE: walk the lists the previous pass of this step made (same cells, same pair counts) with a fresh set of work
+// counters -- the other epoch's, which k_cell_lists zeroed and nobody has used since -- instead of building them again
+template <int OP, bool REUSE = false>
 static int launch_cells_pass(dsmc_ctx *c, const StepParams &p) {
   CellLists L;
-  launch_cell_lists(c, p, L);
+  if (REUSE) {
+    const size_t K = (size_t)c->max_cells;
+    const int e = (int)((c->list_epoch - 1) & 1);  // the epoch of the lists just made
+    for (int k = 0; k < 3; ++k) L.list[k] = c->d_cell_list + k * K;
+    L.ctr = c->d_list_ctr + 8 * e;
+    L.work = c->d_list_ctr + 8 * (1 - e) + 4;
+  } else {
+    launch_cell_lists(c, p, L);
+  }
   {
     auto kern = k_cells<OP>;
     const size_t smem = CellTeam<128>::bytes();
@@ -171,7 +183,7 @@ int launch_collide_cells_split(dsmc_ctx *c, const StepParams &p_in, const MlpTcD
   if (rc != DSMC_OK) return rc;
   rc = launch_chi_rows_tc(c, p.n / 2 + 1, p.feat0, p.feat1, p.chi_pair, net);
   if (rc != DSMC_OK) return rc;
-  return launch_cells_pass<4>(c, p);
+  return launch_cells_pass<4, true>(c, p);
 }
 
 // VHS-NN operator on the tensor cores, split form on the cell-team kernels (default for DSMC_F_BF16_TC;
@@ -196,7 +208,7 @@ int launch_collide_cells_vhs_split(dsmc_ctx *c, const StepParams &p_in, const Ml
   if (rc != DSMC_OK) return rc;
   rc = launch_mlp_rows_tc_split(c, p.n / 2 + 1, p.feat0, np, p.out3[0], p.out3[1], p.out3[2], net, tail);
   if (rc != DSMC_OK) return rc;
-  return launch_cells_pass<6>(c, p);
+  return launch_cells_pass<6, true>(c, p);
 }
 
 }  // namespace dsmc

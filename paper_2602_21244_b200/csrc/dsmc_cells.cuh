@@ -10,7 +10,8 @@ constexpr int kRankWin = 4;   // bucket members compared without a loop
 
 struct CellLists {
   int4 *list[3];  // (cell, first slot, N, M) by size class: N <= 256, <= 1024, <= 2048
-  int32_t *ctr;   // [0..2] entries of each list, [4..6] work counters
+  int32_t *ctr;   // [0..2] entries of each list
+  int32_t *work;  // [0..2] work counters of the kernels that walk the lists
 };
 
 // Four warp sums for the price of six shuffles: returns the total of a in lanes 0-7, b in 8-15, c in 16-23, d in 24-31.

@@ -184,8 +184,8 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
       const uint32_t b0 = base_s + (uint32_t)(8 * NBUF * g * SLICE);
       T.init(b0, ttid - 256 * g, 1 + g);
       T.srv = &srv;
-      if (NBUF == 2) T.run2(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2, b0, b0 + (uint32_t)(8 * SLICE));
-      else T.run(P, Lst.list[2], Lst.ctr + 2, Lst.ctr + 4 + 2);
+      if (NBUF == 2) T.run2(P, Lst.list[2], Lst.ctr + 2, Lst.work + 2, b0, b0 + (uint32_t)(8 * SLICE));
+      else T.run(P, Lst.list[2], Lst.ctr + 2, Lst.work + 2);
       asm volatile("bar.sync %0, 256;" ::"r"(1 + g) : "memory");
     }
     if (tw < 4 * G4) {  // cells of 257..1024 particles: groups of four warps
@@ -194,8 +194,8 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
       const uint32_t b0 = base_s + (uint32_t)(4 * NBUF * g * SLICE);
       T.init(b0, ttid - 128 * g, 1 + G8 + g);
       T.srv = &srv;
-      if (NBUF == 2) T.run2(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1, b0, b0 + (uint32_t)(4 * SLICE));
-      else T.run(P, Lst.list[1], Lst.ctr + 1, Lst.ctr + 4 + 1);
+      if (NBUF == 2) T.run2(P, Lst.list[1], Lst.ctr + 1, Lst.work + 1, b0, b0 + (uint32_t)(4 * SLICE));
+      else T.run(P, Lst.list[1], Lst.ctr + 1, Lst.work + 1);
       asm volatile("bar.sync %0, 128;" ::"r"(1 + G8 + g) : "memory");
     }
     {
@@ -203,8 +203,8 @@ __global__ void __launch_bounds__((NTW + NA + 2) * 32, 1) k_cells_mlp(const Step
       const uint32_t b0 = base_s + (uint32_t)(NBUF * tw * SLICE);
       T.init(b0, lane, 0);
       T.srv = &srv;
-      if (NBUF == 2) T.run2(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0, b0, b0 + (uint32_t)SLICE);
-      else T.run(P, Lst.list[0], Lst.ctr + 0, Lst.ctr + 4 + 0);
+      if (NBUF == 2) T.run2(P, Lst.list[0], Lst.ctr + 0, Lst.work + 0, b0, b0 + (uint32_t)SLICE);
+      else T.run(P, Lst.list[0], Lst.ctr + 0, Lst.work + 0);
     }
     }
     if (lane == 0) {
