@@ -129,21 +129,19 @@ __global__ void __launch_bounds__(kBinThreads) k_prefix(int n_tiles, int n_group
   int run = woff + inc - total + before;
   if (d >= ps.R) return;
   const int t0 = g * tiles_per_group, t1 = min(t0 + tiles_per_group, n_tiles);
-  int t = t0;
-  for (; t + 8 <= t1; t += 8) {
-    int x[8];
+  // the walk is a chain of L2 / DRAM round trips (one CTA per SM, nothing else to run): eighteen loads in flight per
+  // trip, predicated at the end of the group, so that a group of 36 tiles takes two trips (it was 4 trips of 8 and a
+  // serial remainder of 4: the remainder alone was a quarter of the kernel)
+  constexpr int kWalk = 18;
+  for (int t = t0; t < t1; t += kWalk) {
+    int x[kWalk];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) x[u] = hist[(size_t)(t + u) * kBinMaxRadix + d];
+    for (int u = 0; u < kWalk; ++u) x[u] = t + u < t1 ? hist[(size_t)(t + u) * kBinMaxRadix + d] : 0;
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      hist[(size_t)(t + u) * kBinMaxRadix + d] = run;
+    for (int u = 0; u < kWalk; ++u) {
+      if (t + u < t1) hist[(size_t)(t + u) * kBinMaxRadix + d] = run;
       run += x[u];
     }
-  }
-  for (; t < t1; ++t) {
-    const int x = hist[(size_t)t * kBinMaxRadix + d];
-    hist[(size_t)t * kBinMaxRadix + d] = run;
-    run += x;
   }
 }
 
