@@ -267,6 +267,7 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
   mbar_wait(&bar[0], 0);
 
   uint16_t *mywc = wc + warp * kBinMaxRadix;
+  const int nbits = __popc((unsigned)ps.mask);
   const int jbase = warp * (32 * kBinItems) + lane;
   int c[kBinItems], lr[kBinItems];
 #pragma unroll
@@ -278,7 +279,18 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
 #pragma unroll
   for (int r = 0; r < kBinItems; ++r) {
     const int d = c[r] >= 0 ? bin_digit(c[r], ps) : 0xFFFF;
-    const uint32_t m = __match_any_sync(0xffffffffu, d);
+    // lanes with the same digit: one ballot per digit bit (MATCH.ANY takes time in proportion to the number of
+    // distinct values in the warp, and with 512 digits nearly all 32 are distinct: it was the top stall of the pass)
+    uint32_t m = __ballot_sync(0xffffffffu, c[r] >= 0);
+    m = c[r] >= 0 ? m : ~m;
+#pragma unroll
+    for (int b = 0; b < 9; ++b) {
+      if (b < nbits) {
+        const bool bit = (d >> b) & 1;
+        const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+        m &= bit ? bal : ~bal;
+      }
+    }
     const int rk = __popc(m & ((1u << lane) - 1u));
     int old = 0;
     if (rk == 0 && c[r] >= 0) {
