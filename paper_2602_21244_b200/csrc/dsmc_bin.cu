@@ -281,15 +281,22 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_downsweep(int64_t n, int32_t
     const int d = c[r] >= 0 ? bin_digit(c[r], ps) : 0xFFFF;
     // lanes with the same digit: one ballot per digit bit (MATCH.ANY takes time in proportion to the number of
     // distinct values in the warp, and with 512 digits nearly all 32 are distinct: it was the top stall of the pass)
-    uint32_t m = __ballot_sync(0xffffffffu, c[r] >= 0);
-    m = c[r] >= 0 ? m : ~m;
+    // (later passes see fewer distinct digits per warp -- their input is ordered by the lower digits -- and there
+    // match.any is the faster of the two: measured 153 against 158 us)
+    uint32_t m;
+    if (FIRST) {
+      m = __ballot_sync(0xffffffffu, c[r] >= 0);
+      m = c[r] >= 0 ? m : ~m;
 #pragma unroll
-    for (int b = 0; b < 9; ++b) {
-      if (b < nbits) {
-        const bool bit = (d >> b) & 1;
-        const uint32_t bal = __ballot_sync(0xffffffffu, bit);
-        m &= bit ? bal : ~bal;
+      for (int b = 0; b < 9; ++b) {
+        if (b < nbits) {
+          const bool bit = (d >> b) & 1;
+          const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+          m &= bit ? bal : ~bal;
+        }
       }
+    } else {
+      m = __match_any_sync(0xffffffffu, d);
     }
     const int rk = __popc(m & ((1u << lane) - 1u));
     int old = 0;
